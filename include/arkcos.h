@@ -1,0 +1,145 @@
+/* arkcos.h -- C ABI of libarkcos.so: hybrid Fourier/direct-space convolution of a ring-pixelized map on
+ * the sphere with a compact radial kernel (Elsner & Wandelt, "ARKCoS", arXiv:1104.0672), for NVIDIA B200
+ * (sm_100a).  Citations are PAPER.md:<line> of the paper text, plus the section / equation.
+ *
+ * What one call computes (Eq. 1 / Eq. 6, with the quadrature weight of PAPER.md:99):
+ *
+ *     out(p) = sum_{q : gamma_pq < theta_max}  K(gamma_pq) * in(q) * Omega_q
+ *
+ * by the hybrid method of section 4 with the anti-ringing treatment of section 4.3
+ * (PAPER.md:219): real FFT along every isolatitude ring, kernel rows K(gamma(theta_i, theta_j, dphi)) sampled
+ * on a phi grid (Eq. 9) and Fourier-transformed along phi, multiplied with the input-ring spectra
+ * and summed over the input rings j inside the support for every azimuthal mode m, super-Nyquist modes folded
+ * onto the ring's own modes, inverse real FFT.  On an ECP grid and in the HEALPix equatorial region the result
+ * equals the direct sum up to rounding; where a polar-cap ring is involved it carries the interpolation error
+ * of the kernel-row grid (controlled by ell_nyquist / polar_oversample below).
+ *
+ * Every step runs in CUDA kernels of this library on the caller's stream.  There is no CPU fallback and no
+ * cuFFT.  All functions return 0 (ARKCOS_OK) or a negative arkcos_status; nothing throws or aborts across the
+ * ABI.  Unless noted, pointers are HOST pointers.
+ */
+#ifndef ARKCOS_H
+#define ARKCOS_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct arkcos_plan arkcos_plan;          /* opaque; owns all device tables and the workspace */
+
+typedef enum {
+    ARKCOS_OK = 0,
+    ARKCOS_INVALID_ARG = -1,       /* NULL pointer, size out of range, in == out, nmaps > max_nmaps, ... */
+    ARKCOS_UNSUPPORTED = -2,       /* a valid request this build does not implement (see each function) */
+    ARKCOS_CUDA_ERROR = -3,        /* a CUDA runtime call failed (no device, launch failure, ...) */
+    ARKCOS_OUT_OF_MEMORY = -4      /* host or device allocation failed */
+} arkcos_status;
+
+typedef enum { ARKCOS_ECP = 0, ARKCOS_HEALPIX_RING = 1 } arkcos_pix_kind;
+typedef enum { ARKCOS_F32 = 0, ARKCOS_F64 = 1 } arkcos_dtype;
+
+/* Pixelization: pixels grouped into isolatitude rings.
+ *  ECP           ntheta rings at theta_i = (i + 1/2) pi / ntheta, nphi pixels each at phi_k = 2 pi k / nphi,
+ *                Omega_i = sin(theta_i) (pi/ntheta) (2 pi/nphi); pixel index p = i * nphi + k.
+ *                nphi must be a power of two, 4 <= nphi <= 16384 (f32) / 8192 (f64).
+ *  HEALPIX_RING  ring scheme, resolution nside: rings 1 .. 4 nside - 1 north to south, cap ring
+ *                n has 4 n pixels shifted by pi / (4 n), the 2 nside + 1 equatorial rings have 4 nside pixels, every
+ *                other one shifted by pi / (4 nside); Omega = 4 pi / (12 nside^2); pixel index = RING ordering.
+ *                nside must be a power of two, 1 <= nside <= 4096 (f32) / 2048 (f64). */
+typedef struct {
+    arkcos_pix_kind kind;
+    int ntheta, nphi;              /* ECP only */
+    int nside;                     /* HEALPix only */
+} arkcos_pixelization;
+
+/* Radial profile (a precomputed table, interpolated linearly).
+ *  table[t] = K(theta_t), theta_t = t * theta_max / (n - 1), t = 0 .. n-1 (both end points included); host memory,
+ *  copied by arkcos_plan_create (the caller may free it afterwards).  n >= 2.
+ *  The support is gamma < theta_max, strict; 0 < theta_max <= pi, radians, a radius. */
+typedef struct {
+    const double* table;
+    int n;
+    double theta_max;
+} arkcos_kernel;
+
+/* Options; pass NULL for the defaults (all fields zero).
+ *  variant           0: anti-ringing scheme of PAPER.md:219 (periodic extension of the ring spectra, folding of the
+ *                       super-Nyquist modes, ring offsets inside the kernel evaluation).  1: the basic scheme of
+ *                       PAPER.md:125, 142 (zero-pad, truncate) -- ARKCOS_UNSUPPORTED in this build.
+ *  ell_nyquist       length of the phi grid on which a kernel row that touches a polar-cap ring is sampled:
+ *                       M'_i = max(8, 2 ceil(ell_nyquist * smax_i)), smax_i = max sin(theta) over output ring i and
+ *                       its band, i.e. the row resolves wavenumber ell_nyquist along the ring.  0: chosen from the
+ *                       profile at plan time (arkcos_plan_ell_nyquist reports it).  Ignored if polar_oversample > 0.
+ *  polar_oversample  > 0: M' = polar_oversample * 4 nside for every such row; 1 is the paper's choice.
+ *  max_nmaps         largest nmaps arkcos_convolve will be called with (sizes the workspace); 0 means 1.
+ *  cache_kernel_rows 0: the kernel rows are re-evaluated from the profile table inside every arkcos_convolve (the
+ *                       paper's timing includes the kernel evaluation, Table 1); 1: they are
+ *                       evaluated once in arkcos_plan_create. */
+typedef struct {
+    int variant;
+    double ell_nyquist;
+    int polar_oversample;
+    int max_nmaps;
+    int cache_kernel_rows;
+    int reserved[8];               /* must be zero */
+} arkcos_options;
+
+/* Builds the ring-geometry table (theta, N, phi0, offset per ring), the band and ring-pair tables, FFT twiddles,
+ * and allocates the workspace on the CURRENT CUDA device.  On failure *out is untouched. */
+int arkcos_plan_create(arkcos_plan** out, const arkcos_pixelization* pix, const arkcos_kernel* kernel,
+                       arkcos_dtype dtype, const arkcos_options* options /* NULL = defaults */);
+
+/* Same tables, host side only: no CUDA call is made, so it works without a device.  The plan answers the queries
+ * below (geometry, bands, M'_i, work model); arkcos_convolve on it returns ARKCOS_INVALID_ARG. */
+int arkcos_plan_create_tables_only(arkcos_plan** out, const arkcos_pixelization* pix, const arkcos_kernel* kernel,
+                                   arkcos_dtype dtype, const arkcos_options* options);
+
+/* d_in, d_out: DEVICE pointers owned by the caller, element type = the plan's dtype, layout [nmaps][npix]
+ * contiguous, pixels in ring order.  d_in is not modified; d_in == d_out (or overlapping) is rejected.
+ * cuda_stream: a cudaStream_t (NULL = the default stream).  The call only enqueues kernels on that stream: no
+ * synchronisation, no allocation, no host arithmetic.  Two calls on the same plan must not run concurrently
+ * (they share the plan's workspace). */
+int arkcos_convolve(const arkcos_plan* plan, const void* d_in, void* d_out, int nmaps, void* cuda_stream);
+
+/* Same result from HOST buffers (pinned memory makes the copies asynchronous): host -> device copy, arkcos_convolve,
+ * device -> host copy, all on cuda_stream, then a stream synchronisation.  Uses staging buffers inside the plan. */
+int arkcos_convolve_host(const arkcos_plan* plan, const void* h_in, void* h_out, int nmaps, void* cuda_stream);
+
+int arkcos_plan_destroy(arkcos_plan* plan);      /* NULL is a no-op */
+
+/* ---- queries (host side, no CUDA work) ---- */
+int64_t arkcos_plan_npix(const arkcos_plan* plan);
+int arkcos_plan_nrings(const arkcos_plan* plan);
+/* ring = 0 .. nrings-1 north to south; any output pointer may be NULL.  mprime = M'_i of that OUTPUT ring. */
+int arkcos_plan_ring_info(const arkcos_plan* plan, int ring, double* theta, int* n, double* phi0, int64_t* offset,
+                          int* band_lo, int* band_hi, int* mprime);
+double arkcos_plan_ell_nyquist(const arkcos_plan* plan);
+
+/* Work model of one arkcos_convolve with nmaps = 1; any pointer may be NULL.
+ *  ring_pairs        ordered ring pairs (i, j) inside the support
+ *  row_samples       kernel-row samples evaluated (after the even and north/south symmetries)
+ *  mac_flops         flops of the band kernel: cosine transform of the rows + multiply-accumulate over input rings
+ *  fft_flops         flops of the forward + inverse ring FFTs as executed (incl. Bluestein padding)
+ *  workspace_bytes   device memory held by the plan */
+int arkcos_plan_stats(const arkcos_plan* plan, int64_t* ring_pairs, int64_t* row_samples, double* mac_flops,
+                      double* fft_flops, int64_t* workspace_bytes);
+
+/* Optional per-stage timing of arkcos_convolve with CUDA events recorded on the caller's stream between the stages.
+ * arkcos_plan_get_timing waits for the last call and returns milliseconds for
+ *   ms4[0] kernel-row generator, ms4[1] forward ring FFT, ms4[2] band multiply-accumulate, ms4[3] inverse ring FFT. */
+int arkcos_plan_set_timing(const arkcos_plan* plan, int enable);
+int arkcos_plan_get_timing(const arkcos_plan* plan, float* ms4);
+
+/* Measures the FP32 FMA throughput of the current device with a register-resident FFMA chain (the denominator of the
+ * "alu" roofline); result in TFLOP/s, best of `repeats` launches.  Synchronises the device. */
+int arkcos_probe_fp32_peak(double* tflops, int repeats);
+
+const char* arkcos_strerror(int status);
+const char* arkcos_last_error(void);             /* detail of the last failure on this thread ("" if none) */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* ARKCOS_H */

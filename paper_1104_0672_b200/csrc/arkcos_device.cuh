@@ -1,0 +1,45 @@
+// Device-side helpers shared by the kernels of libarkcos (complex arithmetic, exact-phase twiddles).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace arkcos {
+
+template <class T> struct cx { T x, y; };              // complex number (re, im); cx<float> is 8 bytes, cx<double> 16
+
+template <class T> __host__ __device__ __forceinline__ cx<T> mk(T a, T b) { cx<T> r; r.x = a; r.y = b; return r; }
+template <class T> __device__ __forceinline__ cx<T> operator+(cx<T> a, cx<T> b) { return mk<T>(a.x + b.x, a.y + b.y); }
+template <class T> __device__ __forceinline__ cx<T> operator-(cx<T> a, cx<T> b) { return mk<T>(a.x - b.x, a.y - b.y); }
+template <class T> __device__ __forceinline__ cx<T> cmul(cx<T> a, cx<T> b)
+{
+    return mk<T>(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x);
+}
+template <class T> __device__ __forceinline__ cx<T> cmulc(cx<T> a, cx<T> b)   // a * conj(b)
+{
+    return mk<T>(a.x * b.x + a.y * b.y, a.y * b.x - a.x * b.y);
+}
+template <class T> __device__ __forceinline__ cx<T> cconj(cx<T> a) { return mk<T>(a.x, -a.y); }
+template <class T> __device__ __forceinline__ cx<T> cscale(cx<T> a, T s) { return mk<T>(a.x * s, a.y * s); }
+
+__device__ __forceinline__ void sincospi_t(float x, float* s, float* c) { sincospif(x, s, c); }
+__device__ __forceinline__ void sincospi_t(double x, double* s, double* c) { sincospi(x, s, c); }
+
+// exp(i * pi * num / den) for integers 0 <= num < 2 den, den >= 1.  The argument is reduced to the first octant with
+// integer arithmetic, so the result is accurate to about one ulp of T whatever the size of num and den.
+template <class T> __device__ __forceinline__ cx<T> cispi_ratio(uint32_t num, uint32_t den)
+{
+    bool neg = num >= den;                  // e^{i (pi + a)} = -e^{i a}
+    if (neg) num -= den;
+    bool refl = 2u * num > den;             // a -> pi - a
+    if (refl) num = den - num;
+    bool swp = 4u * num > den;              // a -> pi/2 - a
+    uint32_t rr = swp ? (den - 2u * num) : 2u * num;       // angle = pi * rr / (2 den), rr / (2 den) in [0, 1/4]
+    T s, c;
+    sincospi_t((T)rr / (T)(2u * den), &s, &c);
+    if (swp) { T t = s; s = c; c = t; }
+    if (refl) c = -c;
+    if (neg) { c = -c; s = -s; }
+    return mk<T>(c, s);
+}
+
+}  // namespace arkcos

@@ -1,0 +1,566 @@
+// libarkcos: plan construction (host) and the C ABI of include/arkcos.h.
+#include <math.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <algorithm>
+#include <map>
+#include <new>
+
+#include "arkcos_plan.hpp"
+
+using namespace arkcos;
+
+namespace {
+
+thread_local std::string g_last_error;
+
+int fail(int code, const std::string& msg)
+{
+    g_last_error = msg;
+    return code;
+}
+
+#define CUDA_TRY(expr)                                                                                        \
+    do {                                                                                                      \
+        cudaError_t e_ = (expr);                                                                              \
+        if (e_ != cudaSuccess) {                                                                              \
+            cudaGetLastError();                                                                               \
+            return fail(e_ == cudaErrorMemoryAllocation ? ARKCOS_OUT_OF_MEMORY : ARKCOS_CUDA_ERROR,           \
+                        std::string(#expr) + ": " + cudaGetErrorString(e_));                                  \
+        }                                                                                                     \
+    } while (0)
+
+bool is_pow2(int v) { return v > 0 && (v & (v - 1)) == 0; }
+int ilog2(int v) { int l = 0; while ((1 << l) < v) ++l; return l; }
+const double kPi = 3.14159265358979323846264338327950288;
+
+// ---- step 0: ring geometry (HEALPix ring centres: Gorski et al. 2005, cited PAPER.md:125) ----
+int build_geometry(const arkcos_pixelization& pix, HostGeometry& g)
+{
+    if (pix.kind == ARKCOS_ECP) {
+        const int R = pix.ntheta, N = pix.nphi;
+        g.R = R;
+        for (int i = 0; i < R; ++i) {
+            const double th = (i + 0.5) * kPi / R;
+            g.theta.push_back(th);
+            g.n.push_back(N);
+            g.phi0.push_back(0.0);
+            g.shifted.push_back(0);
+            g.omega.push_back(sin(th) * (kPi / R) * (2.0 * kPi / N));
+        }
+    } else {
+        const int ns = pix.nside, R = 4 * ns - 1;
+        g.R = R;
+        const double om = 4.0 * kPi / (12.0 * (double)ns * (double)ns);
+        for (int idx = 0; idx < R; ++idx) {
+            const int i = idx + 1;
+            double th;
+            int n, sh;
+            if (i < ns) {                    // north cap: z = 1 - i^2/(3 ns^2), theta = 2 asin(sqrt((1-z)/2))
+                th = 2.0 * asin(i / (sqrt(6.0) * ns));
+                n = 4 * i;
+                sh = 1;
+            } else if (i <= 3 * ns) {        // equatorial belt: z = 4/3 - 2i/(3 ns)
+                th = acos(4.0 / 3.0 - 2.0 * i / (3.0 * ns));
+                n = 4 * ns;
+                sh = ((i - ns) % 2 == 0) ? 1 : 0;
+            } else {                         // south cap: mirror image
+                const int ii = 4 * ns - i;
+                th = kPi - 2.0 * asin(ii / (sqrt(6.0) * ns));
+                n = 4 * ii;
+                sh = 1;
+            }
+            g.theta.push_back(th);
+            g.n.push_back(n);
+            g.shifted.push_back(sh);
+            g.phi0.push_back(sh ? kPi / n : 0.0);
+            g.omega.push_back(om);
+        }
+    }
+    g.pix_off.assign(g.R + 1, 0);
+    g.spec_off.assign(g.R + 1, 0);
+    for (int i = 0; i < g.R; ++i) {
+        g.pix_off[i + 1] = g.pix_off[i] + g.n[i];
+        g.spec_off[i + 1] = g.spec_off[i] + g.n[i] / 2 + 1;
+    }
+    g.npix = g.pix_off[g.R];
+    g.spec_total = g.spec_off[g.R];
+    return 0;
+}
+
+// band of ring i: rings j with |theta_i - theta_j| < theta_max (contiguous, theta is monotonic)
+void build_bands(HostGeometry& g, double theta_max)
+{
+    g.band_lo.resize(g.R);
+    g.band_hi.resize(g.R);
+    int lo = 0, hi = 0;
+    for (int i = 0; i < g.R; ++i) {
+        while (!(fabs(g.theta[i] - g.theta[lo]) < theta_max)) ++lo;
+        if (hi < i) hi = i;
+        while (hi + 1 < g.R && fabs(g.theta[i] - g.theta[hi + 1]) < theta_max) ++hi;
+        g.band_lo[i] = lo;
+        g.band_hi[i] = hi;
+    }
+}
+
+// Automatic ell_nyquist (reading R10): smallest wavenumber beyond which the 1-D spectra of straight cuts
+// through the profile hold less than `tol` of their L1 mass, capped at ell_cap.  Cuts at offsets 0 and theta_max/2.
+double auto_ell_nyquist(const double* table, int ntab, double theta_max, double ell_cap)
+{
+    const int NL = 1024;
+    const int NS = (int)std::min(65536.0, std::max(2048.0, ceil(2.0 * ell_cap * theta_max)));
+    const double tol = 1e-7;
+    double best = 0.0;
+    std::vector<double> f(NS + 1), spec(NL + 1);
+    for (int cut = 0; cut < 2; ++cut) {
+        const double off = cut * 0.5 * theta_max;
+        const double amax = sqrt(theta_max * theta_max - off * off);
+        for (int s = 0; s <= NS; ++s) {
+            const double a = amax * s / NS, gam = sqrt(a * a + off * off);
+            double u = gam * (ntab - 1) / theta_max;
+            int t = std::min(std::max((int)floor(u), 0), ntab - 2);
+            f[s] = gam < theta_max ? table[t] + (u - t) * (table[t + 1] - table[t]) : 0.0;
+        }
+        double total = 0.0;
+        for (int l = 0; l <= NL; ++l) {
+            const double ell = ell_cap * l / NL;
+            double acc = 0.0;
+            for (int s = 0; s <= NS; ++s) acc += ((s == 0 || s == NS) ? 0.5 : 1.0) * f[s] * cos(ell * amax * s / NS);
+            spec[l] = fabs(acc);
+            total += spec[l];
+        }
+        if (!(total > 0.0)) continue;
+        double tail = 0.0;
+        int l = NL;
+        for (; l > 0; --l) {
+            tail += spec[l];
+            if (tail > tol * total) break;
+        }
+        best = std::max(best, ell_cap * std::min(l + 1, NL) / NL);
+    }
+    return best > 0.0 ? best : ell_cap;
+}
+
+struct HostTables {
+    std::vector<RingRec> rings;
+    std::vector<FftLen> lens;
+    std::vector<int> bluestein_ids;     // lens that need a filter spectrum
+    std::vector<PairRec> pairs;
+    std::vector<NorthRec> north;
+    std::vector<BandItem> items;
+    int64_t filt_total = 0, nsamples = 0;
+    int logPT = 1;
+};
+
+// FFT length table: one entry per distinct ring length
+void build_fft_lens(const HostGeometry& g, HostTables& t, Stats& st)
+{
+    std::map<int, int> id_of;
+    t.rings.resize(g.R);
+    for (int i = 0; i < g.R; ++i) {
+        const int N = g.n[i], L = N / 2;
+        auto it = id_of.find(N);
+        if (it == id_of.end()) {
+            FftLen f{};
+            f.L = L;
+            f.pow2 = is_pow2(L) ? 1 : 0;
+            f.logP = f.pow2 ? ilog2(L) : ilog2(2 * L - 1);
+            f.filt_off = 0;
+            if (!f.pow2) {
+                f.filt_off = t.filt_total;
+                t.filt_total += (int64_t)1 << f.logP;
+                t.bluestein_ids.push_back((int)t.lens.size());
+            }
+            t.logPT = std::max(t.logPT, f.logP);
+            it = id_of.emplace(N, (int)t.lens.size()).first;
+            t.lens.push_back(f);
+        }
+        RingRec r{};
+        r.pix_off = g.pix_off[i];
+        r.spec_off = g.spec_off[i];
+        r.n = N;
+        r.shifted = g.shifted[i];
+        r.len_id = it->second;
+        t.rings[i] = r;
+        const FftLen& f = t.lens[r.len_id];
+        const double P = (double)(1 << f.logP);
+        // forward + inverse: complex FFT(s) + O(N) split / chirps
+        st.fft_flops += 2.0 * (f.pow2 ? 5.0 * P * f.logP + 20.0 * L : 2.0 * 5.0 * P * f.logP + 6.0 * P + 32.0 * L);
+    }
+}
+
+// Ring-pair table for the northern output rings (the southern ones reuse the rows of their mirror images).
+void build_pairs(HostGeometry& g, double theta_max, double ell_nyq, int fixed_mprime, int band_threads, HostTables& t,
+                 Stats& st)
+{
+    const int R = g.R, nnorth = (R + 1) / 2;
+    const double shm = sin(0.5 * theta_max), xmax = 4.0 * shm * shm;
+    g.mprime.assign(R, 0);
+    for (int i = 0; i < R; ++i) {
+        double smax = 0.0;
+        for (int j = g.band_lo[i]; j <= g.band_hi[i]; ++j) smax = std::max(smax, sin(g.theta[j]));
+        g.mprime[i] = fixed_mprime > 0 ? fixed_mprime : std::max(8, 2 * (int)ceil(ell_nyq * smax));
+    }
+    t.north.resize(nnorth);
+    for (int i = 0; i < nnorth; ++i) {
+        t.north[i].pair_lo = (int)t.pairs.size();
+        const bool has_mirror = (R - 1 - i) != i;
+        for (int j = g.band_lo[i]; j <= g.band_hi[i]; ++j) {
+            PairRec p{};
+            const double sd = sin(0.5 * (g.theta[i] - g.theta[j]));
+            p.A = 4.0 * sd * sd;
+            p.B = 4.0 * sin(g.theta[i]) * sin(g.theta[j]);
+            if (g.n[i] == g.n[j]) {          // class E: common grid, ring offset inside the kernel evaluation
+                p.M = g.n[i];
+                p.par = g.shifted[i] != g.shifted[j] ? 1 : 0;
+            } else {                         // class C: a cap ring is involved, Eq. 8 on both rings
+                p.M = g.mprime[i];
+                p.par = 0;
+            }
+            p.scale = g.omega[j] / (double)p.M;
+            int umax = p.M;
+            if (p.B > 0.0) {
+                const double ratio = (xmax - p.A) / p.B;
+                if (ratio < 1.0) {
+                    const double psimax = 2.0 * asin(sqrt(std::max(ratio, 0.0)));
+                    umax = std::min((double)p.M, floor(psimax * p.M / kPi) + 2.0);
+                }
+            }
+            p.cnt = umax >= p.par ? (umax - p.par) / 2 + 1 : 0;
+            p.j = j;
+            p.woff = t.nsamples;
+            t.nsamples += p.cnt;
+            t.pairs.push_back(p);
+            const double modes = p.M / 2 + 1;
+            st.mac_flops += modes * (2.0 * p.cnt + (has_mirror ? 8.0 : 4.0));
+            st.ring_pairs += has_mirror ? 2 : 1;
+        }
+        t.north[i].pair_hi = (int)t.pairs.size();
+        for (int m0 = 0; m0 <= g.n[i] / 2; m0 += band_threads) t.items.push_back(BandItem{i, m0});
+    }
+    st.row_samples = t.nsamples;
+}
+
+template <class V> int upload(V** dst, const std::vector<V>& src, int64_t* bytes)
+{
+    const size_t nb = std::max<size_t>(src.size(), 1) * sizeof(V);
+    CUDA_TRY(cudaMalloc((void**)dst, nb));
+    if (!src.empty()) CUDA_TRY(cudaMemcpy(*dst, src.data(), src.size() * sizeof(V), cudaMemcpyHostToDevice));
+    *bytes += (int64_t)nb;
+    return 0;
+}
+
+// twiddles exp(-2 pi i k / PT) from double precision, Bluestein filters by a plan-time kernel, workspace
+template <class T> int build_device_numeric(arkcos_plan* pl, const HostTables& t)
+{
+    const int PT = 1 << t.logPT;
+    std::vector<cx<T>> tw(std::max(PT / 2, 1));
+    for (int k = 0; k < PT / 2; ++k) tw[k] = mk<T>((T)cos(2.0 * kPi * k / PT), (T)(-sin(2.0 * kPi * k / PT)));
+    cx<T>* d_tw = nullptr;
+    if (int rc = upload(&d_tw, tw, &pl->stats.workspace_bytes)) return rc;
+    pl->d_tw = d_tw;
+    pl->fft_smem = (size_t)PT * sizeof(cx<T>);
+    if (pl->fft_smem > 227 * 1024) return fail(ARKCOS_UNSUPPORTED, "ring too long for the shared-memory FFT");
+    CUDA_TRY(cudaFuncSetAttribute(ring_fft_forward_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl->fft_smem));
+    CUDA_TRY(cudaFuncSetAttribute(ring_fft_inverse_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl->fft_smem));
+    CUDA_TRY(cudaFuncSetAttribute(bluestein_filter_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl->fft_smem));
+
+    const size_t fb = (size_t)std::max<int64_t>(t.filt_total, 1) * sizeof(cx<T>);
+    CUDA_TRY(cudaMalloc(&pl->d_filt, fb));
+    pl->stats.workspace_bytes += (int64_t)fb;
+    if (!t.bluestein_ids.empty()) {
+        int* d_which = nullptr;
+        int64_t dummy = 0;
+        if (int rc = upload(&d_which, t.bluestein_ids, &dummy)) return rc;
+        bluestein_filter_kernel<T><<<(unsigned)t.bluestein_ids.size(), pl->fft_threads, pl->fft_smem>>>(
+            pl->d_lens, d_which, d_tw, pl->logPT, (cx<T>*)pl->d_filt);
+        cudaError_t e = cudaDeviceSynchronize();
+        cudaFree(d_which);
+        CUDA_TRY(e);
+    }
+    const size_t wb = (size_t)std::max<int64_t>(t.nsamples, 1) * sizeof(T);
+    CUDA_TRY(cudaMalloc(&pl->d_W, wb));
+    const size_t sb = (size_t)pl->max_nmaps * (size_t)pl->g.spec_total * sizeof(cx<T>);
+    CUDA_TRY(cudaMalloc(&pl->d_specIn, sb));
+    CUDA_TRY(cudaMalloc(&pl->d_specOut, sb));
+    pl->stats.workspace_bytes += (int64_t)(wb + 2 * sb);
+    return 0;
+}
+}  // namespace
+
+namespace {
+
+template <class T> int enqueue_rows(const arkcos_plan* pl, cudaStream_t st)
+{
+    if (pl->npairs > 0)
+        kernel_rows_kernel<T><<<pl->npairs, 32, 0, st>>>(pl->d_pairs, pl->npairs, pl->d_table, pl->ntab, pl->theta_max,
+                                                         (T*)pl->d_W);
+    return 0;
+}
+
+template <class T> int enqueue_convolve(const arkcos_plan* pl, const void* d_in, void* d_out, int nmaps, cudaStream_t st)
+{
+    const HostGeometry& g = pl->g;
+    const bool tm = pl->timing != 0;
+    if (tm) cudaEventRecord(pl->ev[0], st);
+    if (!pl->opt.cache_kernel_rows) enqueue_rows<T>(pl, st);
+    if (tm) cudaEventRecord(pl->ev[1], st);
+    const dim3 gfft((unsigned)g.R, (unsigned)nmaps);
+    ring_fft_forward_kernel<T><<<gfft, pl->fft_threads, pl->fft_smem, st>>>(
+        (const T*)d_in, g.npix, (cx<T>*)pl->d_specIn, g.spec_total, pl->d_rings, pl->d_lens, (const cx<T>*)pl->d_tw,
+        pl->logPT, (const cx<T>*)pl->d_filt);
+    if (tm) cudaEventRecord(pl->ev[2], st);
+    band_mac_general_kernel<T, 16><<<dim3((unsigned)pl->nitems, (unsigned)nmaps), pl->band_threads, 0, st>>>(
+        pl->d_items, pl->d_north, pl->d_pairs, (const T*)pl->d_W, pl->d_rings, g.R, (const cx<T>*)pl->d_specIn,
+        (cx<T>*)pl->d_specOut, g.spec_total);
+    if (tm) cudaEventRecord(pl->ev[3], st);
+    ring_fft_inverse_kernel<T><<<gfft, pl->fft_threads, pl->fft_smem, st>>>(
+        (const cx<T>*)pl->d_specOut, g.spec_total, (T*)d_out, g.npix, pl->d_rings, pl->d_lens, (const cx<T>*)pl->d_tw,
+        pl->logPT, (const cx<T>*)pl->d_filt);
+    if (tm) cudaEventRecord(pl->ev[4], st);
+    CUDA_TRY(cudaGetLastError());
+    return 0;
+}
+
+__global__ void fma_chain_kernel(float* out, int iters, float a, float b)
+{
+    float x0 = threadIdx.x, x1 = x0 + 1, x2 = x0 + 2, x3 = x0 + 3, x4 = x0 + 4, x5 = x0 + 5, x6 = x0 + 6, x7 = x0 + 7;
+    for (int i = 0; i < iters; ++i) {
+        x0 = fmaf(x0, a, b); x1 = fmaf(x1, a, b); x2 = fmaf(x2, a, b); x3 = fmaf(x3, a, b);
+        x4 = fmaf(x4, a, b); x5 = fmaf(x5, a, b); x6 = fmaf(x6, a, b); x7 = fmaf(x7, a, b);
+    }
+    out[blockIdx.x * blockDim.x + threadIdx.x] = x0 + x1 + x2 + x3 + x4 + x5 + x6 + x7;
+}
+
+size_t elem_size(arkcos_dtype d) { return d == ARKCOS_F64 ? 8 : 4; }
+
+}  // namespace
+
+extern "C" {
+
+static int plan_create_impl(arkcos_plan** out, const arkcos_pixelization* pix, const arkcos_kernel* kernel, arkcos_dtype dtype,
+                            const arkcos_options* options, bool tables_only)
+{
+    if (!out || !pix || !kernel || !kernel->table) return fail(ARKCOS_INVALID_ARG, "NULL argument");
+    if (dtype != ARKCOS_F32 && dtype != ARKCOS_F64) return fail(ARKCOS_INVALID_ARG, "bad dtype");
+    if (kernel->n < 2 || !(kernel->theta_max > 0.0) || !(kernel->theta_max <= kPi + 1e-12))
+        return fail(ARKCOS_INVALID_ARG, "kernel: need n >= 2 and 0 < theta_max <= pi");
+    arkcos_options opt{};
+    if (options) opt = *options;
+    for (int r : opt.reserved) if (r != 0) return fail(ARKCOS_INVALID_ARG, "options.reserved must be zero");
+    if (opt.variant != 0 && opt.variant != 1) return fail(ARKCOS_INVALID_ARG, "options.variant must be 0 or 1");
+    if (opt.variant == 1) return fail(ARKCOS_UNSUPPORTED, "variant 1 (zero-pad / truncate) is not implemented");
+    if (opt.max_nmaps < 0 || opt.polar_oversample < 0 || opt.ell_nyquist < 0.0 || opt.max_nmaps > 65535)
+        return fail(ARKCOS_INVALID_ARG, "negative option");
+    const int maxlen = dtype == ARKCOS_F32 ? 16384 : 8192;
+    if (pix->kind == ARKCOS_ECP) {
+        if (pix->ntheta < 1 || pix->ntheta > (1 << 20) || !is_pow2(pix->nphi) || pix->nphi < 4 || pix->nphi > maxlen)
+            return fail(ARKCOS_INVALID_ARG, "ECP: need ntheta >= 1 and nphi a power of two in [4, 16384 (f32) / 8192 (f64)]");
+    } else if (pix->kind == ARKCOS_HEALPIX_RING) {
+        if (!is_pow2(pix->nside) || 4 * pix->nside > maxlen)
+            return fail(ARKCOS_INVALID_ARG, "HEALPix: nside must be a power of two <= 4096 (f32) / 2048 (f64)");
+    } else return fail(ARKCOS_INVALID_ARG, "bad pixelization kind");
+
+    arkcos_plan* pl = new (std::nothrow) arkcos_plan();
+    if (!pl) return fail(ARKCOS_OUT_OF_MEMORY, "host allocation");
+    struct Guard { arkcos_plan* p; ~Guard() { if (p) arkcos_plan_destroy(p); } } guard{pl};
+    pl->dtype = dtype;
+    pl->pix = *pix;
+    pl->opt = opt;
+    pl->theta_max = kernel->theta_max;
+    pl->ntab = kernel->n;
+    pl->max_nmaps = opt.max_nmaps > 0 ? opt.max_nmaps : 1;
+    pl->tables_only = tables_only;
+    if (!tables_only) CUDA_TRY(cudaGetDevice(&pl->device));
+
+    build_geometry(*pix, pl->g);
+    build_bands(pl->g, pl->theta_max);
+    int fixed_mprime = 0;
+    if (pix->kind == ARKCOS_HEALPIX_RING) {
+        if (opt.polar_oversample > 0) fixed_mprime = opt.polar_oversample * 4 * pix->nside;
+        else pl->ell_nyquist = opt.ell_nyquist > 0.0 ? opt.ell_nyquist
+                                                     : auto_ell_nyquist(kernel->table, kernel->n, kernel->theta_max, 8.0 * pix->nside);
+    }
+    HostTables t;
+    build_fft_lens(pl->g, t, pl->stats);
+    build_pairs(pl->g, pl->theta_max, pl->ell_nyquist, fixed_mprime, pl->band_threads, t, pl->stats);
+    if (t.pairs.size() > (size_t)INT32_MAX || t.items.size() > (size_t)INT32_MAX) return fail(ARKCOS_UNSUPPORTED, "too many ring pairs");
+    pl->nnorth = (int)t.north.size();
+    pl->npairs = (int)t.pairs.size();
+    pl->nitems = (int)t.items.size();
+    pl->nsamples = t.nsamples;
+    pl->logPT = t.logPT;
+
+    if (tables_only) {
+        guard.p = nullptr;
+        *out = pl;
+        return ARKCOS_OK;
+    }
+    int64_t* wsb = &pl->stats.workspace_bytes;
+    if (int rc = upload(&pl->d_rings, t.rings, wsb)) return rc;
+    if (int rc = upload(&pl->d_lens, t.lens, wsb)) return rc;
+    if (int rc = upload(&pl->d_pairs, t.pairs, wsb)) return rc;
+    if (int rc = upload(&pl->d_north, t.north, wsb)) return rc;
+    if (int rc = upload(&pl->d_items, t.items, wsb)) return rc;
+    std::vector<double> tab(kernel->table, kernel->table + kernel->n);
+    if (int rc = upload(&pl->d_table, tab, wsb)) return rc;
+    if (int rc = dtype == ARKCOS_F32 ? build_device_numeric<float>(pl, t) : build_device_numeric<double>(pl, t)) return rc;
+    for (auto& e : pl->ev) CUDA_TRY(cudaEventCreate(&e));
+    if (opt.cache_kernel_rows) {
+        dtype == ARKCOS_F32 ? enqueue_rows<float>(pl, 0) : enqueue_rows<double>(pl, 0);
+        CUDA_TRY(cudaDeviceSynchronize());
+    }
+    CUDA_TRY(cudaGetLastError());
+    guard.p = nullptr;
+    *out = pl;
+    g_last_error.clear();
+    return ARKCOS_OK;
+}
+
+int arkcos_plan_create(arkcos_plan** out, const arkcos_pixelization* pix, const arkcos_kernel* kernel, arkcos_dtype dtype,
+                       const arkcos_options* options)
+{
+    return plan_create_impl(out, pix, kernel, dtype, options, false);
+}
+
+int arkcos_plan_create_tables_only(arkcos_plan** out, const arkcos_pixelization* pix, const arkcos_kernel* kernel,
+                                   arkcos_dtype dtype, const arkcos_options* options)
+{
+    return plan_create_impl(out, pix, kernel, dtype, options, true);
+}
+
+int arkcos_convolve(const arkcos_plan* pl, const void* d_in, void* d_out, int nmaps, void* cuda_stream)
+{
+    if (!pl || !d_in || !d_out) return fail(ARKCOS_INVALID_ARG, "NULL argument");
+    if (pl->tables_only) return fail(ARKCOS_INVALID_ARG, "plan was created with arkcos_plan_create_tables_only");
+    if (nmaps < 1 || nmaps > pl->max_nmaps) return fail(ARKCOS_INVALID_ARG, "nmaps must be in [1, max_nmaps]");
+    const size_t bytes = (size_t)nmaps * (size_t)pl->g.npix * elem_size(pl->dtype);
+    const char *a = (const char*)d_in, *b = (const char*)d_out;
+    if (a < b + bytes && b < a + bytes) return fail(ARKCOS_INVALID_ARG, "d_in and d_out overlap");
+    if (((uintptr_t)d_in | (uintptr_t)d_out) & 15) return fail(ARKCOS_INVALID_ARG, "d_in / d_out must be 16-byte aligned");
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    return pl->dtype == ARKCOS_F32 ? enqueue_convolve<float>(pl, d_in, d_out, nmaps, st)
+                                   : enqueue_convolve<double>(pl, d_in, d_out, nmaps, st);
+}
+
+int arkcos_convolve_host(const arkcos_plan* pl, const void* h_in, void* h_out, int nmaps, void* cuda_stream)
+{
+    if (!pl || !h_in || !h_out) return fail(ARKCOS_INVALID_ARG, "NULL argument");
+    if (pl->tables_only) return fail(ARKCOS_INVALID_ARG, "plan was created with arkcos_plan_create_tables_only");
+    if (nmaps < 1 || nmaps > pl->max_nmaps) return fail(ARKCOS_INVALID_ARG, "nmaps must be in [1, max_nmaps]");
+    const size_t full = (size_t)pl->max_nmaps * (size_t)pl->g.npix * elem_size(pl->dtype);
+    const size_t bytes = (size_t)nmaps * (size_t)pl->g.npix * elem_size(pl->dtype);
+    if (!pl->d_stage_in) CUDA_TRY(cudaMalloc(&pl->d_stage_in, full));
+    if (!pl->d_stage_out) CUDA_TRY(cudaMalloc(&pl->d_stage_out, full));
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    CUDA_TRY(cudaMemcpyAsync(pl->d_stage_in, h_in, bytes, cudaMemcpyHostToDevice, st));
+    if (int rc = arkcos_convolve(pl, pl->d_stage_in, pl->d_stage_out, nmaps, cuda_stream)) return rc;
+    CUDA_TRY(cudaMemcpyAsync(h_out, pl->d_stage_out, bytes, cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaStreamSynchronize(st));
+    return ARKCOS_OK;
+}
+
+int arkcos_plan_destroy(arkcos_plan* pl)
+{
+    if (!pl) return ARKCOS_OK;
+    void* ptrs[] = {pl->d_rings, pl->d_lens, pl->d_pairs, pl->d_north, pl->d_items, pl->d_table, pl->d_tw, pl->d_filt,
+                    pl->d_W, pl->d_specIn, pl->d_specOut, pl->d_stage_in, pl->d_stage_out};
+    for (void* p : ptrs) if (p) cudaFree(p);
+    for (auto& e : pl->ev) if (e) cudaEventDestroy(e);
+    delete pl;
+    return ARKCOS_OK;
+}
+
+int64_t arkcos_plan_npix(const arkcos_plan* pl) { return pl ? pl->g.npix : -1; }
+int arkcos_plan_nrings(const arkcos_plan* pl) { return pl ? pl->g.R : -1; }
+double arkcos_plan_ell_nyquist(const arkcos_plan* pl) { return pl ? pl->ell_nyquist : -1.0; }
+
+int arkcos_plan_ring_info(const arkcos_plan* pl, int ring, double* theta, int* n, double* phi0, int64_t* offset,
+                          int* band_lo, int* band_hi, int* mprime)
+{
+    if (!pl || ring < 0 || ring >= pl->g.R) return fail(ARKCOS_INVALID_ARG, "bad ring");
+    const HostGeometry& g = pl->g;
+    if (theta) *theta = g.theta[ring];
+    if (n) *n = g.n[ring];
+    if (phi0) *phi0 = g.phi0[ring];
+    if (offset) *offset = g.pix_off[ring];
+    if (band_lo) *band_lo = g.band_lo[ring];
+    if (band_hi) *band_hi = g.band_hi[ring];
+    if (mprime) *mprime = g.mprime[ring];
+    return ARKCOS_OK;
+}
+
+int arkcos_plan_stats(const arkcos_plan* pl, int64_t* ring_pairs, int64_t* row_samples, double* mac_flops, double* fft_flops,
+                      int64_t* workspace_bytes)
+{
+    if (!pl) return fail(ARKCOS_INVALID_ARG, "NULL plan");
+    if (ring_pairs) *ring_pairs = pl->stats.ring_pairs;
+    if (row_samples) *row_samples = pl->stats.row_samples;
+    if (mac_flops) *mac_flops = pl->stats.mac_flops;
+    if (fft_flops) *fft_flops = pl->stats.fft_flops;
+    if (workspace_bytes) *workspace_bytes = pl->stats.workspace_bytes;
+    return ARKCOS_OK;
+}
+
+int arkcos_plan_set_timing(const arkcos_plan* pl, int enable)
+{
+    if (!pl) return fail(ARKCOS_INVALID_ARG, "NULL plan");
+    pl->timing = enable ? 1 : 0;
+    return ARKCOS_OK;
+}
+
+int arkcos_plan_get_timing(const arkcos_plan* pl, float* ms4)
+{
+    if (!pl || !ms4) return fail(ARKCOS_INVALID_ARG, "NULL argument");
+    if (!pl->timing) return fail(ARKCOS_INVALID_ARG, "timing is not enabled");
+    CUDA_TRY(cudaEventSynchronize(pl->ev[4]));
+    for (int k = 0; k < 4; ++k) CUDA_TRY(cudaEventElapsedTime(&ms4[k], pl->ev[k], pl->ev[k + 1]));
+    return ARKCOS_OK;
+}
+
+int arkcos_probe_fp32_peak(double* tflops, int repeats)
+{
+    if (!tflops || repeats < 1) return fail(ARKCOS_INVALID_ARG, "bad argument");
+    int dev = 0, sms = 0;
+    CUDA_TRY(cudaGetDevice(&dev));
+    CUDA_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    const int blocks = sms * 8, threads = 256, iters = 1 << 15;
+    float* d = nullptr;
+    CUDA_TRY(cudaMalloc(&d, (size_t)blocks * threads * sizeof(float)));
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0);
+    cudaEventCreate(&e1);
+    double best = 0.0;
+    for (int r = 0; r < repeats + 1; ++r) {
+        cudaEventRecord(e0);
+        fma_chain_kernel<<<blocks, threads>>>(d, iters, 1.0000001f, 1e-9f);
+        cudaEventRecord(e1);
+        cudaEventSynchronize(e1);
+        float ms = 0;
+        cudaEventElapsedTime(&ms, e0, e1);
+        if (r > 0 && ms > 0) best = std::max(best, 2.0 * 8.0 * iters * (double)blocks * threads / (ms * 1e-3) / 1e12);
+    }
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    cudaFree(d);
+    CUDA_TRY(cudaGetLastError());
+    *tflops = best;
+    return ARKCOS_OK;
+}
+
+const char* arkcos_strerror(int status)
+{
+    switch (status) {
+        case ARKCOS_OK: return "success";
+        case ARKCOS_INVALID_ARG: return "invalid argument";
+        case ARKCOS_UNSUPPORTED: return "unsupported request";
+        case ARKCOS_CUDA_ERROR: return "CUDA error";
+        case ARKCOS_OUT_OF_MEMORY: return "out of memory";
+        default: return "unknown status";
+    }
+}
+
+const char* arkcos_last_error(void) { return g_last_error.c_str(); }
+
+}  // extern "C"

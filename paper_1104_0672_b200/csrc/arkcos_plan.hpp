@@ -1,0 +1,62 @@
+// Host-side plan of libarkcos: ring geometry, band / ring-pair tables, FFT length table (step 0 of the hot path,
+// PAPER.md:123-125, 162 "we stored the longitudes of all rings ... in constant memory").
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <string>
+#include <vector>
+
+#include "../../include/arkcos.h"
+#include "arkcos_band.cuh"
+#include "arkcos_fft.cuh"
+
+namespace arkcos {
+
+struct HostGeometry {
+    int R = 0;
+    int64_t npix = 0, spec_total = 0;
+    std::vector<double> theta, phi0, omega;
+    std::vector<int> n, shifted, band_lo, band_hi, mprime;
+    std::vector<int64_t> pix_off, spec_off;
+};
+
+struct Stats {
+    int64_t ring_pairs = 0, row_samples = 0, workspace_bytes = 0;
+    double mac_flops = 0, fft_flops = 0;
+};
+
+}  // namespace arkcos
+
+struct arkcos_plan {
+    arkcos_dtype dtype = ARKCOS_F32;
+    arkcos_pixelization pix{};
+    arkcos_options opt{};
+    double theta_max = 0, ell_nyquist = 0;
+    int ntab = 0, max_nmaps = 1, device = 0;
+    bool tables_only = false;
+    arkcos::HostGeometry g;
+    arkcos::Stats stats;
+
+    int nnorth = 0, npairs = 0, nitems = 0, logPT = 0, band_threads = 128, fft_threads = 256;
+    size_t fft_smem = 0;
+    int64_t nsamples = 0;
+
+    // device tables
+    arkcos::RingRec* d_rings = nullptr;
+    arkcos::FftLen* d_lens = nullptr;
+    arkcos::PairRec* d_pairs = nullptr;
+    arkcos::NorthRec* d_north = nullptr;
+    arkcos::BandItem* d_items = nullptr;
+    double* d_table = nullptr;
+    void* d_tw = nullptr;        // cx<T>[PT/2]
+    void* d_filt = nullptr;      // cx<T>[...] Bluestein filter spectra
+    void* d_W = nullptr;         // T[nsamples] kernel rows
+    void* d_specIn = nullptr;    // cx<T>[max_nmaps][spec_total]
+    void* d_specOut = nullptr;
+    // lazily allocated staging for arkcos_convolve_host
+    mutable void* d_stage_in = nullptr;
+    mutable void* d_stage_out = nullptr;
+    // optional per-stage timing
+    mutable int timing = 0;
+    mutable cudaEvent_t ev[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
+};

@@ -1,0 +1,240 @@
+"""Parity of the CUDA path (through the C ABI) against the CPU oracle, element by element, on seeded inputs.
+
+Tolerances (BASELINE.json north_star):
+  fp64 path          max |gpu - oracle| <= 1e-12 max |oracle|
+  fp32 path, ECP     fractional RMS <= 1e-6 vs the fp64 brute-force sum
+  fp32 path, HEALPix fractional RMS <= 1e-5 vs the brute-force sum; <= 1e-6 vs the fp64 hybrid oracle with the same M'
+"""
+import numpy as np
+import pytest
+
+from oracle import geometry, direct, hybrid
+from paper_1104_0672_b200 import arkcos, inputs
+
+pytestmark = pytest.mark.gpu
+torch = pytest.importorskip("torch")
+
+DEG, ARCMIN = inputs.DEG, inputs.ARCMIN
+
+
+def frms(a, b):
+    a, b = np.asarray(a, float), np.asarray(b, float)
+    return float(np.sqrt(((a - b) ** 2).sum() / (b ** 2).sum()))
+
+
+def maxrel(a, b):
+    return float(np.abs(np.asarray(a, float) - b).max() / np.abs(b).max())
+
+
+def geom_of(pix):
+    return geometry.ecp(pix[1], pix[2]) if pix[0] == "ecp" else geometry.healpix_ring(pix[1])
+
+
+def gpu_convolve(pix, table, tmax, x, dtype=arkcos.F32, plan=None, **opts):
+    """x: numpy [npix] or [nmaps, npix]; returns numpy of the same shape (and the plan)."""
+    tdt = torch.float32 if dtype == arkcos.F32 else torch.float64
+    nmaps = 1 if x.ndim == 1 else x.shape[0]
+    if plan is None:
+        plan = arkcos.Plan(pix, table, tmax, dtype, max_nmaps=nmaps, **opts)
+    d_in = torch.from_numpy(np.ascontiguousarray(x)).to(device="cuda", dtype=tdt)
+    d_out = torch.full_like(d_in, float("nan"))
+    plan.convolve(d_in.data_ptr(), d_out.data_ptr(), nmaps, torch.cuda.current_stream().cuda_stream)
+    torch.cuda.synchronize()
+    return d_out.cpu().numpy(), plan
+
+
+def take_rings(geom, full, rings):
+    return np.concatenate([full[..., geom.ring_slice(int(r))] for r in rings], axis=-1)
+
+
+def sample_rings(geom, extra=(), nrand=8, seed=0):
+    R = geom.nrings
+    base = {0, 1, 2, R // 4, R // 2 - 1, R // 2, R // 2 + 1, (3 * R) // 4, R - 3, R - 2, R - 1}
+    rng = np.random.default_rng(seed)
+    base |= set(int(v) for v in rng.integers(0, R, nrand)) | set(int(e) for e in extra)
+    return np.array(sorted(r for r in base if 0 <= r < R))
+
+
+# ------------------------------------------------------------------ config 1: ECP 64 x 128 -------------------------
+
+def test_cfg1_fp64_and_fp32():
+    c = inputs.config(1)
+    geom, tab, tmax = geom_of(c["pix"]), inputs.kernel_table(c), c["theta_max"]
+    x = inputs.white_noise(geom.npix, 1, dtype=np.float64)
+    ref = direct.direct_sum(geom, tab, tmax, x)
+    out64, _ = gpu_convolve(c["pix"], tab, tmax, x, arkcos.F64)
+    assert maxrel(out64, ref) <= 1e-12
+    x32 = x.astype(np.float32)
+    ref32 = direct.direct_sum(geom, tab, tmax, x32.astype(np.float64))
+    out32, _ = gpu_convolve(c["pix"], tab, tmax, x32, arkcos.F32)
+    assert frms(out32, ref32) <= 1e-6
+    # and against the scheme oracle
+    assert maxrel(out64, hybrid.hybrid_convolve(geom, tab, tmax, x)) <= 1e-12
+
+
+# ------------------------------------------------------------------ config 2: ECP 1024 x 2048 ----------------------
+
+def test_cfg2_fp32_sampled_rings():
+    c = inputs.config(2)
+    geom, tab, tmax = geom_of(c["pix"]), inputs.kernel_table(c), c["theta_max"]
+    x = inputs.white_noise(geom.npix, 2)
+    out, _ = gpu_convolve(c["pix"], tab, tmax, x)
+    assert np.isfinite(out).all()
+    rings = sample_rings(geom, nrand=6, seed=2)
+    ref = direct.direct_sum(geom, tab, tmax, x.astype(np.float64), out_rings=rings)
+    assert frms(take_rings(geom, out, rings), ref) <= 1e-6
+
+
+# ------------------------------------------------------------------ small HEALPix, whole map -----------------------
+
+@pytest.mark.parametrize("nside,dtype", [(1, arkcos.F64), (2, arkcos.F64), (16, arkcos.F64), (16, arkcos.F32),
+                                         (32, arkcos.F32)])
+def test_healpix_small_full_map(nside, dtype):
+    geom = geometry.healpix_ring(nside)
+    pixsz = np.sqrt(4 * np.pi / geom.npix)
+    fwhm = 2.5 * pixsz
+    sigma, tmax = fwhm * inputs.FWHM_TO_SIGMA, min(3 * fwhm, np.pi)
+    tab = inputs.gaussian_table(fwhm, tmax)
+    ell = 5.5 / sigma
+    x = inputs.white_noise(geom.npix, 9, dtype=np.float64 if dtype == arkcos.F64 else np.float32)
+    out, plan = gpu_convolve(("healpix", nside), tab, tmax, x, dtype, ell_nyquist=ell)
+    mp = hybrid.mprime_rule(geom, tmax, ell)
+    assert [plan.ring_info(i)["mprime"] for i in range(geom.nrings)] == list(mp)
+    ref2 = hybrid.hybrid_convolve(geom, tab, tmax, x.astype(np.float64), mprime=mp)
+    ref1 = direct.direct_sum(geom, tab, tmax, x.astype(np.float64))
+    if dtype == arkcos.F64:
+        assert maxrel(out, ref2) <= 1e-12
+    else:
+        assert frms(out, ref2) <= 1e-6
+    if nside >= 16:
+        assert frms(out, ref1) <= 1e-5
+
+
+def test_healpix_paper_grid_polar_oversample():
+    """polar_oversample = 1 is the paper's M = 4 nside: parity with oracle #2 at the same M."""
+    nside = 16
+    geom = geometry.healpix_ring(nside)
+    fwhm = 3 * np.sqrt(4 * np.pi / geom.npix)
+    tmax = 3 * fwhm
+    tab = inputs.gaussian_table(fwhm, tmax)
+    x = inputs.white_noise(geom.npix, 9, dtype=np.float64)
+    out, _ = gpu_convolve(("healpix", nside), tab, tmax, x, arkcos.F64, polar_oversample=1)
+    assert maxrel(out, hybrid.hybrid_convolve(geom, tab, tmax, x, mprime=4 * nside)) <= 1e-12
+
+
+def test_hard_edged_kernels_vs_scheme_oracle():
+    """Top-hat and Mexican hat (config 5's kernels) at nside 32, 3 maps: GPU == oracle #2; equatorial rings == oracle #1."""
+    nside = 32
+    geom = geometry.healpix_ring(nside)
+    pixsz = np.sqrt(4 * np.pi / geom.npix)
+    x = inputs.white_noise_maps(geom.npix, 5, 3)
+    for tab, tmax in [(inputs.tophat_table(5.8 * pixsz), 5.8 * pixsz),
+                      (inputs.mexican_hat_table(2.33 * pixsz, 5 * 2.33 * pixsz), 5 * 2.33 * pixsz)]:
+        ell = 6.0 * nside
+        out, _ = gpu_convolve(("healpix", nside), tab, tmax, x, arkcos.F32, ell_nyquist=ell)
+        mp = hybrid.mprime_rule(geom, tmax, ell)
+        ref2 = hybrid.hybrid_convolve(geom, tab, tmax, x.astype(np.float64), mprime=mp)
+        assert frms(out, ref2) <= 1e-6
+        eq = np.array([i for i in range(geom.nrings) if np.all(geom.n[geometry.band(geom, i, tmax)] == 4 * nside)])
+        ref1 = direct.direct_sum(geom, tab, tmax, x.astype(np.float64), out_rings=eq)
+        assert frms(take_rings(geom, out, eq), ref1) <= 1e-6
+
+
+# ------------------------------------------------------------------ config 3: HEALPix nside 512 --------------------
+
+def test_cfg3_fp32_sampled_rings():
+    c = inputs.config(3)
+    nside = c["pix"][1]
+    geom, tab, tmax = geom_of(c["pix"]), inputs.kernel_table(c), c["theta_max"]
+    x = inputs.white_noise(geom.npix, 3)
+    out, plan = gpu_convolve(c["pix"], tab, tmax, x)
+    assert np.isfinite(out).all()
+    rings = sample_rings(geom, extra=(nside - 2, nside - 1, nside, nside + 5, 2 * nside - 1, 330, 126), seed=3)
+    ref = direct.direct_sum(geom, tab, tmax, x.astype(np.float64), out_rings=rings)
+    assert frms(take_rings(geom, out, rings), ref) <= 1e-5
+    # same M' in the scheme oracle on a few rings
+    mp = np.array([plan.ring_info(i)["mprime"] for i in range(geom.nrings)])
+    assert np.array_equal(mp, hybrid.mprime_rule(geom, tmax, plan.ell_nyquist))
+    few = np.array([0, 5, 126, nside - 1, nside + 3, 2 * nside - 1])
+    ref2 = hybrid.hybrid_convolve(geom, tab, tmax, x.astype(np.float64), mprime=mp, out_rings=few)
+    assert frms(take_rings(geom, out, few), ref2) <= 1e-6
+
+
+# ------------------------------------------------------------------ config 4: HEALPix nside 2048 -------------------
+
+def test_cfg4_full_size_sampled_rings():
+    c = inputs.config(4)
+    nside = c["pix"][1]
+    geom, tab, tmax = geom_of(c["pix"]), inputs.kernel_table(c), c["theta_max"]
+    x = inputs.add_point_sources(inputs.white_noise(geom.npix, 4))
+    out, plan = gpu_convolve(c["pix"], tab, tmax, x)
+    assert np.isfinite(out).all()
+    # rings: poles, prime-length / power-of-two-length cap rings (N = 4 * 509, 4 * 512), cap boundary +- band, equator,
+    # random, and the rings of a few point sources
+    src_rings = np.searchsorted(geom.offset, np.random.default_rng(inputs.BASE_SEED + 499).integers(0, geom.npix, 1000)[:6],
+                                side="right") - 1
+    rings = sample_rings(geom, extra=(508, 511, 1020, nside - 14, nside - 2, nside - 1, nside, nside + 12, 2 * nside - 1,
+                                      3 * nside - 1, 3 * nside + 10, *src_rings), nrand=10, seed=4)
+    ref = direct.direct_sum(geom, tab, tmax, x.astype(np.float64), out_rings=rings)
+    got = take_rings(geom, out, rings)
+    assert frms(got, ref) <= 1e-5
+    # per-ring: no single ring is off (amplitude-100 sources included)
+    o = 0
+    for r in rings:
+        n = int(geom.n[r])
+        assert np.abs(got[o:o + n] - ref[o:o + n]).max() <= 3e-5 * np.abs(ref).max(), int(r)
+        o += n
+
+
+# ------------------------------------------------------------------ API behaviour -----------------------------------
+
+def test_multi_map_equals_single_and_host_path():
+    nside = 16
+    geom = geometry.healpix_ring(nside)
+    fwhm = 3 * np.sqrt(4 * np.pi / geom.npix)
+    tmax = 3 * fwhm
+    tab = inputs.gaussian_table(fwhm, tmax)
+    x = inputs.white_noise_maps(geom.npix, 7, 4)
+    out, plan = gpu_convolve(("healpix", nside), tab, tmax, x)
+    for k in range(4):
+        single, _ = gpu_convolve(("healpix", nside), tab, tmax, x[k], plan=plan)
+        np.testing.assert_array_equal(single, out[k])
+    h_in = torch.from_numpy(x).pin_memory()
+    h_out = torch.empty_like(h_in).pin_memory()
+    plan.convolve_host(h_in.data_ptr(), h_out.data_ptr(), 4, torch.cuda.current_stream().cuda_stream)
+    np.testing.assert_array_equal(h_out.numpy(), out)
+    # cached rows give the same bits
+    out_c, _ = gpu_convolve(("healpix", nside), tab, tmax, x, cache_kernel_rows=1)
+    np.testing.assert_array_equal(out_c, out)
+
+
+def test_argument_errors():
+    tab = inputs.gaussian_table(0.2, 0.4, 256)
+    plan = arkcos.Plan(("ecp", 8, 16), tab, 0.4, arkcos.F32, max_nmaps=2)
+    a = torch.zeros(3, 128, device="cuda")
+    b = torch.zeros(3, 128, device="cuda")
+    s = torch.cuda.current_stream().cuda_stream
+    for args in [(a.data_ptr(), a.data_ptr(), 1), (a.data_ptr(), b.data_ptr(), 3), (a.data_ptr(), b.data_ptr(), 0),
+                 (0, b.data_ptr(), 1), (a.data_ptr(), a.data_ptr() + 256, 1)]:
+        with pytest.raises(arkcos.ArkcosError) as e:
+            plan.convolve(args[0], args[1], args[2], s)
+        assert e.value.status == arkcos.INVALID_ARG
+    plan.convolve(a.data_ptr(), b.data_ptr(), 2, s)
+    torch.cuda.synchronize()
+    assert torch.all(b[:2] == 0)
+
+
+def test_degenerate_kernels():
+    """Support narrower than the ring spacing (only the ring itself contributes) and support = the whole sphere."""
+    geom = geometry.ecp(8, 16)
+    x = inputs.white_noise(geom.npix, 8, dtype=np.float64)
+    for tmax in (0.05, np.pi):
+        tab = inputs.gaussian_table(0.8, tmax, 4096)
+        out, _ = gpu_convolve(("ecp", 8, 16), tab, tmax, x, arkcos.F64)
+        assert maxrel(out, direct.direct_sum(geom, tab, tmax, x)) <= 1e-12
+    geom = geometry.healpix_ring(4)
+    xh = inputs.white_noise(geom.npix, 8, dtype=np.float64)
+    tab = inputs.gaussian_table(0.01, 0.02, 4096)
+    out, _ = gpu_convolve(("healpix", 4), tab, 0.02, xh, arkcos.F64)     # each pixel only sees itself
+    assert maxrel(out, direct.direct_sum(geom, tab, 0.02, xh)) <= 1e-12
+    np.testing.assert_allclose(out, xh * geom.omega[0], rtol=1e-12)
