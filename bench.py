@@ -261,7 +261,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--cfg", type=int, default=4)
-    ap.add_argument("--oracle-rings", type=int, default=96, help="output rings in the CPU-oracle sample")
+    ap.add_argument("--oracle-rings", type=int, default=2048, help="output rings in the CPU-oracle sample")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
