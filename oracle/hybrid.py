@@ -12,11 +12,12 @@ M_ij = length of the phi grid the kernel row is sampled on.
 
 Step 1  B_j[m] = sum_l in(j,l) exp(-2 pi i m l / N_j),  m = 0 .. N_j-1.
 Step 2 for every j in the band of i:
-   class E, N_i == N_j: M_ij = N_i and the row is sampled *with* the offset ("substitute
+   class E, N_i == N_j == N_max (both rings have the full length: every ECP ring, the HEALPix equatorial rings; DESIGN.md
+        reading R11): M_ij = N_i and the row is sampled *with* the offset ("substitute
         cos(phi) with cos(phi - phi0)"): kappa[d] = kappa_ij(delta_ij + 2 pi d / M),
         kt[m] = sum_d kappa[d] exp(-2 pi i m d / M); no phase factor.  This is an exact circulant
         identity (the ECP case of PAPER.md:219 and the HEALPix equatorial region).
-   class C, N_i != N_j (a polar-cap ring is involved): M_ij = M'_i (reading R10), the row is
+   class C, every other pair (a polar-cap ring is involved, including a cap ring paired with itself): M_ij = M'_i (reading R10), the row is
         sampled at delta = 0 and both rings are re-origined by Eq. 8:
         kt[m] <- kt[m] exp(i m delta_ij) for signed |m| < M/2, and the +-M/2 bins carry half the
         Nyquist coefficient each.
@@ -79,11 +80,17 @@ def mprime_rule(geom: RingGeometry, theta_max: float, ell_nyq: float) -> np.ndar
     return out
 
 
+def is_class_e(geom, i, j) -> bool:
+    """Both rings have the full ring length, so their pixels share one phi grid up to the half-pixel offset."""
+    nmax = int(geom.n.max())
+    return int(geom.n[i]) == nmax and int(geom.n[j]) == nmax
+
+
 def pair_spectrum(geom, i, j, table, theta_max, M):
     """(signed mode numbers m, kt[m] incl. Eq. 8 phases) of ring pair (i, j) on an M-point grid."""
     delta = geom.phi0[i] - geom.phi0[j]
     d = np.arange(M)
-    if geom.n[i] == geom.n[j] and M == geom.n[i]:               # class E: offset-aware sampling
+    if is_class_e(geom, i, j) and M == geom.n[i]:                # class E: offset-aware sampling
         kap = kernel_row(geom.theta[i], geom.theta[j], delta + 2.0 * np.pi * d / M, table, theta_max)
         phase_delta = 0.0
     else:                                                         # class C: delta = 0, Eq. 8 on both rings
@@ -135,7 +142,7 @@ def hybrid_convolve(geom: RingGeometry, table, theta_max: float, inp, variant: s
         for j in band(geom, i, theta_max):
             j = int(j)
             Nj = int(geom.n[j])
-            M = Ni if Ni == Nj else int(mprime[i])
+            M = Ni if is_class_e(geom, i, j) else int(mprime[i])
             m, kt = pair_spectrum(geom, i, j, table, theta_max, M)        # step 2
             Bj = ring_spectrum(j)[:, m % Nj]
             if variant == "A":

@@ -21,7 +21,7 @@ struct PairRec {
     int64_t woff;      // first sample of the row in W
     int M;             // length of the phi grid of this row (even)
     int par;           // sample positions psi_t = (2t + par) pi / M ; par = 1: half-step offset
-    int cnt;           // stored samples t = 0 .. cnt-1
+    int cnt;           // evaluated samples t = 0 .. cnt-1; the row is stored zero-padded to a multiple of 4 (woff % 4 == 0)
     int j;             // input ring (northern image)
 };
 
@@ -39,7 +39,9 @@ template <class T> __global__ void kernel_rows_kernel(const PairRec* __restrict_
     const PairRec pr = pairs[p];
     const double inv2M = 1.0 / (2.0 * (double)pr.M);
     const double tscale = (double)(ntab - 1) / theta_max;
-    for (int t = threadIdx.x; t < pr.cnt; t += blockDim.x) {
+    const int cnt4 = (pr.cnt + 3) & ~3;
+    for (int t = threadIdx.x; t < cnt4; t += blockDim.x) {
+        if (t >= pr.cnt) { W[pr.woff + t] = (T)0; continue; }
         const int u = 2 * t + pr.par;
         const double sh = sinpi((double)u * inv2M);                    // sin(psi/2), psi = u pi / M
         const double x = pr.A + pr.B * sh * sh;
@@ -125,6 +127,294 @@ __global__ void band_mac_general_kernel(const BandItem* __restrict__ items, cons
     cx<T>* __restrict__ out = specOut + (int64_t)blockIdx.y * spec_stride;
     out[ri.spec_off + mp] = accN;
     if (iS != i) out[rings[iS].spec_off + mp] = accS;
+}
+
+}  // namespace arkcos
+
+namespace arkcos {
+
+// ---- fast band kernel for "uniform" output rings: every ring pair of the ring is sampled on the same grid length M ----
+// One thread per folded output mode m'.  For each unfolded mode m that folds onto m' the thread builds the cosines
+// cos(m u pi / M) of the row-sample positions ONCE in registers (rotation, re-seeded every 8 steps from an exact
+// sincospi) and reuses them for all input rings of the band; the rows and the per-pair records sit in shared memory.
+constexpr int kBandThreads = 128;
+constexpr int kMaxPairs = 64;
+constexpr int kBandClasses = 5;   // 0: general kernel; 1..4: band_mac_uniform_kernel<12,odd>, <12>, <20>, <32,odd>
+
+struct PairMeta {
+    int64_t offN, offS;   // first coefficient of input ring j (north image) and of its mirror image
+    int Nj;
+    uint32_t magic;       // ceil(2^32 / Nj): m / Nj = umulhi(m, magic) for m < 2^15
+    int cnt;
+    int flags;            // bit 0: par, bit 1: ring j shifted
+};
+
+template <int TMAX, bool HAS_ODD>
+__global__ void __launch_bounds__(kBandThreads)
+band_mac_uniform_kernel(const BandItem* __restrict__ items, const NorthRec* __restrict__ north,
+                        const PairRec* __restrict__ pairs, const float* __restrict__ W,
+                        const RingRec* __restrict__ rings, int R, const cx<float>* __restrict__ specIn,
+                        cx<float>* __restrict__ specOut, int64_t spec_stride)
+{
+    __shared__ __align__(16) float sW[kMaxPairs * TMAX];
+    __shared__ PairMeta sP[kMaxPairs];
+    __shared__ int sTneed;
+    const BandItem it = items[blockIdx.x];
+    const int i = it.ring, iS = R - 1 - i;
+    const RingRec ri = rings[i];
+    const NorthRec nr = north[i];
+    const int np = nr.pair_hi - nr.pair_lo;
+    if (threadIdx.x == 0) sTneed = 0;
+    __syncthreads();
+    for (int p = threadIdx.x; p < np; p += kBandThreads) {
+        const PairRec pr = pairs[nr.pair_lo + p];
+        const RingRec rj = rings[pr.j], rjS = rings[R - 1 - pr.j];
+        PairMeta pm;
+        pm.offN = rj.spec_off;
+        pm.offS = rjS.spec_off;
+        pm.Nj = rj.n;
+        pm.magic = (uint32_t)((0x100000000ull + (uint64_t)rj.n - 1ull) / (uint64_t)rj.n);
+        pm.cnt = pr.cnt;
+        pm.flags = pr.par | (rj.shifted << 1);
+        sP[p] = pm;
+        atomicMax(&sTneed, pr.cnt);
+    }
+    for (int idx = threadIdx.x; idx < np * TMAX; idx += kBandThreads) {
+        const int p = idx / TMAX, t = idx - p * TMAX;
+        const PairRec& pr = pairs[nr.pair_lo + p];
+        sW[idx] = t < pr.cnt ? W[pr.woff + t] : 0.f;
+    }
+    __syncthreads();
+    const int Ni = ri.n, mp = it.m0 + (int)threadIdx.x;
+    if (2 * mp > Ni) return;
+    const int M = pairs[nr.pair_lo].M, Mh = M >> 1, tneed = sTneed;
+    const uint32_t twoM = 2u * (uint32_t)M;
+    const cx<float>* __restrict__ in = specIn + (int64_t)blockIdx.y * spec_stride;
+    cx<float> accN = mk<float>(0, 0), accS = mk<float>(0, 0);
+
+    for (int fam = 0; fam < 2; ++fam) {
+        int wi = fam;
+        for (int m = fam ? Ni - mp : mp; m <= Mh; m += Ni, ++wi) {
+            float ce[TMAX], co[HAS_ODD ? TMAX : 1];
+            {
+                const cx<float> rot = cispi_ratio<float>((2u * (uint32_t)m) % twoM, (uint32_t)M);
+                cx<float> c = mk<float>(1.f, 0.f), d = mk<float>(1.f, 0.f);
+#pragma unroll
+                for (int t = 0; t < TMAX; ++t) {
+                    if (t < tneed) {
+                        if ((t & 7) == 0) {
+                            c = cispi_ratio<float>((2u * (uint32_t)m * (uint32_t)t) % twoM, (uint32_t)M);
+                            if (HAS_ODD) d = cispi_ratio<float>(((uint32_t)m * (uint32_t)(2 * t + 1)) % twoM, (uint32_t)M);
+                        } else {
+                            c = cmul(c, rot);
+                            if (HAS_ODD) d = cmul(d, rot);
+                        }
+                        ce[t] = c.x;
+                        if (HAS_ODD) co[t] = d.x;
+                    } else {
+                        ce[t] = 0.f;
+                        if (HAS_ODD) co[t] = 0.f;
+                    }
+                }
+            }
+            float gs = (2 * m == M) ? 0.5f : 1.f;                       // +-M/2 bins: half the Nyquist term each
+            if (ri.shifted && (wi & 1)) gs = -gs;                        // exp(i m phi0_i) = (-1)^w exp(+-i m' phi0_i)
+            for (int p = 0; p < np; ++p) {
+                const PairMeta pm = sP[p];
+                const float4* __restrict__ w4 = reinterpret_cast<const float4*>(sW + p * TMAX);
+                float G = 0.f;
+                if (HAS_ODD && (pm.flags & 1)) {
+#pragma unroll
+                    for (int t4 = 0; t4 < TMAX / 4; ++t4) {
+                        if (4 * t4 < pm.cnt) {
+                            const float4 w = w4[t4];
+                            G = fmaf(w.x, co[4 * t4], G); G = fmaf(w.y, co[4 * t4 + 1], G);
+                            G = fmaf(w.z, co[4 * t4 + 2], G); G = fmaf(w.w, co[4 * t4 + 3], G);
+                        }
+                    }
+                } else {
+#pragma unroll
+                    for (int t4 = 0; t4 < TMAX / 4; ++t4) {
+                        if (4 * t4 < pm.cnt) {
+                            const float4 w = w4[t4];
+                            G = fmaf(w.x, ce[4 * t4], G); G = fmaf(w.y, ce[4 * t4 + 1], G);
+                            G = fmaf(w.z, ce[4 * t4 + 2], G); G = fmaf(w.w, ce[4 * t4 + 3], G);
+                        }
+                    }
+                }
+                G *= gs;
+                // periodic extension of the stored half spectra (same index for ring j and its mirror image)
+                const int wj = (int)__umulhi((uint32_t)m, pm.magic), r = m - wj * pm.Nj;
+                const bool refl = 2 * r > pm.Nj, shj = (pm.flags & 2) != 0;
+                const int idx = refl ? pm.Nj - r : r;
+                cx<float> vN = in[pm.offN + idx], vS = in[pm.offS + idx];
+                float sre = 1.f, sim = 1.f;                              // signs of (re, im) of the value used
+                if (refl) sim = -1.f;
+                if (shj && (refl != ((wj & 1) != 0))) { sre = -sre; sim = -sim; }
+                if (fam) sim = -sim;
+                const float gr = G * sre, gi = G * sim;
+                accN.x = fmaf(gr, vN.x, accN.x); accN.y = fmaf(gi, vN.y, accN.y);
+                accS.x = fmaf(gr, vS.x, accS.x); accS.y = fmaf(gi, vS.y, accS.y);
+            }
+        }
+    }
+    cx<float>* __restrict__ out = specOut + (int64_t)blockIdx.y * spec_stride;
+    out[ri.spec_off + mp] = accN;
+    if (iS != i) out[rings[iS].spec_off + mp] = accS;
+}
+
+}  // namespace arkcos
+
+namespace arkcos {
+
+// ---- band kernel for runs of output rings whose pairs all live on one common grid (class E: N_i = N_j = M) -------------
+// HEALPix equatorial region and ECP (exact there).  A thread owns MT modes m for a whole chunk of
+// consecutive output rings: the cosines cos(m u pi / M) are built once per thread (exact sincospi each), every input-ring
+// coefficient Bp_j[m] is loaded once per tile of TI output rings and reused from registers, the rows of the tile sit
+// in shared memory.  No index arithmetic on the mode axis: m <= M/2 = N_j/2 needs no periodic extension.
+struct EqChunk { int i0, n; };
+
+template <int TI, int MT, int TMAX>
+__global__ void __launch_bounds__(kBandThreads)
+band_mac_eq_kernel(const EqChunk* __restrict__ chunks, const NorthRec* __restrict__ north,
+                   const PairRec* __restrict__ pairs, const float* __restrict__ W, const RingRec* __restrict__ rings,
+                   int R, const cx<float>* __restrict__ specIn, cx<float>* __restrict__ specOut, int64_t spec_stride)
+{
+    __shared__ __align__(16) float sW[TI * kMaxPairs * TMAX];
+    __shared__ int sPair[TI * kMaxPairs];
+    __shared__ int2 sJ[kMaxPairs + TI];
+    __shared__ int4 sTile[TI];                 // pair index of the ring's first pair (relative), band_lo, band_hi, unused
+    const EqChunk ch = chunks[blockIdx.y];
+    const int M = rings[ch.i0].n, Mh = M >> 1;
+    int m[MT];
+    bool valid[MT];
+    float ce[MT][TMAX], co[MT][TMAX];
+#pragma unroll
+    for (int mt = 0; mt < MT; ++mt) {
+        m[mt] = (int)blockIdx.x * (kBandThreads * MT) + mt * kBandThreads + (int)threadIdx.x;
+        valid[mt] = m[mt] <= Mh;
+        const uint32_t mm = valid[mt] ? (uint32_t)m[mt] : 0u, twoM = 2u * (uint32_t)M;
+#pragma unroll
+        for (int t = 0; t < TMAX; ++t) {
+            ce[mt][t] = cispi_ratio<float>((mm * (uint32_t)(2 * t)) % twoM, (uint32_t)M).x;
+            co[mt][t] = cispi_ratio<float>((mm * (uint32_t)(2 * t + 1)) % twoM, (uint32_t)M).x;
+        }
+    }
+    if ((int)blockIdx.x * (kBandThreads * MT) > Mh) return;
+    const cx<float>* __restrict__ in = specIn + (int64_t)blockIdx.z * spec_stride;
+    cx<float>* __restrict__ out = specOut + (int64_t)blockIdx.z * spec_stride;
+
+    for (int tile = 0; tile < ch.n; tile += TI) {
+        const int nti = min(TI, ch.n - tile), i0 = ch.i0 + tile;
+        __syncthreads();
+        const int p_first = north[i0].pair_lo, p_last = north[i0 + nti - 1].pair_hi;
+        const int64_t wbase = pairs[p_first].woff;
+        const int jlo = pairs[p_first].j, jhi = pairs[p_last - 1].j;
+        {
+            const PairRec& pl = pairs[p_last - 1];
+            const int nw4 = (int)((pl.woff + ((pl.cnt + 3) & ~3) - wbase) >> 2);
+            const float4* __restrict__ src = reinterpret_cast<const float4*>(W + wbase);
+            float4* dst = reinterpret_cast<float4*>(sW);
+            for (int k = threadIdx.x; k < nw4; k += kBandThreads) dst[k] = src[k];
+            for (int p = p_first + threadIdx.x; p < p_last; p += kBandThreads) {
+                const PairRec& pr = pairs[p];
+                sPair[p - p_first] = ((int)(pr.woff - wbase) << 8) | (((pr.cnt + 3) & ~3) << 1) | pr.par;
+            }
+            for (int j = jlo + threadIdx.x; j <= jhi; j += kBandThreads)
+                sJ[j - jlo] = make_int2((int)rings[j].spec_off, (int)rings[R - 1 - j].spec_off);
+            if (threadIdx.x < nti) {
+                const NorthRec nr = north[i0 + threadIdx.x];
+                sTile[threadIdx.x] = make_int4(nr.pair_lo - p_first, pairs[nr.pair_lo].j, pairs[nr.pair_hi - 1].j, 0);
+            }
+        }
+        __syncthreads();
+        int prel[TI], blo[TI], bhi[TI];
+#pragma unroll
+        for (int ii = 0; ii < TI; ++ii) {
+            const int4 tl = sTile[ii < nti ? ii : 0];
+            prel[ii] = tl.x;
+            blo[ii] = ii < nti ? tl.y : 1;
+            bhi[ii] = ii < nti ? tl.z : 0;        // empty band for the missing rings of a ragged last tile
+        }
+        cx<float> acc[TI][2][MT];
+#pragma unroll
+        for (int ii = 0; ii < TI; ++ii)
+#pragma unroll
+            for (int h = 0; h < 2; ++h)
+#pragma unroll
+                for (int mt = 0; mt < MT; ++mt) acc[ii][h][mt] = mk<float>(0.f, 0.f);
+
+        for (int j = jlo; j <= jhi; ++j) {
+            const int2 off = sJ[j - jlo];
+            cx<float> v[2][MT];
+#pragma unroll
+            for (int mt = 0; mt < MT; ++mt) {
+                v[0][mt] = valid[mt] ? in[off.x + m[mt]] : mk<float>(0.f, 0.f);
+                v[1][mt] = valid[mt] ? in[off.y + m[mt]] : mk<float>(0.f, 0.f);
+            }
+#pragma unroll
+            for (int ii = 0; ii < TI; ++ii) {
+                if (j >= blo[ii] && j <= bhi[ii]) {
+                    const int pk = sPair[prel[ii] + j - blo[ii]];
+                    const float4* __restrict__ w4 = reinterpret_cast<const float4*>(sW + (pk >> 8));
+                    const int c4 = (pk >> 1) & 127;
+                    float G[MT];
+#pragma unroll
+                    for (int mt = 0; mt < MT; ++mt) G[mt] = 0.f;
+                    if (pk & 1) {
+#pragma unroll
+                        for (int t4 = 0; t4 < TMAX / 4; ++t4) {
+                            if (4 * t4 < c4) {
+                                const float4 w = w4[t4];
+#pragma unroll
+                                for (int mt = 0; mt < MT; ++mt) {
+                                    G[mt] = fmaf(w.x, co[mt][4 * t4], G[mt]); G[mt] = fmaf(w.y, co[mt][4 * t4 + 1], G[mt]);
+                                    G[mt] = fmaf(w.z, co[mt][4 * t4 + 2], G[mt]); G[mt] = fmaf(w.w, co[mt][4 * t4 + 3], G[mt]);
+                                }
+                            }
+                        }
+                    } else {
+#pragma unroll
+                        for (int t4 = 0; t4 < TMAX / 4; ++t4) {
+                            if (4 * t4 < c4) {
+                                const float4 w = w4[t4];
+#pragma unroll
+                                for (int mt = 0; mt < MT; ++mt) {
+                                    G[mt] = fmaf(w.x, ce[mt][4 * t4], G[mt]); G[mt] = fmaf(w.y, ce[mt][4 * t4 + 1], G[mt]);
+                                    G[mt] = fmaf(w.z, ce[mt][4 * t4 + 2], G[mt]); G[mt] = fmaf(w.w, ce[mt][4 * t4 + 3], G[mt]);
+                                }
+                            }
+                        }
+                    }
+#pragma unroll
+                    for (int h = 0; h < 2; ++h)
+#pragma unroll
+                        for (int mt = 0; mt < MT; ++mt) {
+                            acc[ii][h][mt].x = fmaf(G[mt], v[h][mt].x, acc[ii][h][mt].x);
+                            acc[ii][h][mt].y = fmaf(G[mt], v[h][mt].y, acc[ii][h][mt].y);
+                        }
+                }
+            }
+        }
+#pragma unroll
+        for (int ii = 0; ii < TI; ++ii) {
+            if (ii < nti) {
+                const int i = i0 + ii, iS = R - 1 - i;
+                const RingRec ri = rings[i];
+                const int64_t offS = rings[iS].spec_off;
+#pragma unroll
+                for (int mt = 0; mt < MT; ++mt) {
+                    if (!valid[mt]) continue;
+                    cx<float> a = acc[ii][0][mt], b = acc[ii][1][mt];
+                    if (m[mt] == Mh) {              // +M/2 and -M/2 fold onto the same bin, half weight each
+                        if (ri.shifted) { a.x = 0.f; b.x = 0.f; } else { a.y = 0.f; b.y = 0.f; }
+                    }
+                    out[ri.spec_off + m[mt]] = a;
+                    if (iS != i) out[offS + m[mt]] = b;
+                }
+            }
+        }
+    }
 }
 
 }  // namespace arkcos

@@ -5,7 +5,7 @@
 
 namespace arkcos {
 
-template <class T> struct cx { T x, y; };              // complex number (re, im); cx<float> is 8 bytes, cx<double> 16
+template <class T> struct __align__(2 * sizeof(T)) cx { T x, y; };   // complex (re, im), naturally aligned: one 64/128-bit access
 
 template <class T> __host__ __device__ __forceinline__ cx<T> mk(T a, T b) { cx<T> r; r.x = a; r.y = b; return r; }
 template <class T> __device__ __forceinline__ cx<T> operator+(cx<T> a, cx<T> b) { return mk<T>(a.x + b.x, a.y + b.y); }

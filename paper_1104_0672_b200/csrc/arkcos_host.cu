@@ -2,6 +2,7 @@
 #include <math.h>
 #include <stdio.h>
 #include <string.h>
+#include <stdlib.h>
 
 #include <algorithm>
 #include <map>
@@ -148,7 +149,8 @@ struct HostTables {
     std::vector<int> bluestein_ids;     // lens that need a filter spectrum
     std::vector<PairRec> pairs;
     std::vector<NorthRec> north;
-    std::vector<BandItem> items;
+    std::vector<BandItem> items[kBandClasses];
+    std::vector<EqChunk> eq_chunks;              // runs of consecutive class-E rings for band_mac_eq_kernel   // per band-kernel class (see band_class)
     int64_t filt_total = 0, nsamples = 0;
     int logPT = 1;
 };
@@ -191,12 +193,13 @@ void build_fft_lens(const HostGeometry& g, HostTables& t, Stats& st)
 }
 
 // Ring-pair table for the northern output rings (the southern ones reuse the rows of their mirror images).
-void build_pairs(HostGeometry& g, double theta_max, double ell_nyq, int fixed_mprime, int band_threads, HostTables& t,
-                 Stats& st)
+void build_pairs(HostGeometry& g, double theta_max, double ell_nyq, int fixed_mprime, int band_threads, bool allow_fast,
+                 HostTables& t, Stats& st)
 {
-    const int R = g.R, nnorth = (R + 1) / 2;
+    const int R = g.R, nnorth = (R + 1) / 2, eq_chunk_rings = 32;
     const double shm = sin(0.5 * theta_max), xmax = 4.0 * shm * shm;
     g.mprime.assign(R, 0);
+    const int nmax = *std::max_element(g.n.begin(), g.n.end());
     for (int i = 0; i < R; ++i) {
         double smax = 0.0;
         for (int j = g.band_lo[i]; j <= g.band_hi[i]; ++j) smax = std::max(smax, sin(g.theta[j]));
@@ -211,7 +214,7 @@ void build_pairs(HostGeometry& g, double theta_max, double ell_nyq, int fixed_mp
             const double sd = sin(0.5 * (g.theta[i] - g.theta[j]));
             p.A = 4.0 * sd * sd;
             p.B = 4.0 * sin(g.theta[i]) * sin(g.theta[j]);
-            if (g.n[i] == g.n[j]) {          // class E: common grid, ring offset inside the kernel evaluation
+            if (g.n[i] == nmax && g.n[j] == nmax) {   // class E: common grid, ring offset inside the kernel evaluation
                 p.M = g.n[i];
                 p.par = g.shifted[i] != g.shifted[j] ? 1 : 0;
             } else {                         // class C: a cap ring is involved, Eq. 8 on both rings
@@ -230,16 +233,46 @@ void build_pairs(HostGeometry& g, double theta_max, double ell_nyq, int fixed_mp
             p.cnt = umax >= p.par ? (umax - p.par) / 2 + 1 : 0;
             p.j = j;
             p.woff = t.nsamples;
-            t.nsamples += p.cnt;
+            t.nsamples += (p.cnt + 3) & ~3;          // rows are stored zero-padded to a multiple of four samples
             t.pairs.push_back(p);
             const double modes = p.M / 2 + 1;
             st.mac_flops += modes * (2.0 * p.cnt + (has_mirror ? 8.0 : 4.0));
             st.ring_pairs += has_mirror ? 2 : 1;
         }
         t.north[i].pair_hi = (int)t.pairs.size();
-        for (int m0 = 0; m0 <= g.n[i] / 2; m0 += band_threads) t.items.push_back(BandItem{i, m0});
+        // which band kernel serves this ring: the fast ones need one grid length M for the whole ring, short rows
+        // and few pairs (rows and pair records live in shared memory)
+        int cls = 0;
+        if (allow_fast) {
+            const int lo = t.north[i].pair_lo, hi = t.north[i].pair_hi;
+            bool same = hi - lo <= kMaxPairs, odd = false;
+            int maxcnt = 0;
+            for (int p = lo; p < hi; ++p) {
+                same = same && t.pairs[p].M == t.pairs[lo].M;
+                odd = odd || t.pairs[p].par;
+                maxcnt = std::max(maxcnt, t.pairs[p].cnt);
+            }
+            bool all_e = same;
+            for (int p = lo; p < hi && all_e; ++p) all_e = t.pairs[p].M == g.n[i] && g.n[t.pairs[p].j] == g.n[i];
+            if (all_e && hi > lo && maxcnt <= 12 && g.spec_total < (int64_t)INT32_MAX) {
+                // extend the current chunk if this ring follows it directly, else open a new one
+                if (!t.eq_chunks.empty() && t.eq_chunks.back().i0 + t.eq_chunks.back().n == i &&
+                    t.eq_chunks.back().n < eq_chunk_rings && g.n[t.eq_chunks.back().i0] == g.n[i])
+                    ++t.eq_chunks.back().n;
+                else
+                    t.eq_chunks.push_back(EqChunk{i, 1});
+                continue;
+            }
+            if (same && hi > lo) {
+                if (maxcnt <= 12) cls = odd ? 1 : 2;
+                else if (maxcnt <= 20 && !odd) cls = 3;
+                else if (maxcnt <= 32) cls = 4;
+            }
+        }
+        for (int m0 = 0; m0 <= g.n[i] / 2; m0 += band_threads) t.items[cls].push_back(BandItem{i, m0});
     }
-    st.row_samples = t.nsamples;
+    st.row_samples = 0;
+    for (const PairRec& p : t.pairs) st.row_samples += p.cnt;
 }
 
 template <class V> int upload(V** dst, const std::vector<V>& src, int64_t* bytes)
@@ -299,6 +332,29 @@ template <class T> int enqueue_rows(const arkcos_plan* pl, cudaStream_t st)
     return 0;
 }
 
+template <int TMAX, bool HAS_ODD> void launch_uniform_class(const arkcos_plan* pl, int cls, int nmaps, cudaStream_t st)
+{
+    if (pl->nitems[cls] == 0) return;
+    band_mac_uniform_kernel<TMAX, HAS_ODD><<<dim3((unsigned)pl->nitems[cls], (unsigned)nmaps), kBandThreads, 0, st>>>(
+        pl->d_items[cls], pl->d_north, pl->d_pairs, (const float*)pl->d_W, pl->d_rings, pl->g.R,
+        (const cx<float>*)pl->d_specIn, (cx<float>*)pl->d_specOut, pl->g.spec_total);
+}
+
+void launch_uniform(const arkcos_plan* pl, int nmaps, cudaStream_t st)
+{
+    if (pl->neqchunks > 0) {
+        constexpr int TI = 4, MT = 2;
+        const unsigned gx = (unsigned)((pl->eq_mh + 1 + kBandThreads * MT - 1) / (kBandThreads * MT));
+        band_mac_eq_kernel<TI, MT, 12><<<dim3(gx, (unsigned)pl->neqchunks, (unsigned)nmaps), kBandThreads, 0, st>>>(
+            pl->d_eqchunks, pl->d_north, pl->d_pairs, (const float*)pl->d_W, pl->d_rings, pl->g.R,
+            (const cx<float>*)pl->d_specIn, (cx<float>*)pl->d_specOut, pl->g.spec_total);
+    }
+    launch_uniform_class<12, true>(pl, 1, nmaps, st);
+    launch_uniform_class<12, false>(pl, 2, nmaps, st);
+    launch_uniform_class<20, false>(pl, 3, nmaps, st);
+    launch_uniform_class<32, true>(pl, 4, nmaps, st);
+}
+
 template <class T> int enqueue_convolve(const arkcos_plan* pl, const void* d_in, void* d_out, int nmaps, cudaStream_t st)
 {
     const HostGeometry& g = pl->g;
@@ -311,9 +367,11 @@ template <class T> int enqueue_convolve(const arkcos_plan* pl, const void* d_in,
         (const T*)d_in, g.npix, (cx<T>*)pl->d_specIn, g.spec_total, pl->d_rings, pl->d_lens, (const cx<T>*)pl->d_tw,
         pl->logPT, (const cx<T>*)pl->d_filt);
     if (tm) cudaEventRecord(pl->ev[2], st);
-    band_mac_general_kernel<T, 16><<<dim3((unsigned)pl->nitems, (unsigned)nmaps), pl->band_threads, 0, st>>>(
-        pl->d_items, pl->d_north, pl->d_pairs, (const T*)pl->d_W, pl->d_rings, g.R, (const cx<T>*)pl->d_specIn,
-        (cx<T>*)pl->d_specOut, g.spec_total);
+    if (pl->nitems[0] > 0)
+        band_mac_general_kernel<T, 16><<<dim3((unsigned)pl->nitems[0], (unsigned)nmaps), kBandThreads, 0, st>>>(
+            pl->d_items[0], pl->d_north, pl->d_pairs, (const T*)pl->d_W, pl->d_rings, g.R, (const cx<T>*)pl->d_specIn,
+            (cx<T>*)pl->d_specOut, g.spec_total);
+    launch_uniform(pl, nmaps, st);
     if (tm) cudaEventRecord(pl->ev[3], st);
     ring_fft_inverse_kernel<T><<<gfft, pl->fft_threads, pl->fft_smem, st>>>(
         (const cx<T>*)pl->d_specOut, g.spec_total, (T*)d_out, g.npix, pl->d_rings, pl->d_lens, (const cx<T>*)pl->d_tw,
@@ -384,11 +442,14 @@ static int plan_create_impl(arkcos_plan** out, const arkcos_pixelization* pix, c
     }
     HostTables t;
     build_fft_lens(pl->g, t, pl->stats);
-    build_pairs(pl->g, pl->theta_max, pl->ell_nyquist, fixed_mprime, pl->band_threads, t, pl->stats);
-    if (t.pairs.size() > (size_t)INT32_MAX || t.items.size() > (size_t)INT32_MAX) return fail(ARKCOS_UNSUPPORTED, "too many ring pairs");
+    build_pairs(pl->g, pl->theta_max, pl->ell_nyquist, fixed_mprime, kBandThreads, dtype == ARKCOS_F32 && !getenv("ARKCOS_FORCE_GENERAL"), t, pl->stats);
+    if (t.pairs.size() > (size_t)INT32_MAX) return fail(ARKCOS_UNSUPPORTED, "too many ring pairs");
     pl->nnorth = (int)t.north.size();
     pl->npairs = (int)t.pairs.size();
-    pl->nitems = (int)t.items.size();
+    for (int c = 0; c < kBandClasses; ++c) pl->nitems[c] = (int)t.items[c].size();
+    pl->neqchunks = (int)t.eq_chunks.size();
+    pl->eq_mh = t.eq_chunks.empty() ? 0 : pl->g.n[t.eq_chunks[0].i0] / 2;
+    for (const EqChunk& c : t.eq_chunks) pl->eq_mh = std::max(pl->eq_mh, pl->g.n[c.i0] / 2);
     pl->nsamples = t.nsamples;
     pl->logPT = t.logPT;
 
@@ -402,7 +463,9 @@ static int plan_create_impl(arkcos_plan** out, const arkcos_pixelization* pix, c
     if (int rc = upload(&pl->d_lens, t.lens, wsb)) return rc;
     if (int rc = upload(&pl->d_pairs, t.pairs, wsb)) return rc;
     if (int rc = upload(&pl->d_north, t.north, wsb)) return rc;
-    if (int rc = upload(&pl->d_items, t.items, wsb)) return rc;
+    for (int c = 0; c < kBandClasses; ++c)
+        if (int rc = upload(&pl->d_items[c], t.items[c], wsb)) return rc;
+    if (int rc = upload(&pl->d_eqchunks, t.eq_chunks, wsb)) return rc;
     std::vector<double> tab(kernel->table, kernel->table + kernel->n);
     if (int rc = upload(&pl->d_table, tab, wsb)) return rc;
     if (int rc = dtype == ARKCOS_F32 ? build_device_numeric<float>(pl, t) : build_device_numeric<double>(pl, t)) return rc;
@@ -464,7 +527,8 @@ int arkcos_convolve_host(const arkcos_plan* pl, const void* h_in, void* h_out, i
 int arkcos_plan_destroy(arkcos_plan* pl)
 {
     if (!pl) return ARKCOS_OK;
-    void* ptrs[] = {pl->d_rings, pl->d_lens, pl->d_pairs, pl->d_north, pl->d_items, pl->d_table, pl->d_tw, pl->d_filt,
+    void* ptrs[] = {pl->d_rings, pl->d_lens, pl->d_pairs, pl->d_north, pl->d_items[0], pl->d_items[1], pl->d_items[2], pl->d_items[3],
+                    pl->d_items[4], pl->d_eqchunks, pl->d_table, pl->d_tw, pl->d_filt,
                     pl->d_W, pl->d_specIn, pl->d_specOut, pl->d_stage_in, pl->d_stage_out};
     for (void* p : ptrs) if (p) cudaFree(p);
     for (auto& e : pl->ev) if (e) cudaEventDestroy(e);

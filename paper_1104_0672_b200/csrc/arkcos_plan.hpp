@@ -37,7 +37,7 @@ struct arkcos_plan {
     arkcos::HostGeometry g;
     arkcos::Stats stats;
 
-    int nnorth = 0, npairs = 0, nitems = 0, logPT = 0, band_threads = 128, fft_threads = 256;
+    int nnorth = 0, npairs = 0, nitems[arkcos::kBandClasses] = {0, 0, 0, 0, 0}, logPT = 0, fft_threads = 256;
     size_t fft_smem = 0;
     int64_t nsamples = 0;
 
@@ -46,7 +46,9 @@ struct arkcos_plan {
     arkcos::FftLen* d_lens = nullptr;
     arkcos::PairRec* d_pairs = nullptr;
     arkcos::NorthRec* d_north = nullptr;
-    arkcos::BandItem* d_items = nullptr;
+    arkcos::EqChunk* d_eqchunks = nullptr;
+    int neqchunks = 0, eq_mh = 0;
+    arkcos::BandItem* d_items[arkcos::kBandClasses] = {nullptr, nullptr, nullptr, nullptr, nullptr};
     double* d_table = nullptr;
     void* d_tw = nullptr;        // cx<T>[PT/2]
     void* d_filt = nullptr;      // cx<T>[...] Bluestein filter spectra
