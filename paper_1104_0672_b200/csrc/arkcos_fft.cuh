@@ -3,111 +3,160 @@
 // backward FFT on all output rings"), fused with the re-origin phase of Eq. 8.
 //
 // A ring of N reals (N even) is transformed as one complex FFT of length L = N/2 plus an O(N) split.  Power-of-two L:
-// radix-2 butterflies in shared memory.  Any other L (HEALPix cap rings, N = 4n): Bluestein's chirp-z with a
-// power-of-two convolution length P >= 2L-1, whose filter spectrum is computed once per distinct L at plan time.
+// Stockham radix-8 passes held in registers, exchanged through padded shared memory.  Any other L (HEALPix cap rings,
+// N = 4n): Bluestein's chirp-z with a power-of-two convolution length P >= 2L-1; chirps, phases and the filter
+// spectrum come from tables built once per distinct ring length at plan time.
 #pragma once
 #include "arkcos_device.cuh"
 
 namespace arkcos {
 
-// ---- complex FFT, in place in shared memory, P = 2^logP points ------------------------------------------------------
-// tw[k] = exp(-2 pi i k / PT), k = 0 .. PT/2-1, PT = 2^logPT >= P (global memory, read through L1).
+constexpr int kFftThreads = 512;
 
-// decimation in frequency: natural order in, bit-reversed order out, kernel exp(-i...)
-template <class T> __device__ void fft_dif(cx<T>* s, int logP, const cx<T>* __restrict__ tw, int logPT)
+// shared-memory index padding: one extra slot every 16 complex numbers keeps the radix-8 scatter conflict-free
+__device__ __forceinline__ int phys(int e) { return e + (e >> 4); }
+__host__ __device__ inline size_t fft_smem_elems(int P) { return (size_t)P + (size_t)(P >> 4) + 1; }
+
+template <class T> __device__ __forceinline__ cx<T> mul_mi(cx<T> a) { return mk<T>(a.y, -a.x); }     // a * (-i)
+
+template <class T> __device__ __forceinline__ void dft2(cx<T>* u)
 {
-    const int half = 1 << (logP - 1);
-    for (int lh = logP - 1; lh >= 0; --lh) {
-        const int h = 1 << lh;
-        for (int b = threadIdx.x; b < half; b += blockDim.x) {
-            const int pos = b & (h - 1);
-            const int i0 = ((b >> lh) << (lh + 1)) | pos;
-            const cx<T> a = s[i0], c = s[i0 + h];
-            s[i0] = a + c;
-            s[i0 + h] = cmul(a - c, tw[pos << (logPT - 1 - lh)]);
-        }
-        __syncthreads();
-    }
+    const cx<T> a = u[0] + u[1], b = u[0] - u[1];
+    u[0] = a; u[1] = b;
+}
+template <class T> __device__ __forceinline__ void dft4(cx<T>* u)
+{
+    const cx<T> s02 = u[0] + u[2], d02 = u[0] - u[2], s13 = u[1] + u[3], d13 = mul_mi(u[1] - u[3]);
+    u[0] = s02 + s13; u[2] = s02 - s13; u[1] = d02 + d13; u[3] = d02 - d13;
+}
+template <class T> __device__ __forceinline__ void dft8(cx<T>* u)
+{
+    const T h = (T)0.70710678118654752440;
+    cx<T> a[8];
+#pragma unroll
+    for (int n = 0; n < 4; ++n) { a[n] = u[n] + u[n + 4]; a[n + 4] = u[n] - u[n + 4]; }
+    a[5] = mk<T>(h * (a[5].x + a[5].y), h * (a[5].y - a[5].x));          // * exp(-i pi/4)
+    a[6] = mul_mi(a[6]);                                                  // * exp(-i pi/2)
+    a[7] = mk<T>(h * (a[7].y - a[7].x), -h * (a[7].x + a[7].y));         // * exp(-3 i pi/4)
+    dft4(a);
+    dft4(a + 4);
+    u[0] = a[0]; u[2] = a[1]; u[4] = a[2]; u[6] = a[3];
+    u[1] = a[4]; u[3] = a[5]; u[5] = a[6]; u[7] = a[7];
+}
+template <class T, int R> __device__ __forceinline__ void dftR(cx<T>* u)
+{
+    if (R == 8) dft8(u); else if (R == 4) dft4(u); else dft2(u);
 }
 
-// decimation in time with the conjugate twiddles: bit-reversed order in, natural order out, kernel exp(+i...)
-template <class T> __device__ void ifft_dit(cx<T>* s, int logP, const cx<T>* __restrict__ tw, int logPT)
+// One Stockham pass of radix R over the N = 2^logN points in s (padded indexing), p = 2^logp = product of the radices
+// of the passes already done.  tw[k] = exp(-2 pi i k / PT), k = 0 .. PT-1.
+template <class T, int R, int BPT>
+__device__ __forceinline__ void stockham_pass(cx<T>* s, int logN, int logp, const cx<T>* __restrict__ tw, int logPT)
 {
-    const int half = 1 << (logP - 1);
-    for (int lh = 0; lh < logP; ++lh) {
-        const int h = 1 << lh;
-        for (int b = threadIdx.x; b < half; b += blockDim.x) {
-            const int pos = b & (h - 1);
-            const int i0 = ((b >> lh) << (lh + 1)) | pos;
-            const cx<T> a = s[i0], c = cmulc(s[i0 + h], tw[pos << (logPT - 1 - lh)]);
-            s[i0] = a + c;
-            s[i0 + h] = a - c;
+    constexpr int logR = R == 8 ? 3 : (R == 4 ? 2 : 1);
+    const int nb = 1 << (logN - logR), p = 1 << logp;
+    cx<T> u[BPT][R];
+#pragma unroll
+    for (int b = 0; b < BPT; ++b) {
+        const int i = (int)threadIdx.x + b * kFftThreads;
+        if (i < nb) {
+#pragma unroll
+            for (int r = 0; r < R; ++r) u[b][r] = s[phys(i + r * nb)];
         }
-        __syncthreads();
     }
+    __syncthreads();
+#pragma unroll
+    for (int b = 0; b < BPT; ++b) {
+        const int i = (int)threadIdx.x + b * kFftThreads;
+        if (i < nb) {
+            const int k = i & (p - 1);
+            if (logp > 0) {
+                const int sh = logPT - logp - logR;             // exp(-2 pi i r k / (p R)) = tw[(r k) << sh]
+                if (R == 8) {
+                    const cx<T> w1 = tw[k << sh], w2 = tw[(2 * k) << sh], w4 = tw[(4 * k) << sh];
+                    const cx<T> w3 = cmul(w1, w2);
+                    u[b][1] = cmul(u[b][1], w1); u[b][2] = cmul(u[b][2], w2); u[b][3] = cmul(u[b][3], w3);
+                    u[b][4] = cmul(u[b][4], w4); u[b][5] = cmul(u[b][5], cmul(w4, w1));
+                    u[b][6] = cmul(u[b][6], cmul(w4, w2)); u[b][7] = cmul(u[b][7], cmul(w4, w3));
+                } else if (R == 4) {
+                    const cx<T> w1 = tw[k << sh], w2 = tw[(2 * k) << sh];
+                    u[b][1] = cmul(u[b][1], w1); u[b][2] = cmul(u[b][2], w2); u[b][3] = cmul(u[b][3], cmul(w1, w2));
+                } else {
+                    u[b][1] = cmul(u[b][1], tw[k << sh]);
+                }
+            }
+            dftR<T, R>(u[b]);
+            const int j = ((i - k) << logR) + k;
+#pragma unroll
+            for (int q = 0; q < R; ++q) s[phys(j + q * p)] = u[b][q];
+        }
+    }
+    __syncthreads();
 }
 
-__device__ __forceinline__ int bitrev(int k, int logP) { return (int)(__brev((unsigned)k) >> (32 - logP)); }
+// Forward complex DFT, natural order in and out, of the 2^logN points in s (padded indexing), in place.
+// BPT >= 2^logN / (8 * kFftThreads).  s must be synchronised on entry; it is synchronised on return.
+template <class T, int BPT> __device__ void fft_pow2(cx<T>* s, int logN, const cx<T>* __restrict__ tw, int logPT)
+{
+    int logp = 0;
+    for (; logp + 3 <= logN; logp += 3) stockham_pass<T, 8, BPT>(s, logN, logp, tw, logPT);
+    if (logN - logp == 2) stockham_pass<T, 4, 2 * BPT>(s, logN, logp, tw, logPT);
+    else if (logN - logp == 1) stockham_pass<T, 2, 4 * BPT>(s, logN, logp, tw, logPT);
+}
 
 // Description of one FFT length (one per distinct ring length; device table built at plan time).
 struct FftLen {
-    int L;            // complex length = N/2
-    int logP;         // pow2: P = L; Bluestein: P = smallest power of two >= 2L-1
-    int pow2;         // 1: direct power-of-two transform
+    int L;             // complex length = N/2
+    int logP;          // pow2: P = L; Bluestein: P = smallest power of two >= 2L-1
+    int pow2;          // 1: direct power-of-two transform
     int pad;
-    int64_t filt_off; // Bluestein: offset of the filter spectrum (bit-reversed order, scaled by 1/P) in the filter table
+    int64_t filt_off;  // Bluestein: offset of the filter spectrum FFT_P(b)/P in the filter table
+    int64_t chirp_off; // Bluestein: offset of chirp[n] = exp(-i pi n^2 / L), n < L, in the chirp table
+    int64_t ph_off;    // offset of ph[k] = exp(-i pi k / N), k = 0 .. L, in the phase table
 };
 
-// chirp w[n] = exp(-i pi n^2 / L), n < L <= 8192 (n^2 fits 32 bits)
-template <class T> __device__ __forceinline__ cx<T> chirp(uint32_t n, uint32_t L)
+// Forward complex DFT of length L of the natural-order data in s[phys(0 .. L-1)]; the result replaces it.
+// Bluestein: X[k] = w[k] sum_n (z[n] w[n]) conj(w[k-n]),  w[n] = exp(-i pi n^2 / L), as a cyclic convolution of length P.
+// pre_chirped: the caller already multiplied the input by w[n] and zero-padded s up to P.
+template <class T, int BPT>
+__device__ void fft_len(cx<T>* s, const FftLen& f, const cx<T>* __restrict__ tw, int logPT,
+                        const cx<T>* __restrict__ filt, const cx<T>* __restrict__ chirp)
 {
-    const uint32_t r = (n * n) % (2u * L);
-    return cispi_ratio<T>(r == 0 ? 0u : 2u * L - r, L);
-}
-
-// Forward complex DFT of s[0..L-1] (natural order), X[k] = sum_n s[n] exp(-2 pi i n k / L).
-// On return X[k] is at s[fft_out_index(k)].  All threads of the block must call it; s must hold P elements and be
-// synchronised on entry; it is synchronised on return.
-template <class T> __device__ void fft_len(cx<T>* s, const FftLen& f, const cx<T>* __restrict__ tw, int logPT,
-                                           const cx<T>* __restrict__ filt)
-{
-    if (f.pow2) {
-        if (f.logP > 0) fft_dif(s, f.logP, tw, logPT);
-        return;
-    }
+    fft_pow2<T, BPT>(s, f.logP, tw, logPT);
+    if (f.pow2) return;
     const int L = f.L, P = 1 << f.logP;
-    for (int n = threadIdx.x; n < P; n += blockDim.x)
-        s[n] = n < L ? cmul(s[n], chirp<T>(n, L)) : mk<T>(0, 0);
-    __syncthreads();
-    fft_dif(s, f.logP, tw, logPT);
     const cx<T>* __restrict__ fl = filt + f.filt_off;
-    for (int k = threadIdx.x; k < P; k += blockDim.x) s[k] = cmul(s[k], fl[k]);
+    const cx<T>* __restrict__ cw = chirp + f.chirp_off;
+    // inverse transform of Y F as conj(FFT(conj(Y F)))
+    for (int k = threadIdx.x; k < P; k += kFftThreads) s[phys(k)] = cconj(cmul(s[phys(k)], fl[k]));
     __syncthreads();
-    ifft_dit(s, f.logP, tw, logPT);
-    for (int k = threadIdx.x; k < L; k += blockDim.x) s[k] = cmul(s[k], chirp<T>(k, L));
+    fft_pow2<T, BPT>(s, f.logP, tw, logPT);
+    for (int k = threadIdx.x; k < L; k += kFftThreads) s[phys(k)] = cmul(cconj(s[phys(k)]), cw[k]);
     __syncthreads();
 }
-__device__ __forceinline__ int fft_out_index(int k, const FftLen& f) { return f.pow2 ? bitrev(k, f.logP) : k; }
 
-// Plan time: filter spectrum of Bluestein's convolution for one length per block:
-// b[n] = exp(+i pi n^2 / L) for |n| < L placed circularly on P points; filt = DIF-FFT(b) / P (bit-reversed order).
-template <class T> __global__ void bluestein_filter_kernel(const FftLen* __restrict__ lens, const int* __restrict__ which,
-                                                           const cx<T>* __restrict__ tw, int logPT, cx<T>* __restrict__ filt)
+// Plan time: filter spectrum of Bluestein's convolution, one length per block:
+// b[n] = exp(+i pi n^2 / L) for |n| < L placed circularly on P points; filt = FFT_P(b) / P.
+template <class T, int BPT>
+__global__ void __launch_bounds__(kFftThreads)
+bluestein_filter_kernel(const FftLen* __restrict__ lens, const int* __restrict__ which, const cx<T>* __restrict__ tw,
+                        int logPT, const cx<T>* __restrict__ chirp, cx<T>* __restrict__ filt)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     cx<T>* s = reinterpret_cast<cx<T>*>(smem_raw);
     const FftLen f = lens[which[blockIdx.x]];
     const int L = f.L, P = 1 << f.logP;
-    for (int n = threadIdx.x; n < P; n += blockDim.x) {
+    const cx<T>* __restrict__ cw = chirp + f.chirp_off;
+    for (int n = threadIdx.x; n < P; n += kFftThreads) {
         cx<T> v = mk<T>(0, 0);
-        if (n < L) v = cconj(chirp<T>(n, L));
-        else if (n > P - L) v = cconj(chirp<T>(P - n, L));
-        s[n] = v;
+        if (n < L) v = cconj(cw[n]);
+        else if (n > P - L) v = cconj(cw[P - n]);
+        s[phys(n)] = v;
     }
     __syncthreads();
-    fft_dif(s, f.logP, tw, logPT);
+    fft_pow2<T, BPT>(s, f.logP, tw, logPT);
     const T inv = (T)1 / (T)P;
-    for (int k = threadIdx.x; k < P; k += blockDim.x) filt[f.filt_off + k] = cscale(s[k], inv);
+    for (int k = threadIdx.x; k < P; k += kFftThreads) filt[f.filt_off + k] = cscale(s[phys(k)], inv);
 }
 
 // Per-ring record used by the FFT kernels and the band kernel.
@@ -121,67 +170,80 @@ struct RingRec {
 };
 
 // Step 1 + 2: Bp_j[k] = exp(-i k phi0_j) sum_l in(j,l) exp(-2 pi i k l / N_j), k = 0 .. N_j/2.
-// grid = (rings, nmaps), one ring per block.
-template <class T> __global__ void ring_fft_forward_kernel(const T* __restrict__ in, int64_t npix, cx<T>* __restrict__ spec,
-                                                           int64_t spec_stride, const RingRec* __restrict__ rings,
-                                                           const FftLen* __restrict__ lens, const cx<T>* __restrict__ tw,
-                                                           int logPT, const cx<T>* __restrict__ filt)
+// grid = (rings, nmaps); block b works on ring order[b] (longest transforms first).
+template <class T, int BPT>
+__global__ void __launch_bounds__(kFftThreads)
+ring_fft_forward_kernel(const T* __restrict__ in, int64_t npix, cx<T>* __restrict__ spec, int64_t spec_stride,
+                        const RingRec* __restrict__ rings, const int* __restrict__ order,
+                        const FftLen* __restrict__ lens, const cx<T>* __restrict__ tw, int logPT,
+                        const cx<T>* __restrict__ filt, const cx<T>* __restrict__ chirp, const cx<T>* __restrict__ phase)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     cx<T>* s = reinterpret_cast<cx<T>*>(smem_raw);
-    const RingRec r = rings[blockIdx.x];
+    const RingRec r = rings[order[blockIdx.x]];
     const FftLen f = lens[r.len_id];
-    const int N = r.n, L = N >> 1;
+    const int N = r.n, L = N >> 1, P = 1 << f.logP;
     const cx<T>* __restrict__ x = reinterpret_cast<const cx<T>*>(in + (int64_t)blockIdx.y * npix + r.pix_off);
-    for (int l = threadIdx.x; l < L; l += blockDim.x) s[l] = x[l];          // z[l] = x[2l] + i x[2l+1]
+    if (f.pow2) {
+        for (int l = threadIdx.x; l < L; l += kFftThreads) s[phys(l)] = x[l];          // z[l] = x[2l] + i x[2l+1]
+    } else {
+        const cx<T>* __restrict__ cw = chirp + f.chirp_off;
+        for (int l = threadIdx.x; l < P; l += kFftThreads) s[phys(l)] = l < L ? cmul(x[l], cw[l]) : mk<T>(0, 0);
+    }
     __syncthreads();
-    fft_len(s, f, tw, logPT, filt);
+    fft_len<T, BPT>(s, f, tw, logPT, filt, chirp);
     cx<T>* __restrict__ out = spec + (int64_t)blockIdx.y * spec_stride + r.spec_off;
-    for (int k = threadIdx.x; k <= L; k += blockDim.x) {
-        const cx<T> zk = s[fft_out_index(k == L ? 0 : k, f)];
-        const cx<T> zc = cconj(s[fft_out_index(k == 0 ? 0 : L - k, f)]);
+    const cx<T>* __restrict__ ph = phase + f.ph_off;
+    for (int k = threadIdx.x; k <= L; k += kFftThreads) {
+        const cx<T> zk = s[phys(k == L ? 0 : k)];
+        const cx<T> zc = cconj(s[phys(k == 0 ? 0 : L - k)]);
         const cx<T> e = cscale(zk + zc, (T)0.5), o = cscale(zk - zc, (T)0.5);
-        // X[k] = e - i exp(-2 pi i k / N) o
-        const cx<T> w = cispi_ratio<T>(k == 0 ? 0u : (uint32_t)(2 * N - 2 * k), (uint32_t)N);   // exp(-i pi 2k / N)
-        const cx<T> wo = cmul(w, o);
-        cx<T> X = mk<T>(e.x + wo.y, e.y - wo.x);
-        if (r.shifted) X = cmul(X, cispi_ratio<T>(k == 0 ? 0u : (uint32_t)(2 * N - k), (uint32_t)N));  // exp(-i pi k / N)
+        const cx<T> h = ph[k];                         // exp(-i pi k / N)
+        const cx<T> wo = cmul(cmul(h, h), o);          // exp(-2 pi i k / N) o
+        cx<T> X = mk<T>(e.x + wo.y, e.y - wo.x);       // X[k] = e - i exp(-2 pi i k / N) o
+        if (r.shifted) X = cmul(X, h);
         out[k] = X;
     }
 }
 
 // Step 6 + 7: out(i,k) = sum_{m'} D_i[m'] exp(2 pi i m' k / N_i) with D_i[m'] = exp(+i m' phi0_i) Dp_i[m'] for
 // m' = 0 .. N_i/2 and Hermitian symmetry for the rest.  grid = (rings, nmaps).
-template <class T> __global__ void ring_fft_inverse_kernel(const cx<T>* __restrict__ spec, int64_t spec_stride,
-                                                           T* __restrict__ outmap, int64_t npix,
-                                                           const RingRec* __restrict__ rings, const FftLen* __restrict__ lens,
-                                                           const cx<T>* __restrict__ tw, int logPT,
-                                                           const cx<T>* __restrict__ filt)
+template <class T, int BPT>
+__global__ void __launch_bounds__(kFftThreads)
+ring_fft_inverse_kernel(const cx<T>* __restrict__ spec, int64_t spec_stride, T* __restrict__ outmap, int64_t npix,
+                        const RingRec* __restrict__ rings, const int* __restrict__ order,
+                        const FftLen* __restrict__ lens, const cx<T>* __restrict__ tw, int logPT,
+                        const cx<T>* __restrict__ filt, const cx<T>* __restrict__ chirp, const cx<T>* __restrict__ phase)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     cx<T>* s = reinterpret_cast<cx<T>*>(smem_raw);
-    const RingRec r = rings[blockIdx.x];
+    const RingRec r = rings[order[blockIdx.x]];
     const FftLen f = lens[r.len_id];
-    const int N = r.n, L = N >> 1;
+    const int N = r.n, L = N >> 1, P = 1 << f.logP;
     const cx<T>* __restrict__ D = spec + (int64_t)blockIdx.y * spec_stride + r.spec_off;
-    for (int k = threadIdx.x; k < L; k += blockDim.x) {
-        cx<T> xk = D[k], xl = D[L - k];
-        if (r.shifted) {
-            xk = cmul(xk, cispi_ratio<T>((uint32_t)k, (uint32_t)N));
-            xl = cmul(xl, cispi_ratio<T>((uint32_t)(L - k), (uint32_t)N));
+    const cx<T>* __restrict__ ph = phase + f.ph_off;
+    const cx<T>* __restrict__ cw = chirp + f.chirp_off;
+    for (int k = threadIdx.x; k < (f.pow2 ? L : P); k += kFftThreads) {
+        cx<T> v = mk<T>(0, 0);
+        if (k < L) {
+            cx<T> xk = D[k], xl = D[L - k];
+            const cx<T> hk = cconj(ph[k]), hl = cconj(ph[L - k]);      // exp(+i pi k / N)
+            if (r.shifted) { xk = cmul(xk, hk); xl = cmul(xl, hl); }
+            const cx<T> xc = cconj(xl);
+            const cx<T> a = xk + xc, d = xk - xc;
+            const cx<T> wd = cmul(cmul(hk, hk), d);                    // exp(+2 pi i k / N) d
+            // Z[k] = a + i wd ; the inverse transform is done as conj(FFT(conj Z))
+            v = mk<T>(a.x - wd.y, -(a.y + wd.x));
+            if (!f.pow2) v = cmul(v, cw[k]);
         }
-        const cx<T> xc = cconj(xl);
-        const cx<T> a = xk + xc, d = xk - xc;
-        const cx<T> wd = cmul(cispi_ratio<T>((uint32_t)(2 * k), (uint32_t)N), d);          // exp(+2 pi i k / N) d
-        // Z[k] = a + i wd ; the inverse transform is done as conj(FFT(conj Z))
-        s[k] = mk<T>(a.x - wd.y, -(a.y + wd.x));
+        s[phys(k)] = v;
     }
     __syncthreads();
-    fft_len(s, f, tw, logPT, filt);
+    fft_len<T, BPT>(s, f, tw, logPT, filt, chirp);
     cx<T>* __restrict__ o = reinterpret_cast<cx<T>*>(outmap + (int64_t)blockIdx.y * npix + r.pix_off);
-    for (int n = threadIdx.x; n < L; n += blockDim.x) {
-        const cx<T> z = s[fft_out_index(n, f)];
-        o[n] = mk<T>(z.x, -z.y);                                                             // out[2n], out[2n+1]
+    for (int n = threadIdx.x; n < L; n += kFftThreads) {
+        const cx<T> z = s[phys(n)];
+        o[n] = mk<T>(z.x, -z.y);                                       // out[2n], out[2n+1]
     }
 }
 

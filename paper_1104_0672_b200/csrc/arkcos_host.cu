@@ -151,7 +151,8 @@ struct HostTables {
     std::vector<NorthRec> north;
     std::vector<BandItem> items[kBandClasses];
     std::vector<EqChunk> eq_chunks;              // runs of consecutive class-E rings for band_mac_eq_kernel   // per band-kernel class (see band_class)
-    int64_t filt_total = 0, nsamples = 0;
+    std::vector<int> fft_order;          // rings sorted by decreasing transform size
+    int64_t filt_total = 0, chirp_total = 0, ph_total = 0, nsamples = 0;
     int logPT = 1;
 };
 
@@ -169,9 +170,14 @@ void build_fft_lens(const HostGeometry& g, HostTables& t, Stats& st)
             f.pow2 = is_pow2(L) ? 1 : 0;
             f.logP = f.pow2 ? ilog2(L) : ilog2(2 * L - 1);
             f.filt_off = 0;
+            f.chirp_off = 0;
+            f.ph_off = t.ph_total;
+            t.ph_total += L + 1;
             if (!f.pow2) {
                 f.filt_off = t.filt_total;
                 t.filt_total += (int64_t)1 << f.logP;
+                f.chirp_off = t.chirp_total;
+                t.chirp_total += L;
                 t.bluestein_ids.push_back((int)t.lens.size());
             }
             t.logPT = std::max(t.logPT, f.logP);
@@ -190,6 +196,13 @@ void build_fft_lens(const HostGeometry& g, HostTables& t, Stats& st)
         // forward + inverse: complex FFT(s) + O(N) split / chirps
         st.fft_flops += 2.0 * (f.pow2 ? 5.0 * P * f.logP + 20.0 * L : 2.0 * 5.0 * P * f.logP + 6.0 * P + 32.0 * L);
     }
+    t.fft_order.resize(g.R);
+    for (int i = 0; i < g.R; ++i) t.fft_order[i] = i;
+    std::stable_sort(t.fft_order.begin(), t.fft_order.end(), [&](int a, int b) {
+        const FftLen &fa = t.lens[t.rings[a].len_id], &fb = t.lens[t.rings[b].len_id];
+        const int wa = (fa.pow2 ? 1 : 2) << fa.logP, wb = (fb.pow2 ? 1 : 2) << fb.logP;
+        return wa > wb;
+    });
 }
 
 // Ring-pair table for the northern output rings (the southern ones reuse the rows of their mirror images).
@@ -285,19 +298,44 @@ template <class V> int upload(V** dst, const std::vector<V>& src, int64_t* bytes
 }
 
 // twiddles exp(-2 pi i k / PT) from double precision, Bluestein filters by a plan-time kernel, workspace
+template <class T, int BPT> int set_fft_smem(size_t bytes)
+{
+    CUDA_TRY(cudaFuncSetAttribute(ring_fft_forward_kernel<T, BPT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
+    CUDA_TRY(cudaFuncSetAttribute(ring_fft_inverse_kernel<T, BPT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
+    CUDA_TRY(cudaFuncSetAttribute(bluestein_filter_kernel<T, BPT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
+    return 0;
+}
+
+// twiddles, chirps and phases from double precision, Bluestein filters by a plan-time kernel, workspace
 template <class T> int build_device_numeric(arkcos_plan* pl, const HostTables& t)
 {
     const int PT = 1 << t.logPT;
-    std::vector<cx<T>> tw(std::max(PT / 2, 1));
-    for (int k = 0; k < PT / 2; ++k) tw[k] = mk<T>((T)cos(2.0 * kPi * k / PT), (T)(-sin(2.0 * kPi * k / PT)));
+    std::vector<cx<T>> tw(PT);
+    for (int k = 0; k < PT; ++k) tw[k] = mk<T>((T)cos(2.0 * kPi * k / PT), (T)(-sin(2.0 * kPi * k / PT)));
     cx<T>* d_tw = nullptr;
     if (int rc = upload(&d_tw, tw, &pl->stats.workspace_bytes)) return rc;
     pl->d_tw = d_tw;
-    pl->fft_smem = (size_t)PT * sizeof(cx<T>);
-    if (pl->fft_smem > 227 * 1024) return fail(ARKCOS_UNSUPPORTED, "ring too long for the shared-memory FFT");
-    CUDA_TRY(cudaFuncSetAttribute(ring_fft_forward_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl->fft_smem));
-    CUDA_TRY(cudaFuncSetAttribute(ring_fft_inverse_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl->fft_smem));
-    CUDA_TRY(cudaFuncSetAttribute(bluestein_filter_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl->fft_smem));
+    std::vector<cx<T>> chirp((size_t)t.chirp_total), phase((size_t)t.ph_total);
+    for (const FftLen& f : t.lens) {
+        const int L = f.L, N = 2 * L;
+        for (int k = 0; k <= L; ++k)                       // exp(-i pi k / N)
+            phase[f.ph_off + k] = mk<T>((T)cos(kPi * k / N), (T)(-sin(kPi * k / N)));
+        if (f.pow2) continue;
+        for (int n = 0; n < L; ++n) {                      // exp(-i pi n^2 / L), phase reduced exactly
+            const long long r = ((long long)n * n) % (2LL * L);
+            chirp[f.chirp_off + n] = mk<T>((T)cos(kPi * (double)r / L), (T)(-sin(kPi * (double)r / L)));
+        }
+    }
+    cx<T>*d_chirp = nullptr, *d_phase = nullptr;
+    if (int rc = upload(&d_chirp, chirp, &pl->stats.workspace_bytes)) return rc;
+    pl->d_chirp = d_chirp;
+    if (int rc = upload(&d_phase, phase, &pl->stats.workspace_bytes)) return rc;
+    pl->d_phase = d_phase;
+    if (int rc = upload(&pl->d_fft_order, t.fft_order, &pl->stats.workspace_bytes)) return rc;
+    pl->fft_smem = fft_smem_elems(PT) * sizeof(cx<T>);
+    pl->fft_bpt = PT <= 8 * kFftThreads * 2 ? 2 : 4;
+    if (pl->fft_smem > 227 * 1024 || PT > 8 * kFftThreads * 4) return fail(ARKCOS_UNSUPPORTED, "ring too long for the shared-memory FFT");
+    if (int rc = pl->fft_bpt == 2 ? set_fft_smem<T, 2>(pl->fft_smem) : set_fft_smem<T, 4>(pl->fft_smem)) return rc;
 
     const size_t fb = (size_t)std::max<int64_t>(t.filt_total, 1) * sizeof(cx<T>);
     CUDA_TRY(cudaMalloc(&pl->d_filt, fb));
@@ -306,8 +344,12 @@ template <class T> int build_device_numeric(arkcos_plan* pl, const HostTables& t
         int* d_which = nullptr;
         int64_t dummy = 0;
         if (int rc = upload(&d_which, t.bluestein_ids, &dummy)) return rc;
-        bluestein_filter_kernel<T><<<(unsigned)t.bluestein_ids.size(), pl->fft_threads, pl->fft_smem>>>(
-            pl->d_lens, d_which, d_tw, pl->logPT, (cx<T>*)pl->d_filt);
+        if (pl->fft_bpt == 2)
+            bluestein_filter_kernel<T, 2><<<(unsigned)t.bluestein_ids.size(), kFftThreads, pl->fft_smem>>>(
+                pl->d_lens, d_which, d_tw, pl->logPT, d_chirp, (cx<T>*)pl->d_filt);
+        else
+            bluestein_filter_kernel<T, 4><<<(unsigned)t.bluestein_ids.size(), kFftThreads, pl->fft_smem>>>(
+                pl->d_lens, d_which, d_tw, pl->logPT, d_chirp, (cx<T>*)pl->d_filt);
         cudaError_t e = cudaDeviceSynchronize();
         cudaFree(d_which);
         CUDA_TRY(e);
@@ -363,9 +405,14 @@ template <class T> int enqueue_convolve(const arkcos_plan* pl, const void* d_in,
     if (!pl->opt.cache_kernel_rows) enqueue_rows<T>(pl, st);
     if (tm) cudaEventRecord(pl->ev[1], st);
     const dim3 gfft((unsigned)g.R, (unsigned)nmaps);
-    ring_fft_forward_kernel<T><<<gfft, pl->fft_threads, pl->fft_smem, st>>>(
-        (const T*)d_in, g.npix, (cx<T>*)pl->d_specIn, g.spec_total, pl->d_rings, pl->d_lens, (const cx<T>*)pl->d_tw,
-        pl->logPT, (const cx<T>*)pl->d_filt);
+    if (pl->fft_bpt == 2)
+        ring_fft_forward_kernel<T, 2><<<gfft, kFftThreads, pl->fft_smem, st>>>(
+            (const T*)d_in, g.npix, (cx<T>*)pl->d_specIn, g.spec_total, pl->d_rings, pl->d_fft_order, pl->d_lens,
+            (const cx<T>*)pl->d_tw, pl->logPT, (const cx<T>*)pl->d_filt, (const cx<T>*)pl->d_chirp, (const cx<T>*)pl->d_phase);
+    else
+        ring_fft_forward_kernel<T, 4><<<gfft, kFftThreads, pl->fft_smem, st>>>(
+            (const T*)d_in, g.npix, (cx<T>*)pl->d_specIn, g.spec_total, pl->d_rings, pl->d_fft_order, pl->d_lens,
+            (const cx<T>*)pl->d_tw, pl->logPT, (const cx<T>*)pl->d_filt, (const cx<T>*)pl->d_chirp, (const cx<T>*)pl->d_phase);
     if (tm) cudaEventRecord(pl->ev[2], st);
     if (pl->nitems[0] > 0)
         band_mac_general_kernel<T, 16><<<dim3((unsigned)pl->nitems[0], (unsigned)nmaps), kBandThreads, 0, st>>>(
@@ -373,9 +420,14 @@ template <class T> int enqueue_convolve(const arkcos_plan* pl, const void* d_in,
             (cx<T>*)pl->d_specOut, g.spec_total);
     launch_uniform(pl, nmaps, st);
     if (tm) cudaEventRecord(pl->ev[3], st);
-    ring_fft_inverse_kernel<T><<<gfft, pl->fft_threads, pl->fft_smem, st>>>(
-        (const cx<T>*)pl->d_specOut, g.spec_total, (T*)d_out, g.npix, pl->d_rings, pl->d_lens, (const cx<T>*)pl->d_tw,
-        pl->logPT, (const cx<T>*)pl->d_filt);
+    if (pl->fft_bpt == 2)
+        ring_fft_inverse_kernel<T, 2><<<gfft, kFftThreads, pl->fft_smem, st>>>(
+            (const cx<T>*)pl->d_specOut, g.spec_total, (T*)d_out, g.npix, pl->d_rings, pl->d_fft_order, pl->d_lens,
+            (const cx<T>*)pl->d_tw, pl->logPT, (const cx<T>*)pl->d_filt, (const cx<T>*)pl->d_chirp, (const cx<T>*)pl->d_phase);
+    else
+        ring_fft_inverse_kernel<T, 4><<<gfft, kFftThreads, pl->fft_smem, st>>>(
+            (const cx<T>*)pl->d_specOut, g.spec_total, (T*)d_out, g.npix, pl->d_rings, pl->d_fft_order, pl->d_lens,
+            (const cx<T>*)pl->d_tw, pl->logPT, (const cx<T>*)pl->d_filt, (const cx<T>*)pl->d_chirp, (const cx<T>*)pl->d_phase);
     if (tm) cudaEventRecord(pl->ev[4], st);
     CUDA_TRY(cudaGetLastError());
     return 0;
@@ -528,7 +580,7 @@ int arkcos_plan_destroy(arkcos_plan* pl)
 {
     if (!pl) return ARKCOS_OK;
     void* ptrs[] = {pl->d_rings, pl->d_lens, pl->d_pairs, pl->d_north, pl->d_items[0], pl->d_items[1], pl->d_items[2], pl->d_items[3],
-                    pl->d_items[4], pl->d_eqchunks, pl->d_table, pl->d_tw, pl->d_filt,
+                    pl->d_items[4], pl->d_eqchunks, pl->d_chirp, pl->d_phase, pl->d_fft_order, pl->d_table, pl->d_tw, pl->d_filt,
                     pl->d_W, pl->d_specIn, pl->d_specOut, pl->d_stage_in, pl->d_stage_out};
     for (void* p : ptrs) if (p) cudaFree(p);
     for (auto& e : pl->ev) if (e) cudaEventDestroy(e);

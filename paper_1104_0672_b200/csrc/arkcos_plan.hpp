@@ -37,7 +37,7 @@ struct arkcos_plan {
     arkcos::HostGeometry g;
     arkcos::Stats stats;
 
-    int nnorth = 0, npairs = 0, nitems[arkcos::kBandClasses] = {0, 0, 0, 0, 0}, logPT = 0, fft_threads = 256;
+    int nnorth = 0, npairs = 0, nitems[arkcos::kBandClasses] = {0, 0, 0, 0, 0}, logPT = 0;
     size_t fft_smem = 0;
     int64_t nsamples = 0;
 
@@ -52,6 +52,10 @@ struct arkcos_plan {
     double* d_table = nullptr;
     void* d_tw = nullptr;        // cx<T>[PT/2]
     void* d_filt = nullptr;      // cx<T>[...] Bluestein filter spectra
+    void* d_chirp = nullptr;     // cx<T>[...] Bluestein chirps
+    void* d_phase = nullptr;     // cx<T>[...] exp(-i pi k / N) per ring length
+    int* d_fft_order = nullptr;  // rings by decreasing transform size
+    int fft_bpt = 2;
     void* d_W = nullptr;         // T[nsamples] kernel rows
     void* d_specIn = nullptr;    // cx<T>[max_nmaps][spec_total]
     void* d_specOut = nullptr;
