@@ -268,74 +268,102 @@ band_mac_uniform_kernel(const BandItem* __restrict__ items, const NorthRec* __re
 namespace arkcos {
 
 // ---- band kernel for runs of output rings whose pairs all live on one common grid (class E: N_i = N_j = M) -------------
-// HEALPix equatorial region and ECP (exact there).  A thread owns MT modes m for a whole chunk of
+// HEALPix equatorial region and ECP (exact there).  A thread owns MT modes m < M/2 for a whole chunk of
 // consecutive output rings: the cosines cos(m u pi / M) are built once per thread (exact sincospi each), every input-ring
 // coefficient Bp_j[m] is loaded once per tile of TI output rings and reused from registers, the rows of the tile sit
-// in shared memory.  No index arithmetic on the mode axis: m <= M/2 = N_j/2 needs no periodic extension.
+// in shared memory in a dense [ring of the tile][input ring] layout.  No index arithmetic on the mode axis: m < M/2 = N_j/2
+// needs no periodic extension.  (The Nyquist bin m = M/2 of these rings is left to band_mac_uniform_kernel.)
+// ALT = 1: the half-step parity of pair (i, j) is (i ^ j) & 1 (HEALPix: every other equatorial ring is shifted,
+// PAPER.md:125); ALT = 0: all rows sit on the integer grid (ECP).
 struct EqChunk { int i0, n; };
+constexpr int kEqJMax = kMaxPairs + 8;
 
-template <int TI, int MT, int TMAX>
+template <int TI, int MT, int TMAX, int ALT, int PAR>
+__device__ __forceinline__ void eq_accumulate(const float* __restrict__ sWj, const unsigned char* __restrict__ sCj,
+                                              const float (&ce)[MT][TMAX], const float (&co)[MT][TMAX],
+                                              const cx<float> (&v)[2][MT], cx<float> (&acc)[TI][2][MT])
+{
+#pragma unroll
+    for (int ii = 0; ii < TI; ++ii) {
+        const int c4 = sCj[ii * kEqJMax];
+        if (c4) {
+            const float4* __restrict__ w4 = reinterpret_cast<const float4*>(sWj + ii * (kEqJMax * TMAX));
+            const bool odd = ALT && ((PAR ^ ii) & 1) != 0;          // compile-time after unrolling
+            float G[MT];
+#pragma unroll
+            for (int mt = 0; mt < MT; ++mt) G[mt] = 0.f;
+#pragma unroll
+            for (int t4 = 0; t4 < TMAX / 4; ++t4) {
+                if (t4 < c4) {
+                    const float4 w = w4[t4];
+#pragma unroll
+                    for (int mt = 0; mt < MT; ++mt) {
+                        const float* c = odd ? co[mt] : ce[mt];
+                        G[mt] = fmaf(w.x, c[4 * t4], G[mt]); G[mt] = fmaf(w.y, c[4 * t4 + 1], G[mt]);
+                        G[mt] = fmaf(w.z, c[4 * t4 + 2], G[mt]); G[mt] = fmaf(w.w, c[4 * t4 + 3], G[mt]);
+                    }
+                }
+            }
+#pragma unroll
+            for (int h = 0; h < 2; ++h)
+#pragma unroll
+                for (int mt = 0; mt < MT; ++mt) {
+                    acc[ii][h][mt].x = fmaf(G[mt], v[h][mt].x, acc[ii][h][mt].x);
+                    acc[ii][h][mt].y = fmaf(G[mt], v[h][mt].y, acc[ii][h][mt].y);
+                }
+        }
+    }
+}
+
+template <int TI, int MT, int TMAX, int ALT>
 __global__ void __launch_bounds__(kBandThreads)
 band_mac_eq_kernel(const EqChunk* __restrict__ chunks, const NorthRec* __restrict__ north,
                    const PairRec* __restrict__ pairs, const float* __restrict__ W, const RingRec* __restrict__ rings,
                    int R, const cx<float>* __restrict__ specIn, cx<float>* __restrict__ specOut, int64_t spec_stride)
 {
-    __shared__ __align__(16) float sW[TI * kMaxPairs * TMAX];
-    __shared__ int sPair[TI * kMaxPairs];
-    __shared__ int2 sJ[kMaxPairs + TI];
-    __shared__ int4 sTile[TI];                 // pair index of the ring's first pair (relative), band_lo, band_hi, unused
+    __shared__ __align__(16) float sW[TI * kEqJMax * TMAX];       // [ii][jj][t]
+    __shared__ unsigned char sC[TI * kEqJMax];                     // [ii][jj]: row length / 4, 0 = no such pair
+    __shared__ int2 sJ[kEqJMax];                                   // spectrum offsets of input ring jlo + jj (N, S)
     const EqChunk ch = chunks[blockIdx.y];
     const int M = rings[ch.i0].n, Mh = M >> 1;
     int m[MT];
-    bool valid[MT];
     float ce[MT][TMAX], co[MT][TMAX];
 #pragma unroll
     for (int mt = 0; mt < MT; ++mt) {
         m[mt] = (int)blockIdx.x * (kBandThreads * MT) + mt * kBandThreads + (int)threadIdx.x;
-        valid[mt] = m[mt] <= Mh;
-        const uint32_t mm = valid[mt] ? (uint32_t)m[mt] : 0u, twoM = 2u * (uint32_t)M;
+        const uint32_t mm = (uint32_t)min(m[mt], Mh - 1), twoM = 2u * (uint32_t)M;
 #pragma unroll
         for (int t = 0; t < TMAX; ++t) {
             ce[mt][t] = cispi_ratio<float>((mm * (uint32_t)(2 * t)) % twoM, (uint32_t)M).x;
-            co[mt][t] = cispi_ratio<float>((mm * (uint32_t)(2 * t + 1)) % twoM, (uint32_t)M).x;
+            co[mt][t] = ALT ? cispi_ratio<float>((mm * (uint32_t)(2 * t + 1)) % twoM, (uint32_t)M).x : 0.f;
         }
     }
-    if ((int)blockIdx.x * (kBandThreads * MT) > Mh) return;
-    const cx<float>* __restrict__ in = specIn + (int64_t)blockIdx.z * spec_stride;
+    const cx<float>* __restrict__ inm[MT];
+#pragma unroll
+    for (int mt = 0; mt < MT; ++mt) inm[mt] = specIn + (int64_t)blockIdx.z * spec_stride + min(m[mt], Mh - 1);
     cx<float>* __restrict__ out = specOut + (int64_t)blockIdx.z * spec_stride;
 
     for (int tile = 0; tile < ch.n; tile += TI) {
         const int nti = min(TI, ch.n - tile), i0 = ch.i0 + tile;
-        __syncthreads();
         const int p_first = north[i0].pair_lo, p_last = north[i0 + nti - 1].pair_hi;
-        const int64_t wbase = pairs[p_first].woff;
-        const int jlo = pairs[p_first].j, jhi = pairs[p_last - 1].j;
-        {
-            const PairRec& pl = pairs[p_last - 1];
-            const int nw4 = (int)((pl.woff + ((pl.cnt + 3) & ~3) - wbase) >> 2);
-            const float4* __restrict__ src = reinterpret_cast<const float4*>(W + wbase);
-            float4* dst = reinterpret_cast<float4*>(sW);
-            for (int k = threadIdx.x; k < nw4; k += kBandThreads) dst[k] = src[k];
-            for (int p = p_first + threadIdx.x; p < p_last; p += kBandThreads) {
-                const PairRec& pr = pairs[p];
-                sPair[p - p_first] = ((int)(pr.woff - wbase) << 8) | (((pr.cnt + 3) & ~3) << 1) | pr.par;
-            }
-            for (int j = jlo + threadIdx.x; j <= jhi; j += kBandThreads)
-                sJ[j - jlo] = make_int2((int)rings[j].spec_off, (int)rings[R - 1 - j].spec_off);
-            if (threadIdx.x < nti) {
-                const NorthRec nr = north[i0 + threadIdx.x];
-                sTile[threadIdx.x] = make_int4(nr.pair_lo - p_first, pairs[nr.pair_lo].j, pairs[nr.pair_hi - 1].j, 0);
-            }
+        const int jlo = pairs[p_first].j, jw = pairs[p_last - 1].j - jlo + 1;
+        __syncthreads();
+        for (int k = threadIdx.x; k < TI * kEqJMax; k += kBandThreads) sC[k] = 0;
+        for (int jj = threadIdx.x; jj < jw; jj += kBandThreads)
+            sJ[jj] = make_int2((int)rings[jlo + jj].spec_off, (int)rings[R - 1 - jlo - jj].spec_off);
+        __syncthreads();
+        for (int k = threadIdx.x; k < (p_last - p_first) * (TMAX / 4); k += kBandThreads) {
+            const int p = p_first + k / (TMAX / 4), t4 = k % (TMAX / 4);
+            const PairRec& pr = pairs[p];
+            int ii = 0;                                                     // ring of the tile this pair belongs to
+#pragma unroll
+            for (int q = 1; q < TI; ++q) ii += (q < nti && p >= north[i0 + q].pair_lo) ? 1 : 0;
+            const int slot = ii * kEqJMax + (pr.j - jlo), c4 = (pr.cnt + 3) >> 2;
+            if (t4 < c4)
+                reinterpret_cast<float4*>(sW + slot * TMAX)[t4] = reinterpret_cast<const float4*>(W + pr.woff)[t4];
+            if (t4 == 0) sC[slot] = (unsigned char)c4;
         }
         __syncthreads();
-        int prel[TI], blo[TI], bhi[TI];
-#pragma unroll
-        for (int ii = 0; ii < TI; ++ii) {
-            const int4 tl = sTile[ii < nti ? ii : 0];
-            prel[ii] = tl.x;
-            blo[ii] = ii < nti ? tl.y : 1;
-            bhi[ii] = ii < nti ? tl.z : 0;        // empty band for the missing rings of a ragged last tile
-        }
         cx<float> acc[TI][2][MT];
 #pragma unroll
         for (int ii = 0; ii < TI; ++ii)
@@ -344,73 +372,37 @@ band_mac_eq_kernel(const EqChunk* __restrict__ chunks, const NorthRec* __restric
 #pragma unroll
                 for (int mt = 0; mt < MT; ++mt) acc[ii][h][mt] = mk<float>(0.f, 0.f);
 
-        for (int j = jlo; j <= jhi; ++j) {
-            const int2 off = sJ[j - jlo];
-            cx<float> v[2][MT];
+        cx<float> v[2][MT], vn[2][MT];
+        {
+            const int2 off = sJ[0];
 #pragma unroll
-            for (int mt = 0; mt < MT; ++mt) {
-                v[0][mt] = valid[mt] ? in[off.x + m[mt]] : mk<float>(0.f, 0.f);
-                v[1][mt] = valid[mt] ? in[off.y + m[mt]] : mk<float>(0.f, 0.f);
+            for (int mt = 0; mt < MT; ++mt) { vn[0][mt] = inm[mt][off.x]; vn[1][mt] = inm[mt][off.y]; }
+        }
+        for (int jj = 0; jj < jw; ++jj) {
+#pragma unroll
+            for (int mt = 0; mt < MT; ++mt) { v[0][mt] = vn[0][mt]; v[1][mt] = vn[1][mt]; }
+            {
+                const int2 off = sJ[min(jj + 1, jw - 1)];                  // prefetch the next input ring
+#pragma unroll
+                for (int mt = 0; mt < MT; ++mt) { vn[0][mt] = inm[mt][off.x]; vn[1][mt] = inm[mt][off.y]; }
             }
-#pragma unroll
-            for (int ii = 0; ii < TI; ++ii) {
-                if (j >= blo[ii] && j <= bhi[ii]) {
-                    const int pk = sPair[prel[ii] + j - blo[ii]];
-                    const float4* __restrict__ w4 = reinterpret_cast<const float4*>(sW + (pk >> 8));
-                    const int c4 = (pk >> 1) & 127;
-                    float G[MT];
-#pragma unroll
-                    for (int mt = 0; mt < MT; ++mt) G[mt] = 0.f;
-                    if (pk & 1) {
-#pragma unroll
-                        for (int t4 = 0; t4 < TMAX / 4; ++t4) {
-                            if (4 * t4 < c4) {
-                                const float4 w = w4[t4];
-#pragma unroll
-                                for (int mt = 0; mt < MT; ++mt) {
-                                    G[mt] = fmaf(w.x, co[mt][4 * t4], G[mt]); G[mt] = fmaf(w.y, co[mt][4 * t4 + 1], G[mt]);
-                                    G[mt] = fmaf(w.z, co[mt][4 * t4 + 2], G[mt]); G[mt] = fmaf(w.w, co[mt][4 * t4 + 3], G[mt]);
-                                }
-                            }
-                        }
-                    } else {
-#pragma unroll
-                        for (int t4 = 0; t4 < TMAX / 4; ++t4) {
-                            if (4 * t4 < c4) {
-                                const float4 w = w4[t4];
-#pragma unroll
-                                for (int mt = 0; mt < MT; ++mt) {
-                                    G[mt] = fmaf(w.x, ce[mt][4 * t4], G[mt]); G[mt] = fmaf(w.y, ce[mt][4 * t4 + 1], G[mt]);
-                                    G[mt] = fmaf(w.z, ce[mt][4 * t4 + 2], G[mt]); G[mt] = fmaf(w.w, ce[mt][4 * t4 + 3], G[mt]);
-                                }
-                            }
-                        }
-                    }
-#pragma unroll
-                    for (int h = 0; h < 2; ++h)
-#pragma unroll
-                        for (int mt = 0; mt < MT; ++mt) {
-                            acc[ii][h][mt].x = fmaf(G[mt], v[h][mt].x, acc[ii][h][mt].x);
-                            acc[ii][h][mt].y = fmaf(G[mt], v[h][mt].y, acc[ii][h][mt].y);
-                        }
-                }
-            }
+            const float* sWj = sW + jj * TMAX;
+            const unsigned char* sCj = sC + jj;
+            if (ALT && ((i0 ^ (jlo + jj)) & 1))
+                eq_accumulate<TI, MT, TMAX, ALT, 1>(sWj, sCj, ce, co, v, acc);
+            else
+                eq_accumulate<TI, MT, TMAX, ALT, 0>(sWj, sCj, ce, co, v, acc);
         }
 #pragma unroll
         for (int ii = 0; ii < TI; ++ii) {
             if (ii < nti) {
                 const int i = i0 + ii, iS = R - 1 - i;
-                const RingRec ri = rings[i];
-                const int64_t offS = rings[iS].spec_off;
+                const int64_t offN = rings[i].spec_off, offS = rings[iS].spec_off;
 #pragma unroll
                 for (int mt = 0; mt < MT; ++mt) {
-                    if (!valid[mt]) continue;
-                    cx<float> a = acc[ii][0][mt], b = acc[ii][1][mt];
-                    if (m[mt] == Mh) {              // +M/2 and -M/2 fold onto the same bin, half weight each
-                        if (ri.shifted) { a.x = 0.f; b.x = 0.f; } else { a.y = 0.f; b.y = 0.f; }
-                    }
-                    out[ri.spec_off + m[mt]] = a;
-                    if (iS != i) out[offS + m[mt]] = b;
+                    if (m[mt] >= Mh) continue;
+                    out[offN + m[mt]] = acc[ii][0][mt];
+                    if (iS != i) out[offS + m[mt]] = acc[ii][1][mt];
                 }
             }
         }

@@ -151,6 +151,7 @@ struct HostTables {
     std::vector<NorthRec> north;
     std::vector<BandItem> items[kBandClasses];
     std::vector<EqChunk> eq_chunks;              // runs of consecutive class-E rings for band_mac_eq_kernel   // per band-kernel class (see band_class)
+    int eq_alt = 0;
     std::vector<int> fft_order;          // rings sorted by decreasing transform size
     int64_t filt_total = 0, chirp_total = 0, ph_total = 0, nsamples = 0;
     int logPT = 1;
@@ -207,9 +208,11 @@ void build_fft_lens(const HostGeometry& g, HostTables& t, Stats& st)
 
 // Ring-pair table for the northern output rings (the southern ones reuse the rows of their mirror images).
 void build_pairs(HostGeometry& g, double theta_max, double ell_nyq, int fixed_mprime, int band_threads, bool allow_fast,
-                 HostTables& t, Stats& st)
+                 int sm_count, HostTables& t, Stats& st)
 {
-    const int R = g.R, nnorth = (R + 1) / 2, eq_chunk_rings = 32;
+    const int R = g.R, nnorth = (R + 1) / 2;
+    std::vector<int> eq_rings;
+    bool any_odd = false;
     const double shm = sin(0.5 * theta_max), xmax = 4.0 * shm * shm;
     g.mprime.assign(R, 0);
     const int nmax = *std::max_element(g.n.begin(), g.n.end());
@@ -218,6 +221,9 @@ void build_pairs(HostGeometry& g, double theta_max, double ell_nyq, int fixed_mp
         for (int j = g.band_lo[i]; j <= g.band_hi[i]; ++j) smax = std::max(smax, sin(g.theta[j]));
         g.mprime[i] = fixed_mprime > 0 ? fixed_mprime : std::max(8, 2 * (int)ceil(ell_nyq * smax));
     }
+    for (int i = 0; i < R; ++i) any_odd = any_odd || (g.n[i] == nmax && g.shifted[i] != g.shifted[std::min(i + 1, R - 1)] && g.n[std::min(i + 1, R - 1)] == nmax);
+    const int eq_alt = any_odd ? 1 : 0;
+    t.eq_alt = eq_alt;
     t.north.resize(nnorth);
     for (int i = 0; i < nnorth; ++i) {
         t.north[i].pair_lo = (int)t.pairs.size();
@@ -265,15 +271,14 @@ void build_pairs(HostGeometry& g, double theta_max, double ell_nyq, int fixed_mp
                 odd = odd || t.pairs[p].par;
                 maxcnt = std::max(maxcnt, t.pairs[p].cnt);
             }
-            bool all_e = same;
-            for (int p = lo; p < hi && all_e; ++p) all_e = t.pairs[p].M == g.n[i] && g.n[t.pairs[p].j] == g.n[i];
-            if (all_e && hi > lo && maxcnt <= 12 && g.spec_total < (int64_t)INT32_MAX) {
-                // extend the current chunk if this ring follows it directly, else open a new one
-                if (!t.eq_chunks.empty() && t.eq_chunks.back().i0 + t.eq_chunks.back().n == i &&
-                    t.eq_chunks.back().n < eq_chunk_rings && g.n[t.eq_chunks.back().i0] == g.n[i])
-                    ++t.eq_chunks.back().n;
-                else
-                    t.eq_chunks.push_back(EqChunk{i, 1});
+            bool all_e = same, alt_ok = true;
+            for (int p = lo; p < hi && all_e; ++p) {
+                all_e = t.pairs[p].M == g.n[i] && g.n[t.pairs[p].j] == g.n[i];
+                alt_ok = alt_ok && t.pairs[p].par == (eq_alt ? ((i ^ t.pairs[p].j) & 1) : 0);
+            }
+            if (all_e && alt_ok && hi > lo && maxcnt <= 12 && g.n[i] >= 8 && g.spec_total < (int64_t)INT32_MAX) {
+                eq_rings.push_back(i);
+                t.items[1].push_back(BandItem{i, g.n[i] / 2});      // the Nyquist bin m = M/2 goes to the uniform kernel
                 continue;
             }
             if (same && hi > lo) {
@@ -283,6 +288,21 @@ void build_pairs(HostGeometry& g, double theta_max, double ell_nyq, int fixed_mp
             }
         }
         for (int m0 = 0; m0 <= g.n[i] / 2; m0 += band_threads) t.items[cls].push_back(BandItem{i, m0});
+    }
+    // chunks of consecutive class-E rings: about one block per resident slot of the device (4 blocks per SM)
+    {
+        const int mh = eq_rings.empty() ? 0 : g.n[eq_rings[0]] / 2;
+        const int gx = std::max(1, (mh + kBandThreads * 2 - 1) / (kBandThreads * 2));
+        const int target = std::max(1, (4 * sm_count) / gx);
+        const int chn = std::max(8, ((int)eq_rings.size() + target - 1) / target);
+        for (size_t k = 0; k < eq_rings.size(); ++k) {
+            const int i = eq_rings[k];
+            if (!t.eq_chunks.empty() && t.eq_chunks.back().i0 + t.eq_chunks.back().n == i && t.eq_chunks.back().n < chn &&
+                g.n[t.eq_chunks.back().i0] == g.n[i])
+                ++t.eq_chunks.back().n;
+            else
+                t.eq_chunks.push_back(EqChunk{i, 1});
+        }
     }
     st.row_samples = 0;
     for (const PairRec& p : t.pairs) st.row_samples += p.cnt;
@@ -386,15 +406,20 @@ void launch_uniform(const arkcos_plan* pl, int nmaps, cudaStream_t st)
 {
     if (pl->neqchunks > 0) {
         constexpr int TI = 4, MT = 2;
-        const unsigned gx = (unsigned)((pl->eq_mh + 1 + kBandThreads * MT - 1) / (kBandThreads * MT));
-        band_mac_eq_kernel<TI, MT, 12><<<dim3(gx, (unsigned)pl->neqchunks, (unsigned)nmaps), kBandThreads, 0, st>>>(
-            pl->d_eqchunks, pl->d_north, pl->d_pairs, (const float*)pl->d_W, pl->d_rings, pl->g.R,
-            (const cx<float>*)pl->d_specIn, (cx<float>*)pl->d_specOut, pl->g.spec_total);
+        const dim3 grid((unsigned)((pl->eq_mh + kBandThreads * MT - 1) / (kBandThreads * MT)), (unsigned)pl->neqchunks, (unsigned)nmaps);
+        if (pl->eq_alt)
+            band_mac_eq_kernel<TI, MT, 12, 1><<<grid, kBandThreads, 0, st>>>(
+                pl->d_eqchunks, pl->d_north, pl->d_pairs, (const float*)pl->d_W, pl->d_rings, pl->g.R,
+                (const cx<float>*)pl->d_specIn, (cx<float>*)pl->d_specOut, pl->g.spec_total);
+        else
+            band_mac_eq_kernel<TI, MT, 12, 0><<<grid, kBandThreads, 0, st>>>(
+                pl->d_eqchunks, pl->d_north, pl->d_pairs, (const float*)pl->d_W, pl->d_rings, pl->g.R,
+                (const cx<float>*)pl->d_specIn, (cx<float>*)pl->d_specOut, pl->g.spec_total);
     }
-    launch_uniform_class<12, true>(pl, 1, nmaps, st);
-    launch_uniform_class<12, false>(pl, 2, nmaps, st);
-    launch_uniform_class<20, false>(pl, 3, nmaps, st);
-    launch_uniform_class<32, true>(pl, 4, nmaps, st);
+    launch_uniform_class<12, false>(pl, 2, nmaps, pl->side[1]);
+    launch_uniform_class<20, false>(pl, 3, nmaps, pl->side[1]);
+    launch_uniform_class<32, true>(pl, 4, nmaps, pl->side[2]);
+    launch_uniform_class<12, true>(pl, 1, nmaps, pl->side[2]);
 }
 
 template <class T> int enqueue_convolve(const arkcos_plan* pl, const void* d_in, void* d_out, int nmaps, cudaStream_t st)
@@ -414,11 +439,18 @@ template <class T> int enqueue_convolve(const arkcos_plan* pl, const void* d_in,
             (const T*)d_in, g.npix, (cx<T>*)pl->d_specIn, g.spec_total, pl->d_rings, pl->d_fft_order, pl->d_lens,
             (const cx<T>*)pl->d_tw, pl->logPT, (const cx<T>*)pl->d_filt, (const cx<T>*)pl->d_chirp, (const cx<T>*)pl->d_phase);
     if (tm) cudaEventRecord(pl->ev[2], st);
+    // the band kernels of the different ring classes write disjoint rings: fork them onto the plan's side streams
+    cudaEventRecord(pl->ev_fork, st);
+    for (int k = 0; k < 3; ++k) cudaStreamWaitEvent(pl->side[k], pl->ev_fork, 0);
     if (pl->nitems[0] > 0)
-        band_mac_general_kernel<T, 16><<<dim3((unsigned)pl->nitems[0], (unsigned)nmaps), kBandThreads, 0, st>>>(
+        band_mac_general_kernel<T, 16><<<dim3((unsigned)pl->nitems[0], (unsigned)nmaps), kBandThreads, 0, pl->side[0]>>>(
             pl->d_items[0], pl->d_north, pl->d_pairs, (const T*)pl->d_W, pl->d_rings, g.R, (const cx<T>*)pl->d_specIn,
             (cx<T>*)pl->d_specOut, g.spec_total);
     launch_uniform(pl, nmaps, st);
+    for (int k = 0; k < 3; ++k) {
+        cudaEventRecord(pl->ev_join[k], pl->side[k]);
+        cudaStreamWaitEvent(st, pl->ev_join[k], 0);
+    }
     if (tm) cudaEventRecord(pl->ev[3], st);
     if (pl->fft_bpt == 2)
         ring_fft_inverse_kernel<T, 2><<<gfft, kFftThreads, pl->fft_smem, st>>>(
@@ -492,14 +524,17 @@ static int plan_create_impl(arkcos_plan** out, const arkcos_pixelization* pix, c
         else pl->ell_nyquist = opt.ell_nyquist > 0.0 ? opt.ell_nyquist
                                                      : auto_ell_nyquist(kernel->table, kernel->n, kernel->theta_max, 8.0 * pix->nside);
     }
+    int sm_count = 148;
+    if (!tables_only) CUDA_TRY(cudaDeviceGetAttribute(&sm_count, cudaDevAttrMultiProcessorCount, pl->device));
     HostTables t;
     build_fft_lens(pl->g, t, pl->stats);
-    build_pairs(pl->g, pl->theta_max, pl->ell_nyquist, fixed_mprime, kBandThreads, dtype == ARKCOS_F32 && !getenv("ARKCOS_FORCE_GENERAL"), t, pl->stats);
+    build_pairs(pl->g, pl->theta_max, pl->ell_nyquist, fixed_mprime, kBandThreads, dtype == ARKCOS_F32 && !getenv("ARKCOS_FORCE_GENERAL"), sm_count, t, pl->stats);
     if (t.pairs.size() > (size_t)INT32_MAX) return fail(ARKCOS_UNSUPPORTED, "too many ring pairs");
     pl->nnorth = (int)t.north.size();
     pl->npairs = (int)t.pairs.size();
     for (int c = 0; c < kBandClasses; ++c) pl->nitems[c] = (int)t.items[c].size();
     pl->neqchunks = (int)t.eq_chunks.size();
+    pl->eq_alt = t.eq_alt;
     pl->eq_mh = t.eq_chunks.empty() ? 0 : pl->g.n[t.eq_chunks[0].i0] / 2;
     for (const EqChunk& c : t.eq_chunks) pl->eq_mh = std::max(pl->eq_mh, pl->g.n[c.i0] / 2);
     pl->nsamples = t.nsamples;
@@ -522,6 +557,9 @@ static int plan_create_impl(arkcos_plan** out, const arkcos_pixelization* pix, c
     if (int rc = upload(&pl->d_table, tab, wsb)) return rc;
     if (int rc = dtype == ARKCOS_F32 ? build_device_numeric<float>(pl, t) : build_device_numeric<double>(pl, t)) return rc;
     for (auto& e : pl->ev) CUDA_TRY(cudaEventCreate(&e));
+    CUDA_TRY(cudaEventCreateWithFlags(&pl->ev_fork, cudaEventDisableTiming));
+    for (auto& e : pl->ev_join) CUDA_TRY(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+    for (auto& q : pl->side) CUDA_TRY(cudaStreamCreateWithFlags(&q, cudaStreamNonBlocking));
     if (opt.cache_kernel_rows) {
         dtype == ARKCOS_F32 ? enqueue_rows<float>(pl, 0) : enqueue_rows<double>(pl, 0);
         CUDA_TRY(cudaDeviceSynchronize());
@@ -584,6 +622,9 @@ int arkcos_plan_destroy(arkcos_plan* pl)
                     pl->d_W, pl->d_specIn, pl->d_specOut, pl->d_stage_in, pl->d_stage_out};
     for (void* p : ptrs) if (p) cudaFree(p);
     for (auto& e : pl->ev) if (e) cudaEventDestroy(e);
+    if (pl->ev_fork) cudaEventDestroy(pl->ev_fork);
+    for (auto& e : pl->ev_join) if (e) cudaEventDestroy(e);
+    for (auto& q : pl->side) if (q) cudaStreamDestroy(q);
     delete pl;
     return ARKCOS_OK;
 }

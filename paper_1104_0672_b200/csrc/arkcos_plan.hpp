@@ -47,7 +47,7 @@ struct arkcos_plan {
     arkcos::PairRec* d_pairs = nullptr;
     arkcos::NorthRec* d_north = nullptr;
     arkcos::EqChunk* d_eqchunks = nullptr;
-    int neqchunks = 0, eq_mh = 0;
+    int neqchunks = 0, eq_mh = 0, eq_alt = 0;
     arkcos::BandItem* d_items[arkcos::kBandClasses] = {nullptr, nullptr, nullptr, nullptr, nullptr};
     double* d_table = nullptr;
     void* d_tw = nullptr;        // cx<T>[PT/2]
@@ -65,4 +65,7 @@ struct arkcos_plan {
     // optional per-stage timing
     mutable int timing = 0;
     mutable cudaEvent_t ev[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
+    // fork/join of the band kernels of the different ring classes
+    cudaStream_t side[3] = {nullptr, nullptr, nullptr};
+    cudaEvent_t ev_fork = nullptr, ev_join[3] = {nullptr, nullptr, nullptr};
 };
