@@ -410,3 +410,71 @@ band_mac_eq_kernel(const EqChunk* __restrict__ chunks, const NorthRec* __restric
 }
 
 }  // namespace arkcos
+
+namespace arkcos {
+
+// ---- band kernel for short rings with long rows (the rings next to the poles) ----------------------------------------------
+// There a row covers the whole circle (cnt ~ M/2) and many unfolded modes fold onto each of the few output modes, so the
+// work is spread over the UNFOLDED modes: phase 1, one thread per m in [0, M/2]: T(m) = sum_j G_ij[m] Bp_j[m] into
+// shared memory; phase 2, one thread per folded mode m': the signed sum of T over m = m' + w N_i and w N_i - m'.
+// One block per output ring (and its mirror image); every pair of the ring has the same M.
+constexpr int kPoleThreads = 256;
+
+template <class T, int RESEED>
+__global__ void __launch_bounds__(kPoleThreads)
+band_mac_pole_kernel(const int* __restrict__ ring_list, const NorthRec* __restrict__ north,
+                     const PairRec* __restrict__ pairs, const T* __restrict__ W, const RingRec* __restrict__ rings,
+                     int R, const cx<T>* __restrict__ specIn, cx<T>* __restrict__ specOut, int64_t spec_stride)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cx<T>* sT = reinterpret_cast<cx<T>*>(smem_raw);             // [2][Mh + 1]
+    const int i = ring_list[blockIdx.x], iS = R - 1 - i;
+    const RingRec ri = rings[i];
+    const NorthRec nr = north[i];
+    const int M = pairs[nr.pair_lo].M, Mh = M >> 1, Ni = ri.n;
+    const cx<T>* __restrict__ in = specIn + (int64_t)blockIdx.y * spec_stride;
+    for (int m = threadIdx.x; m <= Mh; m += kPoleThreads) {
+        const cx<T> rot = cispi_ratio<T>((2u * (uint32_t)m) % (2u * (uint32_t)M), (uint32_t)M);
+        cx<T> tN = mk<T>(0, 0), tS = mk<T>(0, 0);
+        for (int p = nr.pair_lo; p < nr.pair_hi; ++p) {
+            const PairRec pr = pairs[p];
+            const T* __restrict__ w = W + pr.woff;
+            T G = 0;
+            for (int t0 = 0; t0 < pr.cnt; t0 += RESEED) {
+                const uint64_t q = ((uint64_t)m * (uint64_t)(2 * t0 + pr.par)) % (uint64_t)(2 * M);
+                cx<T> c = cispi_ratio<T>((uint32_t)q, (uint32_t)M);
+                const int t1 = min(pr.cnt, t0 + RESEED);
+                for (int t = t0; t < t1; ++t) {
+                    G += w[t] * c.x;
+                    c = cmul(c, rot);
+                }
+            }
+            const RingRec rj = rings[pr.j], rjS = rings[R - 1 - pr.j];
+            const cx<T> vN = ext_mode(in + rj.spec_off, m, rj.n, rj.shifted);
+            const cx<T> vS = ext_mode(in + rjS.spec_off, m, rjS.n, rjS.shifted);
+            tN.x += G * vN.x; tN.y += G * vN.y;
+            tS.x += G * vS.x; tS.y += G * vS.y;
+        }
+        if (2 * m == M) { tN = cscale(tN, (T)0.5); tS = cscale(tS, (T)0.5); }   // +-M/2 bins: half the Nyquist term each
+        sT[m] = tN;
+        sT[Mh + 1 + m] = tS;
+    }
+    __syncthreads();
+    cx<T>* __restrict__ out = specOut + (int64_t)blockIdx.y * spec_stride;
+    for (int mp = threadIdx.x; 2 * mp <= Ni; mp += kPoleThreads) {
+        cx<T> aN = mk<T>(0, 0), aS = mk<T>(0, 0);
+        for (int fam = 0; fam < 2; ++fam) {
+            int wi = fam;
+            for (int m = fam ? Ni - mp : mp; m <= Mh; m += Ni, ++wi) {
+                const T sg = (ri.shifted && (wi & 1)) ? (T)-1 : (T)1;        // exp(i m phi0_i) = (-1)^w exp(+-i m' phi0_i)
+                const cx<T> tN = sT[m], tS = sT[Mh + 1 + m];
+                aN.x += sg * tN.x; aN.y += (fam ? -sg : sg) * tN.y;
+                aS.x += sg * tS.x; aS.y += (fam ? -sg : sg) * tS.y;
+            }
+        }
+        out[ri.spec_off + mp] = aN;
+        if (iS != i) out[rings[iS].spec_off + mp] = aS;
+    }
+}
+
+}  // namespace arkcos

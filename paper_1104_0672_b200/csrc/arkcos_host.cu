@@ -143,6 +143,8 @@ double auto_ell_nyquist(const double* table, int ntab, double theta_max, double 
     return best > 0.0 ? best : ell_cap;
 }
 
+constexpr int kPoleMaxModes = 1024;   // longest unfolded spectrum (M/2 + 1) the pole kernel keeps in shared memory
+
 struct HostTables {
     std::vector<RingRec> rings;
     std::vector<FftLen> lens;
@@ -150,6 +152,8 @@ struct HostTables {
     std::vector<PairRec> pairs;
     std::vector<NorthRec> north;
     std::vector<BandItem> items[kBandClasses];
+    std::vector<int> pole_rings;                 // rings for band_mac_pole_kernel
+    int pole_mh = 0;
     std::vector<EqChunk> eq_chunks;              // runs of consecutive class-E rings for band_mac_eq_kernel   // per band-kernel class (see band_class)
     int eq_alt = 0;
     std::vector<int> fft_order;          // rings sorted by decreasing transform size
@@ -285,6 +289,16 @@ void build_pairs(HostGeometry& g, double theta_max, double ell_nyq, int fixed_mp
                 if (maxcnt <= 12) cls = odd ? 1 : 2;
                 else if (maxcnt <= 20 && !odd) cls = 3;
                 else if (maxcnt <= 32) cls = 4;
+            }
+        }
+        if (cls == 0 && t.north[i].pair_hi > t.north[i].pair_lo) {
+            bool same = true;
+            const int M0 = t.pairs[t.north[i].pair_lo].M;
+            for (int p = t.north[i].pair_lo; p < t.north[i].pair_hi; ++p) same = same && t.pairs[p].M == M0;
+            if (same && M0 / 2 + 1 <= kPoleMaxModes) {
+                t.pole_rings.push_back(i);
+                t.pole_mh = std::max(t.pole_mh, M0 / 2);
+                continue;
             }
         }
         for (int m0 = 0; m0 <= g.n[i] / 2; m0 += band_threads) t.items[cls].push_back(BandItem{i, m0});
@@ -446,6 +460,11 @@ template <class T> int enqueue_convolve(const arkcos_plan* pl, const void* d_in,
         band_mac_general_kernel<T, 16><<<dim3((unsigned)pl->nitems[0], (unsigned)nmaps), kBandThreads, 0, pl->side[0]>>>(
             pl->d_items[0], pl->d_north, pl->d_pairs, (const T*)pl->d_W, pl->d_rings, g.R, (const cx<T>*)pl->d_specIn,
             (cx<T>*)pl->d_specOut, g.spec_total);
+    if (pl->npole > 0)
+        band_mac_pole_kernel<T, 16><<<dim3((unsigned)pl->npole, (unsigned)nmaps), kPoleThreads,
+                                       2 * (size_t)(pl->pole_mh + 1) * sizeof(cx<T>), pl->side[0]>>>(
+            pl->d_pole, pl->d_north, pl->d_pairs, (const T*)pl->d_W, pl->d_rings, g.R, (const cx<T>*)pl->d_specIn,
+            (cx<T>*)pl->d_specOut, g.spec_total);
     launch_uniform(pl, nmaps, st);
     for (int k = 0; k < 3; ++k) {
         cudaEventRecord(pl->ev_join[k], pl->side[k]);
@@ -534,6 +553,8 @@ static int plan_create_impl(arkcos_plan** out, const arkcos_pixelization* pix, c
     pl->npairs = (int)t.pairs.size();
     for (int c = 0; c < kBandClasses; ++c) pl->nitems[c] = (int)t.items[c].size();
     pl->neqchunks = (int)t.eq_chunks.size();
+    pl->npole = (int)t.pole_rings.size();
+    pl->pole_mh = t.pole_mh;
     pl->eq_alt = t.eq_alt;
     pl->eq_mh = t.eq_chunks.empty() ? 0 : pl->g.n[t.eq_chunks[0].i0] / 2;
     for (const EqChunk& c : t.eq_chunks) pl->eq_mh = std::max(pl->eq_mh, pl->g.n[c.i0] / 2);
@@ -553,6 +574,7 @@ static int plan_create_impl(arkcos_plan** out, const arkcos_pixelization* pix, c
     for (int c = 0; c < kBandClasses; ++c)
         if (int rc = upload(&pl->d_items[c], t.items[c], wsb)) return rc;
     if (int rc = upload(&pl->d_eqchunks, t.eq_chunks, wsb)) return rc;
+    if (int rc = upload(&pl->d_pole, t.pole_rings, wsb)) return rc;
     std::vector<double> tab(kernel->table, kernel->table + kernel->n);
     if (int rc = upload(&pl->d_table, tab, wsb)) return rc;
     if (int rc = dtype == ARKCOS_F32 ? build_device_numeric<float>(pl, t) : build_device_numeric<double>(pl, t)) return rc;
@@ -618,7 +640,7 @@ int arkcos_plan_destroy(arkcos_plan* pl)
 {
     if (!pl) return ARKCOS_OK;
     void* ptrs[] = {pl->d_rings, pl->d_lens, pl->d_pairs, pl->d_north, pl->d_items[0], pl->d_items[1], pl->d_items[2], pl->d_items[3],
-                    pl->d_items[4], pl->d_eqchunks, pl->d_chirp, pl->d_phase, pl->d_fft_order, pl->d_table, pl->d_tw, pl->d_filt,
+                    pl->d_items[4], pl->d_eqchunks, pl->d_pole, pl->d_chirp, pl->d_phase, pl->d_fft_order, pl->d_table, pl->d_tw, pl->d_filt,
                     pl->d_W, pl->d_specIn, pl->d_specOut, pl->d_stage_in, pl->d_stage_out};
     for (void* p : ptrs) if (p) cudaFree(p);
     for (auto& e : pl->ev) if (e) cudaEventDestroy(e);

@@ -48,6 +48,8 @@ struct arkcos_plan {
     arkcos::NorthRec* d_north = nullptr;
     arkcos::EqChunk* d_eqchunks = nullptr;
     int neqchunks = 0, eq_mh = 0, eq_alt = 0;
+    int* d_pole = nullptr;
+    int npole = 0, pole_mh = 0;
     arkcos::BandItem* d_items[arkcos::kBandClasses] = {nullptr, nullptr, nullptr, nullptr, nullptr};
     double* d_table = nullptr;
     void* d_tw = nullptr;        // cx<T>[PT/2]
