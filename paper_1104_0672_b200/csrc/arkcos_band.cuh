@@ -141,13 +141,16 @@ constexpr int kBandThreads = 128;
 constexpr int kMaxPairs = 64;
 constexpr int kBandClasses = 5;   // 0: general kernel; 1..4: band_mac_uniform_kernel<12,odd>, <12>, <20>, <32,odd>
 
-struct PairMeta {
-    int64_t offN, offS;   // first coefficient of input ring j (north image) and of its mirror image
-    int Nj;
+struct __align__(16) PairMeta {
+    int offN, offS;       // first coefficient of input ring j (north image) and of its mirror image (element offsets)
     uint32_t magic;       // ceil(2^32 / Nj): m / Nj = umulhi(m, magic) for m < 2^15
-    int cnt;
-    int flags;            // bit 0: par, bit 1: ring j shifted
+    uint32_t info;        // bits 0-14: Nj - 1 ... see pack_info()
 };
+// info word: Nj (bits 0-15), ring j shifted (bit 16), par (bit 17), row length / 4 (bits 18-23)
+__host__ __device__ inline uint32_t pack_info(int Nj, int shifted, int par, int c4)
+{
+    return (uint32_t)Nj | ((uint32_t)shifted << 16) | ((uint32_t)par << 17) | ((uint32_t)c4 << 18);
+}
 
 template <int TMAX, bool HAS_ODD>
 __global__ void __launch_bounds__(kBandThreads)
@@ -170,19 +173,17 @@ band_mac_uniform_kernel(const BandItem* __restrict__ items, const NorthRec* __re
         const PairRec pr = pairs[nr.pair_lo + p];
         const RingRec rj = rings[pr.j], rjS = rings[R - 1 - pr.j];
         PairMeta pm;
-        pm.offN = rj.spec_off;
-        pm.offS = rjS.spec_off;
-        pm.Nj = rj.n;
+        pm.offN = (int)rj.spec_off;
+        pm.offS = (int)rjS.spec_off;
         pm.magic = (uint32_t)((0x100000000ull + (uint64_t)rj.n - 1ull) / (uint64_t)rj.n);
-        pm.cnt = pr.cnt;
-        pm.flags = pr.par | (rj.shifted << 1);
+        pm.info = pack_info(rj.n, rj.shifted, pr.par, (pr.cnt + 3) >> 2);
         sP[p] = pm;
         atomicMax(&sTneed, pr.cnt);
     }
-    for (int idx = threadIdx.x; idx < np * TMAX; idx += kBandThreads) {
-        const int p = idx / TMAX, t = idx - p * TMAX;
+    for (int idx = threadIdx.x; idx < np * (TMAX / 4); idx += kBandThreads) {
+        const int p = idx / (TMAX / 4), t4 = idx - p * (TMAX / 4);
         const PairRec& pr = pairs[nr.pair_lo + p];
-        sW[idx] = t < pr.cnt ? W[pr.woff + t] : 0.f;
+        if (4 * t4 < pr.cnt) reinterpret_cast<float4*>(sW + p * TMAX)[t4] = reinterpret_cast<const float4*>(W + pr.woff)[t4];
     }
     __syncthreads();
     const int Ni = ri.n, mp = it.m0 + (int)threadIdx.x;
@@ -201,32 +202,38 @@ band_mac_uniform_kernel(const BandItem* __restrict__ items, const NorthRec* __re
                 cx<float> c = mk<float>(1.f, 0.f), d = mk<float>(1.f, 0.f);
 #pragma unroll
                 for (int t = 0; t < TMAX; ++t) {
-                    if (t < tneed) {
-                        if ((t & 7) == 0) {
+                    if ((t & 7) == 0) {
+                        if (t < tneed) {
                             c = cispi_ratio<float>((2u * (uint32_t)m * (uint32_t)t) % twoM, (uint32_t)M);
                             if (HAS_ODD) d = cispi_ratio<float>(((uint32_t)m * (uint32_t)(2 * t + 1)) % twoM, (uint32_t)M);
-                        } else {
-                            c = cmul(c, rot);
-                            if (HAS_ODD) d = cmul(d, rot);
                         }
-                        ce[t] = c.x;
-                        if (HAS_ODD) co[t] = d.x;
                     } else {
-                        ce[t] = 0.f;
-                        if (HAS_ODD) co[t] = 0.f;
+                        c = cmul(c, rot);
+                        if (HAS_ODD) d = cmul(d, rot);
                     }
+                    ce[t] = c.x;
+                    if (HAS_ODD) co[t] = d.x;
                 }
             }
-            float gs = (2 * m == M) ? 0.5f : 1.f;                       // +-M/2 bins: half the Nyquist term each
-            if (ri.shifted && (wi & 1)) gs = -gs;                        // exp(i m phi0_i) = (-1)^w exp(+-i m' phi0_i)
+            // sign bits: half weight at the +-M/2 bins; exp(i m phi0_i) = (-1)^w exp(+-i m' phi0_i); conjugate family
+            const float gs = (2 * m == M) ? 0.5f : 1.f;
+            const uint32_t sgn_i = (ri.shifted && (wi & 1)) ? 0x80000000u : 0u;
+            const uint32_t sgn_fam = fam ? 0x80000000u : 0u;
+#pragma unroll 2
             for (int p = 0; p < np; ++p) {
                 const PairMeta pm = sP[p];
+                const int Nj = (int)(pm.info & 0xffffu), c4 = (int)(pm.info >> 18);
+                // periodic extension of the stored half spectra (same index for ring j and its mirror image)
+                const int wj = (int)__umulhi((uint32_t)m, pm.magic), r = m - wj * Nj;
+                const bool refl = 2 * r > Nj;
+                const int idx = refl ? Nj - r : r;
+                const cx<float> vN = in[pm.offN + idx], vS = in[pm.offS + idx];
                 const float4* __restrict__ w4 = reinterpret_cast<const float4*>(sW + p * TMAX);
                 float G = 0.f;
-                if (HAS_ODD && (pm.flags & 1)) {
+                if (HAS_ODD && (pm.info & (1u << 17))) {
 #pragma unroll
                     for (int t4 = 0; t4 < TMAX / 4; ++t4) {
-                        if (4 * t4 < pm.cnt) {
+                        if (t4 < c4) {
                             const float4 w = w4[t4];
                             G = fmaf(w.x, co[4 * t4], G); G = fmaf(w.y, co[4 * t4 + 1], G);
                             G = fmaf(w.z, co[4 * t4 + 2], G); G = fmaf(w.w, co[4 * t4 + 3], G);
@@ -235,7 +242,7 @@ band_mac_uniform_kernel(const BandItem* __restrict__ items, const NorthRec* __re
                 } else {
 #pragma unroll
                     for (int t4 = 0; t4 < TMAX / 4; ++t4) {
-                        if (4 * t4 < pm.cnt) {
+                        if (t4 < c4) {
                             const float4 w = w4[t4];
                             G = fmaf(w.x, ce[4 * t4], G); G = fmaf(w.y, ce[4 * t4 + 1], G);
                             G = fmaf(w.z, ce[4 * t4 + 2], G); G = fmaf(w.w, ce[4 * t4 + 3], G);
@@ -243,16 +250,12 @@ band_mac_uniform_kernel(const BandItem* __restrict__ items, const NorthRec* __re
                     }
                 }
                 G *= gs;
-                // periodic extension of the stored half spectra (same index for ring j and its mirror image)
-                const int wj = (int)__umulhi((uint32_t)m, pm.magic), r = m - wj * pm.Nj;
-                const bool refl = 2 * r > pm.Nj, shj = (pm.flags & 2) != 0;
-                const int idx = refl ? pm.Nj - r : r;
-                cx<float> vN = in[pm.offN + idx], vS = in[pm.offS + idx];
-                float sre = 1.f, sim = 1.f;                              // signs of (re, im) of the value used
-                if (refl) sim = -1.f;
-                if (shj && (refl != ((wj & 1) != 0))) { sre = -sre; sim = -sim; }
-                if (fam) sim = -sim;
-                const float gr = G * sre, gi = G * sim;
+                // value used = (+-re, +-im) of the stored coefficient: reflection conjugates, a shifted ring flips the sign
+                // on reflection and on every odd period, the second family conjugates again
+                const uint32_t shj = (pm.info >> 16) & 1u;
+                const uint32_t flip = (shj & ((refl ? 1u : 0u) ^ ((uint32_t)wj & 1u))) << 31;
+                const uint32_t sre = sgn_i ^ flip, sim = sre ^ (refl ? 0x80000000u : 0u) ^ sgn_fam;
+                const float gr = __uint_as_float(__float_as_uint(G) ^ sre), gi = __uint_as_float(__float_as_uint(G) ^ sim);
                 accN.x = fmaf(gr, vN.x, accN.x); accN.y = fmaf(gi, vN.y, accN.y);
                 accS.x = fmaf(gr, vS.x, accS.x); accS.y = fmaf(gi, vS.y, accS.y);
             }
