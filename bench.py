@@ -24,6 +24,7 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
 from paper_1104_0672_b200 import inputs  # noqa: E402
+from paper_1104_0672_b200.sharding import shard_range  # noqa: E402
 
 METRIC = "output Mpix/s per map at HEALPix Nside=2048"
 UNIT = "Mpix/s"
@@ -143,7 +144,8 @@ def run_ours(args):
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     c, tab, x, npix, nmaps, name = workload(args.cfg)
     if world > 1:                       # every rank its own map(s): same shape, different seed
-        x = inputs.white_noise_maps(npix, args.cfg, nmaps * world)[rank * nmaps:(rank + 1) * nmaps]
+        mine = shard_range(nmaps * world, world, rank)
+        x = np.stack([inputs.white_noise(npix, args.cfg, k) for k in mine])
     dtype = arkcos.F32
     t0 = time.perf_counter()
     plan = arkcos.Plan(c["pix"], tab, c["theta_max"], dtype, max_nmaps=nmaps)

@@ -43,9 +43,34 @@ template <class T> __device__ __forceinline__ void dft8(cx<T>* u)
     u[0] = a[0]; u[2] = a[1]; u[4] = a[2]; u[6] = a[3];
     u[1] = a[4]; u[3] = a[5]; u[5] = a[6]; u[7] = a[7];
 }
+template <class T> __device__ __forceinline__ void dft16(cx<T>* u)
+{
+    // 16 = 4 x 4: DFT4 over n1 (stride 4), twiddle exp(-2 pi i n0 k1 / 16), DFT4 over n0; X[k1 + 4 k0]
+    const T c1 = (T)0.92387953251128675613, s1 = (T)0.38268343236508977173, h = (T)0.70710678118654752440;
+    cx<T> a[4][4];
+#pragma unroll
+    for (int n0 = 0; n0 < 4; ++n0) {
+        cx<T> t[4] = {u[n0], u[n0 + 4], u[n0 + 8], u[n0 + 12]};
+        dft4(t);
+#pragma unroll
+        for (int k1 = 0; k1 < 4; ++k1) a[n0][k1] = t[k1];
+    }
+    // twiddles w^(n0 k1), w = exp(-i pi / 8)
+    const cx<T> w1 = mk<T>(c1, -s1), w2 = mk<T>(h, -h), w3 = mk<T>(s1, -c1), w6 = mk<T>(-h, -h), w9 = mk<T>(-c1, s1);
+    a[1][1] = cmul(a[1][1], w1); a[1][2] = cmul(a[1][2], w2); a[1][3] = cmul(a[1][3], w3);
+    a[2][1] = cmul(a[2][1], w2); a[2][2] = mul_mi(a[2][2]);   a[2][3] = cmul(a[2][3], w6);
+    a[3][1] = cmul(a[3][1], w3); a[3][2] = cmul(a[3][2], w6); a[3][3] = cmul(a[3][3], w9);
+#pragma unroll
+    for (int k1 = 0; k1 < 4; ++k1) {
+        cx<T> t[4] = {a[0][k1], a[1][k1], a[2][k1], a[3][k1]};
+        dft4(t);
+#pragma unroll
+        for (int k0 = 0; k0 < 4; ++k0) u[k1 + 4 * k0] = t[k0];
+    }
+}
 template <class T, int R> __device__ __forceinline__ void dftR(cx<T>* u)
 {
-    if (R == 8) dft8(u); else if (R == 4) dft4(u); else dft2(u);
+    if (R == 16) dft16(u); else if (R == 8) dft8(u); else if (R == 4) dft4(u); else dft2(u);
 }
 
 // One Stockham pass of radix R over the N = 2^logN points in s (padded indexing), p = 2^logp = product of the radices
@@ -53,15 +78,36 @@ template <class T, int R> __device__ __forceinline__ void dftR(cx<T>* u)
 template <class T, int R, int BPT>
 __device__ __forceinline__ void stockham_pass(cx<T>* s, int logN, int logp, const cx<T>* __restrict__ tw, int logPT)
 {
-    constexpr int logR = R == 8 ? 3 : (R == 4 ? 2 : 1);
+    constexpr int logR = R == 16 ? 4 : (R == 8 ? 3 : (R == 4 ? 2 : 1));
     const int nb = 1 << (logN - logR), p = 1 << logp;
+    const int sh = logPT - logp - logR;                     // exp(-2 pi i r k / (p R)) = tw[(r k) << sh]
     cx<T> u[BPT][R];
+    cx<T> w1[BPT], w2[BPT], w4[BPT], w8[BPT];
+    // twiddle loads first (global, L1-resident), so their latency overlaps the shared-memory gather
+#pragma unroll
+    for (int b = 0; b < BPT; ++b) {
+        const int i = (int)threadIdx.x + b * kFftThreads;
+        if (i < nb && logp > 0) {
+            const int k = i & (p - 1);
+            w1[b] = tw[k << sh];
+            if (R >= 4) w2[b] = tw[(2 * k) << sh];
+            if (R >= 8) w4[b] = tw[(4 * k) << sh];
+            if (R >= 16) w8[b] = tw[(8 * k) << sh];
+        }
+    }
+    const bool wide_in = nb >= 16, wide_out = p >= 16;      // strides that are multiples of 16 keep the padding affine
 #pragma unroll
     for (int b = 0; b < BPT; ++b) {
         const int i = (int)threadIdx.x + b * kFftThreads;
         if (i < nb) {
+            if (wide_in) {
+                const int base = phys(i), stride = nb + (nb >> 4);
 #pragma unroll
-            for (int r = 0; r < R; ++r) u[b][r] = s[phys(i + r * nb)];
+                for (int r = 0; r < R; ++r) u[b][r] = s[base + r * stride];
+            } else {
+#pragma unroll
+                for (int r = 0; r < R; ++r) u[b][r] = s[phys(i + r * nb)];
+            }
         }
     }
     __syncthreads();
@@ -71,24 +117,32 @@ __device__ __forceinline__ void stockham_pass(cx<T>* s, int logN, int logp, cons
         if (i < nb) {
             const int k = i & (p - 1);
             if (logp > 0) {
-                const int sh = logPT - logp - logR;             // exp(-2 pi i r k / (p R)) = tw[(r k) << sh]
-                if (R == 8) {
-                    const cx<T> w1 = tw[k << sh], w2 = tw[(2 * k) << sh], w4 = tw[(4 * k) << sh];
-                    const cx<T> w3 = cmul(w1, w2);
-                    u[b][1] = cmul(u[b][1], w1); u[b][2] = cmul(u[b][2], w2); u[b][3] = cmul(u[b][3], w3);
-                    u[b][4] = cmul(u[b][4], w4); u[b][5] = cmul(u[b][5], cmul(w4, w1));
-                    u[b][6] = cmul(u[b][6], cmul(w4, w2)); u[b][7] = cmul(u[b][7], cmul(w4, w3));
-                } else if (R == 4) {
-                    const cx<T> w1 = tw[k << sh], w2 = tw[(2 * k) << sh];
-                    u[b][1] = cmul(u[b][1], w1); u[b][2] = cmul(u[b][2], w2); u[b][3] = cmul(u[b][3], cmul(w1, w2));
-                } else {
-                    u[b][1] = cmul(u[b][1], tw[k << sh]);
+                cx<T> w[R];
+                w[1] = w1[b];
+                if (R >= 4) { w[2] = w2[b]; w[3] = cmul(w[1], w[2]); }
+                if (R >= 8) {
+                    w[4] = w4[b];
+#pragma unroll
+                    for (int r = 5; r < 8; ++r) w[r] = cmul(w[4], w[r - 4]);
                 }
+                if (R >= 16) {
+                    w[8] = w8[b];
+#pragma unroll
+                    for (int r = 9; r < 16; ++r) w[r] = cmul(w[8], w[r - 8]);
+                }
+#pragma unroll
+                for (int r = 1; r < R; ++r) u[b][r] = cmul(u[b][r], w[r]);
             }
             dftR<T, R>(u[b]);
             const int j = ((i - k) << logR) + k;
+            if (wide_out) {
+                const int base = phys(j), stride = p + (p >> 4);
 #pragma unroll
-            for (int q = 0; q < R; ++q) s[phys(j + q * p)] = u[b][q];
+                for (int q = 0; q < R; ++q) s[base + q * stride] = u[b][q];
+            } else {
+#pragma unroll
+                for (int q = 0; q < R; ++q) s[phys(j + q * p)] = u[b][q];
+            }
         }
     }
     __syncthreads();
@@ -96,10 +150,16 @@ __device__ __forceinline__ void stockham_pass(cx<T>* s, int logN, int logp, cons
 
 // Forward complex DFT, natural order in and out, of the 2^logN points in s (padded indexing), in place.
 // BPT >= 2^logN / (8 * kFftThreads).  s must be synchronised on entry; it is synchronised on return.
+// Radix plan: radix-8 passes, the remainder absorbed by radix-16 passes (3a+1 = 3(a-1)+4, 3a+2 = 3(a-2)+4+4).
 template <class T, int BPT> __device__ void fft_pow2(cx<T>* s, int logN, const cx<T>* __restrict__ tw, int logPT)
 {
+    constexpr int B16 = BPT > 1 ? BPT / 2 : 1;
     int logp = 0;
-    for (; logp + 3 <= logN; logp += 3) stockham_pass<T, 8, BPT>(s, logN, logp, tw, logPT);
+    int n16 = logN % 3;                                   // number of radix-16 passes wanted
+    if (logN < 4 * n16) n16 = 0;                          // too short: finish with a radix-4 / radix-2 pass instead
+    const int n8 = (logN - 4 * n16) / 3;
+    for (int a = 0; a < n8; ++a, logp += 3) stockham_pass<T, 8, BPT>(s, logN, logp, tw, logPT);
+    for (int a = 0; a < n16; ++a, logp += 4) stockham_pass<T, 16, B16>(s, logN, logp, tw, logPT);
     if (logN - logp == 2) stockham_pass<T, 4, 2 * BPT>(s, logN, logp, tw, logPT);
     else if (logN - logp == 1) stockham_pass<T, 2, 4 * BPT>(s, logN, logp, tw, logPT);
 }
@@ -138,7 +198,7 @@ __device__ void fft_len(cx<T>* s, const FftLen& f, const cx<T>* __restrict__ tw,
 // Plan time: filter spectrum of Bluestein's convolution, one length per block:
 // b[n] = exp(+i pi n^2 / L) for |n| < L placed circularly on P points; filt = FFT_P(b) / P.
 template <class T, int BPT>
-__global__ void __launch_bounds__(kFftThreads)
+__global__ void __launch_bounds__(kFftThreads, sizeof(T) == 4 ? 2 : 1)
 bluestein_filter_kernel(const FftLen* __restrict__ lens, const int* __restrict__ which, const cx<T>* __restrict__ tw,
                         int logPT, const cx<T>* __restrict__ chirp, cx<T>* __restrict__ filt)
 {
@@ -172,7 +232,7 @@ struct RingRec {
 // Step 1 + 2: Bp_j[k] = exp(-i k phi0_j) sum_l in(j,l) exp(-2 pi i k l / N_j), k = 0 .. N_j/2.
 // grid = (rings, nmaps); block b works on ring order[b] (longest transforms first).
 template <class T, int BPT>
-__global__ void __launch_bounds__(kFftThreads)
+__global__ void __launch_bounds__(kFftThreads, sizeof(T) == 4 ? 2 : 1)
 ring_fft_forward_kernel(const T* __restrict__ in, int64_t npix, cx<T>* __restrict__ spec, int64_t spec_stride,
                         const RingRec* __restrict__ rings, const int* __restrict__ order,
                         const FftLen* __restrict__ lens, const cx<T>* __restrict__ tw, int logPT,
@@ -209,7 +269,7 @@ ring_fft_forward_kernel(const T* __restrict__ in, int64_t npix, cx<T>* __restric
 // Step 6 + 7: out(i,k) = sum_{m'} D_i[m'] exp(2 pi i m' k / N_i) with D_i[m'] = exp(+i m' phi0_i) Dp_i[m'] for
 // m' = 0 .. N_i/2 and Hermitian symmetry for the rest.  grid = (rings, nmaps).
 template <class T, int BPT>
-__global__ void __launch_bounds__(kFftThreads)
+__global__ void __launch_bounds__(kFftThreads, sizeof(T) == 4 ? 2 : 1)
 ring_fft_inverse_kernel(const cx<T>* __restrict__ spec, int64_t spec_stride, T* __restrict__ outmap, int64_t npix,
                         const RingRec* __restrict__ rings, const int* __restrict__ order,
                         const FftLen* __restrict__ lens, const cx<T>* __restrict__ tw, int logPT,

@@ -79,3 +79,37 @@ def test_band_is_sufficient():
         rows = gamma[g.ring_slice(i)]
         reached = set(ring_of[np.nonzero((rows < tmax).any(axis=0))[0]].tolist())
         assert reached <= b
+
+
+def test_golden_paper_counts():
+    """The paper's own statements about the ring structure (tests/golden/healpix_counts_paper.txt)."""
+    import os
+    path = os.path.join(os.path.dirname(__file__), "golden", "healpix_counts_paper.txt")
+    for line in open(path):
+        if line.startswith("#") or not line.strip():
+            continue
+        nside, ncaps, nequ, nrings, ncoef, npix = map(int, line.split())
+        g = geometry.healpix_ring(nside)
+        assert ncaps == nside - 1 and nequ == 2 * nside + 1
+        assert g.nrings == nrings == 2 * ncaps + nequ and g.npix == npix
+        assert int((g.n == 4 * nside).sum()) == nequ and int(g.n.max()) // 2 + 1 == ncoef
+        assert list(g.n[:ncaps]) == [4 * n for n in range(1, nside)]
+
+
+def test_golden_point_source_regression():
+    """Oracle #1 against the stored response written by tests/golden/make_golden.py (oracle-only script)."""
+    import os
+    from oracle import direct
+    sys_path = os.path.join(os.path.dirname(__file__), "golden")
+    import importlib.util
+    spec = importlib.util.spec_from_file_location("make_golden", os.path.join(sys_path, "make_golden.py"))
+    mg = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(mg)
+    g = geometry.healpix_ring(mg.NSIDE)
+    x = np.zeros(g.npix)
+    x[mg.Q0] = 1.0
+    out = direct.direct_sum(g, mg.table(), mg.TMAX, x)
+    data = np.loadtxt(os.path.join(sys_path, "point_source_hp8.txt"))
+    ref = np.zeros(g.npix)
+    ref[data[:, 0].astype(int)] = data[:, 1]
+    np.testing.assert_allclose(out, ref, rtol=1e-13, atol=0)
