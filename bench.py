@@ -27,6 +27,9 @@ from paper_1104_0672_b200 import inputs  # noqa: E402
 from paper_1104_0672_b200.sharding import shard_range  # noqa: E402
 
 METRIC = "output Mpix/s per map at HEALPix Nside=2048"
+# dram__bytes_read.sum + dram__bytes_write.sum per launch (bytes) from the ncu --set full captures summarised in
+# profiles/ (config 4, one map); None where no capture exists
+TRAFFIC = {}
 UNIT = "Mpix/s"
 
 
@@ -213,28 +216,43 @@ def run_ours(args):
             dist.destroy_process_group()
         return
 
-    # roofline of the dominant kernel
+    # per-kernel durations: the band kernels normally overlap on side streams; timing mode 2 runs them one after the
+    # other with events in between (same launches, same stream torch handed us)
+    plan.set_timing(2)
+    band_ms = None
+    for _ in range(args.steps):
+        step()
+        cur = [b[2] for b in plan.band_kernels(with_timing=True)]
+        band_ms = cur if band_ms is None else [a + b for a, b in zip(band_ms, cur)]
+    band_info = plan.band_kernels()
+    plan.set_timing(False)
+    band_ms = [v / args.steps for v in band_ms]
+
+    # roofline of the dominant kernel (largest measured duration)
     peaks = {}
     try:
         peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
     except OSError:
         pass
     fp32_peak = arkcos.arkcos_probe_fp32_peak(10)
-    dominant = max(stage, key=stage.get)
-    if dominant == "band":
-        flops = stats["mac_flops"] * nmaps
-        ach = flops / (stage["band"] * 1e-3) / 1e12
-        roof = {"kernel": "band_mac", "bound": "alu", "achieved": ach, "peak": fp32_peak, "unit": "TFLOP/s",
-                "frac": ach / fp32_peak, "traffic": None,
-                "peak_source": "FFMA chain measured in this run (arkcos_probe_fp32_peak); nominal 148*128*2*1.965 GHz = 74.4"}
-    else:
-        hbm = float(peaks.get("hbm_gbs", 6650.0))
+    hbm = float(peaks.get("hbm_gbs", 6650.0))
+    hbm_src = "MEASURED_PEAKS.json hbm_gbs" if "hbm_gbs" in peaks else "fallback 6650 GB/s (B200_PROFILING.md)"
+    alu_src = "FFMA chain measured in this run (arkcos_probe_fp32_peak); nominal 148*128*2*1.965 GHz = 74.4"
+    kernels = []
+    for (kname, flops, _), ms_k in zip(band_info, band_ms):
+        if flops > 0:
+            ach = flops * nmaps / (ms_k * 1e-3) / 1e12
+            kernels.append({"kernel": kname, "ms": ms_k, "bound": "alu", "achieved": ach, "peak": fp32_peak,
+                            "unit": "TFLOP/s", "frac": ach / fp32_peak, "traffic": TRAFFIC.get(kname), "peak_source": alu_src})
+    for kname, key in (("ring_fft_forward_kernel", "fft_forward"), ("ring_fft_inverse_kernel", "fft_inverse")):
         byts = 2.0 * 4.0 * npix * nmaps           # a ring FFT reads and writes every map element once (4 B each way)
-        ach = byts / (stage[dominant] * 1e-3) / 1e9
-        roof = {"kernel": "ring_" + dominant, "bound": "hbm", "achieved": ach, "peak": hbm, "unit": "GB/s",
-                "frac": ach / hbm, "traffic": None,
-                "peak_source": "MEASURED_PEAKS.json hbm_gbs" if "hbm_gbs" in peaks else "fallback 6650 GB/s"}
+        ach = byts / (stage[key] * 1e-3) / 1e9
+        kernels.append({"kernel": kname, "ms": stage[key], "bound": "hbm", "achieved": ach, "peak": hbm, "unit": "GB/s",
+                        "frac": ach / hbm, "traffic": TRAFFIC.get(kname), "peak_source": hbm_src})
+    roof = dict(max(kernels, key=lambda k: k["ms"]))
     roof["stage_ms"] = stage
+    roof["all_kernels"] = [{k: v for k, v in kk.items() if k != "peak_source"} for kk in kernels]
+    launches_per_step = 3 + sum(1 for _, flops, _ in band_info if flops > 0)
 
     cpu = time_oracle(c, tab, x, args.oracle_rings)
     cpu_val = cpu["pixels"] * cpu["maps"] / cpu["seconds"] / 1e6
@@ -249,7 +267,7 @@ def run_ours(args):
             "cpu_baseline": {"value": cpu_val, "unit": UNIT, "cores": cpu["threads"], "kind": "oracle",
                              "sample": f"{cpu['rings']} of {cpu['nrings']} output rings evenly spaced in ring index, "
                                        f"{cpu['pixels']} pixels, {cpu['seconds']:.1f} s"},
-            "e2e": e2e, "gpu_launches": 4 * args.steps, "clocks": clocks,
+            "e2e": e2e, "gpu_launches": launches_per_step * args.steps, "clocks": clocks,
             "paper_context": "2.2 s on a GTX 480 incl. PCIe copies = 22.9 Mpix/s (PAPER.md:195)"}
     print(json.dumps(line))
     if world > 1:

@@ -60,6 +60,7 @@ SYMBOLS = {
                                   POINTER(c_int64)]),
     "arkcos_plan_set_timing": (c_int, [c_void_p, c_int]),
     "arkcos_plan_get_timing": (c_int, [c_void_p, POINTER(c_float)]),
+    "arkcos_plan_band_kernels": (c_int, [c_void_p, POINTER(c_int), POINTER(c_char_p), POINTER(c_double), POINTER(c_float)]),
     "arkcos_probe_fp32_peak": (c_int, [POINTER(c_double), c_int]),
     "arkcos_strerror": (c_char_p, [c_int]),
     "arkcos_last_error": (c_char_p, []),
@@ -162,8 +163,18 @@ class Plan:
         return dict(ring_pairs=rp.value, row_samples=rs.value, mac_flops=mf.value, fft_flops=ff.value,
                     workspace_bytes=ws.value)
 
-    def set_timing(self, enable: bool):
+    def set_timing(self, enable):
         _check(_lib().arkcos_plan_set_timing(self._h, int(enable)), "arkcos_plan_set_timing")
+
+    def band_kernels(self, with_timing: bool = False):
+        """[(name, model_flops, last_ms or None)] of the band kernels (timing needs set_timing(2) before the call)."""
+        n = c_int()
+        names = (c_char_p * 7)()
+        fl = (c_double * 7)()
+        ms = (c_float * 7)()
+        _check(_lib().arkcos_plan_band_kernels(self._h, byref(n), names, fl, ms if with_timing else None),
+               "arkcos_plan_band_kernels")
+        return [(names[k].decode(), fl[k], ms[k] if with_timing else None) for k in range(n.value)]
 
     def get_timing(self):
         ms = (c_float * 4)()

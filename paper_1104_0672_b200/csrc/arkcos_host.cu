@@ -231,6 +231,7 @@ void build_pairs(HostGeometry& g, double theta_max, double ell_nyq, int fixed_mp
     t.north.resize(nnorth);
     for (int i = 0; i < nnorth; ++i) {
         t.north[i].pair_lo = (int)t.pairs.size();
+        double ring_flops = 0.0;
         const bool has_mirror = (R - 1 - i) != i;
         for (int j = g.band_lo[i]; j <= g.band_hi[i]; ++j) {
             PairRec p{};
@@ -259,6 +260,7 @@ void build_pairs(HostGeometry& g, double theta_max, double ell_nyq, int fixed_mp
             t.nsamples += (p.cnt + 3) & ~3;          // rows are stored zero-padded to a multiple of four samples
             t.pairs.push_back(p);
             const double modes = p.M / 2 + 1;
+            ring_flops += modes * (2.0 * p.cnt + (has_mirror ? 8.0 : 4.0));
             st.mac_flops += modes * (2.0 * p.cnt + (has_mirror ? 8.0 : 4.0));
             st.ring_pairs += has_mirror ? 2 : 1;
         }
@@ -282,6 +284,7 @@ void build_pairs(HostGeometry& g, double theta_max, double ell_nyq, int fixed_mp
             }
             if (all_e && alt_ok && hi > lo && maxcnt <= 12 && g.n[i] >= 8 && g.spec_total < (int64_t)INT32_MAX) {
                 eq_rings.push_back(i);
+                st.band_flops[2] += ring_flops;
                 t.items[1].push_back(BandItem{i, g.n[i] / 2});      // the Nyquist bin m = M/2 goes to the uniform kernel
                 continue;
             }
@@ -297,10 +300,14 @@ void build_pairs(HostGeometry& g, double theta_max, double ell_nyq, int fixed_mp
             for (int p = t.north[i].pair_lo; p < t.north[i].pair_hi; ++p) same = same && t.pairs[p].M == M0;
             if (same && M0 / 2 + 1 <= kPoleMaxModes) {
                 t.pole_rings.push_back(i);
+                st.band_flops[1] += ring_flops;
                 t.pole_mh = std::max(t.pole_mh, M0 / 2);
                 continue;
             }
         }
+        // band-kernel slots: 0 general, 1 pole, 2 eq, 3 uniform<12>, 4 uniform<20>, 5 uniform<32,odd>, 6 uniform<12,odd>
+        static const int slot_of_cls[kBandClasses] = {0, 6, 3, 4, 5};
+        st.band_flops[slot_of_cls[cls]] += ring_flops;
         for (int m0 = 0; m0 <= g.n[i] / 2; m0 += band_threads) t.items[cls].push_back(BandItem{i, m0});
     }
     // chunks of consecutive class-E rings: about one block per resident slot of the device (4 blocks per SM)
@@ -416,8 +423,9 @@ template <int TMAX, bool HAS_ODD> void launch_uniform_class(const arkcos_plan* p
         (const cx<float>*)pl->d_specIn, (cx<float>*)pl->d_specOut, pl->g.spec_total);
 }
 
-void launch_uniform(const arkcos_plan* pl, int nmaps, cudaStream_t st)
+void launch_uniform(const arkcos_plan* pl, int nmaps, cudaStream_t st, bool serial)
 {
+    cudaStream_t s1 = serial ? st : pl->side[1], s2 = serial ? st : pl->side[2];
     if (pl->neqchunks > 0) {
         constexpr int TI = 4, MT = 2;
         const dim3 grid((unsigned)((pl->eq_mh + kBandThreads * MT - 1) / (kBandThreads * MT)), (unsigned)pl->neqchunks, (unsigned)nmaps);
@@ -430,10 +438,15 @@ void launch_uniform(const arkcos_plan* pl, int nmaps, cudaStream_t st)
                 pl->d_eqchunks, pl->d_north, pl->d_pairs, (const float*)pl->d_W, pl->d_rings, pl->g.R,
                 (const cx<float>*)pl->d_specIn, (cx<float>*)pl->d_specOut, pl->g.spec_total);
     }
-    launch_uniform_class<12, false>(pl, 2, nmaps, pl->side[1]);
-    launch_uniform_class<20, false>(pl, 3, nmaps, pl->side[1]);
-    launch_uniform_class<32, true>(pl, 4, nmaps, pl->side[2]);
-    launch_uniform_class<12, true>(pl, 1, nmaps, pl->side[2]);
+    if (serial) cudaEventRecord(pl->ev_band[3], st);
+    launch_uniform_class<12, false>(pl, 2, nmaps, s1);
+    if (serial) cudaEventRecord(pl->ev_band[4], st);
+    launch_uniform_class<20, false>(pl, 3, nmaps, s1);
+    if (serial) cudaEventRecord(pl->ev_band[5], st);
+    launch_uniform_class<32, true>(pl, 4, nmaps, s2);
+    if (serial) cudaEventRecord(pl->ev_band[6], st);
+    launch_uniform_class<12, true>(pl, 1, nmaps, s2);
+    if (serial) cudaEventRecord(pl->ev_band[7], st);
 }
 
 template <class T> int enqueue_convolve(const arkcos_plan* pl, const void* d_in, void* d_out, int nmaps, cudaStream_t st)
@@ -454,22 +467,31 @@ template <class T> int enqueue_convolve(const arkcos_plan* pl, const void* d_in,
             (const cx<T>*)pl->d_tw, pl->logPT, (const cx<T>*)pl->d_filt, (const cx<T>*)pl->d_chirp, (const cx<T>*)pl->d_phase);
     if (tm) cudaEventRecord(pl->ev[2], st);
     // the band kernels of the different ring classes write disjoint rings: fork them onto the plan's side streams
-    cudaEventRecord(pl->ev_fork, st);
-    for (int k = 0; k < 3; ++k) cudaStreamWaitEvent(pl->side[k], pl->ev_fork, 0);
+    // (timing mode 2: one after the other on the caller's stream with an event between them)
+    const bool serial = pl->timing == 2;
+    cudaStream_t s0 = serial ? st : pl->side[0];
+    if (!serial) {
+        cudaEventRecord(pl->ev_fork, st);
+        for (int k = 0; k < 3; ++k) cudaStreamWaitEvent(pl->side[k], pl->ev_fork, 0);
+    }
+    if (serial) cudaEventRecord(pl->ev_band[0], st);
     if (pl->nitems[0] > 0)
-        band_mac_general_kernel<T, 16><<<dim3((unsigned)pl->nitems[0], (unsigned)nmaps), kBandThreads, 0, pl->side[0]>>>(
+        band_mac_general_kernel<T, 16><<<dim3((unsigned)pl->nitems[0], (unsigned)nmaps), kBandThreads, 0, s0>>>(
             pl->d_items[0], pl->d_north, pl->d_pairs, (const T*)pl->d_W, pl->d_rings, g.R, (const cx<T>*)pl->d_specIn,
             (cx<T>*)pl->d_specOut, g.spec_total);
+    if (serial) cudaEventRecord(pl->ev_band[1], st);
     if (pl->npole > 0)
         band_mac_pole_kernel<T, 16><<<dim3((unsigned)pl->npole, (unsigned)nmaps), kPoleThreads,
-                                       2 * (size_t)(pl->pole_mh + 1) * sizeof(cx<T>), pl->side[0]>>>(
+                                       2 * (size_t)(pl->pole_mh + 1) * sizeof(cx<T>), s0>>>(
             pl->d_pole, pl->d_north, pl->d_pairs, (const T*)pl->d_W, pl->d_rings, g.R, (const cx<T>*)pl->d_specIn,
             (cx<T>*)pl->d_specOut, g.spec_total);
-    launch_uniform(pl, nmaps, st);
-    for (int k = 0; k < 3; ++k) {
-        cudaEventRecord(pl->ev_join[k], pl->side[k]);
-        cudaStreamWaitEvent(st, pl->ev_join[k], 0);
-    }
+    if (serial) cudaEventRecord(pl->ev_band[2], st);
+    launch_uniform(pl, nmaps, st, serial);
+    if (!serial)
+        for (int k = 0; k < 3; ++k) {
+            cudaEventRecord(pl->ev_join[k], pl->side[k]);
+            cudaStreamWaitEvent(st, pl->ev_join[k], 0);
+        }
     if (tm) cudaEventRecord(pl->ev[3], st);
     if (pl->fft_bpt == 2)
         ring_fft_inverse_kernel<T, 2><<<gfft, kFftThreads, pl->fft_smem, st>>>(
@@ -579,6 +601,7 @@ static int plan_create_impl(arkcos_plan** out, const arkcos_pixelization* pix, c
     if (int rc = upload(&pl->d_table, tab, wsb)) return rc;
     if (int rc = dtype == ARKCOS_F32 ? build_device_numeric<float>(pl, t) : build_device_numeric<double>(pl, t)) return rc;
     for (auto& e : pl->ev) CUDA_TRY(cudaEventCreate(&e));
+    for (auto& e : pl->ev_band) CUDA_TRY(cudaEventCreate(&e));
     CUDA_TRY(cudaEventCreateWithFlags(&pl->ev_fork, cudaEventDisableTiming));
     for (auto& e : pl->ev_join) CUDA_TRY(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
     for (auto& q : pl->side) CUDA_TRY(cudaStreamCreateWithFlags(&q, cudaStreamNonBlocking));
@@ -644,6 +667,7 @@ int arkcos_plan_destroy(arkcos_plan* pl)
                     pl->d_W, pl->d_specIn, pl->d_specOut, pl->d_stage_in, pl->d_stage_out};
     for (void* p : ptrs) if (p) cudaFree(p);
     for (auto& e : pl->ev) if (e) cudaEventDestroy(e);
+    for (auto& e : pl->ev_band) if (e) cudaEventDestroy(e);
     if (pl->ev_fork) cudaEventDestroy(pl->ev_fork);
     for (auto& e : pl->ev_join) if (e) cudaEventDestroy(e);
     for (auto& q : pl->side) if (q) cudaStreamDestroy(q);
@@ -685,7 +709,7 @@ int arkcos_plan_stats(const arkcos_plan* pl, int64_t* ring_pairs, int64_t* row_s
 int arkcos_plan_set_timing(const arkcos_plan* pl, int enable)
 {
     if (!pl) return fail(ARKCOS_INVALID_ARG, "NULL plan");
-    pl->timing = enable ? 1 : 0;
+    pl->timing = enable == 2 ? 2 : (enable ? 1 : 0);
     return ARKCOS_OK;
 }
 
@@ -695,6 +719,25 @@ int arkcos_plan_get_timing(const arkcos_plan* pl, float* ms4)
     if (!pl->timing) return fail(ARKCOS_INVALID_ARG, "timing is not enabled");
     CUDA_TRY(cudaEventSynchronize(pl->ev[4]));
     for (int k = 0; k < 4; ++k) CUDA_TRY(cudaEventElapsedTime(&ms4[k], pl->ev[k], pl->ev[k + 1]));
+    return ARKCOS_OK;
+}
+
+int arkcos_plan_band_kernels(const arkcos_plan* pl, int* n, const char** names, double* model_flops, float* last_ms)
+{
+    static const char* kNames[7] = {"band_mac_general_kernel", "band_mac_pole_kernel", "band_mac_eq_kernel",
+                                    "band_mac_uniform_kernel<12,0>", "band_mac_uniform_kernel<20,0>",
+                                    "band_mac_uniform_kernel<32,1>", "band_mac_uniform_kernel<12,1>"};
+    if (!pl || !n) return fail(ARKCOS_INVALID_ARG, "NULL argument");
+    *n = 7;
+    for (int k = 0; k < 7; ++k) {
+        if (names) names[k] = kNames[k];
+        if (model_flops) model_flops[k] = pl->stats.band_flops[k];
+    }
+    if (last_ms) {
+        if (pl->timing != 2) return fail(ARKCOS_INVALID_ARG, "per-kernel timing needs arkcos_plan_set_timing(plan, 2)");
+        CUDA_TRY(cudaEventSynchronize(pl->ev_band[7]));
+        for (int k = 0; k < 7; ++k) CUDA_TRY(cudaEventElapsedTime(&last_ms[k], pl->ev_band[k], pl->ev_band[k + 1]));
+    }
     return ARKCOS_OK;
 }
 

@@ -23,6 +23,7 @@ struct HostGeometry {
 struct Stats {
     int64_t ring_pairs = 0, row_samples = 0, workspace_bytes = 0;
     double mac_flops = 0, fft_flops = 0;
+    double band_flops[7] = {0, 0, 0, 0, 0, 0, 0};   // per band kernel, see arkcos_plan_band_kernels
 };
 
 }  // namespace arkcos
@@ -67,6 +68,7 @@ struct arkcos_plan {
     // optional per-stage timing
     mutable int timing = 0;
     mutable cudaEvent_t ev[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
+    mutable cudaEvent_t ev_band[8] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
     // fork/join of the band kernels of the different ring classes
     cudaStream_t side[3] = {nullptr, nullptr, nullptr};
     cudaEvent_t ev_fork = nullptr, ev_join[3] = {nullptr, nullptr, nullptr};
