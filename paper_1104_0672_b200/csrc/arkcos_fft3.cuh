@@ -1,0 +1,339 @@
+// Ring FFTs, register-resident version for float rings whose transform size Q is 512 .. 4096 (steps 1+2 and 6+7 of the
+// hot path; "a real-to-complex Fourier transform ... on each ring", Eq. 8
+// "a complex-to-real backward FFT on all output rings").
+//
+// A ring of N reals is one complex FFT of length L = N/2 plus a split (as in arkcos_fft.cuh).  Here a thread keeps 16
+// points of the transform in registers: Q = 16 * 16 * RL (RL = Q/256 = 2..16) is done as radix-16, radix-16, radix-RL
+// Stockham passes with two shared-memory exchanges; T = Q/16 threads per block; every block runs TWO transforms of the
+// same size side by side so that twiddles and index arithmetic are paid once:
+//   * "direct" job  (L = Q a power of two: equatorial rings, ECP): two rings per block;
+//   * "Bluestein" job (any other L <= Q, the HEALPix cap rings N = 4i): one ring per block.  The cyclic convolution of
+//     length P = 2Q is split into its even and odd frequency bins,
+//         Y[2k] = FFT_Q(a)[k],  Y[2k+1] = FFT_Q(a[n] w_P^n)[k],     y[n] = E[n] + conj(w_P^n) O[n]  (n < Q),
+//     (a = chirped input, zero beyond L <= Q; only y[n < L] is needed), so that the two transforms of a block are the
+//     even and the odd half, the filter product needs no exchange (the output layout of one transform is the input
+//     layout of the next) and chirp, filter and half-bin phases are fused into the loads and stores.
+#pragma once
+#include "arkcos_fft.cuh"
+
+namespace arkcos {
+
+struct FftJob { int ring0, ring1; };          // direct: two rings (ring1 = -1: none); Bluestein: ring0 only
+
+template <int LOGQ> struct Fft3 {
+    static constexpr int Q = 1 << LOGQ, T = Q / 16, RL = Q / 256, NC = 16 / RL, SQ = Q + Q / 16;
+    static constexpr int MINB = 512 / T;
+    static constexpr size_t smem_bytes = 2 * (size_t)SQ * sizeof(cx<float>);
+};
+
+// w[r] = tw[r * idx], r = 1 .. R-1 (tw[k] = exp(-2 pi i k / PT)); at most one product per twiddle
+template <int R> __device__ __forceinline__ void load_tw(cx<float>* w, const cx<float>* __restrict__ tw, int idx)
+{
+    w[1] = tw[idx];
+    if (R >= 4) { w[2] = tw[2 * idx]; w[3] = tw[3 * idx]; }
+    if (R >= 8) {
+        w[4] = tw[4 * idx];
+#pragma unroll
+        for (int r = 5; r < 8; ++r) w[r] = cmul(w[4], w[r - 4]);
+    }
+    if (R >= 16) {
+        w[8] = tw[8 * idx];
+        w[12] = tw[12 * idx];
+#pragma unroll
+        for (int r = 9; r < 12; ++r) w[r] = cmul(w[8], w[r - 8]);
+#pragma unroll
+        for (int r = 13; r < 16; ++r) w[r] = cmul(w[12], w[r - 12]);
+    }
+}
+
+// Forward complex DFT of size Q of NB sequences held in registers: in  u[b][r] = x_b[t + T r],  out u[b][q] = X_b[t + T q].
+// s: NB arrays of SQ complex numbers (padded indexing e + e/16).  tw16[16 k + r] = exp(-2 pi i r k / 256).
+// Entry: any earlier readers of s must have passed a barrier.  Exit: results in registers, s free after the next barrier.
+template <int LOGQ, int NB>
+__device__ __forceinline__ void fft3(cx<float> (&u)[NB][16], cx<float>* __restrict__ s, const cx<float>* __restrict__ tw,
+                                     int logPT, const cx<float>* __restrict__ tw16)
+{
+    using F = Fft3<LOGQ>;
+    constexpr int T = F::T, RL = F::RL, NC = F::NC, SQ = F::SQ;
+    const int t = (int)threadIdx.x;
+    // pass 1: radix 16, no twiddles; butterfly t writes X[16 t + q]
+#pragma unroll
+    for (int b = 0; b < NB; ++b) {
+        dft16(u[b]);
+#pragma unroll
+        for (int q = 0; q < 16; ++q) s[b * SQ + 17 * t + q] = u[b][q];
+    }
+    // pass 2 twiddles: row k = t mod 16 of the 16 x 16 table
+    cx<float> w[16];
+    {
+        const float4* __restrict__ row = reinterpret_cast<const float4*>(tw16 + 16 * (t & 15));
+#pragma unroll
+        for (int r2 = 0; r2 < 8; ++r2) {
+            const float4 v = row[r2];
+            w[2 * r2] = mk<float>(v.x, v.y);
+            w[2 * r2 + 1] = mk<float>(v.z, v.w);
+        }
+    }
+    __syncthreads();
+    const int ld0 = t + (t >> 4);
+#pragma unroll
+    for (int b = 0; b < NB; ++b)
+#pragma unroll
+        for (int r = 0; r < 16; ++r) u[b][r] = s[b * SQ + ld0 + r * (T + T / 16)];
+    __syncthreads();
+    // pass 2: radix 16, p = 16; butterfly t writes X[16 (t - k) + k + 16 q]
+    {
+        const int k = t & 15, st0 = 17 * (t - k) + k;
+#pragma unroll
+        for (int b = 0; b < NB; ++b) {
+#pragma unroll
+            for (int r = 1; r < 16; ++r) u[b][r] = cmul(u[b][r], w[r]);
+            dft16(u[b]);
+#pragma unroll
+            for (int q = 0; q < 16; ++q) s[b * SQ + st0 + 17 * q] = u[b][q];
+        }
+    }
+    __syncthreads();
+#pragma unroll
+    for (int b = 0; b < NB; ++b)
+#pragma unroll
+        for (int r = 0; r < 16; ++r) u[b][r] = s[b * SQ + ld0 + r * (T + T / 16)];
+    // pass 3: radix RL, p = 256: butterflies i = t + T c, c < NC, on registers c + NC r'; output layout = input layout
+#pragma unroll
+    for (int c = 0; c < NC; ++c) {
+        const int i = t + T * c;
+        cx<float> wl[RL];
+        load_tw<RL>(wl, tw, i << (logPT - LOGQ));
+#pragma unroll
+        for (int b = 0; b < NB; ++b) {
+            cx<float> v[RL];
+            v[0] = u[b][c];
+#pragma unroll
+            for (int r = 1; r < RL; ++r) v[r] = cmul(u[b][c + NC * r], wl[r]);
+            dftR<float, RL>(v);
+#pragma unroll
+            for (int r = 0; r < RL; ++r) u[b][c + NC * r] = v[r];
+        }
+    }
+}
+
+}  // namespace arkcos
+
+namespace arkcos {
+
+// Asynchronous DRAM -> L2 prefetch of [p, p + bytes) (one thread issues it; 16-byte granularity).
+__device__ __forceinline__ void prefetch_l2(const void* p, uint32_t bytes)
+{
+    const uintptr_t a = (uintptr_t)p & ~(uintptr_t)15;
+    const uint32_t n = (uint32_t)(((uintptr_t)p + bytes + 15 - a) & ~(uintptr_t)15);
+    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(a), "r"(n) : "memory");
+}
+
+// X[k] of a real ring from the packed transform: zk = Z[k], zc = conj(Z[L-k]); h = exp(-i pi k / N).
+__device__ __forceinline__ cx<float> split_fwd(cx<float> zk, cx<float> zc, cx<float> h, int shifted)
+{
+    const cx<float> e = cscale(zk + zc, 0.5f), o = cscale(zk - zc, 0.5f);
+    const cx<float> wo = cmul(cmul(h, h), o);                  // exp(-2 pi i k / N) o
+    cx<float> X = mk<float>(e.x + wo.y, e.y - wo.x);           // e - i exp(-2 pi i k / N) o
+    if (shifted) X = cmul(X, h);                               // re-origin, Eq. 8
+    return X;
+}
+
+// conj(Z[k]) of the packed inverse transform from Dp[k] and Dp[L-k]; hk, hl = exp(+i pi k / N), exp(+i pi (L-k) / N).
+__device__ __forceinline__ cx<float> pack_inv(cx<float> xk, cx<float> xl, cx<float> hk, cx<float> hl, int shifted)
+{
+    if (shifted) { xk = cmul(xk, hk); xl = cmul(xl, hl); }
+    const cx<float> xc = cconj(xl);
+    const cx<float> a = xk + xc, d = xk - xc;
+    const cx<float> wd = cmul(cmul(hk, hk), d);                // exp(+2 pi i k / N) d
+    return mk<float>(a.x - wd.y, -(a.y + wd.x));               // conj(a + i wd)
+}
+
+// Bluestein middle part shared by both directions: u[0][r] = a[t + T r] (chirped input, zero beyond L) on entry;
+// on exit g[q] = conj(y[n]), n = t + T q, y = the cyclic convolution of a with the chirp filter (valid for n < L).
+template <int LOGQ>
+__device__ __forceinline__ void bluestein_core(cx<float> (&u)[2][16], cx<float>* __restrict__ s, const FftLen& f,
+                                               const cx<float>* __restrict__ tw, int logPT,
+                                               const cx<float>* __restrict__ tw16, const cx<float>* __restrict__ filt)
+{
+    using F = Fft3<LOGQ>;
+    constexpr int T = F::T;
+    const int t = (int)threadIdx.x, L = f.L;
+    const int shP = logPT - LOGQ - 1;                           // w_P^n = tw[n << shP], P = 2Q
+#pragma unroll
+    for (int r = 0; r < 16; ++r) {
+        const int n = t + T * r;
+        u[1][r] = n < L ? cmul(u[0][r], tw[n << shP]) : mk<float>(0.f, 0.f);
+    }
+    fft3<LOGQ, 2>(u, s, tw, logPT, tw16);
+    const float4* __restrict__ fl = reinterpret_cast<const float4*>(filt + f.filt_off);     // (F[2k], F[2k+1])
+#pragma unroll
+    for (int q = 0; q < 16; ++q) {
+        const float4 v = fl[t + T * q];
+        u[0][q] = cconj(cmul(u[0][q], mk<float>(v.x, v.y)));
+        u[1][q] = cconj(cmul(u[1][q], mk<float>(v.z, v.w)));
+    }
+    __syncthreads();
+    fft3<LOGQ, 2>(u, s, tw, logPT, tw16);                       // u[0] = conj(E), u[1] = conj(O)
+#pragma unroll
+    for (int q = 0; q < 16; ++q) {
+        const int n = t + T * q;
+        if (n < L) u[0][q] = u[0][q] + cmul(u[1][q], tw[n << shP]);          // conj(y) = conj(E) + w_P^n conj(O)
+    }
+}
+
+// Steps 1 + 2, rings with transform size Q.  grid = (jobs, nmaps), block = Q/16 threads.
+template <int LOGQ>
+__global__ void __launch_bounds__(Fft3<LOGQ>::T, Fft3<LOGQ>::MINB)
+ring_fft3_forward_kernel(const float* __restrict__ in, int64_t npix, cx<float>* __restrict__ spec, int64_t spec_stride,
+                         const RingRec* __restrict__ rings, const FftJob* __restrict__ jobs,
+                         const FftLen* __restrict__ lens, const cx<float>* __restrict__ tw, int logPT,
+                         const cx<float>* __restrict__ tw16, const cx<float>* __restrict__ filt,
+                         const cx<float>* __restrict__ chirp, const cx<float>* __restrict__ phase)
+{
+    using F = Fft3<LOGQ>;
+    constexpr int T = F::T, SQ = F::SQ;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cx<float>* s = reinterpret_cast<cx<float>*>(smem_raw);
+    const int t = (int)threadIdx.x;
+    const FftJob job = jobs[blockIdx.x];
+    const RingRec r0 = rings[job.ring0];
+    const FftLen f = lens[r0.len_id];
+    const int L = f.L;
+    const float* __restrict__ map = in + (int64_t)blockIdx.y * npix;
+    cx<float>* __restrict__ out = spec + (int64_t)blockIdx.y * spec_stride;
+    const cx<float>* __restrict__ ph = phase + f.ph_off;
+    cx<float> u[2][16];
+    if (f.pow2) {
+        const RingRec r1 = rings[job.ring1 >= 0 ? job.ring1 : job.ring0];
+        const cx<float>* __restrict__ x0 = reinterpret_cast<const cx<float>*>(map + r0.pix_off);
+        const cx<float>* __restrict__ x1 = reinterpret_cast<const cx<float>*>(map + r1.pix_off);
+#pragma unroll
+        for (int r = 0; r < 16; ++r) { u[0][r] = x0[t + T * r]; u[1][r] = x1[t + T * r]; }
+        fft3<LOGQ, 2>(u, s, tw, logPT, tw16);
+        __syncthreads();
+#pragma unroll
+        for (int b = 0; b < 2; ++b)
+#pragma unroll
+            for (int q = 0; q < 16; ++q) s[b * SQ + phys(t + T * q)] = u[b][q];
+        __syncthreads();
+#pragma unroll
+        for (int b = 0; b < 2; ++b) {
+            if (b == 1 && job.ring1 < 0) break;
+            const RingRec& rr = b ? r1 : r0;
+            cx<float>* __restrict__ o = out + rr.spec_off;
+#pragma unroll
+            for (int q = 0; q < 16; ++q) {
+                const int k = t + T * q;
+                const cx<float> zc = cconj(s[b * SQ + phys(k == 0 ? 0 : L - k)]);
+                o[k] = split_fwd(u[b][q], zc, ph[k], rr.shifted);
+            }
+            if (t == 0) o[L] = split_fwd(u[b][0], cconj(u[b][0]), ph[L], rr.shifted);
+        }
+    } else {
+        const cx<float>* __restrict__ x0 = reinterpret_cast<const cx<float>*>(map + r0.pix_off);
+        const cx<float>* __restrict__ cw = chirp + f.chirp_off;
+        if (t == 0) {
+            prefetch_l2(filt + f.filt_off, (uint32_t)(2 * F::Q * sizeof(cx<float>)));
+            prefetch_l2(ph, (uint32_t)((L + 1) * sizeof(cx<float>)));
+        }
+#pragma unroll
+        for (int r = 0; r < 16; ++r) {
+            const int n = t + T * r;
+            u[0][r] = n < L ? cmul(x0[n], cw[n]) : mk<float>(0.f, 0.f);
+        }
+        bluestein_core<LOGQ>(u, s, f, tw, logPT, tw16, filt);
+        // phases of the split: loaded now (into the registers of the odd half), used after the exchange
+#pragma unroll
+        for (int q = 0; q < 16; ++q) {
+            const int k = t + T * q;
+            u[1][q] = ph[k < L ? k : L];
+        }
+        __syncthreads();
+        // Z[n] = chirp[n] y[n]
+#pragma unroll
+        for (int q = 0; q < 16; ++q) {
+            const int n = t + T * q;
+            if (n < L) {
+                u[0][q] = cmul(cw[n], cconj(u[0][q]));
+                s[phys(n)] = u[0][q];
+            }
+        }
+        __syncthreads();
+        cx<float>* __restrict__ o = out + r0.spec_off;
+#pragma unroll
+        for (int q = 0; q < 16; ++q) {
+            const int k = t + T * q;
+            if (k < L) {
+                const cx<float> zc = cconj(s[phys(k == 0 ? 0 : L - k)]);
+                o[k] = split_fwd(u[0][q], zc, u[1][q], r0.shifted);
+            }
+        }
+        if (t == 0) o[L] = split_fwd(u[0][0], cconj(u[0][0]), ph[L], r0.shifted);
+    }
+}
+
+// Steps 6 + 7, rings with transform size Q.  grid = (jobs, nmaps), block = Q/16 threads.
+template <int LOGQ>
+__global__ void __launch_bounds__(Fft3<LOGQ>::T, Fft3<LOGQ>::MINB)
+ring_fft3_inverse_kernel(const cx<float>* __restrict__ spec, int64_t spec_stride, float* __restrict__ outmap, int64_t npix,
+                         const RingRec* __restrict__ rings, const FftJob* __restrict__ jobs,
+                         const FftLen* __restrict__ lens, const cx<float>* __restrict__ tw, int logPT,
+                         const cx<float>* __restrict__ tw16, const cx<float>* __restrict__ filt,
+                         const cx<float>* __restrict__ chirp, const cx<float>* __restrict__ phase)
+{
+    using F = Fft3<LOGQ>;
+    constexpr int T = F::T;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cx<float>* s = reinterpret_cast<cx<float>*>(smem_raw);
+    const int t = (int)threadIdx.x;
+    const FftJob job = jobs[blockIdx.x];
+    const RingRec r0 = rings[job.ring0];
+    const FftLen f = lens[r0.len_id];
+    const int L = f.L;
+    const cx<float>* __restrict__ D = spec + (int64_t)blockIdx.y * spec_stride;
+    float* __restrict__ map = outmap + (int64_t)blockIdx.y * npix;
+    const cx<float>* __restrict__ ph = phase + f.ph_off;
+    cx<float> u[2][16];
+    if (f.pow2) {
+        const RingRec r1 = rings[job.ring1 >= 0 ? job.ring1 : job.ring0];
+#pragma unroll
+        for (int r = 0; r < 16; ++r) {
+            const int k = t + T * r;
+            const cx<float> hk = cconj(ph[k]), hl = cconj(ph[L - k]);
+            u[0][r] = pack_inv(D[r0.spec_off + k], D[r0.spec_off + L - k], hk, hl, r0.shifted);
+            u[1][r] = pack_inv(D[r1.spec_off + k], D[r1.spec_off + L - k], hk, hl, r1.shifted);
+        }
+        fft3<LOGQ, 2>(u, s, tw, logPT, tw16);
+        cx<float>* __restrict__ o0 = reinterpret_cast<cx<float>*>(map + r0.pix_off);
+        cx<float>* __restrict__ o1 = reinterpret_cast<cx<float>*>(map + r1.pix_off);
+#pragma unroll
+        for (int q = 0; q < 16; ++q) {
+            o0[t + T * q] = cconj(u[0][q]);
+            if (job.ring1 >= 0) o1[t + T * q] = cconj(u[1][q]);
+        }
+    } else {
+        const cx<float>* __restrict__ cw = chirp + f.chirp_off;
+        if (t == 0) prefetch_l2(filt + f.filt_off, (uint32_t)(2 * F::Q * sizeof(cx<float>)));
+#pragma unroll
+        for (int r = 0; r < 16; ++r) {
+            const int k = t + T * r;
+            cx<float> v = mk<float>(0.f, 0.f);
+            if (k < L) {
+                const cx<float> hk = cconj(ph[k]), hl = cconj(ph[L - k]);
+                v = cmul(pack_inv(D[r0.spec_off + k], D[r0.spec_off + L - k], hk, hl, r0.shifted), cw[k]);
+            }
+            u[0][r] = v;
+        }
+        bluestein_core<LOGQ>(u, s, f, tw, logPT, tw16, filt);
+        // z'[n] = chirp[n] y[n]; out = conj(z') = conj(chirp[n]) conj(y[n])
+        cx<float>* __restrict__ o0 = reinterpret_cast<cx<float>*>(map + r0.pix_off);
+#pragma unroll
+        for (int q = 0; q < 16; ++q) {
+            const int n = t + T * q;
+            if (n < L) o0[n] = cmulc(u[0][q], cw[n]);
+        }
+    }
+}
+
+}  // namespace arkcos

@@ -156,13 +156,14 @@ struct HostTables {
     int pole_mh = 0;
     std::vector<EqChunk> eq_chunks;              // runs of consecutive class-E rings for band_mac_eq_kernel   // per band-kernel class (see band_class)
     int eq_alt = 0;
-    std::vector<int> fft_order;          // rings sorted by decreasing transform size
+    std::vector<int> fft_order;          // rings of the shared-memory FFT kernels, sorted by decreasing transform size
+    std::vector<FftJob> fft3_jobs[4];    // jobs of the register-resident FFT kernels, Q = 512 << k
     int64_t filt_total = 0, chirp_total = 0, ph_total = 0, nsamples = 0;
     int logPT = 1;
 };
 
 // FFT length table: one entry per distinct ring length
-void build_fft_lens(const HostGeometry& g, HostTables& t, Stats& st)
+void build_fft_lens(const HostGeometry& g, HostTables& t, Stats& st, bool use_fft3)
 {
     std::map<int, int> id_of;
     t.rings.resize(g.R);
@@ -201,8 +202,32 @@ void build_fft_lens(const HostGeometry& g, HostTables& t, Stats& st)
         // forward + inverse: complex FFT(s) + O(N) split / chirps
         st.fft_flops += 2.0 * (f.pow2 ? 5.0 * P * f.logP + 20.0 * L : 2.0 * 5.0 * P * f.logP + 6.0 * P + 32.0 * L);
     }
-    t.fft_order.resize(g.R);
-    for (int i = 0; i < g.R; ++i) t.fft_order[i] = i;
+    // Rings whose transform size Q (L for a power of two, half the Bluestein convolution length otherwise) is 512 .. 4096
+    // go to the register-resident kernels: Bluestein rings first, a ring next to its mirror image (same tables), then
+    // the power-of-two rings two per block.  Everything else stays with the shared-memory kernels.
+    std::vector<int> direct[4];
+    std::vector<char> taken(g.R, 0);
+    auto cls_of = [&](int i) {
+        const FftLen& f = t.lens[t.rings[i].len_id];
+        const int logq = f.pow2 ? f.logP : f.logP - 1;
+        return (use_fft3 && logq >= 9 && logq <= 12) ? logq - 9 : -1;
+    };
+    for (int i = g.R / 2; i >= 0; --i) {                 // longest rings first
+        const int twin[2] = {i, g.R - 1 - i};
+        for (int h = 0; h < 2; ++h) {
+            const int r = twin[h];
+            const int c = cls_of(r);
+            if (c < 0 || taken[r]) continue;
+            taken[r] = 1;
+            if (t.lens[t.rings[r].len_id].pow2) direct[c].push_back(r);
+            else t.fft3_jobs[c].push_back(FftJob{r, -1});
+        }
+    }
+    for (int c = 0; c < 4; ++c)
+        for (size_t k = 0; k < direct[c].size(); k += 2)
+            t.fft3_jobs[c].push_back(FftJob{direct[c][k], k + 1 < direct[c].size() ? direct[c][k + 1] : -1});
+    for (int i = 0; i < g.R; ++i)
+        if (!taken[i]) t.fft_order.push_back(i);
     std::stable_sort(t.fft_order.begin(), t.fft_order.end(), [&](int a, int b) {
         const FftLen &fa = t.lens[t.rings[a].len_id], &fb = t.lens[t.rings[b].len_id];
         const int wa = (fa.pow2 ? 1 : 2) << fa.logP, wb = (fb.pow2 ? 1 : 2) << fb.logP;
@@ -347,6 +372,35 @@ template <class T, int BPT> int set_fft_smem(size_t bytes)
     return 0;
 }
 
+template <int LOGQ> int set_fft3_smem()
+{
+    CUDA_TRY(cudaFuncSetAttribute(ring_fft3_forward_kernel<LOGQ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Fft3<LOGQ>::smem_bytes));
+    CUDA_TRY(cudaFuncSetAttribute(ring_fft3_inverse_kernel<LOGQ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Fft3<LOGQ>::smem_bytes));
+    return 0;
+}
+
+// job lists and the 16 x 16 twiddle table of the register-resident FFT kernels (float plans only)
+template <class T> int setup_fft3(arkcos_plan* pl, const HostTables& t)
+{
+    if (sizeof(T) != 4) return 0;
+    for (int c = 0; c < 4; ++c) {
+        pl->nfft3[c] = (int)t.fft3_jobs[c].size();
+        if (int rc = upload(&pl->d_fft3_jobs[c], t.fft3_jobs[c], &pl->stats.workspace_bytes)) return rc;
+    }
+    std::vector<cx<float>> tw16(256);
+    for (int k = 0; k < 16; ++k)
+        for (int r = 0; r < 16; ++r)
+            tw16[16 * k + r] = mk<float>((float)cos(2.0 * kPi * r * k / 256.0), (float)(-sin(2.0 * kPi * r * k / 256.0)));
+    cx<float>* d = nullptr;
+    if (int rc = upload(&d, tw16, &pl->stats.workspace_bytes)) return rc;
+    pl->d_tw16 = d;
+    if (int rc = set_fft3_smem<9>()) return rc;
+    if (int rc = set_fft3_smem<10>()) return rc;
+    if (int rc = set_fft3_smem<11>()) return rc;
+    if (int rc = set_fft3_smem<12>()) return rc;
+    return 0;
+}
+
 // twiddles, chirps and phases from double precision, Bluestein filters by a plan-time kernel, workspace
 template <class T> int build_device_numeric(arkcos_plan* pl, const HostTables& t)
 {
@@ -373,6 +427,8 @@ template <class T> int build_device_numeric(arkcos_plan* pl, const HostTables& t
     if (int rc = upload(&d_phase, phase, &pl->stats.workspace_bytes)) return rc;
     pl->d_phase = d_phase;
     if (int rc = upload(&pl->d_fft_order, t.fft_order, &pl->stats.workspace_bytes)) return rc;
+    pl->nfft_old = (int)t.fft_order.size();
+    if (int rc = setup_fft3<T>(pl, t)) return rc;
     pl->fft_smem = fft_smem_elems(PT) * sizeof(cx<T>);
     pl->fft_bpt = PT <= 8 * kFftThreads * 2 ? 2 : 4;
     if (pl->fft_smem > 227 * 1024 || PT > 8 * kFftThreads * 4) return fail(ARKCOS_UNSUPPORTED, "ring too long for the shared-memory FFT");
@@ -449,6 +505,75 @@ void launch_uniform(const arkcos_plan* pl, int nmaps, cudaStream_t st, bool seri
     if (serial) cudaEventRecord(pl->ev_band[7], st);
 }
 
+// Ring FFTs of one direction (FWD: map -> specIn, else specOut -> map).  Float plans: one launch per transform size of the
+// register-resident kernels (the largest on the caller's stream, the others forked onto the plan's side streams, they
+// touch disjoint rings) plus the shared-memory kernel for whatever is left (very short or very long rings).
+template <int LOGQ, bool FWD>
+void launch_fft3(const arkcos_plan* pl, const void* d_in, void* d_out, int nmaps, cudaStream_t st)
+{
+    const int c = LOGQ - 9;
+    if (pl->nfft3[c] == 0) return;
+    const dim3 grid((unsigned)pl->nfft3[c], (unsigned)nmaps);
+    const HostGeometry& g = pl->g;
+    if (FWD)
+        ring_fft3_forward_kernel<LOGQ><<<grid, Fft3<LOGQ>::T, Fft3<LOGQ>::smem_bytes, st>>>(
+            (const float*)d_in, g.npix, (cx<float>*)pl->d_specIn, g.spec_total, pl->d_rings, pl->d_fft3_jobs[c], pl->d_lens,
+            (const cx<float>*)pl->d_tw, pl->logPT, (const cx<float>*)pl->d_tw16, (const cx<float>*)pl->d_filt,
+            (const cx<float>*)pl->d_chirp, (const cx<float>*)pl->d_phase);
+    else
+        ring_fft3_inverse_kernel<LOGQ><<<grid, Fft3<LOGQ>::T, Fft3<LOGQ>::smem_bytes, st>>>(
+            (const cx<float>*)pl->d_specOut, g.spec_total, (float*)d_out, g.npix, pl->d_rings, pl->d_fft3_jobs[c], pl->d_lens,
+            (const cx<float>*)pl->d_tw, pl->logPT, (const cx<float>*)pl->d_tw16, (const cx<float>*)pl->d_filt,
+            (const cx<float>*)pl->d_chirp, (const cx<float>*)pl->d_phase);
+}
+
+template <class T, bool FWD>
+void launch_ring_ffts(const arkcos_plan* pl, const void* d_in, void* d_out, int nmaps, cudaStream_t st)
+{
+    const HostGeometry& g = pl->g;
+    bool forked = false;
+    if constexpr (sizeof(T) == 4) {
+        const int nside_launches = (pl->nfft3[2] > 0) + (pl->nfft3[1] + pl->nfft3[0] > 0) + (pl->nfft_old > 0);
+        forked = pl->nfft3[3] > 0 && nside_launches > 0 && pl->timing != 2;
+        if (forked) {
+            cudaEventRecord(pl->ev_fork, st);
+            for (int k = 0; k < 3; ++k) cudaStreamWaitEvent(pl->side[k], pl->ev_fork, 0);
+        }
+        launch_fft3<12, FWD>(pl, d_in, d_out, nmaps, st);
+        launch_fft3<11, FWD>(pl, d_in, d_out, nmaps, forked ? pl->side[0] : st);
+        launch_fft3<10, FWD>(pl, d_in, d_out, nmaps, forked ? pl->side[1] : st);
+        launch_fft3<9, FWD>(pl, d_in, d_out, nmaps, forked ? pl->side[1] : st);
+    }
+    if (pl->nfft_old > 0) {
+        cudaStream_t so = forked ? pl->side[2] : st;
+        const dim3 gfft((unsigned)pl->nfft_old, (unsigned)nmaps);
+        if (FWD) {
+            if (pl->fft_bpt == 2)
+                ring_fft_forward_kernel<T, 2><<<gfft, kFftThreads, pl->fft_smem, so>>>(
+                    (const T*)d_in, g.npix, (cx<T>*)pl->d_specIn, g.spec_total, pl->d_rings, pl->d_fft_order, pl->d_lens,
+                    (const cx<T>*)pl->d_tw, pl->logPT, (const cx<T>*)pl->d_filt, (const cx<T>*)pl->d_chirp, (const cx<T>*)pl->d_phase);
+            else
+                ring_fft_forward_kernel<T, 4><<<gfft, kFftThreads, pl->fft_smem, so>>>(
+                    (const T*)d_in, g.npix, (cx<T>*)pl->d_specIn, g.spec_total, pl->d_rings, pl->d_fft_order, pl->d_lens,
+                    (const cx<T>*)pl->d_tw, pl->logPT, (const cx<T>*)pl->d_filt, (const cx<T>*)pl->d_chirp, (const cx<T>*)pl->d_phase);
+        } else {
+            if (pl->fft_bpt == 2)
+                ring_fft_inverse_kernel<T, 2><<<gfft, kFftThreads, pl->fft_smem, so>>>(
+                    (const cx<T>*)pl->d_specOut, g.spec_total, (T*)d_out, g.npix, pl->d_rings, pl->d_fft_order, pl->d_lens,
+                    (const cx<T>*)pl->d_tw, pl->logPT, (const cx<T>*)pl->d_filt, (const cx<T>*)pl->d_chirp, (const cx<T>*)pl->d_phase);
+            else
+                ring_fft_inverse_kernel<T, 4><<<gfft, kFftThreads, pl->fft_smem, so>>>(
+                    (const cx<T>*)pl->d_specOut, g.spec_total, (T*)d_out, g.npix, pl->d_rings, pl->d_fft_order, pl->d_lens,
+                    (const cx<T>*)pl->d_tw, pl->logPT, (const cx<T>*)pl->d_filt, (const cx<T>*)pl->d_chirp, (const cx<T>*)pl->d_phase);
+        }
+    }
+    if (forked)
+        for (int k = 0; k < 3; ++k) {
+            cudaEventRecord(pl->ev_join[k], pl->side[k]);
+            cudaStreamWaitEvent(st, pl->ev_join[k], 0);
+        }
+}
+
 template <class T> int enqueue_convolve(const arkcos_plan* pl, const void* d_in, void* d_out, int nmaps, cudaStream_t st)
 {
     const HostGeometry& g = pl->g;
@@ -456,15 +581,7 @@ template <class T> int enqueue_convolve(const arkcos_plan* pl, const void* d_in,
     if (tm) cudaEventRecord(pl->ev[0], st);
     if (!pl->opt.cache_kernel_rows) enqueue_rows<T>(pl, st);
     if (tm) cudaEventRecord(pl->ev[1], st);
-    const dim3 gfft((unsigned)g.R, (unsigned)nmaps);
-    if (pl->fft_bpt == 2)
-        ring_fft_forward_kernel<T, 2><<<gfft, kFftThreads, pl->fft_smem, st>>>(
-            (const T*)d_in, g.npix, (cx<T>*)pl->d_specIn, g.spec_total, pl->d_rings, pl->d_fft_order, pl->d_lens,
-            (const cx<T>*)pl->d_tw, pl->logPT, (const cx<T>*)pl->d_filt, (const cx<T>*)pl->d_chirp, (const cx<T>*)pl->d_phase);
-    else
-        ring_fft_forward_kernel<T, 4><<<gfft, kFftThreads, pl->fft_smem, st>>>(
-            (const T*)d_in, g.npix, (cx<T>*)pl->d_specIn, g.spec_total, pl->d_rings, pl->d_fft_order, pl->d_lens,
-            (const cx<T>*)pl->d_tw, pl->logPT, (const cx<T>*)pl->d_filt, (const cx<T>*)pl->d_chirp, (const cx<T>*)pl->d_phase);
+    launch_ring_ffts<T, true>(pl, d_in, d_out, nmaps, st);
     if (tm) cudaEventRecord(pl->ev[2], st);
     // the band kernels of the different ring classes write disjoint rings: fork them onto the plan's side streams
     // (timing mode 2: one after the other on the caller's stream with an event between them)
@@ -493,14 +610,7 @@ template <class T> int enqueue_convolve(const arkcos_plan* pl, const void* d_in,
             cudaStreamWaitEvent(st, pl->ev_join[k], 0);
         }
     if (tm) cudaEventRecord(pl->ev[3], st);
-    if (pl->fft_bpt == 2)
-        ring_fft_inverse_kernel<T, 2><<<gfft, kFftThreads, pl->fft_smem, st>>>(
-            (const cx<T>*)pl->d_specOut, g.spec_total, (T*)d_out, g.npix, pl->d_rings, pl->d_fft_order, pl->d_lens,
-            (const cx<T>*)pl->d_tw, pl->logPT, (const cx<T>*)pl->d_filt, (const cx<T>*)pl->d_chirp, (const cx<T>*)pl->d_phase);
-    else
-        ring_fft_inverse_kernel<T, 4><<<gfft, kFftThreads, pl->fft_smem, st>>>(
-            (const cx<T>*)pl->d_specOut, g.spec_total, (T*)d_out, g.npix, pl->d_rings, pl->d_fft_order, pl->d_lens,
-            (const cx<T>*)pl->d_tw, pl->logPT, (const cx<T>*)pl->d_filt, (const cx<T>*)pl->d_chirp, (const cx<T>*)pl->d_phase);
+    launch_ring_ffts<T, false>(pl, d_in, d_out, nmaps, st);
     if (tm) cudaEventRecord(pl->ev[4], st);
     CUDA_TRY(cudaGetLastError());
     return 0;
@@ -568,7 +678,7 @@ static int plan_create_impl(arkcos_plan** out, const arkcos_pixelization* pix, c
     int sm_count = 148;
     if (!tables_only) CUDA_TRY(cudaDeviceGetAttribute(&sm_count, cudaDevAttrMultiProcessorCount, pl->device));
     HostTables t;
-    build_fft_lens(pl->g, t, pl->stats);
+    build_fft_lens(pl->g, t, pl->stats, dtype == ARKCOS_F32 && !getenv("ARKCOS_FORCE_OLD_FFT"));
     build_pairs(pl->g, pl->theta_max, pl->ell_nyquist, fixed_mprime, kBandThreads, dtype == ARKCOS_F32 && !getenv("ARKCOS_FORCE_GENERAL"), sm_count, t, pl->stats);
     if (t.pairs.size() > (size_t)INT32_MAX) return fail(ARKCOS_UNSUPPORTED, "too many ring pairs");
     pl->nnorth = (int)t.north.size();
@@ -664,7 +774,8 @@ int arkcos_plan_destroy(arkcos_plan* pl)
     if (!pl) return ARKCOS_OK;
     void* ptrs[] = {pl->d_rings, pl->d_lens, pl->d_pairs, pl->d_north, pl->d_items[0], pl->d_items[1], pl->d_items[2], pl->d_items[3],
                     pl->d_items[4], pl->d_eqchunks, pl->d_pole, pl->d_chirp, pl->d_phase, pl->d_fft_order, pl->d_table, pl->d_tw, pl->d_filt,
-                    pl->d_W, pl->d_specIn, pl->d_specOut, pl->d_stage_in, pl->d_stage_out};
+                    pl->d_W, pl->d_specIn, pl->d_specOut, pl->d_stage_in, pl->d_stage_out,
+                    pl->d_tw16, pl->d_fft3_jobs[0], pl->d_fft3_jobs[1], pl->d_fft3_jobs[2], pl->d_fft3_jobs[3]};
     for (void* p : ptrs) if (p) cudaFree(p);
     for (auto& e : pl->ev) if (e) cudaEventDestroy(e);
     for (auto& e : pl->ev_band) if (e) cudaEventDestroy(e);

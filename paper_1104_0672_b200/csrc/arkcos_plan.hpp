@@ -9,6 +9,7 @@
 #include "../../include/arkcos.h"
 #include "arkcos_band.cuh"
 #include "arkcos_fft.cuh"
+#include "arkcos_fft3.cuh"
 
 namespace arkcos {
 
@@ -57,7 +58,12 @@ struct arkcos_plan {
     void* d_filt = nullptr;      // cx<T>[...] Bluestein filter spectra
     void* d_chirp = nullptr;     // cx<T>[...] Bluestein chirps
     void* d_phase = nullptr;     // cx<T>[...] exp(-i pi k / N) per ring length
-    int* d_fft_order = nullptr;  // rings by decreasing transform size
+    int* d_fft_order = nullptr;  // rings served by the shared-memory FFT kernels (arkcos_fft.cuh), longest transform first
+    int nfft_old = 0;
+    // register-resident FFT kernels (arkcos_fft3.cuh): job lists for transform sizes Q = 512, 1024, 2048, 4096
+    arkcos::FftJob* d_fft3_jobs[4] = {nullptr, nullptr, nullptr, nullptr};
+    int nfft3[4] = {0, 0, 0, 0};
+    void* d_tw16 = nullptr;      // cx<float>[256]: exp(-2 pi i r k / 256) at [16 k + r]
     int fft_bpt = 2;
     void* d_W = nullptr;         // T[nsamples] kernel rows
     void* d_specIn = nullptr;    // cx<T>[max_nmaps][spec_total]
@@ -72,4 +78,5 @@ struct arkcos_plan {
     // fork/join of the band kernels of the different ring classes
     cudaStream_t side[3] = {nullptr, nullptr, nullptr};
     cudaEvent_t ev_fork = nullptr, ev_join[3] = {nullptr, nullptr, nullptr};
+    cudaEvent_t ev_fork2 = nullptr;
 };
