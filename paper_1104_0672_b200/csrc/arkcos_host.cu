@@ -152,6 +152,8 @@ struct HostTables {
     std::vector<PairRec> pairs;
     std::vector<NorthRec> north;
     std::vector<BandItem> items[kBandClasses];
+    std::vector<CapRing> cap_rings;              // rings for band_mac_cap_kernel, their pairs sorted by row length
+    std::vector<CapPair> cap_pairs;
     std::vector<int> pole_rings;                 // rings for band_mac_pole_kernel
     int pole_mh = 0;
     std::vector<EqChunk> eq_chunks;              // runs of consecutive class-E rings for band_mac_eq_kernel   // per band-kernel class (see band_class)
@@ -317,6 +319,13 @@ void build_pairs(HostGeometry& g, double theta_max, double ell_nyq, int fixed_mp
                 if (maxcnt <= 12) cls = odd ? 1 : 2;
                 else if (maxcnt <= 20 && !odd) cls = 3;
                 else if (maxcnt <= 32) cls = 4;
+                // single-period regime of band_mac_cap_kernel: M/2 below every ring length involved, N_i <= M
+                if ((cls == 2 || cls == 3) && !getenv("ARKCOS_NO_CAP_KERNEL")) {
+                    const int Mh = t.pairs[lo].M / 2;
+                    bool single = g.n[i] >= 512 && g.n[i] <= t.pairs[lo].M && Mh < g.n[i];
+                    for (int p = lo; p < hi; ++p) single = single && Mh < g.n[t.pairs[p].j];
+                    if (single) cls = 5;
+                }
             }
         }
         if (cls == 0 && t.north[i].pair_hi > t.north[i].pair_lo) {
@@ -331,8 +340,40 @@ void build_pairs(HostGeometry& g, double theta_max, double ell_nyq, int fixed_mp
             }
         }
         // band-kernel slots: 0 general, 1 pole, 2 eq, 3 uniform<12>, 4 uniform<20>, 5 uniform<32,odd>, 6 uniform<12,odd>
-        static const int slot_of_cls[kBandClasses] = {0, 6, 3, 4, 5};
+        static const int slot_of_cls[kBandClasses] = {0, 6, 3, 4, 5, 7};
         st.band_flops[slot_of_cls[cls]] += ring_flops;
+        if (cls == 5) {
+            const int lo = t.north[i].pair_lo, hi = t.north[i].pair_hi;
+            CapRing cr{};
+            cr.ring = i;
+            cr.first = (int)t.cap_pairs.size();
+            cr.np = hi - lo;
+            cr.M = t.pairs[lo].M;
+            cr.minN = 1 << 30;
+            std::vector<int> order(hi - lo);
+            for (int p = lo; p < hi; ++p) order[p - lo] = p;
+            auto c4_of = [&](int p) { return std::max(1, (t.pairs[p].cnt + 3) / 4); };
+            std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return c4_of(a) > c4_of(b); });
+            for (int p : order) {
+                const PairRec& pr = t.pairs[p];
+                CapPair cp{};
+                cp.woff = pr.woff;
+                cp.offN = (int)g.spec_off[pr.j];
+                cp.offS = (int)g.spec_off[R - 1 - pr.j];
+                cp.Nj = g.n[pr.j];
+                cp.shj = g.shifted[pr.j];
+                cp.cnt = pr.cnt;
+                t.cap_pairs.push_back(cp);
+                cr.tneed = std::max(cr.tneed, pr.cnt);
+                cr.minN = std::min(cr.minN, cp.Nj);
+                cr.maxN = std::max(cr.maxN, cp.Nj);
+                for (int c = 0; c < c4_of(p); ++c) ++cr.cstart[c];       // cstart[c] = pairs with class > c
+            }
+            const int cidx = (int)t.cap_rings.size();
+            t.cap_rings.push_back(cr);
+            for (int m0 = 0; m0 <= g.n[i] / 2; m0 += kCapThreads) t.items[cls].push_back(BandItem{cidx, m0});
+            continue;
+        }
         for (int m0 = 0; m0 <= g.n[i] / 2; m0 += band_threads) t.items[cls].push_back(BandItem{i, m0});
     }
     // chunks of consecutive class-E rings: about one block per resident slot of the device (4 blocks per SM)
@@ -503,6 +544,11 @@ void launch_uniform(const arkcos_plan* pl, int nmaps, cudaStream_t st, bool seri
     if (serial) cudaEventRecord(pl->ev_band[6], st);
     launch_uniform_class<12, true>(pl, 1, nmaps, s2);
     if (serial) cudaEventRecord(pl->ev_band[7], st);
+    if (pl->nitems[5] > 0)
+        band_mac_cap_kernel<20><<<dim3((unsigned)pl->nitems[5], (unsigned)nmaps), kCapThreads, 0, s1>>>(
+            pl->d_items[5], pl->d_cap_rings, pl->d_cap_pairs, (const float*)pl->d_W, pl->d_rings, pl->g.R,
+            (const cx<float>*)pl->d_specIn, (cx<float>*)pl->d_specOut, pl->g.spec_total);
+    if (serial) cudaEventRecord(pl->ev_band[8], st);
 }
 
 // Ring FFTs of one direction (FWD: map -> specIn, else specOut -> map).  Float plans: one launch per transform size of the
@@ -707,6 +753,8 @@ static int plan_create_impl(arkcos_plan** out, const arkcos_pixelization* pix, c
         if (int rc = upload(&pl->d_items[c], t.items[c], wsb)) return rc;
     if (int rc = upload(&pl->d_eqchunks, t.eq_chunks, wsb)) return rc;
     if (int rc = upload(&pl->d_pole, t.pole_rings, wsb)) return rc;
+    if (int rc = upload(&pl->d_cap_rings, t.cap_rings, wsb)) return rc;
+    if (int rc = upload(&pl->d_cap_pairs, t.cap_pairs, wsb)) return rc;
     std::vector<double> tab(kernel->table, kernel->table + kernel->n);
     if (int rc = upload(&pl->d_table, tab, wsb)) return rc;
     if (int rc = dtype == ARKCOS_F32 ? build_device_numeric<float>(pl, t) : build_device_numeric<double>(pl, t)) return rc;
@@ -773,9 +821,9 @@ int arkcos_plan_destroy(arkcos_plan* pl)
 {
     if (!pl) return ARKCOS_OK;
     void* ptrs[] = {pl->d_rings, pl->d_lens, pl->d_pairs, pl->d_north, pl->d_items[0], pl->d_items[1], pl->d_items[2], pl->d_items[3],
-                    pl->d_items[4], pl->d_eqchunks, pl->d_pole, pl->d_chirp, pl->d_phase, pl->d_fft_order, pl->d_table, pl->d_tw, pl->d_filt,
+                    pl->d_items[4], pl->d_items[5], pl->d_eqchunks, pl->d_pole, pl->d_chirp, pl->d_phase, pl->d_fft_order, pl->d_table, pl->d_tw, pl->d_filt,
                     pl->d_W, pl->d_specIn, pl->d_specOut, pl->d_stage_in, pl->d_stage_out,
-                    pl->d_tw16, pl->d_fft3_jobs[0], pl->d_fft3_jobs[1], pl->d_fft3_jobs[2], pl->d_fft3_jobs[3]};
+                    pl->d_cap_rings, pl->d_cap_pairs, pl->d_tw16, pl->d_fft3_jobs[0], pl->d_fft3_jobs[1], pl->d_fft3_jobs[2], pl->d_fft3_jobs[3]};
     for (void* p : ptrs) if (p) cudaFree(p);
     for (auto& e : pl->ev) if (e) cudaEventDestroy(e);
     for (auto& e : pl->ev_band) if (e) cudaEventDestroy(e);
@@ -835,19 +883,19 @@ int arkcos_plan_get_timing(const arkcos_plan* pl, float* ms4)
 
 int arkcos_plan_band_kernels(const arkcos_plan* pl, int* n, const char** names, double* model_flops, float* last_ms)
 {
-    static const char* kNames[7] = {"band_mac_general_kernel", "band_mac_pole_kernel", "band_mac_eq_kernel",
+    static const char* kNames[8] = {"band_mac_general_kernel", "band_mac_pole_kernel", "band_mac_eq_kernel",
                                     "band_mac_uniform_kernel<12,0>", "band_mac_uniform_kernel<20,0>",
-                                    "band_mac_uniform_kernel<32,1>", "band_mac_uniform_kernel<12,1>"};
+                                    "band_mac_uniform_kernel<32,1>", "band_mac_uniform_kernel<12,1>", "band_mac_cap_kernel<20>"};
     if (!pl || !n) return fail(ARKCOS_INVALID_ARG, "NULL argument");
-    *n = 7;
-    for (int k = 0; k < 7; ++k) {
+    *n = 8;
+    for (int k = 0; k < 8; ++k) {
         if (names) names[k] = kNames[k];
         if (model_flops) model_flops[k] = pl->stats.band_flops[k];
     }
     if (last_ms) {
         if (pl->timing != 2) return fail(ARKCOS_INVALID_ARG, "per-kernel timing needs arkcos_plan_set_timing(plan, 2)");
-        CUDA_TRY(cudaEventSynchronize(pl->ev_band[7]));
-        for (int k = 0; k < 7; ++k) CUDA_TRY(cudaEventElapsedTime(&last_ms[k], pl->ev_band[k], pl->ev_band[k + 1]));
+        CUDA_TRY(cudaEventSynchronize(pl->ev_band[8]));
+        for (int k = 0; k < 8; ++k) CUDA_TRY(cudaEventElapsedTime(&last_ms[k], pl->ev_band[k], pl->ev_band[k + 1]));
     }
     return ARKCOS_OK;
 }

@@ -24,7 +24,7 @@ struct HostGeometry {
 struct Stats {
     int64_t ring_pairs = 0, row_samples = 0, workspace_bytes = 0;
     double mac_flops = 0, fft_flops = 0;
-    double band_flops[7] = {0, 0, 0, 0, 0, 0, 0};   // per band kernel, see arkcos_plan_band_kernels
+    double band_flops[8] = {0, 0, 0, 0, 0, 0, 0, 0};   // per band kernel, see arkcos_plan_band_kernels
 };
 
 }  // namespace arkcos
@@ -39,7 +39,7 @@ struct arkcos_plan {
     arkcos::HostGeometry g;
     arkcos::Stats stats;
 
-    int nnorth = 0, npairs = 0, nitems[arkcos::kBandClasses] = {0, 0, 0, 0, 0}, logPT = 0;
+    int nnorth = 0, npairs = 0, nitems[arkcos::kBandClasses] = {0, 0, 0, 0, 0, 0}, logPT = 0;
     size_t fft_smem = 0;
     int64_t nsamples = 0;
 
@@ -50,9 +50,11 @@ struct arkcos_plan {
     arkcos::NorthRec* d_north = nullptr;
     arkcos::EqChunk* d_eqchunks = nullptr;
     int neqchunks = 0, eq_mh = 0, eq_alt = 0;
+    arkcos::CapRing* d_cap_rings = nullptr;
+    arkcos::CapPair* d_cap_pairs = nullptr;
     int* d_pole = nullptr;
     int npole = 0, pole_mh = 0;
-    arkcos::BandItem* d_items[arkcos::kBandClasses] = {nullptr, nullptr, nullptr, nullptr, nullptr};
+    arkcos::BandItem* d_items[arkcos::kBandClasses] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
     double* d_table = nullptr;
     void* d_tw = nullptr;        // cx<T>[PT/2]
     void* d_filt = nullptr;      // cx<T>[...] Bluestein filter spectra
@@ -74,7 +76,7 @@ struct arkcos_plan {
     // optional per-stage timing
     mutable int timing = 0;
     mutable cudaEvent_t ev[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
-    mutable cudaEvent_t ev_band[8] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+    mutable cudaEvent_t ev_band[9] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
     // fork/join of the band kernels of the different ring classes
     cudaStream_t side[3] = {nullptr, nullptr, nullptr};
     cudaEvent_t ev_fork = nullptr, ev_join[3] = {nullptr, nullptr, nullptr};
