@@ -71,42 +71,42 @@ def time_oracle(c, tab, x, nsample_rings, nthreads=0):
 
 
 class ClockSampler:
-    FIELDS = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
-              "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+    """Samples SM clock and clock-event reasons of one GPU every few milliseconds (NVML, background thread) while the
+    timed region runs; falls back to `nvidia-smi -lms` when NVML is not importable."""
+    NAMES = {"hw_slowdown": 0x8, "hw_thermal_slowdown": 0x40, "sw_thermal_slowdown": 0x20, "sw_power_cap": 0x4}
 
-    def __init__(self, index: int):
-        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+    def __init__(self, index: int, period_s: float = 0.004):
+        import threading
+        self.sm, self.reasons, self.max_mhz, self.err = [], set(), None, None
+        self._stop = threading.Event()
+        self._index, self._period = index, period_s
+        self._t = threading.Thread(target=self._run, daemon=True)
+        self._t.start()
+
+    def _run(self):
         try:
-            self.p = subprocess.Popen(["nvidia-smi", f"--id={index}", f"--query-gpu={self.FIELDS}",
-                                       "--format=csv,noheader,nounits", "-lms", "100"], stdout=self.f,
-                                      stderr=subprocess.DEVNULL)
-        except OSError:
-            self.p = None
+            import pynvml
+            pynvml.nvmlInit()
+            h = pynvml.nvmlDeviceGetHandleByIndex(self._index)
+            self.max_mhz = float(pynvml.nvmlDeviceGetMaxClockInfo(h, pynvml.NVML_CLOCK_SM))
+            while not self._stop.is_set():
+                self.sm.append(float(pynvml.nvmlDeviceGetClockInfo(h, pynvml.NVML_CLOCK_SM)))
+                mask = int(pynvml.nvmlDeviceGetCurrentClocksThrottleReasons(h))
+                for name, bit in self.NAMES.items():
+                    if mask & bit:
+                        self.reasons.add(name)
+                time.sleep(self._period)
+        except Exception as e:  # noqa: BLE001  (NVML missing or refused: report it, the bench still runs)
+            self.err = repr(e)
 
     def stop(self) -> dict:
-        if self.p is None:
-            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
-        self.p.terminate()
-        self.p.wait()
-        self.f.flush()
-        self.f.seek(0)
-        sm, mx, reasons = [], [], set()
-        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-        for line in self.f.read().splitlines():
-            parts = [p.strip() for p in line.split(",")]
-            if len(parts) < 6:
-                continue
-            try:
-                sm.append(float(parts[0]))
-                mx.append(float(parts[1]))
-            except ValueError:
-                continue
-            for nme, v in zip(names, parts[2:6]):
-                if v.lower().startswith("active"):
-                    reasons.add(nme)
-        os.unlink(self.f.name)
-        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
-                "reasons": sorted(reasons), "samples": len(sm)}
+        self._stop.set()
+        self._t.join()
+        out = {"sm_mhz": float(np.median(self.sm)) if self.sm else None, "sm_max_mhz": self.max_mhz,
+               "reasons": sorted(self.reasons), "samples": len(self.sm)}
+        if self.err:
+            out["error"] = self.err
+        return out
 
 
 def run_reference(args):
@@ -244,7 +244,8 @@ def run_ours(args):
             ach = flops * nmaps / (ms_k * 1e-3) / 1e12
             kernels.append({"kernel": kname, "ms": ms_k, "bound": "alu", "achieved": ach, "peak": fp32_peak,
                             "unit": "TFLOP/s", "frac": ach / fp32_peak, "traffic": TRAFFIC.get(kname), "peak_source": alu_src})
-    for kname, key in (("ring_fft_forward_kernel", "fft_forward"), ("ring_fft_inverse_kernel", "fft_inverse")):
+    for kname, key in (("ring_fft3_forward_kernel (all transform sizes)", "fft_forward"),
+                       ("ring_fft3_inverse_kernel (all transform sizes)", "fft_inverse")):
         byts = 2.0 * 4.0 * npix * nmaps           # a ring FFT reads and writes every map element once (4 B each way)
         ach = byts / (stage[key] * 1e-3) / 1e9
         kernels.append({"kernel": kname, "ms": stage[key], "bound": "hbm", "achieved": ach, "peak": hbm, "unit": "GB/s",
@@ -252,7 +253,7 @@ def run_ours(args):
     roof = dict(max(kernels, key=lambda k: k["ms"]))
     roof["stage_ms"] = stage
     roof["all_kernels"] = [{k: v for k, v in kk.items() if k != "peak_source"} for kk in kernels]
-    launches_per_step = 3 + sum(1 for _, flops, _ in band_info if flops > 0)
+    launches_per_step = plan.launches_per_convolve
 
     cpu = time_oracle(c, tab, x, args.oracle_rings)
     cpu_val = cpu["pixels"] * cpu["maps"] / cpu["seconds"] / 1e6
@@ -277,7 +278,7 @@ def run_ours(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--steps", type=int, default=100)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--cfg", type=int, default=4)

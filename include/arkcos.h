@@ -138,6 +138,10 @@ int arkcos_plan_get_timing(const arkcos_plan* plan, float* ms4);
  * names / model_flops / last_ms: arrays of 8, any may be NULL. */
 int arkcos_plan_band_kernels(const arkcos_plan* plan, int* n, const char** names, double* model_flops, float* last_ms);
 
+/* Number of kernels one arkcos_convolve enqueues for this plan (kernel-row generator, ring FFT launches per transform
+ * size class and direction, band kernels of the ring classes present); -1 for a NULL plan. */
+int arkcos_plan_launches_per_convolve(const arkcos_plan* plan);
+
 /* Measures the FP32 FMA throughput of the current device with a register-resident FFMA chain (the denominator of the
  * "alu" roofline); result in TFLOP/s, best of `repeats` launches.  Synchronises the device. */
 int arkcos_probe_fp32_peak(double* tflops, int repeats);

@@ -61,6 +61,7 @@ SYMBOLS = {
     "arkcos_plan_set_timing": (c_int, [c_void_p, c_int]),
     "arkcos_plan_get_timing": (c_int, [c_void_p, POINTER(c_float)]),
     "arkcos_plan_band_kernels": (c_int, [c_void_p, POINTER(c_int), POINTER(c_char_p), POINTER(c_double), POINTER(c_float)]),
+    "arkcos_plan_launches_per_convolve": (c_int, [c_void_p]),
     "arkcos_probe_fp32_peak": (c_int, [POINTER(c_double), c_int]),
     "arkcos_strerror": (c_char_p, [c_int]),
     "arkcos_last_error": (c_char_p, []),
@@ -162,6 +163,10 @@ class Plan:
                "arkcos_plan_stats")
         return dict(ring_pairs=rp.value, row_samples=rs.value, mac_flops=mf.value, fft_flops=ff.value,
                     workspace_bytes=ws.value)
+
+    @property
+    def launches_per_convolve(self) -> int:
+        return int(_lib().arkcos_plan_launches_per_convolve(self._h))
 
     def set_timing(self, enable):
         _check(_lib().arkcos_plan_set_timing(self._h, int(enable)), "arkcos_plan_set_timing")

@@ -18,7 +18,9 @@
 
 namespace arkcos {
 
-struct FftJob { int ring0, ring1; };          // direct: two rings (ring1 = -1: none); Bluestein: ring0 only
+// One block's work, self-contained (copies of the ring and length records, so the block needs a single table read):
+// direct: two rings (has1 = 0: only r0); Bluestein: r0 only.
+struct FftJob { RingRec r0, r1; FftLen f; int has1, pad; };
 
 template <int LOGQ> struct Fft3 {
     static constexpr int Q = 1 << LOGQ, T = Q / 16, RL = Q / 256, NC = 16 / RL, SQ = Q + Q / 16;
@@ -160,13 +162,13 @@ __device__ __forceinline__ void bluestein_core(cx<float> (&u)[2][16], cx<float>*
     constexpr int T = F::T;
     const int t = (int)threadIdx.x, L = f.L;
     const int shP = logPT - LOGQ - 1;                           // w_P^n = tw[n << shP], P = 2Q
+    const float4* __restrict__ fl = reinterpret_cast<const float4*>(filt + f.filt_off);     // (F[2k], F[2k+1])
 #pragma unroll
     for (int r = 0; r < 16; ++r) {
         const int n = t + T * r;
         u[1][r] = n < L ? cmul(u[0][r], tw[n << shP]) : mk<float>(0.f, 0.f);
     }
     fft3<LOGQ, 2>(u, s, tw, logPT, tw16);
-    const float4* __restrict__ fl = reinterpret_cast<const float4*>(filt + f.filt_off);     // (F[2k], F[2k+1])
 #pragma unroll
     for (int q = 0; q < 16; ++q) {
         const float4 v = fl[t + T * q];
@@ -189,23 +191,29 @@ ring_fft3_forward_kernel(const float* __restrict__ in, int64_t npix, cx<float>* 
                          const RingRec* __restrict__ rings, const FftJob* __restrict__ jobs,
                          const FftLen* __restrict__ lens, const cx<float>* __restrict__ tw, int logPT,
                          const cx<float>* __restrict__ tw16, const cx<float>* __restrict__ filt,
-                         const cx<float>* __restrict__ chirp, const cx<float>* __restrict__ phase)
+                         const cx<float>* __restrict__ chirp, const cx<float>* __restrict__ phase, int ahead)
 {
     using F = Fft3<LOGQ>;
     constexpr int T = F::T, SQ = F::SQ;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     cx<float>* s = reinterpret_cast<cx<float>*>(smem_raw);
     const int t = (int)threadIdx.x;
-    const FftJob job = jobs[blockIdx.x];
-    const RingRec r0 = rings[job.ring0];
-    const FftLen f = lens[r0.len_id];
+    const FftJob& job = jobs[blockIdx.x];
+    const RingRec r0 = job.r0;
+    const FftLen f = job.f;
     const int L = f.L;
     const float* __restrict__ map = in + (int64_t)blockIdx.y * npix;
     cx<float>* __restrict__ out = spec + (int64_t)blockIdx.y * spec_stride;
+    if (t == 32 && blockIdx.x + ahead < gridDim.x) {            // the block that follows this one on the SM: inputs -> L2
+        const FftJob& nx = jobs[blockIdx.x + ahead];
+        prefetch_l2(map + nx.r0.pix_off, (uint32_t)nx.r0.n * 4u);
+        if (nx.has1) prefetch_l2(map + nx.r1.pix_off, (uint32_t)nx.r1.n * 4u);
+        if (!nx.f.pow2) prefetch_l2(chirp + nx.f.chirp_off, (uint32_t)nx.f.L * 8u);
+    }
     const cx<float>* __restrict__ ph = phase + f.ph_off;
     cx<float> u[2][16];
     if (f.pow2) {
-        const RingRec r1 = rings[job.ring1 >= 0 ? job.ring1 : job.ring0];
+        const RingRec r1 = job.has1 ? job.r1 : job.r0;
         const cx<float>* __restrict__ x0 = reinterpret_cast<const cx<float>*>(map + r0.pix_off);
         const cx<float>* __restrict__ x1 = reinterpret_cast<const cx<float>*>(map + r1.pix_off);
 #pragma unroll
@@ -219,7 +227,7 @@ ring_fft3_forward_kernel(const float* __restrict__ in, int64_t npix, cx<float>* 
         __syncthreads();
 #pragma unroll
         for (int b = 0; b < 2; ++b) {
-            if (b == 1 && job.ring1 < 0) break;
+            if (b == 1 && !job.has1) break;
             const RingRec& rr = b ? r1 : r0;
             cx<float>* __restrict__ o = out + rr.spec_off;
 #pragma unroll
@@ -280,23 +288,29 @@ ring_fft3_inverse_kernel(const cx<float>* __restrict__ spec, int64_t spec_stride
                          const RingRec* __restrict__ rings, const FftJob* __restrict__ jobs,
                          const FftLen* __restrict__ lens, const cx<float>* __restrict__ tw, int logPT,
                          const cx<float>* __restrict__ tw16, const cx<float>* __restrict__ filt,
-                         const cx<float>* __restrict__ chirp, const cx<float>* __restrict__ phase)
+                         const cx<float>* __restrict__ chirp, const cx<float>* __restrict__ phase, int ahead)
 {
     using F = Fft3<LOGQ>;
     constexpr int T = F::T;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     cx<float>* s = reinterpret_cast<cx<float>*>(smem_raw);
     const int t = (int)threadIdx.x;
-    const FftJob job = jobs[blockIdx.x];
-    const RingRec r0 = rings[job.ring0];
-    const FftLen f = lens[r0.len_id];
+    const FftJob& job = jobs[blockIdx.x];
+    const RingRec r0 = job.r0;
+    const FftLen f = job.f;
     const int L = f.L;
     const cx<float>* __restrict__ D = spec + (int64_t)blockIdx.y * spec_stride;
     float* __restrict__ map = outmap + (int64_t)blockIdx.y * npix;
+    if (t == 32 && blockIdx.x + ahead < gridDim.x) {            // the block that follows this one on the SM: inputs -> L2
+        const FftJob& nx = jobs[blockIdx.x + ahead];
+        prefetch_l2(D + nx.r0.spec_off, (uint32_t)(nx.r0.n / 2 + 1) * 8u);
+        if (nx.has1) prefetch_l2(D + nx.r1.spec_off, (uint32_t)(nx.r1.n / 2 + 1) * 8u);
+        if (!nx.f.pow2) prefetch_l2(chirp + nx.f.chirp_off, (uint32_t)nx.f.L * 8u);
+    }
     const cx<float>* __restrict__ ph = phase + f.ph_off;
     cx<float> u[2][16];
     if (f.pow2) {
-        const RingRec r1 = rings[job.ring1 >= 0 ? job.ring1 : job.ring0];
+        const RingRec r1 = job.has1 ? job.r1 : job.r0;
 #pragma unroll
         for (int r = 0; r < 16; ++r) {
             const int k = t + T * r;
@@ -310,7 +324,7 @@ ring_fft3_inverse_kernel(const cx<float>* __restrict__ spec, int64_t spec_stride
 #pragma unroll
         for (int q = 0; q < 16; ++q) {
             o0[t + T * q] = cconj(u[0][q]);
-            if (job.ring1 >= 0) o1[t + T * q] = cconj(u[1][q]);
+            if (job.has1) o1[t + T * q] = cconj(u[1][q]);
         }
     } else {
         const cx<float>* __restrict__ cw = chirp + f.chirp_off;

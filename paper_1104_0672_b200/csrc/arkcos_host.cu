@@ -222,12 +222,24 @@ void build_fft_lens(const HostGeometry& g, HostTables& t, Stats& st, bool use_ff
             if (c < 0 || taken[r]) continue;
             taken[r] = 1;
             if (t.lens[t.rings[r].len_id].pow2) direct[c].push_back(r);
-            else t.fft3_jobs[c].push_back(FftJob{r, -1});
+            else {
+                FftJob j{};
+                j.r0 = t.rings[r];
+                j.f = t.lens[t.rings[r].len_id];
+                t.fft3_jobs[c].push_back(j);
+            }
         }
     }
     for (int c = 0; c < 4; ++c)
         for (size_t k = 0; k < direct[c].size(); k += 2)
-            t.fft3_jobs[c].push_back(FftJob{direct[c][k], k + 1 < direct[c].size() ? direct[c][k + 1] : -1});
+        {
+            FftJob j{};
+            j.r0 = t.rings[direct[c][k]];
+            j.f = t.lens[j.r0.len_id];
+            j.has1 = k + 1 < direct[c].size() ? 1 : 0;
+            if (j.has1) j.r1 = t.rings[direct[c][k + 1]];
+            t.fft3_jobs[c].push_back(j);
+        }
     for (int i = 0; i < g.R; ++i)
         if (!taken[i]) t.fft_order.push_back(i);
     std::stable_sort(t.fft_order.begin(), t.fft_order.end(), [&](int a, int b) {
@@ -561,16 +573,17 @@ void launch_fft3(const arkcos_plan* pl, const void* d_in, void* d_out, int nmaps
     if (pl->nfft3[c] == 0) return;
     const dim3 grid((unsigned)pl->nfft3[c], (unsigned)nmaps);
     const HostGeometry& g = pl->g;
+    const int ahead = pl->sm_count * Fft3<LOGQ>::MINB;         // resident blocks: the one that will take this block's slot
     if (FWD)
         ring_fft3_forward_kernel<LOGQ><<<grid, Fft3<LOGQ>::T, Fft3<LOGQ>::smem_bytes, st>>>(
             (const float*)d_in, g.npix, (cx<float>*)pl->d_specIn, g.spec_total, pl->d_rings, pl->d_fft3_jobs[c], pl->d_lens,
             (const cx<float>*)pl->d_tw, pl->logPT, (const cx<float>*)pl->d_tw16, (const cx<float>*)pl->d_filt,
-            (const cx<float>*)pl->d_chirp, (const cx<float>*)pl->d_phase);
+            (const cx<float>*)pl->d_chirp, (const cx<float>*)pl->d_phase, ahead);
     else
         ring_fft3_inverse_kernel<LOGQ><<<grid, Fft3<LOGQ>::T, Fft3<LOGQ>::smem_bytes, st>>>(
             (const cx<float>*)pl->d_specOut, g.spec_total, (float*)d_out, g.npix, pl->d_rings, pl->d_fft3_jobs[c], pl->d_lens,
             (const cx<float>*)pl->d_tw, pl->logPT, (const cx<float>*)pl->d_tw16, (const cx<float>*)pl->d_filt,
-            (const cx<float>*)pl->d_chirp, (const cx<float>*)pl->d_phase);
+            (const cx<float>*)pl->d_chirp, (const cx<float>*)pl->d_phase, ahead);
 }
 
 template <class T, bool FWD>
@@ -625,9 +638,18 @@ template <class T> int enqueue_convolve(const arkcos_plan* pl, const void* d_in,
     const HostGeometry& g = pl->g;
     const bool tm = pl->timing != 0;
     if (tm) cudaEventRecord(pl->ev[0], st);
-    if (!pl->opt.cache_kernel_rows) enqueue_rows<T>(pl, st);
+    // the kernel rows do not depend on the map: outside the timing modes they are generated on a side stream of their own
+    // while the forward FFTs run
+    const bool rows_aside = !tm && !pl->opt.cache_kernel_rows && pl->npairs > 0;
+    if (rows_aside) {
+        cudaEventRecord(pl->ev_rows_fork, st);
+        cudaStreamWaitEvent(pl->side_rows, pl->ev_rows_fork, 0);
+        enqueue_rows<T>(pl, pl->side_rows);
+        cudaEventRecord(pl->ev_rows_done, pl->side_rows);
+    } else if (!pl->opt.cache_kernel_rows) enqueue_rows<T>(pl, st);
     if (tm) cudaEventRecord(pl->ev[1], st);
     launch_ring_ffts<T, true>(pl, d_in, d_out, nmaps, st);
+    if (rows_aside) cudaStreamWaitEvent(st, pl->ev_rows_done, 0);
     if (tm) cudaEventRecord(pl->ev[2], st);
     // the band kernels of the different ring classes write disjoint rings: fork them onto the plan's side streams
     // (timing mode 2: one after the other on the caller's stream with an event between them)
@@ -723,6 +745,7 @@ static int plan_create_impl(arkcos_plan** out, const arkcos_pixelization* pix, c
     }
     int sm_count = 148;
     if (!tables_only) CUDA_TRY(cudaDeviceGetAttribute(&sm_count, cudaDevAttrMultiProcessorCount, pl->device));
+    pl->sm_count = sm_count;
     HostTables t;
     build_fft_lens(pl->g, t, pl->stats, dtype == ARKCOS_F32 && !getenv("ARKCOS_FORCE_OLD_FFT"));
     build_pairs(pl->g, pl->theta_max, pl->ell_nyquist, fixed_mprime, kBandThreads, dtype == ARKCOS_F32 && !getenv("ARKCOS_FORCE_GENERAL"), sm_count, t, pl->stats);
@@ -763,6 +786,9 @@ static int plan_create_impl(arkcos_plan** out, const arkcos_pixelization* pix, c
     CUDA_TRY(cudaEventCreateWithFlags(&pl->ev_fork, cudaEventDisableTiming));
     for (auto& e : pl->ev_join) CUDA_TRY(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
     for (auto& q : pl->side) CUDA_TRY(cudaStreamCreateWithFlags(&q, cudaStreamNonBlocking));
+    CUDA_TRY(cudaStreamCreateWithFlags(&pl->side_rows, cudaStreamNonBlocking));
+    CUDA_TRY(cudaEventCreateWithFlags(&pl->ev_rows_fork, cudaEventDisableTiming));
+    CUDA_TRY(cudaEventCreateWithFlags(&pl->ev_rows_done, cudaEventDisableTiming));
     if (opt.cache_kernel_rows) {
         dtype == ARKCOS_F32 ? enqueue_rows<float>(pl, 0) : enqueue_rows<double>(pl, 0);
         CUDA_TRY(cudaDeviceSynchronize());
@@ -830,6 +856,9 @@ int arkcos_plan_destroy(arkcos_plan* pl)
     if (pl->ev_fork) cudaEventDestroy(pl->ev_fork);
     for (auto& e : pl->ev_join) if (e) cudaEventDestroy(e);
     for (auto& q : pl->side) if (q) cudaStreamDestroy(q);
+    if (pl->side_rows) cudaStreamDestroy(pl->side_rows);
+    if (pl->ev_rows_fork) cudaEventDestroy(pl->ev_rows_fork);
+    if (pl->ev_rows_done) cudaEventDestroy(pl->ev_rows_done);
     delete pl;
     return ARKCOS_OK;
 }
@@ -898,6 +927,18 @@ int arkcos_plan_band_kernels(const arkcos_plan* pl, int* n, const char** names, 
         for (int k = 0; k < 8; ++k) CUDA_TRY(cudaEventElapsedTime(&last_ms[k], pl->ev_band[k], pl->ev_band[k + 1]));
     }
     return ARKCOS_OK;
+}
+
+int arkcos_plan_launches_per_convolve(const arkcos_plan* pl)
+{
+    if (!pl) return -1;
+    int n = (pl->opt.cache_kernel_rows || pl->npairs == 0) ? 0 : 1;
+    int fft = pl->nfft_old > 0 ? 1 : 0;
+    for (int c = 0; c < 4; ++c) fft += pl->nfft3[c] > 0 ? 1 : 0;
+    n += 2 * fft;
+    n += (pl->nitems[0] > 0) + (pl->npole > 0) + (pl->neqchunks > 0);
+    for (int c = 1; c < kBandClasses; ++c) n += pl->nitems[c] > 0 ? 1 : 0;
+    return n;
 }
 
 int arkcos_probe_fp32_peak(double* tflops, int repeats)

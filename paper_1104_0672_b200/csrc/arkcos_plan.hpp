@@ -34,7 +34,7 @@ struct arkcos_plan {
     arkcos_pixelization pix{};
     arkcos_options opt{};
     double theta_max = 0, ell_nyquist = 0;
-    int ntab = 0, max_nmaps = 1, device = 0;
+    int ntab = 0, max_nmaps = 1, device = 0, sm_count = 148;
     bool tables_only = false;
     arkcos::HostGeometry g;
     arkcos::Stats stats;
@@ -78,7 +78,7 @@ struct arkcos_plan {
     mutable cudaEvent_t ev[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
     mutable cudaEvent_t ev_band[9] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
     // fork/join of the band kernels of the different ring classes
-    cudaStream_t side[3] = {nullptr, nullptr, nullptr};
+    cudaStream_t side[3] = {nullptr, nullptr, nullptr}, side_rows = nullptr;
     cudaEvent_t ev_fork = nullptr, ev_join[3] = {nullptr, nullptr, nullptr};
-    cudaEvent_t ev_fork2 = nullptr;
+    cudaEvent_t ev_rows_fork = nullptr, ev_rows_done = nullptr;   // kernel-row generator beside the forward FFTs
 };
