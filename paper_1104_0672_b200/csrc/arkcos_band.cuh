@@ -281,40 +281,54 @@ namespace arkcos {
 struct EqChunk { int i0, n; };
 constexpr int kEqJMax = kMaxPairs + 8;
 
-template <int TI, int MT, int TMAX, int ALT, int PAR>
-__device__ __forceinline__ void eq_accumulate(const float* __restrict__ sWj, const unsigned char* __restrict__ sCj,
-                                              const float (&ce)[MT][TMAX], const float (&co)[MT][TMAX],
-                                              const cx<float> (&v)[2][MT], cx<float> (&acc)[TI][2][MT])
+template <int TI, int MT, int TMAX, int ALT, int PAR, int C4>
+__device__ __forceinline__ void eq_accumulate(const float* __restrict__ sWj, const float (&ce)[MT][TMAX],
+                                              const float (&co)[MT][TMAX], const cx<float> (&v)[2][MT],
+                                              cx<float> (&acc)[TI][2][MT])
 {
 #pragma unroll
     for (int ii = 0; ii < TI; ++ii) {
-        const int c4 = sCj[ii * kEqJMax];
-        if (c4) {
-            const float4* __restrict__ w4 = reinterpret_cast<const float4*>(sWj + ii * (kEqJMax * TMAX));
-            const bool odd = ALT && ((PAR ^ ii) & 1) != 0;          // compile-time after unrolling
-            float G[MT];
+        const float4* __restrict__ w4 = reinterpret_cast<const float4*>(sWj + ii * (kEqJMax * TMAX));
+        const bool odd = ALT && ((PAR ^ ii) & 1) != 0;          // compile-time after unrolling
+        float G[MT];
 #pragma unroll
-            for (int mt = 0; mt < MT; ++mt) G[mt] = 0.f;
+        for (int mt = 0; mt < MT; ++mt) G[mt] = 0.f;
 #pragma unroll
-            for (int t4 = 0; t4 < TMAX / 4; ++t4) {
-                if (t4 < c4) {
-                    const float4 w = w4[t4];
+        for (int t4 = 0; t4 < C4; ++t4) {
+            const float4 w = w4[t4];
 #pragma unroll
-                    for (int mt = 0; mt < MT; ++mt) {
-                        const float* c = odd ? co[mt] : ce[mt];
-                        G[mt] = fmaf(w.x, c[4 * t4], G[mt]); G[mt] = fmaf(w.y, c[4 * t4 + 1], G[mt]);
-                        G[mt] = fmaf(w.z, c[4 * t4 + 2], G[mt]); G[mt] = fmaf(w.w, c[4 * t4 + 3], G[mt]);
-                    }
-                }
+            for (int mt = 0; mt < MT; ++mt) {
+                const float* c = odd ? co[mt] : ce[mt];
+                G[mt] = fmaf(w.x, c[4 * t4], G[mt]); G[mt] = fmaf(w.y, c[4 * t4 + 1], G[mt]);
+                G[mt] = fmaf(w.z, c[4 * t4 + 2], G[mt]); G[mt] = fmaf(w.w, c[4 * t4 + 3], G[mt]);
             }
-#pragma unroll
-            for (int h = 0; h < 2; ++h)
-#pragma unroll
-                for (int mt = 0; mt < MT; ++mt) {
-                    acc[ii][h][mt].x = fmaf(G[mt], v[h][mt].x, acc[ii][h][mt].x);
-                    acc[ii][h][mt].y = fmaf(G[mt], v[h][mt].y, acc[ii][h][mt].y);
-                }
         }
+#pragma unroll
+        for (int h = 0; h < 2; ++h)
+#pragma unroll
+            for (int mt = 0; mt < MT; ++mt) {
+                acc[ii][h][mt].x = fmaf(G[mt], v[h][mt].x, acc[ii][h][mt].x);
+                acc[ii][h][mt].y = fmaf(G[mt], v[h][mt].y, acc[ii][h][mt].y);
+            }
+    }
+}
+
+// one input ring of the tile: rows of the TI output rings, all taken with the longest row length of this input ring
+// (shorter and missing rows are zero-filled)
+template <int TI, int MT, int TMAX, int ALT>
+__device__ __forceinline__ void eq_input_ring(const float* __restrict__ sWj, int c4, bool par, const float (&ce)[MT][TMAX],
+                                              const float (&co)[MT][TMAX], const cx<float> (&v)[2][MT],
+                                              cx<float> (&acc)[TI][2][MT])
+{
+    static_assert(TMAX == 12, "row length classes 1..3");
+    if (ALT && par) {
+        if (c4 == 3) eq_accumulate<TI, MT, TMAX, ALT, 1, 3>(sWj, ce, co, v, acc);
+        else if (c4 == 2) eq_accumulate<TI, MT, TMAX, ALT, 1, 2>(sWj, ce, co, v, acc);
+        else eq_accumulate<TI, MT, TMAX, ALT, 1, 1>(sWj, ce, co, v, acc);
+    } else {
+        if (c4 == 3) eq_accumulate<TI, MT, TMAX, ALT, 0, 3>(sWj, ce, co, v, acc);
+        else if (c4 == 2) eq_accumulate<TI, MT, TMAX, ALT, 0, 2>(sWj, ce, co, v, acc);
+        else eq_accumulate<TI, MT, TMAX, ALT, 0, 1>(sWj, ce, co, v, acc);
     }
 }
 
@@ -325,8 +339,9 @@ band_mac_eq_kernel(const EqChunk* __restrict__ chunks, const NorthRec* __restric
                    int R, const cx<float>* __restrict__ specIn, cx<float>* __restrict__ specOut, int64_t spec_stride)
 {
     __shared__ __align__(16) float sW[TI * kEqJMax * TMAX];       // [ii][jj][t]
-    __shared__ unsigned char sC[TI * kEqJMax];                     // [ii][jj]: row length / 4, 0 = no such pair
+    __shared__ int sC[kEqJMax];                                    // [jj]: longest row length / 4 over the tile's rings
     __shared__ int2 sJ[kEqJMax];                                   // spectrum offsets of input ring jlo + jj (N, S)
+    __shared__ cx<float> sB[4][2][MT][kBandThreads];               // in-flight input-ring coefficients, [stage][N/S][mode][thread]
     const EqChunk ch = chunks[blockIdx.y];
     const int M = rings[ch.i0].n, Mh = M >> 1;
     int m[MT];
@@ -351,7 +366,11 @@ band_mac_eq_kernel(const EqChunk* __restrict__ chunks, const NorthRec* __restric
         const int p_first = north[i0].pair_lo, p_last = north[i0 + nti - 1].pair_hi;
         const int jlo = pairs[p_first].j, jw = pairs[p_last - 1].j - jlo + 1;
         __syncthreads();
-        for (int k = threadIdx.x; k < TI * kEqJMax; k += kBandThreads) sC[k] = 0;
+        for (int k = threadIdx.x; k < jw; k += kBandThreads) sC[k] = 0;
+        for (int k = threadIdx.x; k < TI * jw * (TMAX / 4); k += kBandThreads) {
+            const int ii = k / (jw * (TMAX / 4)), r = k - ii * (jw * (TMAX / 4));
+            reinterpret_cast<float4*>(sW + ii * (kEqJMax * TMAX))[r] = make_float4(0.f, 0.f, 0.f, 0.f);
+        }
         for (int jj = threadIdx.x; jj < jw; jj += kBandThreads)
             sJ[jj] = make_int2((int)rings[jlo + jj].spec_off, (int)rings[R - 1 - jlo - jj].spec_off);
         __syncthreads();
@@ -364,7 +383,7 @@ band_mac_eq_kernel(const EqChunk* __restrict__ chunks, const NorthRec* __restric
             const int slot = ii * kEqJMax + (pr.j - jlo), c4 = (pr.cnt + 3) >> 2;
             if (t4 < c4)
                 reinterpret_cast<float4*>(sW + slot * TMAX)[t4] = reinterpret_cast<const float4*>(W + pr.woff)[t4];
-            if (t4 == 0) sC[slot] = (unsigned char)c4;
+            if (t4 == 0) atomicMax(&sC[pr.j - jlo], c4);
         }
         __syncthreads();
         cx<float> acc[TI][2][MT];
@@ -375,26 +394,28 @@ band_mac_eq_kernel(const EqChunk* __restrict__ chunks, const NorthRec* __restric
 #pragma unroll
                 for (int mt = 0; mt < MT; ++mt) acc[ii][h][mt] = mk<float>(0.f, 0.f);
 
-        cx<float> v[2][MT], vn[2][MT];
-        {
-            const int2 off = sJ[0];
+        // Bp_j[m] of the window's input rings: cp.async into a four-deep ring of thread-private shared-memory slots
+        // (three input rings in flight while one is accumulated; no barrier, a thread only reads what it copied itself)
+        auto fetch = [&](int jj) {
+            if (jj < jw) {
+                const int2 off = sJ[jj];
 #pragma unroll
-            for (int mt = 0; mt < MT; ++mt) { vn[0][mt] = inm[mt][off.x]; vn[1][mt] = inm[mt][off.y]; }
-        }
-        for (int jj = 0; jj < jw; ++jj) {
-#pragma unroll
-            for (int mt = 0; mt < MT; ++mt) { v[0][mt] = vn[0][mt]; v[1][mt] = vn[1][mt]; }
-            {
-                const int2 off = sJ[min(jj + 1, jw - 1)];                  // prefetch the next input ring
-#pragma unroll
-                for (int mt = 0; mt < MT; ++mt) { vn[0][mt] = inm[mt][off.x]; vn[1][mt] = inm[mt][off.y]; }
+                for (int mt = 0; mt < MT; ++mt) {
+                    cp_async8(&sB[jj & 3][0][mt][threadIdx.x], inm[mt] + off.x);
+                    cp_async8(&sB[jj & 3][1][mt][threadIdx.x], inm[mt] + off.y);
+                }
             }
-            const float* sWj = sW + jj * TMAX;
-            const unsigned char* sCj = sC + jj;
-            if (ALT && ((i0 ^ (jlo + jj)) & 1))
-                eq_accumulate<TI, MT, TMAX, ALT, 1>(sWj, sCj, ce, co, v, acc);
-            else
-                eq_accumulate<TI, MT, TMAX, ALT, 0>(sWj, sCj, ce, co, v, acc);
+            cp_async_commit();
+        };
+        fetch(0); fetch(1); fetch(2);
+        const bool par0 = ALT && ((i0 ^ jlo) & 1);
+        for (int jj = 0; jj < jw; ++jj) {
+            fetch(jj + 3);
+            cp_async_wait<3>();
+            cx<float> v[2][MT];
+#pragma unroll
+            for (int mt = 0; mt < MT; ++mt) { v[0][mt] = sB[jj & 3][0][mt][threadIdx.x]; v[1][mt] = sB[jj & 3][1][mt][threadIdx.x]; }
+            eq_input_ring<TI, MT, TMAX, ALT>(sW + jj * TMAX, sC[jj], par0 != ((jj & 1) != 0), ce, co, v, acc);
         }
 #pragma unroll
         for (int ii = 0; ii < TI; ++ii) {
