@@ -67,7 +67,8 @@ typedef struct {
 /* Options; pass NULL for the defaults (all fields zero).
  *  variant           0: anti-ringing scheme of PAPER.md:219 (periodic extension of the ring spectra, folding of the
  *                       super-Nyquist modes, ring offsets inside the kernel evaluation).  1: the basic scheme of
- *                       PAPER.md:125, 142 (zero-pad, truncate) -- ARKCOS_UNSUPPORTED in this build.
+ *                       PAPER.md:125, 142 (ring spectra zero-padded above their Nyquist frequency, output truncated at
+ *                       the output ring's Nyquist frequency); served by the general band kernel only (slow path).
  *  ell_nyquist       length of the phi grid on which a kernel row that touches a polar-cap ring is sampled:
  *                       M'_i = max(8, 2 ceil(ell_nyquist * smax_i)), smax_i = max sin(theta) over output ring i and
  *                       its band, i.e. the row resolves wavenumber ell_nyquist along the ring.  0: chosen from the

@@ -82,7 +82,7 @@ template <class T, int RESEED>
 __global__ void band_mac_general_kernel(const BandItem* __restrict__ items, const NorthRec* __restrict__ north,
                                         const PairRec* __restrict__ pairs, const T* __restrict__ W,
                                         const RingRec* __restrict__ rings, int R, const cx<T>* __restrict__ specIn,
-                                        cx<T>* __restrict__ specOut, int64_t spec_stride)
+                                        cx<T>* __restrict__ specOut, int64_t spec_stride, int variant_a)
 {
     const BandItem it = items[blockIdx.x];
     const int i = it.ring, iS = R - 1 - i;
@@ -115,6 +115,12 @@ __global__ void band_mac_general_kernel(const BandItem* __restrict__ items, cons
                     }
                 }
                 if (2 * m == M) G *= (T)0.5;                         // the +-M/2 bins carry half the Nyquist term each
+                if (variant_a) {
+                    // basic variant: Bp_j zero-padded above ring j's Nyquist frequency (its own bin
+                    // split half/half when the grid extends past it), output truncated at ring i's Nyquist frequency
+                    if (2 * m > Ni || 2 * m > rj.n) continue;
+                    if (2 * m == rj.n && M > rj.n) G *= (T)0.5;
+                }
                 if (ri.shifted && (wi & 1)) G = -G;                   // exp(i m phi0_i) = (-1)^w exp(+-i m' phi0_i)
                 cx<T> vN = ext_mode(bN, m, rj.n, rj.shifted);
                 cx<T> vS = ext_mode(bS, m, rjS.n, rjS.shifted);

@@ -250,7 +250,7 @@ void build_fft_lens(const HostGeometry& g, HostTables& t, Stats& st, bool use_ff
 }
 
 // Ring-pair table for the northern output rings (the southern ones reuse the rows of their mirror images).
-void build_pairs(HostGeometry& g, double theta_max, double ell_nyq, int fixed_mprime, int band_threads, bool allow_fast,
+void build_pairs(HostGeometry& g, double theta_max, double ell_nyq, int fixed_mprime, int band_threads, bool allow_fast, bool allow_pole,
                  int sm_count, HostTables& t, Stats& st)
 {
     const int R = g.R, nnorth = (R + 1) / 2;
@@ -340,7 +340,7 @@ void build_pairs(HostGeometry& g, double theta_max, double ell_nyq, int fixed_mp
                 }
             }
         }
-        if (cls == 0 && t.north[i].pair_hi > t.north[i].pair_lo) {
+        if (cls == 0 && allow_pole && t.north[i].pair_hi > t.north[i].pair_lo) {
             bool same = true;
             const int M0 = t.pairs[t.north[i].pair_lo].M;
             for (int p = t.north[i].pair_lo; p < t.north[i].pair_hi; ++p) same = same && t.pairs[p].M == M0;
@@ -663,7 +663,7 @@ template <class T> int enqueue_convolve(const arkcos_plan* pl, const void* d_in,
     if (pl->nitems[0] > 0)
         band_mac_general_kernel<T, 16><<<dim3((unsigned)pl->nitems[0], (unsigned)nmaps), kBandThreads, 0, s0>>>(
             pl->d_items[0], pl->d_north, pl->d_pairs, (const T*)pl->d_W, pl->d_rings, g.R, (const cx<T>*)pl->d_specIn,
-            (cx<T>*)pl->d_specOut, g.spec_total);
+            (cx<T>*)pl->d_specOut, g.spec_total, pl->opt.variant == 1 ? 1 : 0);
     if (serial) cudaEventRecord(pl->ev_band[1], st);
     if (pl->npole > 0)
         band_mac_pole_kernel<T, 16><<<dim3((unsigned)pl->npole, (unsigned)nmaps), kPoleThreads,
@@ -711,7 +711,6 @@ static int plan_create_impl(arkcos_plan** out, const arkcos_pixelization* pix, c
     if (options) opt = *options;
     for (int r : opt.reserved) if (r != 0) return fail(ARKCOS_INVALID_ARG, "options.reserved must be zero");
     if (opt.variant != 0 && opt.variant != 1) return fail(ARKCOS_INVALID_ARG, "options.variant must be 0 or 1");
-    if (opt.variant == 1) return fail(ARKCOS_UNSUPPORTED, "variant 1 (zero-pad / truncate) is not implemented");
     if (opt.max_nmaps < 0 || opt.polar_oversample < 0 || opt.ell_nyquist < 0.0 || opt.max_nmaps > 65535)
         return fail(ARKCOS_INVALID_ARG, "negative option");
     const int maxlen = dtype == ARKCOS_F32 ? 16384 : 8192;
@@ -748,7 +747,7 @@ static int plan_create_impl(arkcos_plan** out, const arkcos_pixelization* pix, c
     pl->sm_count = sm_count;
     HostTables t;
     build_fft_lens(pl->g, t, pl->stats, dtype == ARKCOS_F32 && !getenv("ARKCOS_FORCE_OLD_FFT"));
-    build_pairs(pl->g, pl->theta_max, pl->ell_nyquist, fixed_mprime, kBandThreads, dtype == ARKCOS_F32 && !getenv("ARKCOS_FORCE_GENERAL"), sm_count, t, pl->stats);
+    build_pairs(pl->g, pl->theta_max, pl->ell_nyquist, fixed_mprime, kBandThreads, dtype == ARKCOS_F32 && opt.variant == 0 && !getenv("ARKCOS_FORCE_GENERAL"), opt.variant == 0, sm_count, t, pl->stats);
     if (t.pairs.size() > (size_t)INT32_MAX) return fail(ARKCOS_UNSUPPORTED, "too many ring pairs");
     pl->nnorth = (int)t.north.size();
     pl->npairs = (int)t.pairs.size();

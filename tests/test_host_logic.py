@@ -31,8 +31,9 @@ def test_strerror_and_bad_args():
             arkcos.Plan(bad, tab, 0.2, tables_only=True)
         assert e.value.status == arkcos.INVALID_ARG
     with pytest.raises(arkcos.ArkcosError) as e:
-        arkcos.Plan(("healpix", 4), tab, 0.2, variant=1, tables_only=True)
-    assert e.value.status == arkcos.UNSUPPORTED
+        arkcos.Plan(("healpix", 4), tab, 0.2, variant=2, tables_only=True)
+    assert e.value.status == arkcos.INVALID_ARG
+    assert arkcos.Plan(("healpix", 4), tab, 0.2, variant=1, tables_only=True).nrings == 15     # the basic scheme
     with pytest.raises(arkcos.ArkcosError):
         arkcos.Plan(("healpix", 4), tab, -1.0, tables_only=True)
     p = arkcos.Plan(("healpix", 4), tab, 0.2, tables_only=True)

@@ -122,6 +122,32 @@ def test_healpix_paper_grid_polar_oversample():
     assert maxrel(out, hybrid.hybrid_convolve(geom, tab, tmax, x, mprime=4 * nside)) <= 1e-12
 
 
+@pytest.mark.parametrize("dtype,oversample", [(arkcos.F64, 1), (arkcos.F64, 0), (arkcos.F32, 1)])
+def test_variant_a_zero_pad_truncate(dtype, oversample):
+    """variant = 1 is the paper's basic scheme: parity with oracle #2 run as variant "A"."""
+    nside = 16
+    geom = geometry.healpix_ring(nside)
+    fwhm = 3 * np.sqrt(4 * np.pi / geom.npix)
+    tmax = 3 * fwhm
+    tab = inputs.gaussian_table(fwhm, tmax)
+    x = inputs.white_noise(geom.npix, 9, dtype=np.float64 if dtype == arkcos.F64 else np.float32)
+    out, plan = gpu_convolve(("healpix", nside), tab, tmax, x, dtype, variant=1, polar_oversample=oversample)
+    mp = np.array([plan.ring_info(i)["mprime"] for i in range(geom.nrings)])
+    ref = hybrid.hybrid_convolve(geom, tab, tmax, x.astype(np.float64), variant="A", mprime=mp)
+    refB = hybrid.hybrid_convolve(geom, tab, tmax, x.astype(np.float64), variant="B", mprime=mp)
+    assert maxrel(refB, ref) > 1e-4                      # the two variants really differ on white noise
+    if dtype == arkcos.F64:
+        assert maxrel(out, ref) <= 1e-12
+    else:
+        assert frms(out, ref) <= 1e-6
+    # ECP: both variants coincide (every pair is class E, nothing above the common Nyquist frequency)
+    ge = geometry.ecp(16, 32)
+    te = inputs.gaussian_table(0.5, 1.0, 4096)
+    xe = inputs.white_noise(ge.npix, 8, dtype=np.float64)
+    oa, _ = gpu_convolve(("ecp", 16, 32), te, 1.0, xe, arkcos.F64, variant=1)
+    assert maxrel(oa, direct.direct_sum(ge, te, 1.0, xe)) <= 1e-12
+
+
 def test_hard_edged_kernels_vs_scheme_oracle():
     """Top-hat and Mexican hat (config 5's kernels) at nside 32, 3 maps: GPU == oracle #2; equatorial rings == oracle #1."""
     nside = 32
