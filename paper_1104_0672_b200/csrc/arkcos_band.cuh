@@ -296,26 +296,29 @@ __device__ __forceinline__ void eq_accumulate(const float* __restrict__ sWj, con
     for (int ii = 0; ii < TI; ++ii) {
         const float4* __restrict__ w4 = reinterpret_cast<const float4*>(sWj + ii * (kEqJMax * TMAX));
         const bool odd = ALT && ((PAR ^ ii) & 1) != 0;          // compile-time after unrolling
-        float G[MT];
+        float2 sG[MT];                                          // (even-sample sum, odd-sample sum): packed FMAs (FFMA2)
 #pragma unroll
-        for (int mt = 0; mt < MT; ++mt) G[mt] = 0.f;
+        for (int mt = 0; mt < MT; ++mt) sG[mt] = make_float2(0.f, 0.f);
 #pragma unroll
         for (int t4 = 0; t4 < C4; ++t4) {
             const float4 w = w4[t4];
 #pragma unroll
             for (int mt = 0; mt < MT; ++mt) {
                 const float* c = odd ? co[mt] : ce[mt];
-                G[mt] = fmaf(w.x, c[4 * t4], G[mt]); G[mt] = fmaf(w.y, c[4 * t4 + 1], G[mt]);
-                G[mt] = fmaf(w.z, c[4 * t4 + 2], G[mt]); G[mt] = fmaf(w.w, c[4 * t4 + 3], G[mt]);
+                sG[mt] = ffma2(make_float2(w.x, w.y), make_float2(c[4 * t4], c[4 * t4 + 1]), sG[mt]);
+                sG[mt] = ffma2(make_float2(w.z, w.w), make_float2(c[4 * t4 + 2], c[4 * t4 + 3]), sG[mt]);
             }
         }
 #pragma unroll
-        for (int h = 0; h < 2; ++h)
+        for (int mt = 0; mt < MT; ++mt) {
+            const float G = sG[mt].x + sG[mt].y;
 #pragma unroll
-            for (int mt = 0; mt < MT; ++mt) {
-                acc[ii][h][mt].x = fmaf(G[mt], v[h][mt].x, acc[ii][h][mt].x);
-                acc[ii][h][mt].y = fmaf(G[mt], v[h][mt].y, acc[ii][h][mt].y);
+            for (int h = 0; h < 2; ++h) {
+                const float2 a = ffma2(make_float2(G, G), make_float2(v[h][mt].x, v[h][mt].y),
+                                       make_float2(acc[ii][h][mt].x, acc[ii][h][mt].y));
+                acc[ii][h][mt] = mk<float>(a.x, a.y);
             }
+        }
     }
 }
 
@@ -347,14 +350,15 @@ band_mac_eq_kernel(const EqChunk* __restrict__ chunks, const NorthRec* __restric
     __shared__ __align__(16) float sW[TI * kEqJMax * TMAX];       // [ii][jj][t]
     __shared__ int sC[kEqJMax];                                    // [jj]: longest row length / 4 over the tile's rings
     __shared__ int2 sJ[kEqJMax];                                   // spectrum offsets of input ring jlo + jj (N, S)
-    __shared__ cx<float> sB[4][2][MT][kBandThreads];               // in-flight input-ring coefficients, [stage][N/S][mode][thread]
+    static_assert(MT == 2, "a thread owns two adjacent modes: one 16-byte access per ring");
+    __shared__ float4 sB[4][2][kBandThreads];                      // in-flight input-ring coefficients, [stage][N/S][thread]
     const EqChunk ch = chunks[blockIdx.y];
     const int M = rings[ch.i0].n, Mh = M >> 1;
     int m[MT];
     float ce[MT][TMAX], co[MT][TMAX];
 #pragma unroll
     for (int mt = 0; mt < MT; ++mt) {
-        m[mt] = (int)blockIdx.x * (kBandThreads * MT) + mt * kBandThreads + (int)threadIdx.x;
+        m[mt] = (int)blockIdx.x * (kBandThreads * MT) + MT * (int)threadIdx.x + mt;
         const uint32_t mm = (uint32_t)min(m[mt], Mh - 1), twoM = 2u * (uint32_t)M;
 #pragma unroll
         for (int t = 0; t < TMAX; ++t) {
@@ -362,9 +366,8 @@ band_mac_eq_kernel(const EqChunk* __restrict__ chunks, const NorthRec* __restric
             co[mt][t] = ALT ? cispi_ratio<float>((mm * (uint32_t)(2 * t + 1)) % twoM, (uint32_t)M).x : 0.f;
         }
     }
-    const cx<float>* __restrict__ inm[MT];
-#pragma unroll
-    for (int mt = 0; mt < MT; ++mt) inm[mt] = specIn + (int64_t)blockIdx.z * spec_stride + min(m[mt], Mh - 1);
+    // ring rows start on even coefficient indices (plan), so the thread's mode pair is one aligned 16-byte word
+    const cx<float>* __restrict__ in0 = specIn + (int64_t)blockIdx.z * spec_stride + min(m[0], Mh - 2);
     cx<float>* __restrict__ out = specOut + (int64_t)blockIdx.z * spec_stride;
 
     for (int tile = 0; tile < ch.n; tile += TI) {
@@ -405,11 +408,8 @@ band_mac_eq_kernel(const EqChunk* __restrict__ chunks, const NorthRec* __restric
         auto fetch = [&](int jj) {
             if (jj < jw) {
                 const int2 off = sJ[jj];
-#pragma unroll
-                for (int mt = 0; mt < MT; ++mt) {
-                    cp_async8(&sB[jj & 3][0][mt][threadIdx.x], inm[mt] + off.x);
-                    cp_async8(&sB[jj & 3][1][mt][threadIdx.x], inm[mt] + off.y);
-                }
+                cp_async16(&sB[jj & 3][0][threadIdx.x], in0 + off.x);
+                cp_async16(&sB[jj & 3][1][threadIdx.x], in0 + off.y);
             }
             cp_async_commit();
         };
@@ -420,7 +420,11 @@ band_mac_eq_kernel(const EqChunk* __restrict__ chunks, const NorthRec* __restric
             cp_async_wait<3>();
             cx<float> v[2][MT];
 #pragma unroll
-            for (int mt = 0; mt < MT; ++mt) { v[0][mt] = sB[jj & 3][0][mt][threadIdx.x]; v[1][mt] = sB[jj & 3][1][mt][threadIdx.x]; }
+            for (int h = 0; h < 2; ++h) {
+                const float4 q = sB[jj & 3][h][threadIdx.x];
+                v[h][0] = mk<float>(q.x, q.y);
+                v[h][1] = mk<float>(q.z, q.w);
+            }
             eq_input_ring<TI, MT, TMAX, ALT>(sW + jj * TMAX, sC[jj], par0 != ((jj & 1) != 0), ce, co, v, acc);
         }
 #pragma unroll
@@ -428,11 +432,12 @@ band_mac_eq_kernel(const EqChunk* __restrict__ chunks, const NorthRec* __restric
             if (ii < nti) {
                 const int i = i0 + ii, iS = R - 1 - i;
                 const int64_t offN = rings[i].spec_off, offS = rings[iS].spec_off;
-#pragma unroll
-                for (int mt = 0; mt < MT; ++mt) {
-                    if (m[mt] >= Mh) continue;
-                    out[offN + m[mt]] = acc[ii][0][mt];
-                    if (iS != i) out[offS + m[mt]] = acc[ii][1][mt];
+                if (m[0] < Mh) {
+                    *reinterpret_cast<float4*>(out + offN + m[0]) =
+                        make_float4(acc[ii][0][0].x, acc[ii][0][0].y, acc[ii][0][1].x, acc[ii][0][1].y);
+                    if (iS != i)
+                        *reinterpret_cast<float4*>(out + offS + m[0]) =
+                            make_float4(acc[ii][1][0].x, acc[ii][1][0].y, acc[ii][1][1].x, acc[ii][1][1].y);
                 }
             }
         }
@@ -534,17 +539,17 @@ __device__ __forceinline__ void cap_row(const float* __restrict__ w, const float
                                         float& G1, float& G2)
 {
     const float4* __restrict__ w4 = reinterpret_cast<const float4*>(w);
-    float a1 = 0.f, a2 = 0.f, b1 = 0.f, b2 = 0.f;                       // two partial sums per mode
+    float2 s1 = make_float2(0.f, 0.f), s2 = make_float2(0.f, 0.f);      // (even-sample sum, odd-sample sum) per mode
 #pragma unroll
-    for (int t4 = 0; t4 < C4; ++t4) {
+    for (int t4 = 0; t4 < C4; ++t4) {                                   // packed FMAs (FFMA2): two samples per issue slot
         const float4 v = w4[t4];
-        a1 = fmaf(v.x, c1[4 * t4], a1);     a2 = fmaf(v.x, c2[4 * t4], a2);
-        b1 = fmaf(v.y, c1[4 * t4 + 1], b1); b2 = fmaf(v.y, c2[4 * t4 + 1], b2);
-        a1 = fmaf(v.z, c1[4 * t4 + 2], a1); a2 = fmaf(v.z, c2[4 * t4 + 2], a2);
-        b1 = fmaf(v.w, c1[4 * t4 + 3], b1); b2 = fmaf(v.w, c2[4 * t4 + 3], b2);
+        s1 = ffma2(make_float2(v.x, v.y), make_float2(c1[4 * t4], c1[4 * t4 + 1]), s1);
+        s2 = ffma2(make_float2(v.x, v.y), make_float2(c2[4 * t4], c2[4 * t4 + 1]), s2);
+        s1 = ffma2(make_float2(v.z, v.w), make_float2(c1[4 * t4 + 2], c1[4 * t4 + 3]), s1);
+        s2 = ffma2(make_float2(v.z, v.w), make_float2(c2[4 * t4 + 2], c2[4 * t4 + 3]), s2);
     }
-    G1 = a1 + b1;
-    G2 = a2 + b2;
+    G1 = s1.x + s1.y;
+    G2 = s2.x + s2.y;
 }
 
 struct CapVals { cx<float> v1N, v1S, v2N, v2S; };

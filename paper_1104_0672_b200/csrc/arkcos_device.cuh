@@ -42,6 +42,19 @@ template <class T> __device__ __forceinline__ cx<T> cispi_ratio(uint32_t num, ui
     return mk<T>(c, s);
 }
 
+// Packed FP32 FMA of sm_100 (SASS FFMA2): two fused multiply-adds in one issue slot, d = a * b + c per component.
+__device__ __forceinline__ float2 ffma2(float2 a, float2 b, float2 c)
+{
+    unsigned long long ra, rb, rc, rd;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(ra) : "f"(a.x), "f"(a.y));
+    asm("mov.b64 %0, {%1, %2};" : "=l"(rb) : "f"(b.x), "f"(b.y));
+    asm("mov.b64 %0, {%1, %2};" : "=l"(rc) : "f"(c.x), "f"(c.y));
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(rd) : "l"(ra), "l"(rb), "l"(rc));
+    float2 d;
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(d.x), "=f"(d.y) : "l"(rd));
+    return d;
+}
+
 // cp.async (LDGSTS) of 8 bytes global -> shared, and its group bookkeeping
 __device__ __forceinline__ void cp_async8(void* smem_dst, const void* gsrc)
 {

@@ -83,7 +83,7 @@ int build_geometry(const arkcos_pixelization& pix, HostGeometry& g)
     g.spec_off.assign(g.R + 1, 0);
     for (int i = 0; i < g.R; ++i) {
         g.pix_off[i + 1] = g.pix_off[i] + g.n[i];
-        g.spec_off[i + 1] = g.spec_off[i] + g.n[i] / 2 + 1;
+        g.spec_off[i + 1] = g.spec_off[i] + ((g.n[i] / 2 + 2) & ~1);     // N/2 + 1 coefficients, rows start 16-byte aligned
     }
     g.npix = g.pix_off[g.R];
     g.spec_total = g.spec_off[g.R];
