@@ -760,6 +760,8 @@ static int plan_create_impl(arkcos_plan** out, const arkcos_pixelization* pix, c
     for (const EqChunk& c : t.eq_chunks) pl->eq_mh = std::max(pl->eq_mh, pl->g.n[c.i0] / 2);
     pl->nsamples = t.nsamples;
     pl->logPT = t.logPT;
+    pl->nfft_old = (int)t.fft_order.size();
+    for (int c = 0; c < 4; ++c) pl->nfft3[c] = (int)t.fft3_jobs[c].size();
 
     if (tables_only) {
         guard.p = nullptr;
