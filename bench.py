@@ -213,9 +213,28 @@ def run_ours(args):
     t = torch.tensor([e0.elapsed_time(e1)], device="cuda", dtype=torch.float64)
     if world > 1:
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    e2e_sync_ms = float(t.item()) / args.steps
+    # the streaming form of the same call (arkcos_convolve_host_async): every step still uploads its input and
+    # downloads its result inside the timed region, but the upload of step k+1 and the download of step k-1 overlap
+    # the kernels of step k (two staging sets in the plan)
+    plan.convolve_host_async(h_in.data_ptr(), h_out.data_ptr(), nmaps)
+    plan.synchronize()
+    barrier()
+    e0.record()
+    for _ in range(args.steps):
+        plan.convolve_host_async(h_in.data_ptr(), h_out.data_ptr(), nmaps)
+    plan.synchronize()
+    e1.record()
+    barrier()
+    t = torch.tensor([e0.elapsed_time(e1)], device="cuda", dtype=torch.float64)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
     e2e_ms = float(t.item()) / args.steps
     e2e = {"value": world * npix * nmaps / (e2e_ms * 1e-3) / 1e6, "unit": UNIT, "ms_per_step": e2e_ms,
-           "h2d_bytes_per_step": int(x.nbytes), "d2h_bytes_per_step": int(x.nbytes)}
+           "h2d_bytes_per_step": int(x.nbytes), "d2h_bytes_per_step": int(x.nbytes),
+           "api": "arkcos_convolve_host_async x steps + arkcos_plan_synchronize (copies of neighbouring steps overlap)",
+           "blocking_call_ms_per_step": e2e_sync_ms,
+           "blocking_call_value": world * npix * nmaps / (e2e_sync_ms * 1e-3) / 1e6}
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()

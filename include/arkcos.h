@@ -108,6 +108,16 @@ int arkcos_convolve(const arkcos_plan* plan, const void* d_in, void* d_out, int 
  * device -> host copy, all on cuda_stream, then a stream synchronisation.  Uses staging buffers inside the plan. */
 int arkcos_convolve_host(const arkcos_plan* plan, const void* h_in, void* h_out, int nmaps, void* cuda_stream);
 
+/* Streaming form of the same for a sequence of maps (the paper's use case: one map per detector): the call
+ * returns as soon as its three stages are enqueued on plan-owned streams -- host -> device copy, arkcos_convolve,
+ * device -> host copy -- with two sets of staging buffers, so that the upload of call k+1 and the download of call k-1
+ * overlap the kernels of call k.  h_in must stay valid and unmodified, and h_out unread, until
+ * arkcos_plan_synchronize returns (or two further calls have been made and synchronised).  Pinned host memory is needed
+ * for the copies to overlap.  Do not mix with arkcos_convolve / arkcos_convolve_host on the same plan without an
+ * arkcos_plan_synchronize in between. */
+int arkcos_convolve_host_async(const arkcos_plan* plan, const void* h_in, void* h_out, int nmaps);
+int arkcos_plan_synchronize(const arkcos_plan* plan);
+
 int arkcos_plan_destroy(arkcos_plan* plan);      /* NULL is a no-op */
 
 /* ---- queries (host side, no CUDA work) ---- */

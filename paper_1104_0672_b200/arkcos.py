@@ -50,6 +50,8 @@ SYMBOLS = {
                                                POINTER(Options)]),
     "arkcos_convolve": (c_int, [c_void_p, c_void_p, c_void_p, c_int, c_void_p]),
     "arkcos_convolve_host": (c_int, [c_void_p, c_void_p, c_void_p, c_int, c_void_p]),
+    "arkcos_convolve_host_async": (c_int, [c_void_p, c_void_p, c_void_p, c_int]),
+    "arkcos_plan_synchronize": (c_int, [c_void_p]),
     "arkcos_plan_destroy": (c_int, [c_void_p]),
     "arkcos_plan_npix": (c_int64, [c_void_p]),
     "arkcos_plan_nrings": (c_int, [c_void_p]),
@@ -127,6 +129,14 @@ class Plan:
     def convolve_host(self, h_in: int, h_out: int, nmaps: int = 1, stream: int = 0):
         _check(_lib().arkcos_convolve_host(self._h, c_void_p(h_in), c_void_p(h_out), int(nmaps), c_void_p(stream)),
                "arkcos_convolve_host")
+
+    def convolve_host_async(self, h_in: int, h_out: int, nmaps: int = 1):
+        """Streaming form: returns once upload, kernels and download are enqueued; finish with synchronize()."""
+        _check(_lib().arkcos_convolve_host_async(self._h, c_void_p(h_in), c_void_p(h_out), int(nmaps)),
+               "arkcos_convolve_host_async")
+
+    def synchronize(self):
+        _check(_lib().arkcos_plan_synchronize(self._h), "arkcos_plan_synchronize")
 
     def destroy(self):
         if getattr(self, "_h", None) is not None and self._h:

@@ -844,9 +844,66 @@ int arkcos_convolve_host(const arkcos_plan* pl, const void* h_in, void* h_out, i
     return ARKCOS_OK;
 }
 
+int arkcos_convolve_host_async(const arkcos_plan* pl, const void* h_in, void* h_out, int nmaps)
+{
+    if (!pl || !h_in || !h_out) return fail(ARKCOS_INVALID_ARG, "NULL argument");
+    if (pl->tables_only) return fail(ARKCOS_INVALID_ARG, "plan was created with arkcos_plan_create_tables_only");
+    if (nmaps < 1 || nmaps > pl->max_nmaps) return fail(ARKCOS_INVALID_ARG, "nmaps must be in [1, max_nmaps]");
+    const size_t full = (size_t)pl->max_nmaps * (size_t)pl->g.npix * elem_size(pl->dtype);
+    const size_t bytes = (size_t)nmaps * (size_t)pl->g.npix * elem_size(pl->dtype);
+    if (!pl->s_h2d) {
+        for (int b = 0; b < 2; ++b) {
+            CUDA_TRY(cudaMalloc(&pl->d_pipe_in[b], full));
+            CUDA_TRY(cudaMalloc(&pl->d_pipe_out[b], full));
+            CUDA_TRY(cudaEventCreateWithFlags(&pl->ev_h2d[b], cudaEventDisableTiming));
+            CUDA_TRY(cudaEventCreateWithFlags(&pl->ev_comp[b], cudaEventDisableTiming));
+            CUDA_TRY(cudaEventCreateWithFlags(&pl->ev_d2h[b], cudaEventDisableTiming));
+        }
+        CUDA_TRY(cudaStreamCreateWithFlags(&pl->s_comp, cudaStreamNonBlocking));
+        CUDA_TRY(cudaStreamCreateWithFlags(&pl->s_d2h, cudaStreamNonBlocking));
+        CUDA_TRY(cudaStreamCreateWithFlags(&pl->s_h2d, cudaStreamNonBlocking));
+    }
+    const int b = (int)(pl->pipe_calls & 1);
+    const bool reuse = pl->pipe_calls >= 2;
+    // upload into set b once the kernels of the call before last have read it
+    if (reuse) CUDA_TRY(cudaStreamWaitEvent(pl->s_h2d, pl->ev_comp[b], 0));
+    CUDA_TRY(cudaMemcpyAsync(pl->d_pipe_in[b], h_in, bytes, cudaMemcpyHostToDevice, pl->s_h2d));
+    CUDA_TRY(cudaEventRecord(pl->ev_h2d[b], pl->s_h2d));
+    // kernels: after the upload, and after the download of the call before last has read the output set
+    CUDA_TRY(cudaStreamWaitEvent(pl->s_comp, pl->ev_h2d[b], 0));
+    if (reuse) CUDA_TRY(cudaStreamWaitEvent(pl->s_comp, pl->ev_d2h[b], 0));
+    if (int rc = arkcos_convolve(pl, pl->d_pipe_in[b], pl->d_pipe_out[b], nmaps, (void*)pl->s_comp)) return rc;
+    CUDA_TRY(cudaEventRecord(pl->ev_comp[b], pl->s_comp));
+    // download
+    CUDA_TRY(cudaStreamWaitEvent(pl->s_d2h, pl->ev_comp[b], 0));
+    CUDA_TRY(cudaMemcpyAsync(h_out, pl->d_pipe_out[b], bytes, cudaMemcpyDeviceToHost, pl->s_d2h));
+    CUDA_TRY(cudaEventRecord(pl->ev_d2h[b], pl->s_d2h));
+    ++pl->pipe_calls;
+    return ARKCOS_OK;
+}
+
+int arkcos_plan_synchronize(const arkcos_plan* pl)
+{
+    if (!pl) return fail(ARKCOS_INVALID_ARG, "NULL plan");
+    if (pl->s_h2d) {
+        CUDA_TRY(cudaStreamSynchronize(pl->s_h2d));
+        CUDA_TRY(cudaStreamSynchronize(pl->s_comp));
+        CUDA_TRY(cudaStreamSynchronize(pl->s_d2h));
+    }
+    return ARKCOS_OK;
+}
+
 int arkcos_plan_destroy(arkcos_plan* pl)
 {
     if (!pl) return ARKCOS_OK;
+    for (int b = 0; b < 2; ++b) {
+        if (pl->d_pipe_in[b]) cudaFree(pl->d_pipe_in[b]);
+        if (pl->d_pipe_out[b]) cudaFree(pl->d_pipe_out[b]);
+        if (pl->ev_h2d[b]) cudaEventDestroy(pl->ev_h2d[b]);
+        if (pl->ev_comp[b]) cudaEventDestroy(pl->ev_comp[b]);
+        if (pl->ev_d2h[b]) cudaEventDestroy(pl->ev_d2h[b]);
+    }
+    for (cudaStream_t q : {pl->s_h2d, pl->s_comp, pl->s_d2h}) if (q) cudaStreamDestroy(q);
     void* ptrs[] = {pl->d_rings, pl->d_lens, pl->d_pairs, pl->d_north, pl->d_items[0], pl->d_items[1], pl->d_items[2], pl->d_items[3],
                     pl->d_items[4], pl->d_items[5], pl->d_eqchunks, pl->d_pole, pl->d_chirp, pl->d_phase, pl->d_fft_order, pl->d_table, pl->d_tw, pl->d_filt,
                     pl->d_W, pl->d_specIn, pl->d_specOut, pl->d_stage_in, pl->d_stage_out,

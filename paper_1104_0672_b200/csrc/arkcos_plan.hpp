@@ -73,6 +73,12 @@ struct arkcos_plan {
     // lazily allocated staging for arkcos_convolve_host
     mutable void* d_stage_in = nullptr;
     mutable void* d_stage_out = nullptr;
+    // arkcos_convolve_host_async: two staging sets, copy / compute streams, events of the last use of each set
+    mutable void* d_pipe_in[2] = {nullptr, nullptr};
+    mutable void* d_pipe_out[2] = {nullptr, nullptr};
+    mutable cudaStream_t s_h2d = nullptr, s_comp = nullptr, s_d2h = nullptr;
+    mutable cudaEvent_t ev_h2d[2] = {nullptr, nullptr}, ev_comp[2] = {nullptr, nullptr}, ev_d2h[2] = {nullptr, nullptr};
+    mutable uint64_t pipe_calls = 0;
     // optional per-stage timing
     mutable int timing = 0;
     mutable cudaEvent_t ev[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};

@@ -234,6 +234,26 @@ def test_multi_map_equals_single_and_host_path():
     np.testing.assert_array_equal(out_c, out)
 
 
+def test_streaming_host_path_equals_device_path():
+    """arkcos_convolve_host_async: five maps streamed through the two staging sets give the bits of arkcos_convolve."""
+    nside = 32
+    geom = geometry.healpix_ring(nside)
+    fwhm = 3 * np.sqrt(4 * np.pi / geom.npix)
+    tmax = 3 * fwhm
+    tab = inputs.gaussian_table(fwhm, tmax)
+    x = inputs.white_noise_maps(geom.npix, 7, 5)
+    plan = arkcos.Plan(("healpix", nside), tab, tmax, arkcos.F32)
+    ref = np.stack([gpu_convolve(("healpix", nside), tab, tmax, x[k], plan=plan)[0] for k in range(5)])
+    h_in = torch.from_numpy(x).pin_memory()
+    h_out = torch.full_like(h_in, float("nan")).pin_memory()
+    for rep in range(2):
+        for k in range(5):
+            plan.convolve_host_async(h_in[k].data_ptr(), h_out[k].data_ptr(), 1)
+        plan.synchronize()
+        np.testing.assert_array_equal(h_out.numpy(), ref)
+        h_out.fill_(float("nan"))
+
+
 def test_argument_errors():
     tab = inputs.gaussian_table(0.2, 0.4, 256)
     plan = arkcos.Plan(("ecp", 8, 16), tab, 0.4, arkcos.F32, max_nmaps=2)
