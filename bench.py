@@ -119,9 +119,12 @@ def run_reference(args):
     if int(os.environ.get("RANK", "0")) != 0:
         return
     c, tab, x, npix, nmaps, name = workload(args.cfg)
-    nsample = args.oracle_rings
-    for _ in range(args.warmup):
+    # size the per-step sample so that the whole run stays near two minutes on this host: calibrate on 32 rings
+    cal = time_oracle(c, tab, x, 32)
+    for _ in range(max(args.warmup - 1, 0)):
         time_oracle(c, tab, x, 4)
+    per_ring = cal["seconds"] / max(cal["rings"], 1)
+    nsample = int(min(args.oracle_rings, max(8, 120.0 / (per_ring * max(args.steps, 1)))))
     tot_t, tot_px, info = 0.0, 0, None
     for _ in range(args.steps):
         info = time_oracle(c, tab, x, nsample)
