@@ -519,7 +519,7 @@ namespace {
 template <class T> int enqueue_rows(const arkcos_plan* pl, cudaStream_t st)
 {
     if (pl->npairs > 0)
-        kernel_rows_kernel<T><<<pl->npairs, 32, 0, st>>>(pl->d_pairs, pl->npairs, pl->d_table, pl->ntab, pl->theta_max,
+        kernel_rows_kernel<T><<<(pl->npairs + 3) / 4, 128, 0, st>>>(pl->d_pairs, pl->npairs, pl->d_table, pl->ntab, pl->theta_max,
                                                          (T*)pl->d_W);
     return 0;
 }
