@@ -28,32 +28,15 @@ template <int LOGQ> struct Fft3 {
     static constexpr size_t smem_bytes = 2 * (size_t)SQ * sizeof(cx<float>);
 };
 
-// w[r] = tw[r * idx], r = 1 .. R-1 (tw[k] = exp(-2 pi i k / PT)); at most one product per twiddle
-template <int R> __device__ __forceinline__ void load_tw(cx<float>* w, const cx<float>* __restrict__ tw, int idx)
-{
-    w[1] = tw[idx];
-    if (R >= 4) { w[2] = tw[2 * idx]; w[3] = tw[3 * idx]; }
-    if (R >= 8) {
-        w[4] = tw[4 * idx];
-#pragma unroll
-        for (int r = 5; r < 8; ++r) w[r] = cmul(w[4], w[r - 4]);
-    }
-    if (R >= 16) {
-        w[8] = tw[8 * idx];
-        w[12] = tw[12 * idx];
-#pragma unroll
-        for (int r = 9; r < 12; ++r) w[r] = cmul(w[8], w[r - 8]);
-#pragma unroll
-        for (int r = 13; r < 16; ++r) w[r] = cmul(w[12], w[r - 12]);
-    }
-}
-
 // Forward complex DFT of size Q of NB sequences held in registers: in  u[b][r] = x_b[t + T r],  out u[b][q] = X_b[t + T q].
-// s: NB arrays of SQ complex numbers (padded indexing e + e/16).  tw16[16 k + r] = exp(-2 pi i r k / 256).
+// s: NB arrays of SQ complex numbers (padded indexing e + e/16).  Twiddle tables laid out so that a warp reads whole
+// 128-byte lines (the L1 data pipe is the busiest unit of these kernels):
+//   tw16[16 r + k] = exp(-2 pi i r k / 256)  (pass 2: lane k = t mod 16),
+//   tw3[256 (r - 1) + i] = exp(-2 pi i r i / Q), r = 1 .. RL-1, i < 256  (pass 3, one table per transform size).
 // Entry: any earlier readers of s must have passed a barrier.  Exit: results in registers, s free after the next barrier.
 template <int LOGQ, int NB>
 __device__ __forceinline__ void fft3(cx<float> (&u)[NB][16], cx<float>* __restrict__ s, const cx<float>* __restrict__ tw,
-                                     int logPT, const cx<float>* __restrict__ tw16)
+                                     int logPT, const cx<float>* __restrict__ tw16, const cx<float>* __restrict__ tw3)
 {
     using F = Fft3<LOGQ>;
     constexpr int T = F::T, RL = F::RL, NC = F::NC, SQ = F::SQ;
@@ -67,15 +50,8 @@ __device__ __forceinline__ void fft3(cx<float> (&u)[NB][16], cx<float>* __restri
     }
     // pass 2 twiddles: row k = t mod 16 of the 16 x 16 table
     cx<float> w[16];
-    {
-        const float4* __restrict__ row = reinterpret_cast<const float4*>(tw16 + 16 * (t & 15));
 #pragma unroll
-        for (int r2 = 0; r2 < 8; ++r2) {
-            const float4 v = row[r2];
-            w[2 * r2] = mk<float>(v.x, v.y);
-            w[2 * r2 + 1] = mk<float>(v.z, v.w);
-        }
-    }
+    for (int r = 1; r < 16; ++r) w[r] = tw16[16 * r + (t & 15)];
     __syncthreads();
     const int ld0 = t + (t >> 4);
 #pragma unroll
@@ -105,7 +81,8 @@ __device__ __forceinline__ void fft3(cx<float> (&u)[NB][16], cx<float>* __restri
     for (int c = 0; c < NC; ++c) {
         const int i = t + T * c;
         cx<float> wl[RL];
-        load_tw<RL>(wl, tw, i << (logPT - LOGQ));
+#pragma unroll
+        for (int r = 1; r < RL; ++r) wl[r] = tw3[256 * (r - 1) + i];
 #pragma unroll
         for (int b = 0; b < NB; ++b) {
             cx<float> v[RL];
@@ -156,7 +133,8 @@ __device__ __forceinline__ cx<float> pack_inv(cx<float> xk, cx<float> xl, cx<flo
 template <int LOGQ>
 __device__ __forceinline__ void bluestein_core(cx<float> (&u)[2][16], cx<float>* __restrict__ s, const FftLen& f,
                                                const cx<float>* __restrict__ tw, int logPT,
-                                               const cx<float>* __restrict__ tw16, const cx<float>* __restrict__ filt)
+                                               const cx<float>* __restrict__ tw16, const cx<float>* __restrict__ tw3,
+                                               const cx<float>* __restrict__ filt)
 {
     using F = Fft3<LOGQ>;
     constexpr int T = F::T;
@@ -168,7 +146,7 @@ __device__ __forceinline__ void bluestein_core(cx<float> (&u)[2][16], cx<float>*
         const int n = t + T * r;
         u[1][r] = n < L ? cmul(u[0][r], tw[n << shP]) : mk<float>(0.f, 0.f);
     }
-    fft3<LOGQ, 2>(u, s, tw, logPT, tw16);
+    fft3<LOGQ, 2>(u, s, tw, logPT, tw16, tw3);
 #pragma unroll
     for (int q = 0; q < 16; ++q) {
         const float4 v = fl[t + T * q];
@@ -176,7 +154,7 @@ __device__ __forceinline__ void bluestein_core(cx<float> (&u)[2][16], cx<float>*
         u[1][q] = cconj(cmul(u[1][q], mk<float>(v.z, v.w)));
     }
     __syncthreads();
-    fft3<LOGQ, 2>(u, s, tw, logPT, tw16);                       // u[0] = conj(E), u[1] = conj(O)
+    fft3<LOGQ, 2>(u, s, tw, logPT, tw16, tw3);                       // u[0] = conj(E), u[1] = conj(O)
 #pragma unroll
     for (int q = 0; q < 16; ++q) {
         const int n = t + T * q;
@@ -190,8 +168,9 @@ __global__ void __launch_bounds__(Fft3<LOGQ>::T, Fft3<LOGQ>::MINB)
 ring_fft3_forward_kernel(const float* __restrict__ in, int64_t npix, cx<float>* __restrict__ spec, int64_t spec_stride,
                          const RingRec* __restrict__ rings, const FftJob* __restrict__ jobs,
                          const FftLen* __restrict__ lens, const cx<float>* __restrict__ tw, int logPT,
-                         const cx<float>* __restrict__ tw16, const cx<float>* __restrict__ filt,
-                         const cx<float>* __restrict__ chirp, const cx<float>* __restrict__ phase, int ahead)
+                         const cx<float>* __restrict__ tw16, const cx<float>* __restrict__ tw3,
+                         const cx<float>* __restrict__ filt, const cx<float>* __restrict__ chirp,
+                         const cx<float>* __restrict__ phase, int ahead)
 {
     using F = Fft3<LOGQ>;
     constexpr int T = F::T, SQ = F::SQ;
@@ -218,7 +197,7 @@ ring_fft3_forward_kernel(const float* __restrict__ in, int64_t npix, cx<float>* 
         const cx<float>* __restrict__ x1 = reinterpret_cast<const cx<float>*>(map + r1.pix_off);
 #pragma unroll
         for (int r = 0; r < 16; ++r) { u[0][r] = x0[t + T * r]; u[1][r] = x1[t + T * r]; }
-        fft3<LOGQ, 2>(u, s, tw, logPT, tw16);
+        fft3<LOGQ, 2>(u, s, tw, logPT, tw16, tw3);
         __syncthreads();
 #pragma unroll
         for (int b = 0; b < 2; ++b)
@@ -250,7 +229,7 @@ ring_fft3_forward_kernel(const float* __restrict__ in, int64_t npix, cx<float>* 
             const int n = t + T * r;
             u[0][r] = n < L ? cmul(x0[n], cw[n]) : mk<float>(0.f, 0.f);
         }
-        bluestein_core<LOGQ>(u, s, f, tw, logPT, tw16, filt);
+        bluestein_core<LOGQ>(u, s, f, tw, logPT, tw16, tw3, filt);
         // phases of the split: loaded now (into the registers of the odd half), used after the exchange
 #pragma unroll
         for (int q = 0; q < 16; ++q) {
@@ -287,8 +266,9 @@ __global__ void __launch_bounds__(Fft3<LOGQ>::T, Fft3<LOGQ>::MINB)
 ring_fft3_inverse_kernel(const cx<float>* __restrict__ spec, int64_t spec_stride, float* __restrict__ outmap, int64_t npix,
                          const RingRec* __restrict__ rings, const FftJob* __restrict__ jobs,
                          const FftLen* __restrict__ lens, const cx<float>* __restrict__ tw, int logPT,
-                         const cx<float>* __restrict__ tw16, const cx<float>* __restrict__ filt,
-                         const cx<float>* __restrict__ chirp, const cx<float>* __restrict__ phase, int ahead)
+                         const cx<float>* __restrict__ tw16, const cx<float>* __restrict__ tw3,
+                         const cx<float>* __restrict__ filt, const cx<float>* __restrict__ chirp,
+                         const cx<float>* __restrict__ phase, int ahead)
 {
     using F = Fft3<LOGQ>;
     constexpr int T = F::T;
@@ -318,7 +298,7 @@ ring_fft3_inverse_kernel(const cx<float>* __restrict__ spec, int64_t spec_stride
             u[0][r] = pack_inv(D[r0.spec_off + k], D[r0.spec_off + L - k], hk, hl, r0.shifted);
             u[1][r] = pack_inv(D[r1.spec_off + k], D[r1.spec_off + L - k], hk, hl, r1.shifted);
         }
-        fft3<LOGQ, 2>(u, s, tw, logPT, tw16);
+        fft3<LOGQ, 2>(u, s, tw, logPT, tw16, tw3);
         cx<float>* __restrict__ o0 = reinterpret_cast<cx<float>*>(map + r0.pix_off);
         cx<float>* __restrict__ o1 = reinterpret_cast<cx<float>*>(map + r1.pix_off);
 #pragma unroll
@@ -339,7 +319,7 @@ ring_fft3_inverse_kernel(const cx<float>* __restrict__ spec, int64_t spec_stride
             }
             u[0][r] = v;
         }
-        bluestein_core<LOGQ>(u, s, f, tw, logPT, tw16, filt);
+        bluestein_core<LOGQ>(u, s, f, tw, logPT, tw16, tw3, filt);
         // z'[n] = chirp[n] y[n]; out = conj(z') = conj(chirp[n]) conj(y[n])
         cx<float>* __restrict__ o0 = reinterpret_cast<cx<float>*>(map + r0.pix_off);
 #pragma unroll

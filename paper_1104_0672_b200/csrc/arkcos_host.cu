@@ -443,10 +443,22 @@ template <class T> int setup_fft3(arkcos_plan* pl, const HostTables& t)
     std::vector<cx<float>> tw16(256);
     for (int k = 0; k < 16; ++k)
         for (int r = 0; r < 16; ++r)
-            tw16[16 * k + r] = mk<float>((float)cos(2.0 * kPi * r * k / 256.0), (float)(-sin(2.0 * kPi * r * k / 256.0)));
+            tw16[16 * r + k] = mk<float>((float)cos(2.0 * kPi * r * k / 256.0), (float)(-sin(2.0 * kPi * r * k / 256.0)));
     cx<float>* d = nullptr;
     if (int rc = upload(&d, tw16, &pl->stats.workspace_bytes)) return rc;
     pl->d_tw16 = d;
+    // pass-3 twiddles of the four transform sizes: exp(-2 pi i r i / Q) at [256 (r - 1) + i], Q = 512 << c, r < Q / 256
+    std::vector<cx<float>> tw3;
+    for (int c = 0; c < 4; ++c) {
+        const int Q = 512 << c, RL = Q / 256;
+        pl->tw3_off[c] = (int)tw3.size();
+        for (int r = 1; r < RL; ++r)
+            for (int i = 0; i < 256; ++i)
+                tw3.push_back(mk<float>((float)cos(2.0 * kPi * r * i / Q), (float)(-sin(2.0 * kPi * r * i / Q))));
+    }
+    cx<float>* d3 = nullptr;
+    if (int rc = upload(&d3, tw3, &pl->stats.workspace_bytes)) return rc;
+    pl->d_tw3 = d3;
     if (int rc = set_fft3_smem<9>()) return rc;
     if (int rc = set_fft3_smem<10>()) return rc;
     if (int rc = set_fft3_smem<11>()) return rc;
@@ -577,12 +589,14 @@ void launch_fft3(const arkcos_plan* pl, const void* d_in, void* d_out, int nmaps
     if (FWD)
         ring_fft3_forward_kernel<LOGQ><<<grid, Fft3<LOGQ>::T, Fft3<LOGQ>::smem_bytes, st>>>(
             (const float*)d_in, g.npix, (cx<float>*)pl->d_specIn, g.spec_total, pl->d_rings, pl->d_fft3_jobs[c], pl->d_lens,
-            (const cx<float>*)pl->d_tw, pl->logPT, (const cx<float>*)pl->d_tw16, (const cx<float>*)pl->d_filt,
+            (const cx<float>*)pl->d_tw, pl->logPT, (const cx<float>*)pl->d_tw16, (const cx<float>*)pl->d_tw3 + pl->tw3_off[c],
+            (const cx<float>*)pl->d_filt,
             (const cx<float>*)pl->d_chirp, (const cx<float>*)pl->d_phase, ahead);
     else
         ring_fft3_inverse_kernel<LOGQ><<<grid, Fft3<LOGQ>::T, Fft3<LOGQ>::smem_bytes, st>>>(
             (const cx<float>*)pl->d_specOut, g.spec_total, (float*)d_out, g.npix, pl->d_rings, pl->d_fft3_jobs[c], pl->d_lens,
-            (const cx<float>*)pl->d_tw, pl->logPT, (const cx<float>*)pl->d_tw16, (const cx<float>*)pl->d_filt,
+            (const cx<float>*)pl->d_tw, pl->logPT, (const cx<float>*)pl->d_tw16, (const cx<float>*)pl->d_tw3 + pl->tw3_off[c],
+            (const cx<float>*)pl->d_filt,
             (const cx<float>*)pl->d_chirp, (const cx<float>*)pl->d_phase, ahead);
 }
 
@@ -907,7 +921,7 @@ int arkcos_plan_destroy(arkcos_plan* pl)
     void* ptrs[] = {pl->d_rings, pl->d_lens, pl->d_pairs, pl->d_north, pl->d_items[0], pl->d_items[1], pl->d_items[2], pl->d_items[3],
                     pl->d_items[4], pl->d_items[5], pl->d_eqchunks, pl->d_pole, pl->d_chirp, pl->d_phase, pl->d_fft_order, pl->d_table, pl->d_tw, pl->d_filt,
                     pl->d_W, pl->d_specIn, pl->d_specOut, pl->d_stage_in, pl->d_stage_out,
-                    pl->d_cap_rings, pl->d_cap_pairs, pl->d_tw16, pl->d_fft3_jobs[0], pl->d_fft3_jobs[1], pl->d_fft3_jobs[2], pl->d_fft3_jobs[3]};
+                    pl->d_cap_rings, pl->d_cap_pairs, pl->d_tw3, pl->d_tw16, pl->d_fft3_jobs[0], pl->d_fft3_jobs[1], pl->d_fft3_jobs[2], pl->d_fft3_jobs[3]};
     for (void* p : ptrs) if (p) cudaFree(p);
     for (auto& e : pl->ev) if (e) cudaEventDestroy(e);
     for (auto& e : pl->ev_band) if (e) cudaEventDestroy(e);
