@@ -77,14 +77,20 @@ typedef struct {
  *  max_nmaps         largest nmaps arkcos_convolve will be called with (sizes the workspace); 0 means 1.
  *  cache_kernel_rows 0: the kernel rows are re-evaluated from the profile table inside every arkcos_convolve (the
  *                       paper's timing includes the kernel evaluation, Table 1); 1: they are
- *                       evaluated once in arkcos_plan_create. */
+ *                       evaluated once in arkcos_plan_create.
+ *  exact_caps        1 (HEALPix only): every output ring whose band contains a ring shorter than 4 nside (the polar caps
+ *                       and the equatorial rings next to them) is recomputed by the direct-space sum of Eq. 6
+ *                        after the hybrid pass, so that hard-edged kernels, for which the Fourier
+ *                       scheme only suppresses ringing in the caps, are exact everywhere.  Slow path:
+ *                       fp64 distances per pixel pair, weights shared by the maps of a call. */
 typedef struct {
     int variant;
     double ell_nyquist;
     int polar_oversample;
     int max_nmaps;
     int cache_kernel_rows;
-    int reserved[8];               /* must be zero */
+    int exact_caps;
+    int reserved[7];               /* must be zero */
 } arkcos_options;
 
 /* Builds the ring-geometry table (theta, N, phi0, offset per ring), the band and ring-pair tables, FFT twiddles,

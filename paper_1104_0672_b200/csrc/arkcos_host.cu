@@ -7,6 +7,7 @@
 #include <algorithm>
 #include <map>
 #include <new>
+#include <type_traits>
 
 #include "arkcos_plan.hpp"
 
@@ -693,6 +694,18 @@ template <class T> int enqueue_convolve(const arkcos_plan* pl, const void* d_in,
         }
     if (tm) cudaEventRecord(pl->ev[3], st);
     launch_ring_ffts<T, false>(pl, d_in, d_out, nmaps, st);
+    if (pl->ndirect > 0) {                      // exact_caps: overwrite the cap-zone rings with the direct-space sum
+        const double sh = sin(0.5 * pl->theta_max), xmax = 4.0 * sh * sh;
+        auto launch = [&](auto nm_tag, int chunks) {
+            constexpr int NM = decltype(nm_tag)::value;
+            direct_rings_kernel<T, NM><<<dim3((unsigned)pl->ndirect, (unsigned)chunks), kDirectThreads, 0, st>>>(
+                pl->d_direct_items, pl->d_north, pl->d_pairs, pl->d_rings, g.R, pl->d_table, pl->ntab, pl->theta_max, xmax,
+                (const T*)d_in, (T*)d_out, g.npix, nmaps);
+        };
+        if (nmaps >= 8) launch(std::integral_constant<int, 16>{}, (nmaps + 15) / 16);
+        else if (nmaps >= 2) launch(std::integral_constant<int, 4>{}, (nmaps + 3) / 4);
+        else launch(std::integral_constant<int, 1>{}, 1);
+    }
     if (tm) cudaEventRecord(pl->ev[4], st);
     CUDA_TRY(cudaGetLastError());
     return 0;
@@ -725,6 +738,7 @@ static int plan_create_impl(arkcos_plan** out, const arkcos_pixelization* pix, c
     if (options) opt = *options;
     for (int r : opt.reserved) if (r != 0) return fail(ARKCOS_INVALID_ARG, "options.reserved must be zero");
     if (opt.variant != 0 && opt.variant != 1) return fail(ARKCOS_INVALID_ARG, "options.variant must be 0 or 1");
+    if (opt.exact_caps != 0 && opt.exact_caps != 1) return fail(ARKCOS_INVALID_ARG, "options.exact_caps must be 0 or 1");
     if (opt.max_nmaps < 0 || opt.polar_oversample < 0 || opt.ell_nyquist < 0.0 || opt.max_nmaps > 65535)
         return fail(ARKCOS_INVALID_ARG, "negative option");
     const int maxlen = dtype == ARKCOS_F32 ? 16384 : 8192;
@@ -791,6 +805,20 @@ static int plan_create_impl(arkcos_plan** out, const arkcos_pixelization* pix, c
         if (int rc = upload(&pl->d_items[c], t.items[c], wsb)) return rc;
     if (int rc = upload(&pl->d_eqchunks, t.eq_chunks, wsb)) return rc;
     if (int rc = upload(&pl->d_pole, t.pole_rings, wsb)) return rc;
+    if (opt.exact_caps && pix->kind == ARKCOS_HEALPIX_RING) {
+        // rings whose band contains a ring shorter than the longest one: caps + the equatorial rings next to them
+        const HostGeometry& g = pl->g;
+        const int nmax = *std::max_element(g.n.begin(), g.n.end());
+        std::vector<BandItem> items;
+        for (int i = 0; i < (g.R + 1) / 2; ++i) {
+            bool all_full = true;
+            for (int j = g.band_lo[i]; j <= g.band_hi[i]; ++j) all_full = all_full && g.n[j] == nmax;
+            if (all_full) continue;
+            for (int k0 = 0; k0 < g.n[i]; k0 += kDirectThreads) items.push_back(BandItem{i, k0});
+        }
+        pl->ndirect = (int)items.size();
+        if (int rc = upload(&pl->d_direct_items, items, wsb)) return rc;
+    }
     if (int rc = upload(&pl->d_cap_rings, t.cap_rings, wsb)) return rc;
     if (int rc = upload(&pl->d_cap_pairs, t.cap_pairs, wsb)) return rc;
     std::vector<double> tab(kernel->table, kernel->table + kernel->n);
@@ -921,7 +949,7 @@ int arkcos_plan_destroy(arkcos_plan* pl)
     void* ptrs[] = {pl->d_rings, pl->d_lens, pl->d_pairs, pl->d_north, pl->d_items[0], pl->d_items[1], pl->d_items[2], pl->d_items[3],
                     pl->d_items[4], pl->d_items[5], pl->d_eqchunks, pl->d_pole, pl->d_chirp, pl->d_phase, pl->d_fft_order, pl->d_table, pl->d_tw, pl->d_filt,
                     pl->d_W, pl->d_specIn, pl->d_specOut, pl->d_stage_in, pl->d_stage_out,
-                    pl->d_cap_rings, pl->d_cap_pairs, pl->d_tw3, pl->d_tw16, pl->d_fft3_jobs[0], pl->d_fft3_jobs[1], pl->d_fft3_jobs[2], pl->d_fft3_jobs[3]};
+                    pl->d_cap_rings, pl->d_cap_pairs, pl->d_direct_items, pl->d_tw3, pl->d_tw16, pl->d_fft3_jobs[0], pl->d_fft3_jobs[1], pl->d_fft3_jobs[2], pl->d_fft3_jobs[3]};
     for (void* p : ptrs) if (p) cudaFree(p);
     for (auto& e : pl->ev) if (e) cudaEventDestroy(e);
     for (auto& e : pl->ev_band) if (e) cudaEventDestroy(e);
@@ -1010,6 +1038,7 @@ int arkcos_plan_launches_per_convolve(const arkcos_plan* pl)
     n += 2 * fft;
     n += (pl->nitems[0] > 0) + (pl->npole > 0) + (pl->neqchunks > 0);
     for (int c = 1; c < kBandClasses; ++c) n += pl->nitems[c] > 0 ? 1 : 0;
+    n += pl->ndirect > 0 ? 1 : 0;
     return n;
 }
 

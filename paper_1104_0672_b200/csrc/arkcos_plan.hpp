@@ -10,6 +10,7 @@
 #include "arkcos_band.cuh"
 #include "arkcos_fft.cuh"
 #include "arkcos_fft3.cuh"
+#include "arkcos_direct.cuh"
 
 namespace arkcos {
 
@@ -50,6 +51,8 @@ struct arkcos_plan {
     arkcos::NorthRec* d_north = nullptr;
     arkcos::EqChunk* d_eqchunks = nullptr;
     int neqchunks = 0, eq_mh = 0, eq_alt = 0;
+    arkcos::BandItem* d_direct_items = nullptr;   // exact_caps: {northern ring, first pixel} per block of direct_rings_kernel
+    int ndirect = 0;
     arkcos::CapRing* d_cap_rings = nullptr;
     arkcos::CapPair* d_cap_pairs = nullptr;
     int* d_pole = nullptr;

@@ -166,6 +166,28 @@ def test_hard_edged_kernels_vs_scheme_oracle():
         assert frms(take_rings(geom, out, eq), ref1) <= 1e-6
 
 
+@pytest.mark.parametrize("dtype,nmaps", [(arkcos.F32, 3), (arkcos.F32, 1), (arkcos.F64, 9)])
+def test_exact_caps_hard_edged_kernels(dtype, nmaps):
+    """exact_caps = 1: cap-zone rings by the direct-space sum: the WHOLE map equals the
+    brute-force oracle for the disc and the cut Mexican hat, which the Fourier scheme alone cannot do (reading R18)."""
+    nside = 32
+    geom = geometry.healpix_ring(nside)
+    pixsz = np.sqrt(4 * np.pi / geom.npix)
+    x = inputs.white_noise_maps(geom.npix, 5, nmaps)
+    if dtype == arkcos.F64:
+        x = x.astype(np.float64)
+    for tab, tmax in [(inputs.tophat_table(5.8 * pixsz), 5.8 * pixsz),
+                      (inputs.mexican_hat_table(2.33 * pixsz, 5 * 2.33 * pixsz), 5 * 2.33 * pixsz)]:
+        out, _ = gpu_convolve(("healpix", nside), tab, tmax, x, dtype, exact_caps=1)
+        ref1 = direct.direct_sum(geom, tab, tmax, x.astype(np.float64))
+        if dtype == arkcos.F64:
+            assert maxrel(out, ref1) <= 1e-12
+        else:
+            assert frms(out, ref1) <= 1e-6
+        plain, _ = gpu_convolve(("healpix", nside), tab, tmax, x, dtype)
+        assert frms(plain, ref1) > 1e-5            # without the option the caps carry the scheme's artifact level
+
+
 # ------------------------------------------------------------------ config 3: HEALPix nside 512 --------------------
 
 def test_cfg3_fp32_sampled_rings():
@@ -312,7 +334,13 @@ def test_cfg5_full_size(which):
     assert all(np.all(geom.n[geometry.band(geom, int(i), tmax)] == 4 * nside) for i in eq)
     ref1 = direct.direct_sum(geom, tab, tmax, x.astype(np.float64), out_rings=eq)
     assert frms(take_rings(geom, out, eq), ref1) <= 1e-6
-    cap = np.array([100, 1000, nside - 5])
+    cap = np.array([100, 1000, nside - 5, nside + 3, geom.nrings - 700])
     refc = direct.direct_sum(geom, tab, tmax, x.astype(np.float64), out_rings=cap)
     print(f"\ncfg5 {spec['kernel']}: cap-ring fractional RMS vs brute force = {frms(take_rings(geom, out, cap), refc):.2e}"
           f" (ell_nyquist {plan.ell_nyquist:.0f})")
+    # with exact_caps the cap zone is the direct-space sum: the 1e-5 of north_star holds on every ring
+    del plan
+    out_x, _ = gpu_convolve(c["pix"], tab, tmax, x, exact_caps=1)
+    assert frms(take_rings(geom, out_x, cap), refc) <= 1e-6
+    assert frms(take_rings(geom, out_x, eq), ref1) <= 1e-6
+    np.testing.assert_array_equal(take_rings(geom, out_x, eq), take_rings(geom, out, eq))
