@@ -31,7 +31,7 @@ METRIC = "output Mpix/s per map at HEALPix Nside=2048"
 # profiles/ (config 4, one map); None where no capture exists
 TRAFFIC = {  # profiles/r1_v7_final.md (ncu --set full, config 4, one map); FFT entries = sum over the size classes
     "band_mac_eq_kernel": 238e6 + 110e6,
-    "band_mac_cap_kernel<20>": 71e6 + 35e6,
+    "band_mac_capchunk_kernel<4,20>": None,
     "ring_fft3_forward_kernel (all transform sizes)": 306e6 + 154e6 + 42e6 + 1e6 + 11e6 + 3e6,
     "ring_fft3_inverse_kernel (all transform sizes)": 311e6 + 154e6 + 42e6 + 1e6 + 11e6 + 3e6,
 }

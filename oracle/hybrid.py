@@ -77,6 +77,8 @@ def mprime_rule(geom: RingGeometry, theta_max: float, ell_nyq: float) -> np.ndar
     for i in range(geom.nrings):
         smax = s[band(geom, i, theta_max)].max()
         out[i] = max(8, 2 * int(np.ceil(ell_nyq * smax)))
+        if out[i] >= 512:                       # runs of consecutive cap rings share one grid length (reading R10)
+            out[i] = (out[i] + 127) // 128 * 128
     return out
 
 

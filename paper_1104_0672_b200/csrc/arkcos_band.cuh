@@ -160,7 +160,7 @@ namespace arkcos {
 // sincospi) and reuses them for all input rings of the band; the rows and the per-pair records sit in shared memory.
 constexpr int kBandThreads = 128;
 constexpr int kMaxPairs = 64;
-constexpr int kBandClasses = 6;   // 0: general kernel; 1..4: band_mac_uniform_kernel<12,odd>, <12>, <20>, <32,odd>; 5: band_mac_cap_kernel<20>
+constexpr int kBandClasses = 6;   // 0: general kernel; 1..4: band_mac_uniform_kernel<12,odd>, <12>, <20>, <32,odd>; 5: band_mac_capchunk_kernel (cap rings in the single-period regime)
 
 struct __align__(16) PairMeta {
     int offN, offS;       // first coefficient of input ring j (north image) and of its mirror image (element offsets)
@@ -531,194 +531,143 @@ band_mac_pole_kernel(const int* __restrict__ ring_list, const NorthRec* __restri
 
 namespace arkcos {
 
-// ---- cap kernel: uniform output rings in the "single period" regime -----------------------------------------------------
-// Every pair of output ring i is sampled on the same grid M (class C, integer grid), and M/2 < N_i <= M, M/2 < N_j for
-// every input ring j of the band (all HEALPix cap rings except the few next to the poles: M'_i ~ 1.7 N_i).  Then the
-// unfolded modes that fold onto m' are just m1 = m' and m2 = N_i - m' (if <= M/2), and the periodic extension of Bp_j is
-// the stored value or its reflection, no division.  A thread owns one folded mode m': two cosine tables in registers,
-// both unfolded modes share the row loads.  The plan stores the pairs of such a ring sorted by row length, so the inner
-// loops are fully unrolled per length class, and the coefficients of the next pair are loaded while the current one is
-// accumulated.  Blocks whose modes are away from the ring Nyquist ("interior": m1 is never reflected, m2 always) run
-// a path with per-pair constant signs and precomputed pointers.
-// grid = (items, nmaps), one item = kCapThreads folded modes of one ring.
-constexpr int kCapThreads = 256;
-constexpr int kCapClasses = 5;                 // row length classes c4 = ceil(cnt / 4) = 1 .. 5 (TMAX = 20)
+// ---- cap kernel, chunked: runs of consecutive cap rings that share one grid length M' --------------------------------------
+// The plan rounds M'_i up to a multiple of 128 (reading R10), so ~18 consecutive cap rings share M'.  Such a run is
+// processed like a run of equatorial rings (band_mac_eq_kernel): a thread owns two adjacent UNFOLDED modes m <= M'/2 for
+// the whole chunk, its cosine table is built once, the (periodically extended) coefficient Bp_j[m] of an input ring is
+// loaded once per tile of TI output rings and reused from registers, rows are staged per tile with one row length per
+// input ring.  What differs from the equatorial case: the extension of Bp_j (reflection above N_j/2: conjugate, sign on
+// a shifted ring; single-period regime M'/2 < N_j) and the fold: T_i[m] belongs to the folded mode m (m <= N_i/2) or
+// N_i - m (conjugated, sign on a shifted ring i), so the block adds it into the zero-initialised output spectrum with a
+// vector reduction.  Every output coefficient receives at most two such terms, so the sum does not depend on their order.
+constexpr int kCapChunkRings = 8;          // longest run handed to one block (two tiles): enough blocks to balance the device
+struct CapChunk { int i0, n, M, pad; };
+struct CapChunkItem { int chunk, bx; };
 
-struct CapPair { int64_t woff; int offN, offS, Nj, shj, cnt, pad; };      // plan table, sorted by decreasing c4 within a ring
-struct CapRing { int ring, first, np, M, tneed, minN, maxN, cstart[kCapClasses + 1]; };   // cstart[c] = pairs with class > c
-struct __align__(16) CapMeta { int offN, offS, Nj, shj; };
-struct __align__(16) CapPtr { const cx<float>*p1N, *p1S, *p2N, *p2S; };  // interior path: Bp_j + idx for m' = 0 of both families
-
-template <int TMAX, int C4>
-__device__ __forceinline__ void cap_row(const float* __restrict__ w, const float (&c1)[TMAX], const float (&c2)[TMAX],
-                                        float& G1, float& G2)
+template <int TI, int TMAX>
+__global__ void __launch_bounds__(kBandThreads)
+band_mac_capchunk_kernel(const CapChunkItem* __restrict__ items, const CapChunk* __restrict__ chunks,
+                         const NorthRec* __restrict__ north, const PairRec* __restrict__ pairs,
+                         const float* __restrict__ W, const RingRec* __restrict__ rings, int R,
+                         const cx<float>* __restrict__ specIn, cx<float>* __restrict__ specOut, int64_t spec_stride)
 {
-    const float4* __restrict__ w4 = reinterpret_cast<const float4*>(w);
-    float2 s1 = make_float2(0.f, 0.f), s2 = make_float2(0.f, 0.f);      // (even-sample sum, odd-sample sum) per mode
+    constexpr int MT = 2, G4 = TMAX / 4;
+    __shared__ __align__(16) float sW[TI * kEqJMax * TMAX];       // [ii][jj][t]
+    __shared__ int sC[kEqJMax];                                    // [jj]: longest row length / 4 over the tile's rings
+    __shared__ int4 sJ[kEqJMax];                                   // input ring jlo + jj: spectrum offsets (N, S), N_j, shifted
+    const CapChunkItem it = items[blockIdx.x];
+    const CapChunk ch = chunks[it.chunk];
+    const int M = ch.M, Mh = M >> 1;
+    const int m0 = it.bx * (kBandThreads * MT) + MT * (int)threadIdx.x;      // modes m0, m0 + 1
+    float ce[MT][TMAX];
 #pragma unroll
-    for (int t4 = 0; t4 < C4; ++t4) {                                   // packed FMAs (FFMA2): two samples per issue slot
-        const float4 v = w4[t4];
-        s1 = ffma2(make_float2(v.x, v.y), make_float2(c1[4 * t4], c1[4 * t4 + 1]), s1);
-        s2 = ffma2(make_float2(v.x, v.y), make_float2(c2[4 * t4], c2[4 * t4 + 1]), s2);
-        s1 = ffma2(make_float2(v.z, v.w), make_float2(c1[4 * t4 + 2], c1[4 * t4 + 3]), s1);
-        s2 = ffma2(make_float2(v.z, v.w), make_float2(c2[4 * t4 + 2], c2[4 * t4 + 3]), s2);
-    }
-    G1 = s1.x + s1.y;
-    G2 = s2.x + s2.y;
-}
-
-struct CapVals { cx<float> v1N, v1S, v2N, v2S; };
-
-__device__ __forceinline__ CapVals cap_load_fast(const CapPtr* __restrict__ sF, int p, uint32_t off1, uint32_t off2)
-{
-    const CapPtr pf = sF[p];
-    CapVals v;
-    v.v1N = *reinterpret_cast<const cx<float>*>(reinterpret_cast<const char*>(pf.p1N) + off1);
-    v.v1S = *reinterpret_cast<const cx<float>*>(reinterpret_cast<const char*>(pf.p1S) + off1);
-    v.v2N = *reinterpret_cast<const cx<float>*>(reinterpret_cast<const char*>(pf.p2N) + off2);
-    v.v2S = *reinterpret_cast<const cx<float>*>(reinterpret_cast<const char*>(pf.p2S) + off2);
-    return v;
-}
-
-// interior path, pairs [p0, p1) all with row length class C4; nxt holds the coefficients of pair p0 on entry and those
-// of pair p1 (if < np) on exit
-template <int TMAX, int C4>
-__device__ __forceinline__ void cap_fast_run(int p0, int p1, int np, const float* __restrict__ sW, const CapPtr* __restrict__ sF,
-                                             const uint32_t* __restrict__ sS2, const float (&c1)[TMAX], const float (&c2)[TMAX],
-                                             uint32_t off1, uint32_t off2, CapVals& nxt, cx<float>& accN, cx<float>& accS)
-{
-    for (int p = p0; p < p1; ++p) {
-        const CapVals v = nxt;
-        nxt = cap_load_fast(sF, min(p + 1, np - 1), off1, off2);
-        float G1, G2;
-        cap_row<TMAX, C4>(sW + p * TMAX, c1, c2, G1, G2);
-        G2 = __uint_as_float(__float_as_uint(G2) ^ sS2[p]);
-        accN.x = fmaf(G1, v.v1N.x, accN.x); accN.y = fmaf(G1, v.v1N.y, accN.y);
-        accS.x = fmaf(G1, v.v1S.x, accS.x); accS.y = fmaf(G1, v.v1S.y, accS.y);
-        accN.x = fmaf(G2, v.v2N.x, accN.x); accN.y = fmaf(G2, v.v2N.y, accN.y);
-        accS.x = fmaf(G2, v.v2S.x, accS.x); accS.y = fmaf(G2, v.v2S.y, accS.y);
-    }
-}
-
-// general path (blocks next to the ring Nyquist), pairs [p0, p1) with row length class C4
-template <int TMAX, int C4>
-__device__ __forceinline__ void cap_edge_run(int p0, int p1, const float* __restrict__ sW, const CapMeta* __restrict__ sP,
-                                             const float (&c1)[TMAX], const float (&c2)[TMAX],
-                                             const cx<float>* __restrict__ in, int m1, int m2c, uint32_t shi,
-                                             cx<float>& accN, cx<float>& accS)
-{
-    for (int p = p0; p < p1; ++p) {
-        const CapMeta pm = sP[p];
-        const bool refl1 = 2 * m1 > pm.Nj, refl2 = 2 * m2c > pm.Nj;
-        const int idx1 = refl1 ? pm.Nj - m1 : m1, idx2 = refl2 ? pm.Nj - m2c : m2c;
-        const cx<float> v1N = in[pm.offN + idx1], v1S = in[pm.offS + idx1];
-        const cx<float> v2N = in[pm.offN + idx2], v2S = in[pm.offS + idx2];
-        float G1, G2;
-        cap_row<TMAX, C4>(sW + p * TMAX, c1, c2, G1, G2);
-        // stored coefficient -> value used: reflection conjugates (and flips the sign on a shifted ring); the second
-        // family is the w = 1 period of ring i (sign if ring i is shifted) and enters conjugated
-        const uint32_t shj = pm.shj ? 0x80000000u : 0u;
-        const uint32_t sre1 = refl1 ? shj : 0u, sim1 = sre1 ^ (refl1 ? 0x80000000u : 0u);
-        const uint32_t sre2 = shi ^ (refl2 ? shj : 0u), sim2 = sre2 ^ (refl2 ? 0u : 0x80000000u);
-        const float g1r = __uint_as_float(__float_as_uint(G1) ^ sre1), g1i = __uint_as_float(__float_as_uint(G1) ^ sim1);
-        const float g2r = __uint_as_float(__float_as_uint(G2) ^ sre2), g2i = __uint_as_float(__float_as_uint(G2) ^ sim2);
-        accN.x = fmaf(g1r, v1N.x, accN.x); accN.y = fmaf(g1i, v1N.y, accN.y);
-        accS.x = fmaf(g1r, v1S.x, accS.x); accS.y = fmaf(g1i, v1S.y, accS.y);
-        accN.x = fmaf(g2r, v2N.x, accN.x); accN.y = fmaf(g2i, v2N.y, accN.y);
-        accS.x = fmaf(g2r, v2S.x, accS.x); accS.y = fmaf(g2i, v2S.y, accS.y);
-    }
-}
-
-template <int TMAX>
-__global__ void __launch_bounds__(kCapThreads)
-band_mac_cap_kernel(const BandItem* __restrict__ items, const CapRing* __restrict__ crings,
-                    const CapPair* __restrict__ cpairs, const float* __restrict__ W,
-                    const RingRec* __restrict__ rings, int R, const cx<float>* __restrict__ specIn,
-                    cx<float>* __restrict__ specOut, int64_t spec_stride)
-{
-    static_assert(TMAX == 4 * kCapClasses, "row length classes");
-    __shared__ __align__(16) float sW[kMaxPairs * TMAX];
-    __shared__ CapMeta sP[kMaxPairs];
-    __shared__ CapPtr sF[kMaxPairs];
-    __shared__ uint32_t sS2[kMaxPairs];
-    const BandItem it = items[blockIdx.x];
-    const CapRing cr = crings[it.ring];
-    const int i = cr.ring, iS = R - 1 - i, np = cr.np;
-    const RingRec ri = rings[i];
-    const int Ni = ri.n;
-    const cx<float>* __restrict__ in = specIn + (int64_t)blockIdx.y * spec_stride;
-    if ((int)threadIdx.x < np) {
-        const CapPair cp = cpairs[cr.first + threadIdx.x];
-        CapMeta pm;
-        pm.offN = cp.offN; pm.offS = cp.offS; pm.Nj = cp.Nj; pm.shj = cp.shj;
-        sP[threadIdx.x] = pm;
-        CapPtr pf;
-        pf.p1N = in + cp.offN; pf.p1S = in + cp.offS;
-        pf.p2N = in + (cp.offN + cp.Nj - Ni); pf.p2S = in + (cp.offS + cp.Nj - Ni);
-        sF[threadIdx.x] = pf;
-        sS2[threadIdx.x] = ((ri.shifted != 0) != (cp.shj != 0)) ? 0x80000000u : 0u;
-    }
-    for (int idx = threadIdx.x; idx < np * (TMAX / 4); idx += kCapThreads) {
-        const int p = idx / (TMAX / 4), t4 = idx - p * (TMAX / 4);
-        const CapPair& cp = cpairs[cr.first + p];
-        float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
-        if (4 * t4 < cp.cnt) v = reinterpret_cast<const float4*>(W + cp.woff)[t4];
-        reinterpret_cast<float4*>(sW + p * TMAX)[t4] = v;
-    }
-    __syncthreads();
-    const int mp = it.m0 + (int)threadIdx.x;
-    if (2 * mp > Ni) return;
-    const int M = cr.M, Mh = M >> 1, tneed = cr.tneed;
-    const uint32_t twoM = 2u * (uint32_t)M;
-    const int m1 = mp, m2 = Ni - mp;
-    const bool has2 = m2 <= Mh;
-    const int m2c = has2 ? m2 : 0;
-    float c1[TMAX], c2[TMAX];
-    {
-        // half weight at the +-M/2 bins; a missing second mode contributes nothing
-        const float gs1 = (2 * m1 == M) ? 0.5f : 1.f;
-        const float gs2 = has2 ? ((2 * m2 == M) ? 0.5f : 1.f) : 0.f;
-        const cx<float> rot1 = cispi_ratio<float>((2u * (uint32_t)m1) % twoM, (uint32_t)M);
-        const cx<float> rot2 = cispi_ratio<float>((2u * (uint32_t)m2c) % twoM, (uint32_t)M);
-        cx<float> a = mk<float>(1.f, 0.f), b = mk<float>(1.f, 0.f);
+    for (int mt = 0; mt < MT; ++mt) {
+        const uint32_t mm = (uint32_t)min(m0 + mt, Mh), twoM = 2u * (uint32_t)M;
+        const cx<float> rot = cispi_ratio<float>((2u * mm) % twoM, (uint32_t)M);
+        cx<float> a = mk<float>(1.f, 0.f);
 #pragma unroll
         for (int t = 0; t < TMAX; ++t) {
-            if ((t & 7) == 0) {
-                if (t > 0 && t < tneed) {
-                    a = cispi_ratio<float>((2u * (uint32_t)m1 * (uint32_t)t) % twoM, (uint32_t)M);
-                    b = cispi_ratio<float>((2u * (uint32_t)m2c * (uint32_t)t) % twoM, (uint32_t)M);
-                }
-            } else {
-                a = cmul(a, rot1);
-                b = cmul(b, rot2);
-            }
-            c1[t] = a.x * gs1;
-            c2[t] = b.x * gs2;
+            if ((t & 7) == 0) { if (t > 0) a = cispi_ratio<float>((2u * mm * (uint32_t)t) % twoM, (uint32_t)M); }
+            else a = cmul(a, rot);
+            ce[mt][t] = a.x;
         }
     }
-    cx<float> accN = mk<float>(0, 0), accS = mk<float>(0, 0);
-    // interior block: no m1 of the block is reflected on any input ring, every m2 is
-    const int mlast = min(it.m0 + kCapThreads - 1, Ni >> 1);
-    const bool interior = 2 * mlast <= cr.minN && 2 * (Ni - mlast) > cr.maxN;
-    if (interior) {
-        const uint32_t off1 = (uint32_t)mp * 8u, off2 = (uint32_t)(has2 ? mp : 128) * 8u;
-        CapVals nxt = cap_load_fast(sF, 0, off1, off2);
-        cap_fast_run<TMAX, 5>(cr.cstart[5], cr.cstart[4], np, sW, sF, sS2, c1, c2, off1, off2, nxt, accN, accS);
-        cap_fast_run<TMAX, 4>(cr.cstart[4], cr.cstart[3], np, sW, sF, sS2, c1, c2, off1, off2, nxt, accN, accS);
-        cap_fast_run<TMAX, 3>(cr.cstart[3], cr.cstart[2], np, sW, sF, sS2, c1, c2, off1, off2, nxt, accN, accS);
-        cap_fast_run<TMAX, 2>(cr.cstart[2], cr.cstart[1], np, sW, sF, sS2, c1, c2, off1, off2, nxt, accN, accS);
-        cap_fast_run<TMAX, 1>(cr.cstart[1], cr.cstart[0], np, sW, sF, sS2, c1, c2, off1, off2, nxt, accN, accS);
-    } else {
-        const uint32_t shi = ri.shifted ? 0x80000000u : 0u;      // second family: w = 1
-        cap_edge_run<TMAX, 5>(cr.cstart[5], cr.cstart[4], sW, sP, c1, c2, in, m1, m2c, shi, accN, accS);
-        cap_edge_run<TMAX, 4>(cr.cstart[4], cr.cstart[3], sW, sP, c1, c2, in, m1, m2c, shi, accN, accS);
-        cap_edge_run<TMAX, 3>(cr.cstart[3], cr.cstart[2], sW, sP, c1, c2, in, m1, m2c, shi, accN, accS);
-        cap_edge_run<TMAX, 2>(cr.cstart[2], cr.cstart[1], sW, sP, c1, c2, in, m1, m2c, shi, accN, accS);
-        cap_edge_run<TMAX, 1>(cr.cstart[1], cr.cstart[0], sW, sP, c1, c2, in, m1, m2c, shi, accN, accS);
-    }
+    const cx<float>* __restrict__ in = specIn + (int64_t)blockIdx.y * spec_stride;
     cx<float>* __restrict__ out = specOut + (int64_t)blockIdx.y * spec_stride;
-    out[ri.spec_off + mp] = accN;
-    if (iS != i) out[rings[iS].spec_off + mp] = accS;
+    const int mA = min(m0, Mh), mB = min(m0 + 1, Mh);
+
+    // extended coefficient of input ring (Nj, shj) at mode m from the stored half spectrum (single period: m < Nj)
+    auto ext_index = [](int m, int Nj) { return 2 * m > Nj ? Nj - m : m; };
+    auto ext_value = [](cx<float> b, int m, int Nj, int shj) {
+        if (2 * m > Nj) { b.y = -b.y; if (shj) { b.x = -b.x; b.y = -b.y; } }
+        return b;
+    };
+
+    for (int tile = 0; tile < ch.n; tile += TI) {
+        const int nti = min(TI, ch.n - tile), i0 = ch.i0 + tile;
+        const int p_first = north[i0].pair_lo, p_last = north[i0 + nti - 1].pair_hi;
+        const int jlo = pairs[p_first].j, jw = pairs[p_last - 1].j - jlo + 1;
+        __syncthreads();
+        for (int k = threadIdx.x; k < jw; k += kBandThreads) sC[k] = 0;
+        for (int k = threadIdx.x; k < TI * jw * G4; k += kBandThreads) {
+            const int ii = k / (jw * G4), r = k - ii * (jw * G4);
+            reinterpret_cast<float4*>(sW + ii * (kEqJMax * TMAX))[r] = make_float4(0.f, 0.f, 0.f, 0.f);
+        }
+        for (int jj = threadIdx.x; jj < jw; jj += kBandThreads) {
+            const RingRec rj = rings[jlo + jj];
+            sJ[jj] = make_int4((int)rj.spec_off, (int)rings[R - 1 - jlo - jj].spec_off, rj.n, rj.shifted);
+        }
+        __syncthreads();
+        for (int k = threadIdx.x; k < (p_last - p_first) * G4; k += kBandThreads) {
+            const int p = p_first + k / G4, t4 = k % G4;
+            const PairRec& pr = pairs[p];
+            int ii = 0;                                                     // ring of the tile this pair belongs to
+#pragma unroll
+            for (int q = 1; q < TI; ++q) ii += (q < nti && p >= north[i0 + q].pair_lo) ? 1 : 0;
+            const int slot = ii * kEqJMax + (pr.j - jlo), c4 = (pr.cnt + 3) >> 2;
+            if (t4 < c4)
+                reinterpret_cast<float4*>(sW + slot * TMAX)[t4] = reinterpret_cast<const float4*>(W + pr.woff)[t4];
+            if (t4 == 0) atomicMax(&sC[pr.j - jlo], c4);
+        }
+        __syncthreads();
+        cx<float> acc[TI][2][MT];
+#pragma unroll
+        for (int ii = 0; ii < TI; ++ii)
+#pragma unroll
+            for (int h = 0; h < 2; ++h)
+#pragma unroll
+                for (int mt = 0; mt < MT; ++mt) acc[ii][h][mt] = mk<float>(0.f, 0.f);
+
+        cx<float> nx[2][MT];                                                // coefficients of the next input ring (raw)
+        auto fetch = [&](int jj) {
+            const int4 rj = sJ[min(jj, jw - 1)];
+            const int ia = ext_index(mA, rj.z), ib = ext_index(mB, rj.z);
+            nx[0][0] = in[rj.x + ia]; nx[0][1] = in[rj.x + ib];
+            nx[1][0] = in[rj.y + ia]; nx[1][1] = in[rj.y + ib];
+        };
+        fetch(0);
+        for (int jj = 0; jj < jw; ++jj) {
+            const int4 rj = sJ[jj];
+            cx<float> v[2][MT];
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                v[h][0] = ext_value(nx[h][0], mA, rj.z, rj.w);
+                v[h][1] = ext_value(nx[h][1], mB, rj.z, rj.w);
+            }
+            fetch(jj + 1);
+            const float* sWj = sW + jj * TMAX;
+            const int c4 = sC[jj];
+            if (c4 >= 5) eq_accumulate<TI, MT, TMAX, 0, 0, (G4 >= 5 ? 5 : 1)>(sWj, ce, ce, v, acc);
+            else if (c4 == 4) eq_accumulate<TI, MT, TMAX, 0, 0, (G4 >= 4 ? 4 : 1)>(sWj, ce, ce, v, acc);
+            else if (c4 == 3) eq_accumulate<TI, MT, TMAX, 0, 0, 3>(sWj, ce, ce, v, acc);
+            else if (c4 == 2) eq_accumulate<TI, MT, TMAX, 0, 0, 2>(sWj, ce, ce, v, acc);
+            else eq_accumulate<TI, MT, TMAX, 0, 0, 1>(sWj, ce, ce, v, acc);
+        }
+        // fold: mode m adds to m (m <= N_i/2) and / or to N_i - m (conjugated; sign if ring i is shifted)
+#pragma unroll
+        for (int ii = 0; ii < TI; ++ii) {
+            if (ii < nti) {
+                const int i = i0 + ii, iS = R - 1 - i;
+                const RingRec ri = rings[i];
+                const int64_t offS = rings[iS].spec_off;
+                const float sg = ri.shifted ? -1.f : 1.f;
+#pragma unroll
+                for (int mt = 0; mt < MT; ++mt) {
+                    const int m = m0 + mt;
+                    if (m > Mh) continue;
+                    const float hw = (2 * m == M) ? 0.5f : 1.f;          // the +-M/2 bins carry half the Nyquist term each
+#pragma unroll
+                    for (int h = 0; h < 2; ++h) {
+                        if (h == 1 && iS == i) continue;
+                        float2* dst = reinterpret_cast<float2*>(out + (h ? offS : ri.spec_off));
+                        const float tx = hw * acc[ii][h][mt].x, ty = hw * acc[ii][h][mt].y;
+                        if (2 * m <= ri.n) atomicAdd(dst + m, make_float2(tx, ty));
+                        if (2 * m >= ri.n) atomicAdd(dst + (ri.n - m), make_float2(sg * tx, -sg * ty));
+                    }
+                }
+            }
+        }
+    }
 }
 
 }  // namespace arkcos

@@ -153,8 +153,9 @@ struct HostTables {
     std::vector<PairRec> pairs;
     std::vector<NorthRec> north;
     std::vector<BandItem> items[kBandClasses];
-    std::vector<CapRing> cap_rings;              // rings for band_mac_cap_kernel, their pairs sorted by row length
-    std::vector<CapPair> cap_pairs;
+    std::vector<CapChunk> cap_chunks;            // runs of cap rings with one grid length for band_mac_capchunk_kernel
+    std::vector<CapChunkItem> cap_chunk_items;
+    std::vector<std::pair<int64_t, int64_t>> cap_zero;   // (first coefficient, count) ranges of the output spectrum to clear
     std::vector<int> pole_rings;                 // rings for band_mac_pole_kernel
     int pole_mh = 0;
     std::vector<EqChunk> eq_chunks;              // runs of consecutive class-E rings for band_mac_eq_kernel   // per band-kernel class (see band_class)
@@ -264,6 +265,9 @@ void build_pairs(HostGeometry& g, double theta_max, double ell_nyq, int fixed_mp
         double smax = 0.0;
         for (int j = g.band_lo[i]; j <= g.band_hi[i]; ++j) smax = std::max(smax, sin(g.theta[j]));
         g.mprime[i] = fixed_mprime > 0 ? fixed_mprime : std::max(8, 2 * (int)ceil(ell_nyq * smax));
+        // grids of 512 points and more are rounded up to a multiple of 128 so that runs of consecutive cap rings share one
+        // grid length (reading R10; band_mac_capchunk_kernel)
+        if (fixed_mprime <= 0 && g.mprime[i] >= 512) g.mprime[i] = (g.mprime[i] + 127) / 128 * 128;
     }
     for (int i = 0; i < R; ++i) any_odd = any_odd || (g.n[i] == nmax && g.shifted[i] != g.shifted[std::min(i + 1, R - 1)] && g.n[std::min(i + 1, R - 1)] == nmax);
     const int eq_alt = any_odd ? 1 : 0;
@@ -332,7 +336,7 @@ void build_pairs(HostGeometry& g, double theta_max, double ell_nyq, int fixed_mp
                 if (maxcnt <= 12) cls = odd ? 1 : 2;
                 else if (maxcnt <= 20 && !odd) cls = 3;
                 else if (maxcnt <= 32) cls = 4;
-                // single-period regime of band_mac_cap_kernel: M/2 below every ring length involved, N_i <= M
+                // single-period regime of band_mac_capchunk_kernel: M/2 below every ring length involved, N_i <= M
                 if ((cls == 2 || cls == 3) && !getenv("ARKCOS_NO_CAP_KERNEL")) {
                     const int Mh = t.pairs[lo].M / 2;
                     bool single = g.n[i] >= 512 && g.n[i] <= t.pairs[lo].M && Mh < g.n[i];
@@ -356,35 +360,12 @@ void build_pairs(HostGeometry& g, double theta_max, double ell_nyq, int fixed_mp
         static const int slot_of_cls[kBandClasses] = {0, 6, 3, 4, 5, 7};
         st.band_flops[slot_of_cls[cls]] += ring_flops;
         if (cls == 5) {
-            const int lo = t.north[i].pair_lo, hi = t.north[i].pair_hi;
-            CapRing cr{};
-            cr.ring = i;
-            cr.first = (int)t.cap_pairs.size();
-            cr.np = hi - lo;
-            cr.M = t.pairs[lo].M;
-            cr.minN = 1 << 30;
-            std::vector<int> order(hi - lo);
-            for (int p = lo; p < hi; ++p) order[p - lo] = p;
-            auto c4_of = [&](int p) { return std::max(1, (t.pairs[p].cnt + 3) / 4); };
-            std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return c4_of(a) > c4_of(b); });
-            for (int p : order) {
-                const PairRec& pr = t.pairs[p];
-                CapPair cp{};
-                cp.woff = pr.woff;
-                cp.offN = (int)g.spec_off[pr.j];
-                cp.offS = (int)g.spec_off[R - 1 - pr.j];
-                cp.Nj = g.n[pr.j];
-                cp.shj = g.shifted[pr.j];
-                cp.cnt = pr.cnt;
-                t.cap_pairs.push_back(cp);
-                cr.tneed = std::max(cr.tneed, pr.cnt);
-                cr.minN = std::min(cr.minN, cp.Nj);
-                cr.maxN = std::max(cr.maxN, cp.Nj);
-                for (int c = 0; c < c4_of(p); ++c) ++cr.cstart[c];       // cstart[c] = pairs with class > c
-            }
-            const int cidx = (int)t.cap_rings.size();
-            t.cap_rings.push_back(cr);
-            for (int m0 = 0; m0 <= g.n[i] / 2; m0 += kCapThreads) t.items[cls].push_back(BandItem{cidx, m0});
+            const int M = t.pairs[t.north[i].pair_lo].M;
+            if (!t.cap_chunks.empty() && t.cap_chunks.back().i0 + t.cap_chunks.back().n == i && t.cap_chunks.back().M == M &&
+                t.cap_chunks.back().n < kCapChunkRings)
+                ++t.cap_chunks.back().n;
+            else
+                t.cap_chunks.push_back(CapChunk{i, 1, M, 0});
             continue;
         }
         for (int m0 = 0; m0 <= g.n[i] / 2; m0 += band_threads) t.items[cls].push_back(BandItem{i, m0});
@@ -403,6 +384,28 @@ void build_pairs(HostGeometry& g, double theta_max, double ell_nyq, int fixed_mp
             else
                 t.eq_chunks.push_back(EqChunk{i, 1});
         }
+    }
+    for (size_t c = 0; c < t.cap_chunks.size(); ++c) {
+        const CapChunk& ch = t.cap_chunks[c];
+        for (int bx = 0; bx * (kBandThreads * 2) <= ch.M / 2; ++bx) t.cap_chunk_items.push_back(CapChunkItem{(int)c, bx});
+        // output coefficients of the chunk's rings (north and mirror image) are accumulated: they start from zero
+        const int iA = ch.i0, iB = ch.i0 + ch.n - 1;
+        auto add_range = [&](int ra, int rb) {
+            const int64_t a = g.spec_off[ra], n = g.spec_off[rb + 1] - a;
+            if (!t.cap_zero.empty() && t.cap_zero.back().first + t.cap_zero.back().second == a) t.cap_zero.back().second += n;
+            else t.cap_zero.push_back({a, n});
+        };
+        add_range(iA, iB);
+        if (R - 1 - iB > iB) add_range(R - 1 - iB, R - 1 - iA);
+    }
+    // longest blocks first (the chunks run from the pole towards the equator, M' grows)
+    std::reverse(t.cap_chunk_items.begin(), t.cap_chunk_items.end());
+    std::sort(t.cap_zero.begin(), t.cap_zero.end());
+    for (size_t k = 1; k < t.cap_zero.size();) {                             // merge adjacent ranges
+        if (t.cap_zero[k - 1].first + t.cap_zero[k - 1].second == t.cap_zero[k].first) {
+            t.cap_zero[k - 1].second += t.cap_zero[k].second;
+            t.cap_zero.erase(t.cap_zero.begin() + k);
+        } else ++k;
     }
     st.row_samples = 0;
     for (const PairRec& p : t.pairs) st.row_samples += p.cnt;
@@ -569,10 +572,15 @@ void launch_uniform(const arkcos_plan* pl, int nmaps, cudaStream_t st, bool seri
     if (serial) cudaEventRecord(pl->ev_band[6], st);
     launch_uniform_class<12, true>(pl, 1, nmaps, s2);
     if (serial) cudaEventRecord(pl->ev_band[7], st);
-    if (pl->nitems[5] > 0)
-        band_mac_cap_kernel<20><<<dim3((unsigned)pl->nitems[5], (unsigned)nmaps), kCapThreads, 0, s1>>>(
-            pl->d_items[5], pl->d_cap_rings, pl->d_cap_pairs, (const float*)pl->d_W, pl->d_rings, pl->g.R,
+    if (pl->ncapitems > 0) {
+        for (const auto& z : pl->cap_zero)
+            for (int q = 0; q < nmaps; ++q)
+                cudaMemsetAsync((cx<float>*)pl->d_specOut + (int64_t)q * pl->g.spec_total + z.first, 0,
+                                (size_t)z.second * sizeof(cx<float>), s1);
+        band_mac_capchunk_kernel<4, 20><<<dim3((unsigned)pl->ncapitems, (unsigned)nmaps), kBandThreads, 0, s1>>>(
+            pl->d_cap_chunk_items, pl->d_cap_chunks, pl->d_north, pl->d_pairs, (const float*)pl->d_W, pl->d_rings, pl->g.R,
             (const cx<float>*)pl->d_specIn, (cx<float>*)pl->d_specOut, pl->g.spec_total);
+    }
     if (serial) cudaEventRecord(pl->ev_band[8], st);
 }
 
@@ -819,8 +827,10 @@ static int plan_create_impl(arkcos_plan** out, const arkcos_pixelization* pix, c
         pl->ndirect = (int)items.size();
         if (int rc = upload(&pl->d_direct_items, items, wsb)) return rc;
     }
-    if (int rc = upload(&pl->d_cap_rings, t.cap_rings, wsb)) return rc;
-    if (int rc = upload(&pl->d_cap_pairs, t.cap_pairs, wsb)) return rc;
+    if (int rc = upload(&pl->d_cap_chunks, t.cap_chunks, wsb)) return rc;
+    if (int rc = upload(&pl->d_cap_chunk_items, t.cap_chunk_items, wsb)) return rc;
+    pl->ncapitems = (int)t.cap_chunk_items.size();
+    pl->cap_zero = t.cap_zero;
     std::vector<double> tab(kernel->table, kernel->table + kernel->n);
     if (int rc = upload(&pl->d_table, tab, wsb)) return rc;
     if (int rc = dtype == ARKCOS_F32 ? build_device_numeric<float>(pl, t) : build_device_numeric<double>(pl, t)) return rc;
@@ -949,7 +959,7 @@ int arkcos_plan_destroy(arkcos_plan* pl)
     void* ptrs[] = {pl->d_rings, pl->d_lens, pl->d_pairs, pl->d_north, pl->d_items[0], pl->d_items[1], pl->d_items[2], pl->d_items[3],
                     pl->d_items[4], pl->d_items[5], pl->d_eqchunks, pl->d_pole, pl->d_chirp, pl->d_phase, pl->d_fft_order, pl->d_table, pl->d_tw, pl->d_filt,
                     pl->d_W, pl->d_specIn, pl->d_specOut, pl->d_stage_in, pl->d_stage_out,
-                    pl->d_cap_rings, pl->d_cap_pairs, pl->d_direct_items, pl->d_tw3, pl->d_tw16, pl->d_fft3_jobs[0], pl->d_fft3_jobs[1], pl->d_fft3_jobs[2], pl->d_fft3_jobs[3]};
+                    pl->d_cap_chunks, pl->d_cap_chunk_items, pl->d_direct_items, pl->d_tw3, pl->d_tw16, pl->d_fft3_jobs[0], pl->d_fft3_jobs[1], pl->d_fft3_jobs[2], pl->d_fft3_jobs[3]};
     for (void* p : ptrs) if (p) cudaFree(p);
     for (auto& e : pl->ev) if (e) cudaEventDestroy(e);
     for (auto& e : pl->ev_band) if (e) cudaEventDestroy(e);
@@ -1014,7 +1024,7 @@ int arkcos_plan_band_kernels(const arkcos_plan* pl, int* n, const char** names, 
 {
     static const char* kNames[8] = {"band_mac_general_kernel", "band_mac_pole_kernel", "band_mac_eq_kernel",
                                     "band_mac_uniform_kernel<12,0>", "band_mac_uniform_kernel<20,0>",
-                                    "band_mac_uniform_kernel<32,1>", "band_mac_uniform_kernel<12,1>", "band_mac_cap_kernel<20>"};
+                                    "band_mac_uniform_kernel<32,1>", "band_mac_uniform_kernel<12,1>", "band_mac_capchunk_kernel<4,20>"};
     if (!pl || !n) return fail(ARKCOS_INVALID_ARG, "NULL argument");
     *n = 8;
     for (int k = 0; k < 8; ++k) {
@@ -1039,6 +1049,7 @@ int arkcos_plan_launches_per_convolve(const arkcos_plan* pl)
     n += (pl->nitems[0] > 0) + (pl->npole > 0) + (pl->neqchunks > 0);
     for (int c = 1; c < kBandClasses; ++c) n += pl->nitems[c] > 0 ? 1 : 0;
     n += pl->ndirect > 0 ? 1 : 0;
+    n += pl->ncapitems > 0 ? 1 : 0;
     return n;
 }
 

@@ -53,8 +53,10 @@ struct arkcos_plan {
     int neqchunks = 0, eq_mh = 0, eq_alt = 0;
     arkcos::BandItem* d_direct_items = nullptr;   // exact_caps: {northern ring, first pixel} per block of direct_rings_kernel
     int ndirect = 0;
-    arkcos::CapRing* d_cap_rings = nullptr;
-    arkcos::CapPair* d_cap_pairs = nullptr;
+    arkcos::CapChunk* d_cap_chunks = nullptr;
+    arkcos::CapChunkItem* d_cap_chunk_items = nullptr;
+    int ncapitems = 0;
+    std::vector<std::pair<int64_t, int64_t>> cap_zero;    // output-spectrum ranges cleared before band_mac_capchunk_kernel
     int* d_pole = nullptr;
     int npole = 0, pole_mh = 0;
     arkcos::BandItem* d_items[arkcos::kBandClasses] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
