@@ -573,10 +573,6 @@ void launch_uniform(const arkcos_plan* pl, int nmaps, cudaStream_t st, bool seri
     launch_uniform_class<12, true>(pl, 1, nmaps, s2);
     if (serial) cudaEventRecord(pl->ev_band[7], st);
     if (pl->ncapitems > 0) {
-        for (const auto& z : pl->cap_zero)
-            for (int q = 0; q < nmaps; ++q)
-                cudaMemsetAsync((cx<float>*)pl->d_specOut + (int64_t)q * pl->g.spec_total + z.first, 0,
-                                (size_t)z.second * sizeof(cx<float>), s1);
         band_mac_capchunk_kernel<4, 20><<<dim3((unsigned)pl->ncapitems, (unsigned)nmaps), kBandThreads, 0, s1>>>(
             pl->d_cap_chunk_items, pl->d_cap_chunks, pl->d_north, pl->d_pairs, (const float*)pl->d_W, pl->d_rings, pl->g.R,
             (const cx<float>*)pl->d_specIn, (cx<float>*)pl->d_specOut, pl->g.spec_total);
@@ -664,15 +660,28 @@ template <class T> int enqueue_convolve(const arkcos_plan* pl, const void* d_in,
     // the kernel rows do not depend on the map: outside the timing modes they are generated on a side stream of their own
     // while the forward FFTs run
     const bool rows_aside = !tm && !pl->opt.cache_kernel_rows && pl->npairs > 0;
-    if (rows_aside) {
+    // the cap fold accumulates into the output spectrum: clear those ranges early, beside the forward FFTs as well
+    auto clear_cap_ranges = [&](cudaStream_t q) {
+        if (pl->ncapitems > 0)
+            for (const auto& z : pl->cap_zero)
+                for (int k = 0; k < nmaps; ++k)
+                    cudaMemsetAsync((cx<float>*)pl->d_specOut + (int64_t)k * g.spec_total + z.first, 0,
+                                    (size_t)z.second * sizeof(cx<float>), q);
+    };
+    const bool aside = !tm && pl->ncapitems > 0 && !rows_aside;
+    if (rows_aside || aside) {
         cudaEventRecord(pl->ev_rows_fork, st);
         cudaStreamWaitEvent(pl->side_rows, pl->ev_rows_fork, 0);
-        enqueue_rows<T>(pl, pl->side_rows);
+        clear_cap_ranges(pl->side_rows);
+        if (rows_aside) enqueue_rows<T>(pl, pl->side_rows);
         cudaEventRecord(pl->ev_rows_done, pl->side_rows);
-    } else if (!pl->opt.cache_kernel_rows) enqueue_rows<T>(pl, st);
+    } else {
+        clear_cap_ranges(st);
+        if (!pl->opt.cache_kernel_rows) enqueue_rows<T>(pl, st);
+    }
     if (tm) cudaEventRecord(pl->ev[1], st);
     launch_ring_ffts<T, true>(pl, d_in, d_out, nmaps, st);
-    if (rows_aside) cudaStreamWaitEvent(st, pl->ev_rows_done, 0);
+    if (rows_aside || aside) cudaStreamWaitEvent(st, pl->ev_rows_done, 0);
     if (tm) cudaEventRecord(pl->ev[2], st);
     // the band kernels of the different ring classes write disjoint rings: fork them onto the plan's side streams
     // (timing mode 2: one after the other on the caller's stream with an event between them)
