@@ -29,11 +29,11 @@ from paper_1104_0672_b200.sharding import shard_range  # noqa: E402
 METRIC = "output Mpix/s per map at HEALPix Nside=2048"
 # dram__bytes_read.sum + dram__bytes_write.sum per launch (bytes) from the ncu --set full captures summarised in
 # profiles/ (config 4, one map); None where no capture exists
-TRAFFIC = {  # profiles/r1_v7_final.md (ncu --set full, config 4, one map); FFT entries = sum over the size classes
-    "band_mac_eq_kernel": 238e6 + 110e6,
-    "band_mac_capchunk_kernel<4,20>": None,
-    "ring_fft3_forward_kernel (all transform sizes)": 306e6 + 154e6 + 42e6 + 1e6 + 11e6 + 3e6,
-    "ring_fft3_inverse_kernel (all transform sizes)": 311e6 + 154e6 + 42e6 + 1e6 + 11e6 + 3e6,
+TRAFFIC = {  # profiles/r1_v8_final.md (ncu --set full, config 4, one map); FFT entries = sum over the size classes
+    "band_mac_eq_kernel": 224e6 + 111e6,
+    "band_mac_capchunk_kernel<4,20>": 138e6 + 30e6,
+    "ring_fft3_forward_kernel (all transform sizes)": 306e6 + 149e6 + 42e6 + 1e6 + 11e6 + 3e6,
+    "ring_fft3_inverse_kernel (all transform sizes)": 309e6 + 149e6 + 42e6 + 1e6 + 11e6 + 3e6,
 }
 UNIT = "Mpix/s"
 
