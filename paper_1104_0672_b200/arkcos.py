@@ -140,8 +140,8 @@ class Plan:
         _check(_lib().arkcos_plan_synchronize(self._h), "arkcos_plan_synchronize")
 
     def destroy(self):
-        if getattr(self, "_h", None) is not None and self._h:
-            _lib().arkcos_plan_destroy(self._h)
+        if getattr(self, "_h", None) is not None and self._h and _LIB is not None:   # _LIB is gone at interpreter exit
+            _LIB.arkcos_plan_destroy(self._h)
             self._h = c_void_p()
 
     __del__ = destroy
