@@ -234,6 +234,20 @@ def test_cfg4_full_size_sampled_rings():
         o += n
 
 
+def test_nside4096_maximum_size_sampled_rings():
+    """The largest HEALPix grid an fp32 plan accepts (ring length 16384: the shared-memory FFT path for the belt)."""
+    nside = 4096
+    geom = geometry.healpix_ring(nside)
+    fwhm, tmax = 2.5 * ARCMIN, 7.5 * ARCMIN
+    tab = inputs.gaussian_table(fwhm, tmax)
+    x = inputs.white_noise(geom.npix, 6)
+    out, _ = gpu_convolve(("healpix", nside), tab, tmax, x)
+    assert np.isfinite(out).all()
+    rings = np.array([0, 3, 700, 2047, 2048, 3000, nside - 1, nside, nside + 5, 2 * nside - 1, 3 * nside + 2, geom.nrings - 1])
+    ref = direct.direct_sum(geom, tab, tmax, x.astype(np.float64), out_rings=rings)
+    assert frms(take_rings(geom, out, rings), ref) <= 1e-5
+
+
 # ------------------------------------------------------------------ API behaviour -----------------------------------
 
 def test_multi_map_equals_single_and_host_path():
