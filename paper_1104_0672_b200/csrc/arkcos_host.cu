@@ -439,7 +439,7 @@ template <int LOGQ> int set_fft3_smem()
 // job lists and the 16 x 16 twiddle table of the register-resident FFT kernels (float plans only)
 template <class T> int setup_fft3(arkcos_plan* pl, const HostTables& t)
 {
-    if (sizeof(T) != 4) return 0;
+    if constexpr (sizeof(T) == 4) {
     for (int c = 0; c < 4; ++c) {
         pl->nfft3[c] = (int)t.fft3_jobs[c].size();
         if (int rc = upload(&pl->d_fft3_jobs[c], t.fft3_jobs[c], &pl->stats.workspace_bytes)) return rc;
@@ -467,6 +467,7 @@ template <class T> int setup_fft3(arkcos_plan* pl, const HostTables& t)
     if (int rc = set_fft3_smem<10>()) return rc;
     if (int rc = set_fft3_smem<11>()) return rc;
     if (int rc = set_fft3_smem<12>()) return rc;
+    }
     return 0;
 }
 
