@@ -4,11 +4,12 @@
 //
 // A ring of N reals is one complex FFT of length L = N/2 plus a split (as in arkcos_fft.cuh).  Here a thread keeps 16
 // points of the transform in registers: Q = 16 * 16 * RL (RL = Q/256 = 2..16) is done as radix-16, radix-16, radix-RL
-// Stockham passes with two shared-memory exchanges; T = Q/16 threads per block; every block runs TWO transforms of the
-// same size side by side so that twiddles and index arithmetic are paid once:
-//   * "direct" job  (L = Q a power of two: equatorial rings, ECP): two rings per block;
-//   * "Bluestein" job (any other L <= Q, the HEALPix cap rings N = 4i): one ring per block.  The cyclic convolution of
-//     length P = 2Q is split into its even and odd frequency bins,
+// Stockham passes with two shared-memory exchanges; T = Q/16 threads per block.
+//   * power-of-two rings (L = Q: equatorial rings, ECP): one ring per block (ring_fft3_direct1_kernel, 64 registers, four
+//     blocks of the largest size per SM, so that the memory phases of some blocks overlap the butterflies of others);
+//   * any other length L <= Q (the HEALPix cap rings N = 4i): Bluestein, one ring per block, TWO transforms side by side
+//     (twiddles and index arithmetic paid once).  The cyclic convolution of length P = 2Q is split into its even and odd
+//     frequency bins,
 //         Y[2k] = FFT_Q(a)[k],  Y[2k+1] = FFT_Q(a[n] w_P^n)[k],     y[n] = E[n] + conj(w_P^n) O[n]  (n < Q),
 //     (a = chirped input, zero beyond L <= Q; only y[n < L] is needed), so that the two transforms of a block are the
 //     even and the odd half, the filter product needs no exchange (the output layout of one transform is the input
@@ -18,8 +19,8 @@
 
 namespace arkcos {
 
-// One block's work, self-contained (copies of the ring and length records, so the block needs a single table read):
-// direct: two rings (has1 = 0: only r0); Bluestein: r0 only.
+// One job, self-contained (copies of the ring and length records, so a block needs a single table read):
+// power-of-two rings: two rings, served by two blocks (has1 = 0: only r0); Bluestein: r0 only.
 struct FftJob { RingRec r0, r1; FftLen f; int has1, pad; };
 
 template <int LOGQ> struct Fft3 {
@@ -162,7 +163,7 @@ __device__ __forceinline__ void bluestein_core(cx<float> (&u)[2][16], cx<float>*
     }
 }
 
-// Steps 1 + 2, rings with transform size Q.  grid = (jobs, nmaps), block = Q/16 threads.
+// Steps 1 + 2, Bluestein rings with transform size Q.  grid = (Bluestein jobs, nmaps), block = Q/16 threads.
 template <int LOGQ>
 __global__ void __launch_bounds__(Fft3<LOGQ>::T, Fft3<LOGQ>::MINB)
 ring_fft3_forward_kernel(const float* __restrict__ in, int64_t npix, cx<float>* __restrict__ spec, int64_t spec_stride,
@@ -173,7 +174,7 @@ ring_fft3_forward_kernel(const float* __restrict__ in, int64_t npix, cx<float>* 
                          const cx<float>* __restrict__ phase, int ahead)
 {
     using F = Fft3<LOGQ>;
-    constexpr int T = F::T, SQ = F::SQ;
+    constexpr int T = F::T;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     cx<float>* s = reinterpret_cast<cx<float>*>(smem_raw);
     const int t = (int)threadIdx.x;
@@ -191,33 +192,7 @@ ring_fft3_forward_kernel(const float* __restrict__ in, int64_t npix, cx<float>* 
     }
     const cx<float>* __restrict__ ph = phase + f.ph_off;
     cx<float> u[2][16];
-    if (f.pow2) {
-        const RingRec r1 = job.has1 ? job.r1 : job.r0;
-        const cx<float>* __restrict__ x0 = reinterpret_cast<const cx<float>*>(map + r0.pix_off);
-        const cx<float>* __restrict__ x1 = reinterpret_cast<const cx<float>*>(map + r1.pix_off);
-#pragma unroll
-        for (int r = 0; r < 16; ++r) { u[0][r] = x0[t + T * r]; u[1][r] = x1[t + T * r]; }
-        fft3<LOGQ, 2>(u, s, tw, logPT, tw16, tw3);
-        __syncthreads();
-#pragma unroll
-        for (int b = 0; b < 2; ++b)
-#pragma unroll
-            for (int q = 0; q < 16; ++q) s[b * SQ + phys(t + T * q)] = u[b][q];
-        __syncthreads();
-#pragma unroll
-        for (int b = 0; b < 2; ++b) {
-            if (b == 1 && !job.has1) break;
-            const RingRec& rr = b ? r1 : r0;
-            cx<float>* __restrict__ o = out + rr.spec_off;
-#pragma unroll
-            for (int q = 0; q < 16; ++q) {
-                const int k = t + T * q;
-                const cx<float> zc = cconj(s[b * SQ + phys(k == 0 ? 0 : L - k)]);
-                o[k] = split_fwd(u[b][q], zc, ph[k], rr.shifted);
-            }
-            if (t == 0) o[L] = split_fwd(u[b][0], cconj(u[b][0]), ph[L], rr.shifted);
-        }
-    } else {
+    {
         const cx<float>* __restrict__ x0 = reinterpret_cast<const cx<float>*>(map + r0.pix_off);
         const cx<float>* __restrict__ cw = chirp + f.chirp_off;
         if (t == 0) {
@@ -260,7 +235,7 @@ ring_fft3_forward_kernel(const float* __restrict__ in, int64_t npix, cx<float>* 
     }
 }
 
-// Steps 6 + 7, rings with transform size Q.  grid = (jobs, nmaps), block = Q/16 threads.
+// Steps 6 + 7, Bluestein rings with transform size Q.  grid = (Bluestein jobs, nmaps), block = Q/16 threads.
 template <int LOGQ>
 __global__ void __launch_bounds__(Fft3<LOGQ>::T, Fft3<LOGQ>::MINB)
 ring_fft3_inverse_kernel(const cx<float>* __restrict__ spec, int64_t spec_stride, float* __restrict__ outmap, int64_t npix,
@@ -289,24 +264,7 @@ ring_fft3_inverse_kernel(const cx<float>* __restrict__ spec, int64_t spec_stride
     }
     const cx<float>* __restrict__ ph = phase + f.ph_off;
     cx<float> u[2][16];
-    if (f.pow2) {
-        const RingRec r1 = job.has1 ? job.r1 : job.r0;
-#pragma unroll
-        for (int r = 0; r < 16; ++r) {
-            const int k = t + T * r;
-            const cx<float> hk = cconj(ph[k]), hl = cconj(ph[L - k]);
-            u[0][r] = pack_inv(D[r0.spec_off + k], D[r0.spec_off + L - k], hk, hl, r0.shifted);
-            u[1][r] = pack_inv(D[r1.spec_off + k], D[r1.spec_off + L - k], hk, hl, r1.shifted);
-        }
-        fft3<LOGQ, 2>(u, s, tw, logPT, tw16, tw3);
-        cx<float>* __restrict__ o0 = reinterpret_cast<cx<float>*>(map + r0.pix_off);
-        cx<float>* __restrict__ o1 = reinterpret_cast<cx<float>*>(map + r1.pix_off);
-#pragma unroll
-        for (int q = 0; q < 16; ++q) {
-            o0[t + T * q] = cconj(u[0][q]);
-            if (job.has1) o1[t + T * q] = cconj(u[1][q]);
-        }
-    } else {
+    {
         const cx<float>* __restrict__ cw = chirp + f.chirp_off;
         if (t == 0) prefetch_l2(filt + f.filt_off, (uint32_t)(2 * F::Q * sizeof(cx<float>)));
 #pragma unroll
@@ -327,6 +285,60 @@ ring_fft3_inverse_kernel(const cx<float>* __restrict__ spec, int64_t spec_stride
             const int n = t + T * q;
             if (n < L) o0[n] = cmulc(u[0][q], cw[n]);
         }
+    }
+}
+
+}  // namespace arkcos
+
+namespace arkcos {
+
+// Power-of-two rings, ONE transform per block (block b works on ring b & 1 of direct job b >> 1): twice as many resident
+// blocks at half the registers, so that the load / store phases of some blocks overlap the butterflies of the others.
+template <int LOGQ, bool FWD>
+__global__ void __launch_bounds__(Fft3<LOGQ>::T, 2 * Fft3<LOGQ>::MINB)
+ring_fft3_direct1_kernel(const float* __restrict__ in, float* __restrict__ outmap, int64_t npix,
+                         cx<float>* __restrict__ spec, int64_t spec_stride, const FftJob* __restrict__ jobs,
+                         const cx<float>* __restrict__ tw, int logPT, const cx<float>* __restrict__ tw16,
+                         const cx<float>* __restrict__ tw3, const cx<float>* __restrict__ phase)
+{
+    using F = Fft3<LOGQ>;
+    constexpr int T = F::T;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cx<float>* s = reinterpret_cast<cx<float>*>(smem_raw);
+    const int t = (int)threadIdx.x;
+    const FftJob& job = jobs[blockIdx.x >> 1];
+    if ((blockIdx.x & 1) && !job.has1) return;
+    const RingRec rr = (blockIdx.x & 1) ? job.r1 : job.r0;
+    const int L = job.f.L;
+    const cx<float>* __restrict__ ph = phase + job.f.ph_off;
+    cx<float>* __restrict__ sp = spec + (int64_t)blockIdx.y * spec_stride + rr.spec_off;
+    cx<float> u[1][16];
+    if (FWD) {
+        const cx<float>* __restrict__ x0 = reinterpret_cast<const cx<float>*>(in + (int64_t)blockIdx.y * npix + rr.pix_off);
+#pragma unroll
+        for (int r = 0; r < 16; ++r) u[0][r] = x0[t + T * r];
+        fft3<LOGQ, 1>(u, s, tw, logPT, tw16, tw3);
+        __syncthreads();
+#pragma unroll
+        for (int q = 0; q < 16; ++q) s[phys(t + T * q)] = u[0][q];
+        __syncthreads();
+#pragma unroll
+        for (int q = 0; q < 16; ++q) {
+            const int k = t + T * q;
+            const cx<float> zc = cconj(s[phys(k == 0 ? 0 : L - k)]);
+            sp[k] = split_fwd(u[0][q], zc, ph[k], rr.shifted);
+        }
+        if (t == 0) sp[L] = split_fwd(u[0][0], cconj(u[0][0]), ph[L], rr.shifted);
+    } else {
+#pragma unroll
+        for (int r = 0; r < 16; ++r) {
+            const int k = t + T * r;
+            u[0][r] = pack_inv(sp[k], sp[L - k], cconj(ph[k]), cconj(ph[L - k]), rr.shifted);
+        }
+        fft3<LOGQ, 1>(u, s, tw, logPT, tw16, tw3);
+        cx<float>* __restrict__ o0 = reinterpret_cast<cx<float>*>(outmap + (int64_t)blockIdx.y * npix + rr.pix_off);
+#pragma unroll
+        for (int q = 0; q < 16; ++q) o0[t + T * q] = cconj(u[0][q]);
     }
 }
 

@@ -433,6 +433,8 @@ template <int LOGQ> int set_fft3_smem()
 {
     CUDA_TRY(cudaFuncSetAttribute(ring_fft3_forward_kernel<LOGQ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Fft3<LOGQ>::smem_bytes));
     CUDA_TRY(cudaFuncSetAttribute(ring_fft3_inverse_kernel<LOGQ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Fft3<LOGQ>::smem_bytes));
+    CUDA_TRY(cudaFuncSetAttribute(ring_fft3_direct1_kernel<LOGQ, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Fft3<LOGQ>::smem_bytes / 2));
+    CUDA_TRY(cudaFuncSetAttribute(ring_fft3_direct1_kernel<LOGQ, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Fft3<LOGQ>::smem_bytes / 2));
     return 0;
 }
 
@@ -589,8 +591,18 @@ void launch_fft3(const arkcos_plan* pl, const void* d_in, void* d_out, int nmaps
 {
     const int c = LOGQ - 9;
     if (pl->nfft3[c] == 0) return;
-    const dim3 grid((unsigned)pl->nfft3[c], (unsigned)nmaps);
     const HostGeometry& g = pl->g;
+    int njobs = pl->nfft3[c];
+    if (pl->nfft3[c] > pl->nfft3_bluestein[c]) {      // power-of-two rings: one transform per block
+        const int nb = pl->nfft3_bluestein[c], nd = pl->nfft3[c] - nb;
+        ring_fft3_direct1_kernel<LOGQ, FWD><<<dim3(2u * (unsigned)nd, (unsigned)nmaps), Fft3<LOGQ>::T, Fft3<LOGQ>::smem_bytes / 2, st>>>(
+            (const float*)d_in, (float*)d_out, g.npix, (cx<float>*)(FWD ? pl->d_specIn : pl->d_specOut), g.spec_total,
+            pl->d_fft3_jobs[c] + nb, (const cx<float>*)pl->d_tw, pl->logPT, (const cx<float>*)pl->d_tw16,
+            (const cx<float>*)pl->d_tw3 + pl->tw3_off[c], (const cx<float>*)pl->d_phase);
+        njobs = nb;
+        if (njobs == 0) return;
+    }
+    const dim3 grid((unsigned)njobs, (unsigned)nmaps);
     const int ahead = pl->sm_count * Fft3<LOGQ>::MINB;         // resident blocks: the one that will take this block's slot
     if (FWD)
         ring_fft3_forward_kernel<LOGQ><<<grid, Fft3<LOGQ>::T, Fft3<LOGQ>::smem_bytes, st>>>(
@@ -807,7 +819,11 @@ static int plan_create_impl(arkcos_plan** out, const arkcos_pixelization* pix, c
     pl->nsamples = t.nsamples;
     pl->logPT = t.logPT;
     pl->nfft_old = (int)t.fft_order.size();
-    for (int c = 0; c < 4; ++c) pl->nfft3[c] = (int)t.fft3_jobs[c].size();
+    for (int c = 0; c < 4; ++c) {
+        pl->nfft3[c] = (int)t.fft3_jobs[c].size();
+        pl->nfft3_bluestein[c] = 0;
+        for (const FftJob& j : t.fft3_jobs[c]) pl->nfft3_bluestein[c] += j.f.pow2 ? 0 : 1;
+    }
 
     if (tables_only) {
         guard.p = nullptr;
@@ -1054,7 +1070,7 @@ int arkcos_plan_launches_per_convolve(const arkcos_plan* pl)
     if (!pl) return -1;
     int n = (pl->opt.cache_kernel_rows || pl->npairs == 0) ? 0 : 1;
     int fft = pl->nfft_old > 0 ? 1 : 0;
-    for (int c = 0; c < 4; ++c) fft += pl->nfft3[c] > 0 ? 1 : 0;
+    for (int c = 0; c < 4; ++c) fft += (pl->nfft3_bluestein[c] > 0 ? 1 : 0) + (pl->nfft3[c] > pl->nfft3_bluestein[c] ? 1 : 0);
     n += 2 * fft;
     n += (pl->nitems[0] > 0) + (pl->npole > 0) + (pl->neqchunks > 0);
     for (int c = 1; c < kBandClasses; ++c) n += pl->nitems[c] > 0 ? 1 : 0;

@@ -70,6 +70,7 @@ struct arkcos_plan {
     // register-resident FFT kernels (arkcos_fft3.cuh): job lists for transform sizes Q = 512, 1024, 2048, 4096
     arkcos::FftJob* d_fft3_jobs[4] = {nullptr, nullptr, nullptr, nullptr};
     int nfft3[4] = {0, 0, 0, 0};
+    int nfft3_bluestein[4] = {0, 0, 0, 0};   // the first jobs of each list are the Bluestein rings, the rest pairs of power-of-two rings
     void* d_tw3 = nullptr;       // cx<float>: pass-3 twiddles of the four transform sizes, see arkcos_fft3.cuh
     int tw3_off[4] = {0, 0, 0, 0};
     void* d_tw16 = nullptr;      // cx<float>[256]: exp(-2 pi i r k / 256) at [16 r + k]
