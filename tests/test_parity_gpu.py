@@ -110,6 +110,28 @@ def test_healpix_small_full_map(nside, dtype):
         assert frms(out, ref1) <= 1e-5
 
 
+@pytest.mark.parametrize("nside,fwhm_px,nmaps", [(128, 2.0, 2), (256, 3.0, 3), (256, 1.5, 1)])
+def test_healpix_mid_size_all_kernel_classes(nside, fwhm_px, nmaps):
+    """Sizes at which the cap-run kernel, the register-resident FFTs (Q = 512, 1024) and the pole / general / uniform
+    kernels all serve some rings: every sampled ring equals oracle #2 at the plan's M' and oracle #1 to 1e-5."""
+    geom = geometry.healpix_ring(nside)
+    fwhm = fwhm_px * np.sqrt(4 * np.pi / geom.npix)
+    tmax = 3 * fwhm
+    tab = inputs.gaussian_table(fwhm, tmax)
+    x = inputs.white_noise_maps(geom.npix, 11, nmaps)
+    out, plan = gpu_convolve(("healpix", nside), tab, tmax, x)
+    assert np.isfinite(out).all()
+    mp = np.array([plan.ring_info(i)["mprime"] for i in range(geom.nrings)])
+    assert np.array_equal(mp, hybrid.mprime_rule(geom, tmax, plan.ell_nyquist))
+    R = geom.nrings
+    rings = np.unique(np.concatenate([np.arange(0, 12), np.arange(nside // 8 - 2, nside // 8 + 3), [nside // 2, nside // 2 + 1],
+                                      np.arange(nside - 16, nside + 16, 3), [2 * nside - 1, 3 * nside], R - 1 - np.arange(0, 40, 7)]))
+    ref2 = hybrid.hybrid_convolve(geom, tab, tmax, x.astype(np.float64), mprime=mp, out_rings=rings)
+    assert frms(take_rings(geom, out, rings), ref2) <= 1e-6
+    ref1 = direct.direct_sum(geom, tab, tmax, x.astype(np.float64), out_rings=rings)
+    assert frms(take_rings(geom, out, rings), ref1) <= 1e-5
+
+
 def test_healpix_paper_grid_polar_oversample():
     """polar_oversample = 1 is the paper's M = 4 nside: parity with oracle #2 at the same M."""
     nside = 16
