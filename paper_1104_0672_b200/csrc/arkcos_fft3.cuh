@@ -272,7 +272,7 @@ ring_fft3_inverse_kernel(const cx<float>* __restrict__ spec, int64_t spec_stride
             const int k = t + T * r;
             cx<float> v = mk<float>(0.f, 0.f);
             if (k < L) {
-                const cx<float> hk = cconj(ph[k]), hl = cconj(ph[L - k]);
+                const cx<float> hk = cconj(ph[k]), hl = mk<float>(hk.y, hk.x);     // exp(i pi (L-k)/N) = i conj(exp(i pi k/N))
                 v = cmul(pack_inv(D[r0.spec_off + k], D[r0.spec_off + L - k], hk, hl, r0.shifted), cw[k]);
             }
             u[0][r] = v;
@@ -333,7 +333,8 @@ ring_fft3_direct1_kernel(const float* __restrict__ in, float* __restrict__ outma
 #pragma unroll
         for (int r = 0; r < 16; ++r) {
             const int k = t + T * r;
-            u[0][r] = pack_inv(sp[k], sp[L - k], cconj(ph[k]), cconj(ph[L - k]), rr.shifted);
+            const cx<float> hk = cconj(ph[k]);                                 // exp(+i pi k / N)
+            u[0][r] = pack_inv(sp[k], sp[L - k], hk, mk<float>(hk.y, hk.x), rr.shifted);   // exp(i pi (L-k)/N) = i conj(hk)
         }
         fft3<LOGQ, 1>(u, s, tw, logPT, tw16, tw3);
         cx<float>* __restrict__ o0 = reinterpret_cast<cx<float>*>(outmap + (int64_t)blockIdx.y * npix + rr.pix_off);
