@@ -78,6 +78,10 @@ typedef struct {
  *  cache_kernel_rows 0: the kernel rows are re-evaluated from the profile table inside every arkcos_convolve (the
  *                       paper's timing includes the kernel evaluation, Table 1); 1: they are
  *                       evaluated once in arkcos_plan_create.
+ *  cache_kernel_spectra 1 (float plans): the cosine transforms G_ij[m] of the kernel rows (and the rows) are computed
+ *                       once in arkcos_plan_create and kept in device memory (4 bytes per ring pair and mode: 1.4 GB at
+ *                       nside 2048 for a 15' support); arkcos_convolve then only streams them, two maps per read when
+ *                       nmaps > 1.  For many maps with one kernel; rows of any length take the fast path.
  *  exact_caps        1 (HEALPix only): every output ring whose band contains a ring shorter than 4 nside (the polar caps
  *                       and the equatorial rings next to them) is recomputed by the direct-space sum of Eq. 6
  *                        after the hybrid pass, so that hard-edged kernels, for which the Fourier
@@ -90,7 +94,8 @@ typedef struct {
     int max_nmaps;
     int cache_kernel_rows;
     int exact_caps;
-    int reserved[7];               /* must be zero */
+    int cache_kernel_spectra;
+    int reserved[6];               /* must be zero */
 } arkcos_options;
 
 /* Builds the ring-geometry table (theta, N, phi0, offset per ring), the band and ring-pair tables, FFT twiddles,

@@ -537,14 +537,16 @@ namespace arkcos {
 // the whole chunk, its cosine table is built once, the (periodically extended) coefficient Bp_j[m] of an input ring is
 // loaded once per tile of TI output rings and reused from registers, rows are staged per tile with one row length per
 // input ring.  What differs from the equatorial case: the extension of Bp_j (reflection above N_j/2: conjugate, sign on
-// a shifted ring; single-period regime M'/2 < N_j) and the fold: T_i[m] belongs to the folded mode m (m <= N_i/2) or
-// N_i - m (conjugated, sign on a shifted ring i), so the block adds it into the zero-initialised output spectrum with a
-// vector reduction.  Every output coefficient receives at most two such terms, so the sum does not depend on their order.
+// a shifted ring and on its odd periods) and the fold: T_i[m], m = w N_i + r, belongs to the folded mode r (r <= N_i/2) or
+// N_i - r (conjugated; sign on the odd periods of a shifted ring i), so the block adds it into the zero-initialised
+// output spectrum with a vector reduction.  With M'/2 < N_i (Gaussian-like kernels: M' ~ 1.7 N_i) every output
+// coefficient receives at most two such terms and the sum does not depend on their order; hard-edged kernels (M' up to
+// 3 N_i) fold three or four terms, whose order of addition is then not fixed (last-bit differences between runs).
 constexpr int kCapChunkRings = 8;          // longest run handed to one block (two tiles): enough blocks to balance the device
-struct CapChunk { int i0, n, M, pad; };
+struct CapChunk { int i0, n, M, multi; };    // multi = 1: M/2 reaches past a ring length (several periods)
 struct CapChunkItem { int chunk, bx; };
 
-template <int TI, int TMAX>
+template <int TI, int TMAX, bool MULTI>
 __global__ void __launch_bounds__(kBandThreads)
 band_mac_capchunk_kernel(const CapChunkItem* __restrict__ items, const CapChunk* __restrict__ chunks,
                          const NorthRec* __restrict__ north, const PairRec* __restrict__ pairs,
@@ -577,9 +579,19 @@ band_mac_capchunk_kernel(const CapChunkItem* __restrict__ items, const CapChunk*
     const int mA = min(m0, Mh), mB = min(m0 + 1, Mh);
 
     // extended coefficient of input ring (Nj, shj) at mode m from the stored half spectrum (single period: m < Nj)
-    auto ext_index = [](int m, int Nj) { return 2 * m > Nj ? Nj - m : m; };
-    auto ext_value = [](cx<float> b, int m, int Nj, int shj) {
-        if (2 * m > Nj) { b.y = -b.y; if (shj) { b.x = -b.x; b.y = -b.y; } }
+    // periodic extension of the stored half spectrum of a ring (N_j, shifted flag in bit 31, magic = ceil(2^32 / N_j)):
+    // m = w N_j + r; above N_j/2 the coefficient is the conjugate of the one at N_j - r; a shifted ring changes sign on
+    // reflection and on every odd period (reading R8)
+    // (MULTI = false: the plan guarantees M'/2 < N_j and M'/2 < N_i for every ring involved, period 0 only)
+    auto ext_index = [](int m, int nj_sh, uint32_t magic) {
+        const int Nj = nj_sh & 0x7fffffff, w = MULTI ? (int)__umulhi((uint32_t)m, magic) : 0, r = m - w * Nj;
+        return 2 * r > Nj ? Nj - r : r;
+    };
+    auto ext_value = [](cx<float> b, int m, int nj_sh, uint32_t magic) {
+        const int Nj = nj_sh & 0x7fffffff, w = MULTI ? (int)__umulhi((uint32_t)m, magic) : 0, r = m - w * Nj;
+        const bool refl = 2 * r > Nj;
+        if (refl) b.y = -b.y;
+        if (nj_sh < 0 && (refl != ((w & 1) != 0))) { b.x = -b.x; b.y = -b.y; }
         return b;
     };
 
@@ -595,7 +607,8 @@ band_mac_capchunk_kernel(const CapChunkItem* __restrict__ items, const CapChunk*
         }
         for (int jj = threadIdx.x; jj < jw; jj += kBandThreads) {
             const RingRec rj = rings[jlo + jj];
-            sJ[jj] = make_int4((int)rj.spec_off, (int)rings[R - 1 - jlo - jj].spec_off, rj.n, rj.shifted);
+            sJ[jj] = make_int4((int)rj.spec_off, (int)rings[R - 1 - jlo - jj].spec_off, rj.n | (rj.shifted ? (int)0x80000000 : 0),
+                               MULTI ? (int)(uint32_t)((0x100000000ull + (uint64_t)rj.n - 1ull) / (uint64_t)rj.n) : 0);
         }
         __syncthreads();
         for (int k = threadIdx.x; k < (p_last - p_first) * G4; k += kBandThreads) {
@@ -621,7 +634,7 @@ band_mac_capchunk_kernel(const CapChunkItem* __restrict__ items, const CapChunk*
         cx<float> nx[2][MT];                                                // coefficients of the next input ring (raw)
         auto fetch = [&](int jj) {
             const int4 rj = sJ[min(jj, jw - 1)];
-            const int ia = ext_index(mA, rj.z), ib = ext_index(mB, rj.z);
+            const int ia = ext_index(mA, rj.z, (uint32_t)rj.w), ib = ext_index(mB, rj.z, (uint32_t)rj.w);
             nx[0][0] = in[rj.x + ia]; nx[0][1] = in[rj.x + ib];
             nx[1][0] = in[rj.y + ia]; nx[1][1] = in[rj.y + ib];
         };
@@ -631,8 +644,8 @@ band_mac_capchunk_kernel(const CapChunkItem* __restrict__ items, const CapChunk*
             cx<float> v[2][MT];
 #pragma unroll
             for (int h = 0; h < 2; ++h) {
-                v[h][0] = ext_value(nx[h][0], mA, rj.z, rj.w);
-                v[h][1] = ext_value(nx[h][1], mB, rj.z, rj.w);
+                v[h][0] = ext_value(nx[h][0], mA, rj.z, (uint32_t)rj.w);
+                v[h][1] = ext_value(nx[h][1], mB, rj.z, (uint32_t)rj.w);
             }
             fetch(jj + 1);
             const float* sWj = sW + jj * TMAX;
@@ -650,19 +663,23 @@ band_mac_capchunk_kernel(const CapChunkItem* __restrict__ items, const CapChunk*
                 const int i = i0 + ii, iS = R - 1 - i;
                 const RingRec ri = rings[i];
                 const int64_t offS = rings[iS].spec_off;
-                const float sg = ri.shifted ? -1.f : 1.f;
 #pragma unroll
                 for (int mt = 0; mt < MT; ++mt) {
                     const int m = m0 + mt;
                     if (m > Mh) continue;
                     const float hw = (2 * m == M) ? 0.5f : 1.f;          // the +-M/2 bins carry half the Nyquist term each
+                    // m = w N_i + r: folded mode r in period w (r <= N_i/2) and / or N_i - r in period w + 1 (conjugated);
+                    // a shifted ring changes sign on every odd period
+                    const int w = MULTI ? m / ri.n : 0, r = m - w * ri.n;
+                    const float s0 = (ri.shifted && (w & 1)) ? -1.f : 1.f, s1 = ri.shifted ? -s0 : s0;
 #pragma unroll
                     for (int h = 0; h < 2; ++h) {
                         if (h == 1 && iS == i) continue;
                         float2* dst = reinterpret_cast<float2*>(out + (h ? offS : ri.spec_off));
                         const float tx = hw * acc[ii][h][mt].x, ty = hw * acc[ii][h][mt].y;
-                        if (2 * m <= ri.n) atomicAdd(dst + m, make_float2(tx, ty));
-                        if (2 * m >= ri.n) atomicAdd(dst + (ri.n - m), make_float2(sg * tx, -sg * ty));
+                        if (2 * r <= ri.n) atomicAdd(dst + r, make_float2(s0 * tx, s0 * ty));
+                        if (2 * r >= ri.n) atomicAdd(dst + (ri.n - r), make_float2(s1 * tx, -s1 * ty));
+                        if (MULTI && r == 0 && w > 0) atomicAdd(dst, make_float2(s0 * tx, -s0 * ty));     // m = -w N_i folds onto 0 as well
                     }
                 }
             }

@@ -153,6 +153,8 @@ struct HostTables {
     std::vector<PairRec> pairs;
     std::vector<NorthRec> north;
     std::vector<BandItem> items[kBandClasses];
+    std::vector<CapChunkItem> cap_chunk_items_multi;   // items of runs that need more than one period of the ring spectra
+    int cap_nsingle = 0;
     std::vector<CapChunk> cap_chunks;            // runs of cap rings with one grid length for band_mac_capchunk_kernel
     std::vector<CapChunkItem> cap_chunk_items;
     std::vector<std::pair<int64_t, int64_t>> cap_zero;   // (first coefficient, count) ranges of the output spectrum to clear
@@ -252,7 +254,7 @@ void build_fft_lens(const HostGeometry& g, HostTables& t, Stats& st, bool use_ff
 }
 
 // Ring-pair table for the northern output rings (the southern ones reuse the rows of their mirror images).
-void build_pairs(HostGeometry& g, double theta_max, double ell_nyq, int fixed_mprime, int band_threads, bool allow_fast, bool allow_pole,
+void build_pairs(HostGeometry& g, double theta_max, double ell_nyq, int fixed_mprime, int band_threads, bool allow_fast, bool allow_pole, bool cached,
                  int sm_count, HostTables& t, Stats& st)
 {
     const int R = g.R, nnorth = (R + 1) / 2;
@@ -271,6 +273,10 @@ void build_pairs(HostGeometry& g, double theta_max, double ell_nyq, int fixed_mp
     }
     for (int i = 0; i < R; ++i) any_odd = any_odd || (g.n[i] == nmax && g.shifted[i] != g.shifted[std::min(i + 1, R - 1)] && g.n[std::min(i + 1, R - 1)] == nmax);
     const int eq_alt = any_odd ? 1 : 0;
+    int ncap_long = 0, ncap_multi = 0;                     // cap rings of 512+ pixels, and those whose grid spans several periods
+    for (int i = 0; i < nnorth; ++i)
+        if (g.n[i] >= 512 && g.n[i] < nmax) { ++ncap_long; ncap_multi += g.mprime[i] / 2 >= g.n[i] ? 1 : 0; }
+    const bool multi_is_rule = 4 * ncap_multi > ncap_long;
     t.eq_alt = eq_alt;
     t.north.resize(nnorth);
     for (int i = 0; i < nnorth; ++i) {
@@ -326,7 +332,7 @@ void build_pairs(HostGeometry& g, double theta_max, double ell_nyq, int fixed_mp
                 all_e = t.pairs[p].M == g.n[i] && g.n[t.pairs[p].j] == g.n[i];
                 alt_ok = alt_ok && t.pairs[p].par == (eq_alt ? ((i ^ t.pairs[p].j) & 1) : 0);
             }
-            if (all_e && alt_ok && hi > lo && maxcnt <= 12 && g.n[i] >= 8 && g.spec_total < (int64_t)INT32_MAX) {
+            if (all_e && alt_ok && hi > lo && (maxcnt <= 12 || cached) && g.n[i] >= 8 && g.spec_total < (int64_t)INT32_MAX) {
                 eq_rings.push_back(i);
                 st.band_flops[2] += ring_flops;
                 t.items[1].push_back(BandItem{i, g.n[i] / 2});      // the Nyquist bin m = M/2 goes to the uniform kernel
@@ -336,12 +342,13 @@ void build_pairs(HostGeometry& g, double theta_max, double ell_nyq, int fixed_mp
                 if (maxcnt <= 12) cls = odd ? 1 : 2;
                 else if (maxcnt <= 20 && !odd) cls = 3;
                 else if (maxcnt <= 32) cls = 4;
-                // single-period regime of band_mac_capchunk_kernel: M/2 below every ring length involved, N_i <= M
-                if ((cls == 2 || cls == 3) && !getenv("ARKCOS_NO_CAP_KERNEL")) {
-                    const int Mh = t.pairs[lo].M / 2;
-                    bool single = g.n[i] >= 512 && g.n[i] <= t.pairs[lo].M && Mh < g.n[i];
-                    for (int p = lo; p < hi; ++p) single = single && Mh < g.n[t.pairs[p].j];
-                    if (single) cls = 5;
+                // runs of band_mac_capchunk_kernel: one grid length, integer grid, rings long enough for 256-mode blocks
+                if ((cls == 2 || cls == 3 || (cached && !odd)) && !getenv("ARKCOS_NO_CAP_KERNEL")) {
+                    bool single_period = t.pairs[lo].M / 2 < g.n[i] && g.n[i] <= t.pairs[lo].M;
+                    for (int p = lo; p < hi; ++p) single_period = single_period && t.pairs[lo].M / 2 < g.n[t.pairs[p].j];
+                    // multi-period rings join the run kernel when they are the rule (hard-edged kernels: M' up to 3 N_i) or when
+                    // the spectra are cached; a few stragglers of a Gaussian plan stay with the uniform kernels
+                    if (g.n[i] >= 512 && t.pairs[lo].M / 2 < (1 << 15) && (single_period || cached || multi_is_rule)) cls = 5;
                 }
             }
         }
@@ -361,11 +368,15 @@ void build_pairs(HostGeometry& g, double theta_max, double ell_nyq, int fixed_mp
         st.band_flops[slot_of_cls[cls]] += ring_flops;
         if (cls == 5) {
             const int M = t.pairs[t.north[i].pair_lo].M;
+            // single-period ring: M/2 below the length of ring i and of every ring of its band (a run is homogeneous)
+            bool single = M / 2 < g.n[i] && g.n[i] <= M;
+            for (int p = t.north[i].pair_lo; p < t.north[i].pair_hi; ++p) single = single && M / 2 < g.n[t.pairs[p].j];
+            const int multi = single ? 0 : 1;
             if (!t.cap_chunks.empty() && t.cap_chunks.back().i0 + t.cap_chunks.back().n == i && t.cap_chunks.back().M == M &&
-                t.cap_chunks.back().n < kCapChunkRings)
+                t.cap_chunks.back().multi == multi && t.cap_chunks.back().n < kCapChunkRings)
                 ++t.cap_chunks.back().n;
             else
-                t.cap_chunks.push_back(CapChunk{i, 1, M, 0});
+                t.cap_chunks.push_back(CapChunk{i, 1, M, multi});
             continue;
         }
         for (int m0 = 0; m0 <= g.n[i] / 2; m0 += band_threads) t.items[cls].push_back(BandItem{i, m0});
@@ -387,7 +398,8 @@ void build_pairs(HostGeometry& g, double theta_max, double ell_nyq, int fixed_mp
     }
     for (size_t c = 0; c < t.cap_chunks.size(); ++c) {
         const CapChunk& ch = t.cap_chunks[c];
-        for (int bx = 0; bx * (kBandThreads * 2) <= ch.M / 2; ++bx) t.cap_chunk_items.push_back(CapChunkItem{(int)c, bx});
+        for (int bx = 0; bx * (kBandThreads * 2) <= ch.M / 2; ++bx)
+            (ch.multi ? t.cap_chunk_items_multi : t.cap_chunk_items).push_back(CapChunkItem{(int)c, bx});
         // output coefficients of the chunk's rings (north and mirror image) are accumulated: they start from zero
         const int iA = ch.i0, iB = ch.i0 + ch.n - 1;
         auto add_range = [&](int ra, int rb) {
@@ -400,6 +412,9 @@ void build_pairs(HostGeometry& g, double theta_max, double ell_nyq, int fixed_mp
     }
     // longest blocks first (the chunks run from the pole towards the equator, M' grows)
     std::reverse(t.cap_chunk_items.begin(), t.cap_chunk_items.end());
+    std::reverse(t.cap_chunk_items_multi.begin(), t.cap_chunk_items_multi.end());
+    t.cap_nsingle = (int)t.cap_chunk_items.size();                               // single-period items first, then the others
+    t.cap_chunk_items.insert(t.cap_chunk_items.end(), t.cap_chunk_items_multi.begin(), t.cap_chunk_items_multi.end());
     std::sort(t.cap_zero.begin(), t.cap_zero.end());
     for (size_t k = 1; k < t.cap_zero.size();) {                             // merge adjacent ranges
         if (t.cap_zero[k - 1].first + t.cap_zero[k - 1].second == t.cap_zero[k].first) {
@@ -554,7 +569,17 @@ template <int TMAX, bool HAS_ODD> void launch_uniform_class(const arkcos_plan* p
 void launch_uniform(const arkcos_plan* pl, int nmaps, cudaStream_t st, bool serial)
 {
     cudaStream_t s1 = serial ? st : pl->side[1], s2 = serial ? st : pl->side[2];
-    if (pl->neqchunks > 0) {
+    if (pl->neqchunks > 0 && pl->d_G) {
+        const unsigned gx = (unsigned)((pl->eq_mh + kBandThreads * 2 - 1) / (kBandThreads * 2));
+        if (nmaps > 1)
+            band_mac_eq_cached_kernel<4, 2><<<dim3(gx, (unsigned)pl->neqchunks, (unsigned)((nmaps + 1) / 2)), kBandThreads, 0, st>>>(
+                pl->d_eqchunks, pl->d_north, pl->d_pairs, pl->d_goff, pl->d_G, pl->d_rings, pl->g.R,
+                (const cx<float>*)pl->d_specIn, (cx<float>*)pl->d_specOut, pl->g.spec_total, nmaps);
+        else
+            band_mac_eq_cached_kernel<4, 1><<<dim3(gx, (unsigned)pl->neqchunks, 1), kBandThreads, 0, st>>>(
+                pl->d_eqchunks, pl->d_north, pl->d_pairs, pl->d_goff, pl->d_G, pl->d_rings, pl->g.R,
+                (const cx<float>*)pl->d_specIn, (cx<float>*)pl->d_specOut, pl->g.spec_total, nmaps);
+    } else if (pl->neqchunks > 0) {
         constexpr int TI = 4, MT = 2;
         const dim3 grid((unsigned)((pl->eq_mh + kBandThreads * MT - 1) / (kBandThreads * MT)), (unsigned)pl->neqchunks, (unsigned)nmaps);
         if (pl->eq_alt)
@@ -576,9 +601,26 @@ void launch_uniform(const arkcos_plan* pl, int nmaps, cudaStream_t st, bool seri
     launch_uniform_class<12, true>(pl, 1, nmaps, s2);
     if (serial) cudaEventRecord(pl->ev_band[7], st);
     if (pl->ncapitems > 0) {
-        band_mac_capchunk_kernel<4, 20><<<dim3((unsigned)pl->ncapitems, (unsigned)nmaps), kBandThreads, 0, s1>>>(
-            pl->d_cap_chunk_items, pl->d_cap_chunks, pl->d_north, pl->d_pairs, (const float*)pl->d_W, pl->d_rings, pl->g.R,
-            (const cx<float>*)pl->d_specIn, (cx<float>*)pl->d_specOut, pl->g.spec_total);
+        auto launch_cap = [&](auto multi_tag, int first, int count) {
+            constexpr bool MULTI = decltype(multi_tag)::value;
+            if (count <= 0) return;
+            const unsigned n = (unsigned)count;
+            const CapChunkItem* items = pl->d_cap_chunk_items + first;
+            if (pl->d_G && nmaps > 1)
+                band_mac_capchunk_cached_kernel<4, 2, MULTI><<<dim3(n, (unsigned)((nmaps + 1) / 2)), kBandThreads, 0, s1>>>(
+                    items, pl->d_cap_chunks, pl->d_north, pl->d_pairs, pl->d_goff, pl->d_G, pl->d_rings, pl->g.R,
+                    (const cx<float>*)pl->d_specIn, (cx<float>*)pl->d_specOut, pl->g.spec_total, nmaps);
+            else if (pl->d_G)
+                band_mac_capchunk_cached_kernel<4, 1, MULTI><<<dim3(n, 1), kBandThreads, 0, s1>>>(
+                    items, pl->d_cap_chunks, pl->d_north, pl->d_pairs, pl->d_goff, pl->d_G, pl->d_rings, pl->g.R,
+                    (const cx<float>*)pl->d_specIn, (cx<float>*)pl->d_specOut, pl->g.spec_total, nmaps);
+            else
+                band_mac_capchunk_kernel<4, 20, MULTI><<<dim3(n, (unsigned)nmaps), kBandThreads, 0, s1>>>(
+                    items, pl->d_cap_chunks, pl->d_north, pl->d_pairs, (const float*)pl->d_W, pl->d_rings, pl->g.R,
+                    (const cx<float>*)pl->d_specIn, (cx<float>*)pl->d_specOut, pl->g.spec_total);
+        };
+        launch_cap(std::false_type{}, 0, pl->ncapsingle);
+        launch_cap(std::true_type{}, pl->ncapsingle, pl->ncapitems - pl->ncapsingle);
     }
     if (serial) cudaEventRecord(pl->ev_band[8], st);
 }
@@ -769,6 +811,11 @@ static int plan_create_impl(arkcos_plan** out, const arkcos_pixelization* pix, c
     for (int r : opt.reserved) if (r != 0) return fail(ARKCOS_INVALID_ARG, "options.reserved must be zero");
     if (opt.variant != 0 && opt.variant != 1) return fail(ARKCOS_INVALID_ARG, "options.variant must be 0 or 1");
     if (opt.exact_caps != 0 && opt.exact_caps != 1) return fail(ARKCOS_INVALID_ARG, "options.exact_caps must be 0 or 1");
+    if (opt.cache_kernel_spectra != 0 && opt.cache_kernel_spectra != 1)
+        return fail(ARKCOS_INVALID_ARG, "options.cache_kernel_spectra must be 0 or 1");
+    if (opt.cache_kernel_spectra && (dtype != ARKCOS_F32 || opt.variant != 0))
+        return fail(ARKCOS_UNSUPPORTED, "cache_kernel_spectra needs a float plan of variant 0");
+    if (opt.cache_kernel_spectra) opt.cache_kernel_rows = 1;     // the spectra are made from the rows, once
     if (opt.max_nmaps < 0 || opt.polar_oversample < 0 || opt.ell_nyquist < 0.0 || opt.max_nmaps > 65535)
         return fail(ARKCOS_INVALID_ARG, "negative option");
     const int maxlen = dtype == ARKCOS_F32 ? 16384 : 8192;
@@ -805,7 +852,7 @@ static int plan_create_impl(arkcos_plan** out, const arkcos_pixelization* pix, c
     pl->sm_count = sm_count;
     HostTables t;
     build_fft_lens(pl->g, t, pl->stats, dtype == ARKCOS_F32 && !getenv("ARKCOS_FORCE_OLD_FFT"));
-    build_pairs(pl->g, pl->theta_max, pl->ell_nyquist, fixed_mprime, kBandThreads, dtype == ARKCOS_F32 && opt.variant == 0 && !getenv("ARKCOS_FORCE_GENERAL"), opt.variant == 0, sm_count, t, pl->stats);
+    build_pairs(pl->g, pl->theta_max, pl->ell_nyquist, fixed_mprime, kBandThreads, dtype == ARKCOS_F32 && opt.variant == 0 && !getenv("ARKCOS_FORCE_GENERAL"), opt.variant == 0, opt.cache_kernel_spectra != 0, sm_count, t, pl->stats);
     if (t.pairs.size() > (size_t)INT32_MAX) return fail(ARKCOS_UNSUPPORTED, "too many ring pairs");
     pl->nnorth = (int)t.north.size();
     pl->npairs = (int)t.pairs.size();
@@ -856,6 +903,7 @@ static int plan_create_impl(arkcos_plan** out, const arkcos_pixelization* pix, c
     if (int rc = upload(&pl->d_cap_chunks, t.cap_chunks, wsb)) return rc;
     if (int rc = upload(&pl->d_cap_chunk_items, t.cap_chunk_items, wsb)) return rc;
     pl->ncapitems = (int)t.cap_chunk_items.size();
+    pl->ncapsingle = t.cap_nsingle;
     pl->cap_zero = t.cap_zero;
     std::vector<double> tab(kernel->table, kernel->table + kernel->n);
     if (int rc = upload(&pl->d_table, tab, wsb)) return rc;
@@ -870,6 +918,25 @@ static int plan_create_impl(arkcos_plan** out, const arkcos_pixelization* pix, c
     CUDA_TRY(cudaEventCreateWithFlags(&pl->ev_rows_done, cudaEventDisableTiming));
     if (opt.cache_kernel_rows) {
         dtype == ARKCOS_F32 ? enqueue_rows<float>(pl, 0) : enqueue_rows<double>(pl, 0);
+        CUDA_TRY(cudaDeviceSynchronize());
+    }
+    if (opt.cache_kernel_spectra && pl->npairs > 0) {
+        // one row of M/2 + 1 floats per northern ring pair, padded to a multiple of four
+        std::vector<uint32_t> goff(t.pairs.size());
+        uint64_t n4 = 0;
+        int mh_max = 0;
+        for (size_t p = 0; p < t.pairs.size(); ++p) {
+            goff[p] = (uint32_t)n4;
+            n4 += (uint64_t)(t.pairs[p].M / 2 + 1 + 3) / 4;
+            mh_max = std::max(mh_max, t.pairs[p].M / 2);
+        }
+        if (n4 >= 0xffffffffull) return fail(ARKCOS_UNSUPPORTED, "kernel spectra too large to cache");
+        if (int rc = upload(&pl->d_goff, goff, wsb)) return rc;
+        CUDA_TRY(cudaMalloc(&pl->d_G, (size_t)n4 * 16));
+        pl->stats.workspace_bytes += (int64_t)n4 * 16;
+        CUDA_TRY(cudaMemset(pl->d_G, 0, (size_t)n4 * 16));
+        kernel_spectra_kernel<<<dim3((unsigned)pl->npairs, (unsigned)(mh_max / 256 + 1)), 256>>>(
+            pl->d_pairs, (const float*)pl->d_W, pl->d_goff, pl->d_G);
         CUDA_TRY(cudaDeviceSynchronize());
     }
     CUDA_TRY(cudaGetLastError());
@@ -985,7 +1052,7 @@ int arkcos_plan_destroy(arkcos_plan* pl)
     void* ptrs[] = {pl->d_rings, pl->d_lens, pl->d_pairs, pl->d_north, pl->d_items[0], pl->d_items[1], pl->d_items[2], pl->d_items[3],
                     pl->d_items[4], pl->d_items[5], pl->d_eqchunks, pl->d_pole, pl->d_chirp, pl->d_phase, pl->d_fft_order, pl->d_table, pl->d_tw, pl->d_filt,
                     pl->d_W, pl->d_specIn, pl->d_specOut, pl->d_stage_in, pl->d_stage_out,
-                    pl->d_cap_chunks, pl->d_cap_chunk_items, pl->d_direct_items, pl->d_tw3, pl->d_tw16, pl->d_fft3_jobs[0], pl->d_fft3_jobs[1], pl->d_fft3_jobs[2], pl->d_fft3_jobs[3]};
+                    pl->d_cap_chunks, pl->d_cap_chunk_items, pl->d_goff, pl->d_G, pl->d_direct_items, pl->d_tw3, pl->d_tw16, pl->d_fft3_jobs[0], pl->d_fft3_jobs[1], pl->d_fft3_jobs[2], pl->d_fft3_jobs[3]};
     for (void* p : ptrs) if (p) cudaFree(p);
     for (auto& e : pl->ev) if (e) cudaEventDestroy(e);
     for (auto& e : pl->ev_band) if (e) cudaEventDestroy(e);
@@ -1075,7 +1142,7 @@ int arkcos_plan_launches_per_convolve(const arkcos_plan* pl)
     n += (pl->nitems[0] > 0) + (pl->npole > 0) + (pl->neqchunks > 0);
     for (int c = 1; c < kBandClasses; ++c) n += pl->nitems[c] > 0 ? 1 : 0;
     n += pl->ndirect > 0 ? 1 : 0;
-    n += pl->ncapitems > 0 ? 1 : 0;
+    n += (pl->ncapsingle > 0 ? 1 : 0) + (pl->ncapitems > pl->ncapsingle ? 1 : 0);
     return n;
 }
 

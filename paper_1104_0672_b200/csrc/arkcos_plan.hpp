@@ -11,6 +11,7 @@
 #include "arkcos_fft.cuh"
 #include "arkcos_fft3.cuh"
 #include "arkcos_direct.cuh"
+#include "arkcos_band_cached.cuh"
 
 namespace arkcos {
 
@@ -51,11 +52,14 @@ struct arkcos_plan {
     arkcos::NorthRec* d_north = nullptr;
     arkcos::EqChunk* d_eqchunks = nullptr;
     int neqchunks = 0, eq_mh = 0, eq_alt = 0;
+    uint32_t* d_goff = nullptr;       // cache_kernel_spectra: first float4 of each northern pair's row in d_G
+    float* d_G = nullptr;
     arkcos::BandItem* d_direct_items = nullptr;   // exact_caps: {northern ring, first pixel} per block of direct_rings_kernel
     int ndirect = 0;
     arkcos::CapChunk* d_cap_chunks = nullptr;
     arkcos::CapChunkItem* d_cap_chunk_items = nullptr;
     int ncapitems = 0;
+    int ncapsingle = 0;               // the first ncapsingle items are single-period runs
     std::vector<std::pair<int64_t, int64_t>> cap_zero;    // output-spectrum ranges cleared before band_mac_capchunk_kernel
     int* d_pole = nullptr;
     int npole = 0, pole_mh = 0;

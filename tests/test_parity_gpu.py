@@ -132,6 +132,30 @@ def test_healpix_mid_size_all_kernel_classes(nside, fwhm_px, nmaps):
     assert frms(take_rings(geom, out, rings), ref1) <= 1e-5
 
 
+@pytest.mark.parametrize("cache", [0, 1], ids=["computed", "cached_spectra"])
+@pytest.mark.parametrize("kernel", ["gauss", "tophat", "mexhat"])
+def test_healpix_256_cap_runs_and_cached_spectra(kernel, cache):
+    """nside 256, 3 maps: single-period cap runs (Gaussian), multi-period ones (hard-edged kernels: M' up to 3 N_i) and
+    the cached-spectra kernels (options.cache_kernel_spectra, two maps per read of G) against oracle #2 at the plan's M'."""
+    nside, nmaps = 256, 3
+    geom = geometry.healpix_ring(nside)
+    px = np.sqrt(4 * np.pi / geom.npix)
+    tab, tmax = {"gauss": (inputs.gaussian_table(2.5 * px, 7.5 * px), 7.5 * px),
+                 "tophat": (inputs.tophat_table(5.8 * px), 5.8 * px),
+                 "mexhat": (inputs.mexican_hat_table(2.33 * px, 5 * 2.33 * px), 5 * 2.33 * px)}[kernel]
+    x = inputs.white_noise_maps(geom.npix, 12, nmaps)
+    out, plan = gpu_convolve(("healpix", nside), tab, tmax, x, cache_kernel_spectra=cache)
+    assert np.isfinite(out).all()
+    mp = np.array([plan.ring_info(i)["mprime"] for i in range(geom.nrings)])
+    R = geom.nrings
+    rings = np.unique(np.concatenate([[0, 5, 40, 127, 128, 129, 160, 200, 255, 256, 257, 300, 511, 700], R - 1 - np.array([0, 50, 130, 250])]))
+    ref2 = hybrid.hybrid_convolve(geom, tab, tmax, x.astype(np.float64), mprime=mp, out_rings=rings)
+    assert frms(take_rings(geom, out, rings), ref2) <= 1e-6
+    # a second call on the same plan (accumulating fold: the output spectrum must be cleared every time)
+    out2, _ = gpu_convolve(("healpix", nside), tab, tmax, x, plan=plan)
+    assert frms(take_rings(geom, out2, rings), ref2) <= 1e-6
+
+
 def test_healpix_paper_grid_polar_oversample():
     """polar_oversample = 1 is the paper's M = 4 nside: parity with oracle #2 at the same M."""
     nside = 16
