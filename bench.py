@@ -282,6 +282,22 @@ def run_ours(args):
     roof["all_kernels"] = [{k: v for k, v in kk.items() if k != "peak_source"} for kk in kernels]
     launches_per_step = plan.launches_per_convolve
 
+    # beside the headline (kernel rows regenerated every step, Table 1): the plan-cached mode for many maps
+    # with one kernel, rows and their transforms computed once at plan time
+    plan_c = arkcos.Plan(c["pix"], tab, c["theta_max"], dtype, max_nmaps=nmaps, cache_kernel_spectra=1)
+    for _ in range(3):
+        plan_c.convolve(d_in.data_ptr(), d_out.data_ptr(), nmaps, stream)
+    torch.cuda.synchronize()
+    e0.record()
+    for _ in range(args.steps):
+        plan_c.convolve(d_in.data_ptr(), d_out.data_ptr(), nmaps, stream)
+    e1.record()
+    torch.cuda.synchronize()
+    cached_ms = e0.elapsed_time(e1) / args.steps
+    cached = {"ms_per_step": cached_ms, "value": npix * nmaps / (cached_ms * 1e-3) / 1e6, "unit": UNIT,
+              "workspace_gb": plan_c.stats()["workspace_bytes"] / 1e9, "note": "options.cache_kernel_spectra = 1; not the headline"}
+    del plan_c
+
     cpu = time_oracle(c, tab, x, args.oracle_rings)
     cpu_val = cpu["pixels"] * cpu["maps"] / cpu["seconds"] / 1e6
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
@@ -295,7 +311,7 @@ def run_ours(args):
             "cpu_baseline": {"value": cpu_val, "unit": UNIT, "cores": cpu["threads"], "kind": "oracle",
                              "sample": f"{cpu['rings']} of {cpu['nrings']} output rings evenly spaced in ring index, "
                                        f"{cpu['pixels']} pixels, {cpu['seconds']:.1f} s"},
-            "e2e": e2e, "gpu_launches": launches_per_step * args.steps, "clocks": clocks,
+            "cached_spectra_mode": cached, "e2e": e2e, "gpu_launches": launches_per_step * args.steps, "clocks": clocks,
             "paper_context": "2.2 s on a GTX 480 incl. PCIe copies = 22.9 Mpix/s (PAPER.md:195)"}
     print(json.dumps(line))
     if world > 1:
