@@ -282,3 +282,70 @@ def test_funk_hecke_l0_l1():
         for op in (direct.direct_sum, hybrid.hybrid_convolve):
             out = op(geom, tab, tmax, Y, out_rings=rings)
             assert np.abs(out - Kl * Y[sel]).max() < 2e-3 * abs(Kl), lm
+
+
+# ---------------------------------------------------------------- oracle #2, variant A ------------------------
+# The basic scheme (PAPER.md:125 zero-padding, PAPER.md:142 truncation at the ring's Nyquist frequency) treats the samples
+# of input ring j as their band-limited trigonometric interpolant.  A single azimuthal harmonic on one input ring is
+# therefore mapped to the same harmonic on every output ring of the band, scaled by the cosine transform of the
+# kernel row:   in(j, l) = trig(m0 phi_jl)   =>   out(i, k) = Omega_j (N_j / M) kt_ij[m0] trig(m0 phi_ik)
+# for m0 <= N_j / 2 and m0 <= N_i / 2, and 0 for m0 > N_i / 2; kt_ij[m0] = sum_d kappa_ij(psi_d) cos(m0 psi_d) over the
+# M sample positions psi_d of the row (offset by phi0_i - phi0_j for two full-length rings).
+# The expectation is evaluated here from that closed statement (hybrid.kernel_row is pinned by the Jacobi-Anger test).
+
+def _variant_a_expectation(geom, i, j, m0, trig, tab, tmax, M):
+    class_e = geom.n[i] == geom.n.max() and geom.n[j] == geom.n.max()
+    delta = geom.phi0[i] - geom.phi0[j] if class_e else 0.0
+    psi = delta + 2.0 * np.pi * np.arange(M) / M
+    kt = float((hybrid.kernel_row(geom.theta[i], geom.theta[j], psi, tab, tmax) * np.cos(m0 * psi)).sum())
+    if 2 * m0 > geom.n[i] or 2 * m0 > geom.n[j]:
+        return np.zeros(int(geom.n[i]))
+    return geom.omega[j] * (geom.n[j] / M) * kt * trig(m0 * geom.phi(i))
+
+
+@pytest.mark.parametrize("case", ["interior", "nyquist_of_j", "edge_of_i"])
+def test_variant_a_single_harmonic(case):
+    """Pins the zero-pad weights (half/half split of ring j's own Nyquist bin, nothing above it), the truncation edge
+    of the output ring (|m| = N_i/2 kept, N_i/2 + 1 dropped), the sign of Eq. 8 and the normalisation of variant A."""
+    nside = 8
+    geom = geometry.healpix_ring(nside)
+    tmax = 40 * DEG
+    tab = gauss(25 * DEG, tmax)
+    M = 64
+    if case == "interior":          # harmonic well below both Nyquist frequencies; cap, cap-boundary and equatorial pairs
+        todo = [(5, 6, 3, np.cos), (6, 5, 3, np.sin), (7, 8, 7, np.cos), (9, 6, 4, np.sin), (12, 13, 9, np.cos), (13, 12, 9, np.sin)]
+    elif case == "nyquist_of_j":    # m0 = N_j / 2 exactly: on a shifted ring cos(m0 phi_jl) = 0, sin(m0 phi_jl) = (-1)^l
+        todo = [(6, 4, 10, np.sin), (5, 5, 12, np.sin), (7, 3, 8, np.sin), (3, 4, 10, np.sin)]      # last: N_i < N_j, truncated
+    else:                           # output ring shorter than the input ring: m0 = N_i/2 - 1, N_i/2, N_i/2 + 1
+        todo = [(3, 6, 7, np.cos), (3, 6, 8, np.sin), (3, 6, 9, np.cos), (3, 6, 9, np.sin), (4, 9, 11, np.cos)]
+    for i, j, m0, trig in todo:
+        x = np.zeros(geom.npix)
+        x[geom.ring_slice(j)] = trig(m0 * geom.phi(j))
+        assert np.abs(x).max() > 0.5
+        out = hybrid.hybrid_convolve(geom, tab, tmax, x, variant="A", mprime=M, out_rings=np.array([i]))
+        expect = _variant_a_expectation(geom, i, j, m0, trig, tab, tmax, int(geom.n[i]) if geom.n[i] == geom.n[j] == 4 * nside else M)
+        scale = geom.omega[j] * geom.n[j]
+        assert np.abs(out - expect).max() <= 1e-13 * scale, (case, i, j, m0)
+        if case != "interior" and 2 * m0 <= geom.n[i] and 2 * m0 <= geom.n[j]:
+            assert np.abs(expect).max() > 1e-4 * scale          # the kept edge modes really carry signal
+
+
+def test_variant_a_ecp_equals_direct():
+    """On ECP every pair is class E and N_i = N_j = M: zero-padding and truncation do nothing, so variant A is the
+    same exact circulant identity as variant B ("vanish exactly")."""
+    geom = geometry.ecp(12, 24)
+    tmax = 35 * DEG
+    tab = inputs.tophat_table(tmax)
+    x = np.random.default_rng(17).standard_normal(geom.npix)
+    a = direct.direct_sum(geom, tab, tmax, x)
+    b = hybrid.hybrid_convolve(geom, tab, tmax, x, variant="A")
+    assert np.abs(a - b).max() <= 1e-13 * np.abs(a).max()
+
+
+def test_direct_dft_beyond_library_switch():
+    """hybrid.dft switches to the library FFT above 1024 points: one direct-definition spot check at a longer length."""
+    N = 1500
+    x = np.random.default_rng(2).standard_normal(N) + 1j * np.random.default_rng(3).standard_normal(N)
+    X = hybrid.dft(x)
+    for m in (0, 1, 749, 750, 1499):
+        assert abs(X[m] - (x * np.exp(-2j * np.pi * ((m * np.arange(N)) % N) / N)).sum()) <= 1e-10 * np.abs(x).sum()
