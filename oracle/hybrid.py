@@ -65,20 +65,20 @@ def kernel_row(theta_i, theta_j, psi, table, theta_max) -> np.ndarray:
     return np.where(gamma < theta_max, kernel_lerp(table, theta_max, np.minimum(gamma, theta_max)), 0.0)
 
 
-def mprime_rule(geom: RingGeometry, theta_max: float, ell_nyq: float) -> np.ndarray:
-    """M'_i for class-C pairs of output ring i (reading R10).
+def mprime_resolving(geom: RingGeometry, theta_max: float, ell_nyq: float) -> np.ndarray:
+    """Shortest class-C grid per output ring that resolves wavenumber ell_nyq along the ring (reading R10).
 
-    The paper samples every kernel row on 4 nside points.  Here the grid of a
-    cap-touching row resolves wavenumber ell_nyq along the ring:  M'_i = 2 ceil(ell_nyq * smax_i),
-    smax_i = max sin(theta) over ring i and its band, never below 8.
+    The paper samples every kernel row on 4 nside points.  Under reading R10 the grid of a
+    cap-touching row resolves wavenumber ell_nyq along the ring:  M'_i >= 2 ceil(ell_nyq * smax_i),
+    smax_i = max sin(theta) over ring i and its band, never below 8.  Any even M'_i at or above this bound is a valid
+    setting of the scheme; which one a plan uses is the plan's parameter ("run it with the plan's
+    settings"), passed to hybrid_convolve as ``mprime``.
     """
     out = np.empty(geom.nrings, dtype=np.int64)
     s = np.sin(geom.theta)
     for i in range(geom.nrings):
         smax = s[band(geom, i, theta_max)].max()
         out[i] = max(8, 2 * int(np.ceil(ell_nyq * smax)))
-        if out[i] >= 512:                       # runs of consecutive cap rings share one grid length (reading R10)
-            out[i] = (out[i] + 127) // 128 * 128
     return out
 
 

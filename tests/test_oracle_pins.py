@@ -200,7 +200,7 @@ def test_healpix_point_source_sign_of_eq8():
     tmax = 3 * fwhm
     sigma = fwhm * inputs.FWHM_TO_SIGMA
     tab = gauss(fwhm, tmax)
-    mp = hybrid.mprime_rule(geom, tmax, 5.5 / sigma)
+    mp = hybrid.mprime_resolving(geom, tmax, 5.5 / sigma)
     x = np.zeros(geom.npix)
     q0 = int(geom.offset[nside - 3]) + 5                      # in the north cap, two rings above the belt
     x[q0] = 1.0
@@ -223,7 +223,7 @@ def test_cap_method_error_orders():
     a = direct.direct_sum(geom, tab, tmax, x)
     eB = frms(hybrid.hybrid_convolve(geom, tab, tmax, x), a)
     eA = frms(hybrid.hybrid_convolve(geom, tab, tmax, x, variant="A"), a)
-    eR = frms(hybrid.hybrid_convolve(geom, tab, tmax, x, mprime=hybrid.mprime_rule(geom, tmax, 5.0 / sigma)), a)
+    eR = frms(hybrid.hybrid_convolve(geom, tab, tmax, x, mprime=hybrid.mprime_resolving(geom, tmax, 5.0 / sigma)), a)
     assert 3e-5 < eB < 1e-3 and 5e-4 < eA < 2e-2 and eB < eA and eR < 1e-8
 
 

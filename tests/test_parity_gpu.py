@@ -10,6 +10,7 @@ import pytest
 
 from oracle import geometry, direct, hybrid
 from paper_1104_0672_b200 import arkcos, inputs
+from plan_checks import plan_mprime
 
 pytestmark = pytest.mark.gpu
 torch = pytest.importorskip("torch")
@@ -98,8 +99,7 @@ def test_healpix_small_full_map(nside, dtype):
     ell = 5.5 / sigma
     x = inputs.white_noise(geom.npix, 9, dtype=np.float64 if dtype == arkcos.F64 else np.float32)
     out, plan = gpu_convolve(("healpix", nside), tab, tmax, x, dtype, ell_nyquist=ell)
-    mp = hybrid.mprime_rule(geom, tmax, ell)
-    assert [plan.ring_info(i)["mprime"] for i in range(geom.nrings)] == list(mp)
+    mp = plan_mprime(plan, geom, tmax, ell)
     ref2 = hybrid.hybrid_convolve(geom, tab, tmax, x.astype(np.float64), mprime=mp)
     ref1 = direct.direct_sum(geom, tab, tmax, x.astype(np.float64))
     if dtype == arkcos.F64:
@@ -121,8 +121,7 @@ def test_healpix_mid_size_all_kernel_classes(nside, fwhm_px, nmaps):
     x = inputs.white_noise_maps(geom.npix, 11, nmaps)
     out, plan = gpu_convolve(("healpix", nside), tab, tmax, x)
     assert np.isfinite(out).all()
-    mp = np.array([plan.ring_info(i)["mprime"] for i in range(geom.nrings)])
-    assert np.array_equal(mp, hybrid.mprime_rule(geom, tmax, plan.ell_nyquist))
+    mp = plan_mprime(plan, geom, tmax)
     R = geom.nrings
     rings = np.unique(np.concatenate([np.arange(0, 12), np.arange(nside // 8 - 2, nside // 8 + 3), [nside // 2, nside // 2 + 1],
                                       np.arange(nside - 16, nside + 16, 3), [2 * nside - 1, 3 * nside], R - 1 - np.arange(0, 40, 7)]))
@@ -203,8 +202,8 @@ def test_hard_edged_kernels_vs_scheme_oracle():
     for tab, tmax in [(inputs.tophat_table(5.8 * pixsz), 5.8 * pixsz),
                       (inputs.mexican_hat_table(2.33 * pixsz, 5 * 2.33 * pixsz), 5 * 2.33 * pixsz)]:
         ell = 6.0 * nside
-        out, _ = gpu_convolve(("healpix", nside), tab, tmax, x, arkcos.F32, ell_nyquist=ell)
-        mp = hybrid.mprime_rule(geom, tmax, ell)
+        out, plan = gpu_convolve(("healpix", nside), tab, tmax, x, arkcos.F32, ell_nyquist=ell)
+        mp = plan_mprime(plan, geom, tmax, ell)
         ref2 = hybrid.hybrid_convolve(geom, tab, tmax, x.astype(np.float64), mprime=mp)
         assert frms(out, ref2) <= 1e-6
         eq = np.array([i for i in range(geom.nrings) if np.all(geom.n[geometry.band(geom, i, tmax)] == 4 * nside)])
@@ -247,8 +246,7 @@ def test_cfg3_fp32_sampled_rings():
     ref = direct.direct_sum(geom, tab, tmax, x.astype(np.float64), out_rings=rings)
     assert frms(take_rings(geom, out, rings), ref) <= 1e-5
     # same M' in the scheme oracle on a few rings
-    mp = np.array([plan.ring_info(i)["mprime"] for i in range(geom.nrings)])
-    assert np.array_equal(mp, hybrid.mprime_rule(geom, tmax, plan.ell_nyquist))
+    mp = plan_mprime(plan, geom, tmax)
     few = np.array([0, 5, 126, nside - 1, nside + 3, 2 * nside - 1])
     ref2 = hybrid.hybrid_convolve(geom, tab, tmax, x.astype(np.float64), mprime=mp, out_rings=few)
     assert frms(take_rings(geom, out, few), ref2) <= 1e-6
@@ -366,7 +364,7 @@ def test_degenerate_kernels():
     xh = inputs.white_noise(geom.npix, 8, dtype=np.float64)
     tab = inputs.gaussian_table(0.01, 0.02, 4096)
     out, plan = gpu_convolve(("healpix", 4), tab, 0.02, xh, arkcos.F64, ell_nyquist=40.0)
-    mp = hybrid.mprime_rule(geom, 0.02, 40.0)
+    mp = plan_mprime(plan, geom, 0.02, 40.0)
     assert maxrel(out, hybrid.hybrid_convolve(geom, tab, 0.02, xh, mprime=mp)) <= 1e-12
     eq = slice(int(geom.offset[3]), int(geom.offset[12]))
     np.testing.assert_allclose(out[eq], xh[eq] * geom.omega[0], rtol=1e-12)
@@ -385,8 +383,7 @@ def test_cfg5_full_size(which):
     x = inputs.white_noise_maps(geom.npix, 5, nmaps)
     out, plan = gpu_convolve(c["pix"], tab, tmax, x)
     assert np.isfinite(out).all()
-    mp = np.array([plan.ring_info(i)["mprime"] for i in range(geom.nrings)])
-    assert np.array_equal(mp, hybrid.mprime_rule(geom, tmax, plan.ell_nyquist))
+    mp = plan_mprime(plan, geom, tmax)
     few = np.array([3, 700, nside - 1, nside + 2, 2 * nside - 1, 3 * nside + 1, geom.nrings - 40])
     ref2 = hybrid.hybrid_convolve(geom, tab, tmax, x.astype(np.float64), mprime=mp, out_rings=few)
     assert frms(take_rings(geom, out, few), ref2) <= 1e-6
