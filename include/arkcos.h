@@ -86,7 +86,10 @@ typedef struct {
  *                       and the equatorial rings next to them) is recomputed by the direct-space sum of Eq. 6
  *                        after the hybrid pass, so that hard-edged kernels, for which the Fourier
  *                       scheme only suppresses ringing in the caps, are exact everywhere.  Slow path:
- *                       fp64 distances per pixel pair, weights shared by the maps of a call. */
+ *                       fp64 distances per pixel pair, weights shared by the maps of a call.
+ *  no_tensor_cores   0: float plans run the kernel-row phi-transform of the class-E and cap-ring runs as
+ *                       3xTF32 tcgen05 matrix products (FP32-level accuracy); 1: every band kernel
+ *                       uses FP32 FMAs only (the round-1 kernels; also what small grids and cached-spectra plans use). */
 typedef struct {
     int variant;
     double ell_nyquist;
@@ -95,7 +98,8 @@ typedef struct {
     int cache_kernel_rows;
     int exact_caps;
     int cache_kernel_spectra;
-    int reserved[6];               /* must be zero */
+    int no_tensor_cores;
+    int reserved[5];               /* must be zero */
 } arkcos_options;
 
 /* Builds the ring-geometry table (theta, N, phi0, offset per ring), the band and ring-pair tables, FFT twiddles,

@@ -162,6 +162,9 @@ struct HostTables {
     int pole_mh = 0;
     std::vector<EqChunk> eq_chunks;              // runs of consecutive class-E rings for band_mac_eq_kernel   // per band-kernel class (see band_class)
     int eq_alt = 0;
+    bool use_tc = false;                         // tensor-core band kernels (arkcos_band_tc.cuh) serve the class-E and cap runs
+    std::vector<CapChunk> tc_eq_chunks;          // the class-E runs again, as (first ring, rings, M) for band_mac_tc_kernel
+    std::vector<CapChunkItem> tc_eq_items;       // (run, block of 128 modes)
     std::vector<int> fft_order;          // rings of the shared-memory FFT kernels, sorted by decreasing transform size
     std::vector<FftJob> fft3_jobs[4];    // jobs of the register-resident FFT kernels, Q = 512 << k
     int64_t filt_total = 0, chirp_total = 0, ph_total = 0, nsamples = 0;
@@ -255,9 +258,15 @@ void build_fft_lens(const HostGeometry& g, HostTables& t, Stats& st, bool use_ff
 
 // Ring-pair table for the northern output rings (the southern ones reuse the rows of their mirror images).
 void build_pairs(HostGeometry& g, double theta_max, double ell_nyq, int fixed_mprime, int band_threads, bool allow_fast, bool allow_pole, bool cached,
-                 int sm_count, HostTables& t, Stats& st)
+                 bool allow_tc, int sm_count, HostTables& t, Stats& st)
 {
     const int R = g.R, nnorth = (R + 1) / 2;
+    // tensor-core band kernels: float plans with computed spectra; the window of a tile of kTcTI consecutive output rings
+    // must fit the kernel's kTcJW slots for every tile the plan could form
+    bool use_tc = allow_tc && allow_fast && !cached;
+    for (int i = 0; i < nnorth && use_tc; ++i)
+        use_tc = g.band_hi[std::min(i + kTcTI - 1, nnorth - 1)] - g.band_lo[i] + 1 <= kTcJW;
+    t.use_tc = use_tc;
     std::vector<int> eq_rings;
     bool any_odd = false;
     const double shm = sin(0.5 * theta_max), xmax = 4.0 * shm * shm;
@@ -332,10 +341,13 @@ void build_pairs(HostGeometry& g, double theta_max, double ell_nyq, int fixed_mp
                 all_e = t.pairs[p].M == g.n[i] && g.n[t.pairs[p].j] == g.n[i];
                 alt_ok = alt_ok && t.pairs[p].par == (eq_alt ? ((i ^ t.pairs[p].j) & 1) : 0);
             }
-            if (all_e && alt_ok && hi > lo && (maxcnt <= 12 || cached) && g.n[i] >= 8 && g.spec_total < (int64_t)INT32_MAX) {
+            // rows of the tensor-core kernel hold kTcK sample positions: 12 samples with half-step positions, 24 without
+            const bool tc_eq = use_tc && (g.n[i] / 2) % 128 == 0;
+            if (all_e && alt_ok && hi > lo && (maxcnt <= (tc_eq && !eq_alt ? kTcK : 12) || cached) && g.n[i] >= 8 && g.spec_total < (int64_t)INT32_MAX) {
                 eq_rings.push_back(i);
                 st.band_flops[2] += ring_flops;
-                t.items[1].push_back(BandItem{i, g.n[i] / 2});      // the Nyquist bin m = M/2 goes to the uniform kernel
+                // the Nyquist bin m = M/2 goes to a per-mode kernel that holds the whole row (cached plans admit long rows)
+                t.items[maxcnt <= 12 ? 1 : (maxcnt <= 32 ? 4 : 0)].push_back(BandItem{i, g.n[i] / 2});
                 continue;
             }
             if (same && hi > lo) {
@@ -343,7 +355,10 @@ void build_pairs(HostGeometry& g, double theta_max, double ell_nyq, int fixed_mp
                 else if (maxcnt <= 20 && !odd) cls = 3;
                 else if (maxcnt <= 32) cls = 4;
                 // runs of band_mac_capchunk_kernel: one grid length, integer grid, rings long enough for 256-mode blocks
-                if ((cls == 2 || cls == 3 || (cached && !odd)) && !getenv("ARKCOS_NO_CAP_KERNEL")) {
+                if (use_tc) {
+                    // tensor-core run kernel: integer grid, rows of at most kTcK samples, any number of periods
+                    if (!odd && maxcnt <= kTcK && g.n[i] >= 256 && g.n[i] < nmax && t.pairs[lo].M / 2 < (1 << 15)) cls = 5;
+                } else if ((cls == 2 || cls == 3 || (cached && !odd))) {
                     bool single_period = t.pairs[lo].M / 2 < g.n[i] && g.n[i] <= t.pairs[lo].M;
                     for (int p = lo; p < hi; ++p) single_period = single_period && t.pairs[lo].M / 2 < g.n[t.pairs[p].j];
                     // multi-period rings join the run kernel when they are the rule (hard-edged kernels: M' up to 3 N_i) or when
@@ -373,7 +388,7 @@ void build_pairs(HostGeometry& g, double theta_max, double ell_nyq, int fixed_mp
             for (int p = t.north[i].pair_lo; p < t.north[i].pair_hi; ++p) single = single && M / 2 < g.n[t.pairs[p].j];
             const int multi = single ? 0 : 1;
             if (!t.cap_chunks.empty() && t.cap_chunks.back().i0 + t.cap_chunks.back().n == i && t.cap_chunks.back().M == M &&
-                t.cap_chunks.back().multi == multi && t.cap_chunks.back().n < kCapChunkRings)
+                t.cap_chunks.back().multi == multi && t.cap_chunks.back().n < (use_tc ? kTcChunkRings : kCapChunkRings))
                 ++t.cap_chunks.back().n;
             else
                 t.cap_chunks.push_back(CapChunk{i, 1, M, multi});
@@ -396,9 +411,17 @@ void build_pairs(HostGeometry& g, double theta_max, double ell_nyq, int fixed_mp
                 t.eq_chunks.push_back(EqChunk{i, 1});
         }
     }
+    if (use_tc)
+        for (const EqChunk& e : t.eq_chunks) {
+            const int M = g.n[e.i0];
+            if ((M / 2) % 128 != 0) continue;              // (such rings were not admitted with long rows, see above)
+            t.tc_eq_chunks.push_back(CapChunk{e.i0, e.n, M, 0});
+            for (int bx = 0; bx * 128 < M / 2; ++bx) t.tc_eq_items.push_back(CapChunkItem{(int)t.tc_eq_chunks.size() - 1, bx});
+        }
     for (size_t c = 0; c < t.cap_chunks.size(); ++c) {
         const CapChunk& ch = t.cap_chunks[c];
-        for (int bx = 0; bx * (kBandThreads * 2) <= ch.M / 2; ++bx)
+        const int modes_per_block = use_tc ? 128 : kBandThreads * 2;
+        for (int bx = 0; bx * modes_per_block <= ch.M / 2; ++bx)
             (ch.multi ? t.cap_chunk_items_multi : t.cap_chunk_items).push_back(CapChunkItem{(int)c, bx});
         // output coefficients of the chunk's rings (north and mirror image) are accumulated: they start from zero
         const int iA = ch.i0, iB = ch.i0 + ch.n - 1;
@@ -408,7 +431,9 @@ void build_pairs(HostGeometry& g, double theta_max, double ell_nyq, int fixed_mp
             else t.cap_zero.push_back({a, n});
         };
         add_range(iA, iB);
-        if (R - 1 - iB > iB) add_range(R - 1 - iB, R - 1 - iA);
+        // mirror images of the run's rings, without the rings of the run itself (a run may end on the self-mirror middle ring)
+        const int lo = std::max(R - 1 - iB, iB + 1);
+        if (lo <= R - 1 - iA) add_range(lo, R - 1 - iA);
     }
     // longest blocks first (the chunks run from the pole towards the equator, M' grows)
     std::reverse(t.cap_chunk_items.begin(), t.cap_chunk_items.end());
@@ -579,6 +604,16 @@ void launch_uniform(const arkcos_plan* pl, int nmaps, cudaStream_t st, bool seri
             band_mac_eq_cached_kernel<4, 1><<<dim3(gx, (unsigned)pl->neqchunks, 1), kBandThreads, 0, st>>>(
                 pl->d_eqchunks, pl->d_north, pl->d_pairs, pl->d_goff, pl->d_G, pl->d_rings, pl->g.R,
                 (const cx<float>*)pl->d_specIn, (cx<float>*)pl->d_specOut, pl->g.spec_total, nmaps);
+    } else if (pl->neqchunks > 0 && pl->use_tc && pl->ntc_eq_items > 0) {
+        const dim3 grid((unsigned)pl->ntc_eq_items, (unsigned)nmaps);
+        if (pl->eq_alt)
+            band_mac_tc_kernel<0><<<grid, kTcThreads, kTcSmemBytes, st>>>(
+                pl->d_tc_eq_items, pl->d_tc_eq_chunks, pl->d_north, pl->d_pairs, (const float*)pl->d_W, pl->d_rings, pl->g.R,
+                (const cx<float>*)pl->d_specIn, (cx<float>*)pl->d_specOut, pl->g.spec_total);
+        else
+            band_mac_tc_kernel<1><<<grid, kTcThreads, kTcSmemBytes, st>>>(
+                pl->d_tc_eq_items, pl->d_tc_eq_chunks, pl->d_north, pl->d_pairs, (const float*)pl->d_W, pl->d_rings, pl->g.R,
+                (const cx<float>*)pl->d_specIn, (cx<float>*)pl->d_specOut, pl->g.spec_total);
     } else if (pl->neqchunks > 0) {
         constexpr int TI = 4, MT = 2;
         const dim3 grid((unsigned)((pl->eq_mh + kBandThreads * MT - 1) / (kBandThreads * MT)), (unsigned)pl->neqchunks, (unsigned)nmaps);
@@ -614,6 +649,10 @@ void launch_uniform(const arkcos_plan* pl, int nmaps, cudaStream_t st, bool seri
                 band_mac_capchunk_cached_kernel<4, 1, MULTI><<<dim3(n, 1), kBandThreads, 0, s1>>>(
                     items, pl->d_cap_chunks, pl->d_north, pl->d_pairs, pl->d_goff, pl->d_G, pl->d_rings, pl->g.R,
                     (const cx<float>*)pl->d_specIn, (cx<float>*)pl->d_specOut, pl->g.spec_total, nmaps);
+            else if (pl->use_tc)
+                band_mac_tc_kernel<MULTI ? 3 : 2><<<dim3(n, (unsigned)nmaps), kTcThreads, kTcSmemBytes, s1>>>(
+                    items, pl->d_cap_chunks, pl->d_north, pl->d_pairs, (const float*)pl->d_W, pl->d_rings, pl->g.R,
+                    (const cx<float>*)pl->d_specIn, (cx<float>*)pl->d_specOut, pl->g.spec_total);
             else
                 band_mac_capchunk_kernel<4, 20, MULTI><<<dim3(n, (unsigned)nmaps), kBandThreads, 0, s1>>>(
                     items, pl->d_cap_chunks, pl->d_north, pl->d_pairs, (const float*)pl->d_W, pl->d_rings, pl->g.R,
@@ -813,6 +852,7 @@ static int plan_create_impl(arkcos_plan** out, const arkcos_pixelization* pix, c
     if (opt.exact_caps != 0 && opt.exact_caps != 1) return fail(ARKCOS_INVALID_ARG, "options.exact_caps must be 0 or 1");
     if (opt.cache_kernel_spectra != 0 && opt.cache_kernel_spectra != 1)
         return fail(ARKCOS_INVALID_ARG, "options.cache_kernel_spectra must be 0 or 1");
+    if (opt.no_tensor_cores != 0 && opt.no_tensor_cores != 1) return fail(ARKCOS_INVALID_ARG, "options.no_tensor_cores must be 0 or 1");
     if (opt.cache_kernel_spectra && (dtype != ARKCOS_F32 || opt.variant != 0))
         return fail(ARKCOS_UNSUPPORTED, "cache_kernel_spectra needs a float plan of variant 0");
     if (opt.cache_kernel_spectra) opt.cache_kernel_rows = 1;     // the spectra are made from the rows, once
@@ -840,6 +880,8 @@ static int plan_create_impl(arkcos_plan** out, const arkcos_pixelization* pix, c
     if (!tables_only) CUDA_TRY(cudaGetDevice(&pl->device));
 
     build_geometry(*pix, pl->g);
+    // the band kernels index the ring spectra of one map with 32-bit offsets
+    if (pl->g.spec_total >= (int64_t)INT32_MAX) return fail(ARKCOS_UNSUPPORTED, "pixelization too large: ring spectra of one map exceed 2^31 coefficients");
     build_bands(pl->g, pl->theta_max);
     int fixed_mprime = 0;
     if (pix->kind == ARKCOS_HEALPIX_RING) {
@@ -851,13 +893,15 @@ static int plan_create_impl(arkcos_plan** out, const arkcos_pixelization* pix, c
     if (!tables_only) CUDA_TRY(cudaDeviceGetAttribute(&sm_count, cudaDevAttrMultiProcessorCount, pl->device));
     pl->sm_count = sm_count;
     HostTables t;
-    build_fft_lens(pl->g, t, pl->stats, dtype == ARKCOS_F32 && !getenv("ARKCOS_FORCE_OLD_FFT"));
-    build_pairs(pl->g, pl->theta_max, pl->ell_nyquist, fixed_mprime, kBandThreads, dtype == ARKCOS_F32 && opt.variant == 0 && !getenv("ARKCOS_FORCE_GENERAL"), opt.variant == 0, opt.cache_kernel_spectra != 0, sm_count, t, pl->stats);
+    build_fft_lens(pl->g, t, pl->stats, dtype == ARKCOS_F32);
+    build_pairs(pl->g, pl->theta_max, pl->ell_nyquist, fixed_mprime, kBandThreads, dtype == ARKCOS_F32 && opt.variant == 0, opt.variant == 0, opt.cache_kernel_spectra != 0, opt.no_tensor_cores == 0, sm_count, t, pl->stats);
     if (t.pairs.size() > (size_t)INT32_MAX) return fail(ARKCOS_UNSUPPORTED, "too many ring pairs");
     pl->nnorth = (int)t.north.size();
     pl->npairs = (int)t.pairs.size();
     for (int c = 0; c < kBandClasses; ++c) pl->nitems[c] = (int)t.items[c].size();
     pl->neqchunks = (int)t.eq_chunks.size();
+    pl->use_tc = t.use_tc;
+    pl->ntc_eq_items = (int)t.tc_eq_items.size();
     pl->npole = (int)t.pole_rings.size();
     pl->pole_mh = t.pole_mh;
     pl->eq_alt = t.eq_alt;
@@ -899,6 +943,14 @@ static int plan_create_impl(arkcos_plan** out, const arkcos_pixelization* pix, c
         }
         pl->ndirect = (int)items.size();
         if (int rc = upload(&pl->d_direct_items, items, wsb)) return rc;
+    }
+    if (pl->use_tc) {
+        if (int rc = upload(&pl->d_tc_eq_chunks, t.tc_eq_chunks, wsb)) return rc;
+        if (int rc = upload(&pl->d_tc_eq_items, t.tc_eq_items, wsb)) return rc;
+        CUDA_TRY(cudaFuncSetAttribute(band_mac_tc_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kTcSmemBytes));
+        CUDA_TRY(cudaFuncSetAttribute(band_mac_tc_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kTcSmemBytes));
+        CUDA_TRY(cudaFuncSetAttribute(band_mac_tc_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kTcSmemBytes));
+        CUDA_TRY(cudaFuncSetAttribute(band_mac_tc_kernel<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kTcSmemBytes));
     }
     if (int rc = upload(&pl->d_cap_chunks, t.cap_chunks, wsb)) return rc;
     if (int rc = upload(&pl->d_cap_chunk_items, t.cap_chunk_items, wsb)) return rc;
@@ -968,6 +1020,9 @@ int arkcos_convolve(const arkcos_plan* pl, const void* d_in, void* d_out, int nm
     if (a < b + bytes && b < a + bytes) return fail(ARKCOS_INVALID_ARG, "d_in and d_out overlap");
     if (((uintptr_t)d_in | (uintptr_t)d_out) & 15) return fail(ARKCOS_INVALID_ARG, "d_in / d_out must be 16-byte aligned");
     cudaStream_t st = (cudaStream_t)cuda_stream;
+    int dev = -1;
+    CUDA_TRY(cudaGetDevice(&dev));
+    if (dev != pl->device) return fail(ARKCOS_INVALID_ARG, "the current device is not the device the plan was created on");
     return pl->dtype == ARKCOS_F32 ? enqueue_convolve<float>(pl, d_in, d_out, nmaps, st)
                                    : enqueue_convolve<double>(pl, d_in, d_out, nmaps, st);
 }
@@ -1052,7 +1107,7 @@ int arkcos_plan_destroy(arkcos_plan* pl)
     void* ptrs[] = {pl->d_rings, pl->d_lens, pl->d_pairs, pl->d_north, pl->d_items[0], pl->d_items[1], pl->d_items[2], pl->d_items[3],
                     pl->d_items[4], pl->d_items[5], pl->d_eqchunks, pl->d_pole, pl->d_chirp, pl->d_phase, pl->d_fft_order, pl->d_table, pl->d_tw, pl->d_filt,
                     pl->d_W, pl->d_specIn, pl->d_specOut, pl->d_stage_in, pl->d_stage_out,
-                    pl->d_cap_chunks, pl->d_cap_chunk_items, pl->d_goff, pl->d_G, pl->d_direct_items, pl->d_tw3, pl->d_tw16, pl->d_fft3_jobs[0], pl->d_fft3_jobs[1], pl->d_fft3_jobs[2], pl->d_fft3_jobs[3]};
+                    pl->d_cap_chunks, pl->d_cap_chunk_items, pl->d_tc_eq_chunks, pl->d_tc_eq_items, pl->d_goff, pl->d_G, pl->d_direct_items, pl->d_tw3, pl->d_tw16, pl->d_fft3_jobs[0], pl->d_fft3_jobs[1], pl->d_fft3_jobs[2], pl->d_fft3_jobs[3]};
     for (void* p : ptrs) if (p) cudaFree(p);
     for (auto& e : pl->ev) if (e) cudaEventDestroy(e);
     for (auto& e : pl->ev_band) if (e) cudaEventDestroy(e);

@@ -12,6 +12,7 @@
 #include "arkcos_fft3.cuh"
 #include "arkcos_direct.cuh"
 #include "arkcos_band_cached.cuh"
+#include "arkcos_band_tc.cuh"
 
 namespace arkcos {
 
@@ -61,6 +62,12 @@ struct arkcos_plan {
     int ncapitems = 0;
     int ncapsingle = 0;               // the first ncapsingle items are single-period runs
     std::vector<std::pair<int64_t, int64_t>> cap_zero;    // output-spectrum ranges cleared before band_mac_capchunk_kernel
+    // tensor-core band kernels (arkcos_band_tc.cuh): class-E runs as (run, block of 128 modes) items; the cap runs use
+    // d_cap_chunks / d_cap_chunk_items with blocks of 128 modes
+    bool use_tc = false;
+    arkcos::CapChunk* d_tc_eq_chunks = nullptr;
+    arkcos::CapChunkItem* d_tc_eq_items = nullptr;
+    int ntc_eq_items = 0;
     int* d_pole = nullptr;
     int npole = 0, pole_mh = 0;
     arkcos::BandItem* d_items[arkcos::kBandClasses] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};

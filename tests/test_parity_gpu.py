@@ -401,3 +401,43 @@ def test_cfg5_full_size(which):
     assert frms(take_rings(geom, out_x, cap), refc) <= 1e-6
     assert frms(take_rings(geom, out_x, eq), ref1) <= 1e-6
     np.testing.assert_array_equal(take_rings(geom, out_x, eq), take_rings(geom, out, eq))
+
+
+# ------------------------------------------------------------------ regressions found by review ---------------------
+
+def test_ecp_odd_ntheta_run_ending_on_middle_ring():
+    """ECP with an odd number of rings and rows of 13..20 samples at the equator: the cap-run kernel serves a run that
+    ends on the self-mirror middle ring; the mirror images of the other rings of that run must be cleared on every
+    call (round-1 review: they were not, the result drifted from call to call)."""
+    pix = ("ecp", 511, 1024)
+    geom = geom_of(pix)
+    tmax = 0.1
+    tab = inputs.gaussian_table(0.06, tmax)
+    x = inputs.white_noise(geom.npix, 21)
+    out, plan = gpu_convolve(pix, tab, tmax, x)
+    rings = np.array([0, 3, 100, 250, 254, 255, 256, 257, 260, 262, 400, 510])
+    ref1 = direct.direct_sum(geom, tab, tmax, x.astype(np.float64), out_rings=rings)
+    assert frms(take_rings(geom, out, rings), ref1) <= 1e-6
+    out2, _ = gpu_convolve(pix, tab, tmax, x, plan=plan)
+    assert frms(take_rings(geom, out2, rings), ref1) <= 1e-6
+    np.testing.assert_array_equal(out, out2)
+
+
+def test_cached_spectra_long_equatorial_rows():
+    """cache_kernel_spectra with equatorial rows longer than 12 samples (disc of 14 pixels at nside 256): every bin,
+    the Nyquist bin m = M/2 included, must come from the whole row (round-1 review: that bin used a row cut at 12)."""
+    nside, nmaps = 256, 2
+    geom = geometry.healpix_ring(nside)
+    px = np.sqrt(4 * np.pi / geom.npix)
+    tmax = 14 * px
+    tab = inputs.tophat_table(tmax)
+    x = inputs.white_noise_maps(geom.npix, 13, nmaps)
+    # an input that lives at the Nyquist frequency of the equatorial rings makes that bin visible
+    x[:, geom.offset[400]:geom.offset[401]] += 50.0 * (-1.0) ** np.arange(4 * nside, dtype=np.float32)
+    x[:, geom.offset[511]:geom.offset[512]] += 50.0 * (-1.0) ** np.arange(4 * nside, dtype=np.float32)
+    out, plan = gpu_convolve(("healpix", nside), tab, tmax, x, cache_kernel_spectra=1)
+    eq = np.array([i for i in range(geom.nrings) if np.all(geom.n[geometry.band(geom, i, tmax)] == 4 * nside)])
+    rings = eq[[0, 1, len(eq) // 3, len(eq) // 2, len(eq) - 1]]
+    rings = np.unique(np.concatenate([rings, [398, 400, 403, 509, 511, 514]]))
+    ref1 = direct.direct_sum(geom, tab, tmax, x.astype(np.float64), out_rings=rings)
+    assert frms(take_rings(geom, out, rings), ref1) <= 1e-6
