@@ -164,6 +164,12 @@ int arkcos_plan_get_timing(const arkcos_plan* plan, float* ms4);
  * names / model_flops / last_ms: arrays of 8, any may be NULL. */
 int arkcos_plan_band_kernels(const arkcos_plan* plan, int* n, const char** names, double* model_flops, float* last_ms);
 
+/* Whether the plan's band step runs on the tensor cores (options.no_tensor_cores = 0, a float plan with computed spectra,
+ * band windows that fit): *blocks = blocks of band_mac_tc_kernel launched per arkcos_convolve and map (class-E runs, cap
+ * runs single period, cap runs several periods), *resident_per_sm = how many of them one SM holds.  Pointers may be NULL.
+ * Returns 1 if the tensor-core kernels are used, 0 if not, negative on error. */
+int arkcos_plan_tensor_cores(const arkcos_plan* plan, int blocks[3], int* resident_per_sm);
+
 /* Number of kernels one arkcos_convolve enqueues for this plan (kernel-row generator, ring FFT launches per transform
  * size class and direction, band kernels of the ring classes present); -1 for a NULL plan. */
 int arkcos_plan_launches_per_convolve(const arkcos_plan* plan);

@@ -64,6 +64,7 @@ SYMBOLS = {
     "arkcos_plan_set_timing": (c_int, [c_void_p, c_int]),
     "arkcos_plan_get_timing": (c_int, [c_void_p, POINTER(c_float)]),
     "arkcos_plan_band_kernels": (c_int, [c_void_p, POINTER(c_int), POINTER(c_char_p), POINTER(c_double), POINTER(c_float)]),
+    "arkcos_plan_tensor_cores": (c_int, [c_void_p, POINTER(c_int), POINTER(c_int)]),
     "arkcos_plan_launches_per_convolve": (c_int, [c_void_p]),
     "arkcos_probe_fp32_peak": (c_int, [POINTER(c_double), c_int]),
     "arkcos_strerror": (c_char_p, [c_int]),
@@ -175,6 +176,15 @@ class Plan:
                "arkcos_plan_stats")
         return dict(ring_pairs=rp.value, row_samples=rs.value, mac_flops=mf.value, fft_flops=ff.value,
                     workspace_bytes=ws.value)
+
+    def tensor_cores(self) -> dict:
+        """Whether the band step runs on the tensor cores, with the blocks per launch class and the blocks one SM holds."""
+        blocks = (c_int * 3)()
+        res = c_int()
+        used = _lib().arkcos_plan_tensor_cores(self._h, blocks, byref(res))
+        if used < 0:
+            raise ArkcosError(used, "arkcos_plan_tensor_cores")
+        return dict(used=bool(used), blocks=list(blocks), resident_per_sm=res.value)
 
     @property
     def launches_per_convolve(self) -> int:

@@ -23,13 +23,17 @@
 
 namespace arkcos {
 
-constexpr int kTcThreads = 128;            // one thread per TMEM lane
+constexpr int kTcMT = 2;                   // blocks of 128 modes (TMEM lanes) per thread block, one consumer warpgroup each
+constexpr int kTcConsumers = 128 * kTcMT;  // multiply-accumulate threads: thread = mode
+constexpr int kTcProducers = 128;          // B-operand threads: thread = accumulator column; its thread 0 issues the MMAs
+constexpr int kTcThreads = kTcConsumers + kTcProducers;
 constexpr int kTcTI = 4;                   // output rings per tile
 constexpr int kTcJW = 32;                  // input rings a tile's window can hold
-constexpr int kTcN = kTcTI * kTcJW;        // accumulator columns
+constexpr int kTcN = kTcTI * kTcJW;        // accumulator columns per block of modes
 constexpr int kTcK = 24;                   // sample positions u per row
 constexpr int kTcChunkRings = 24;          // longest run of cap rings handed to one block
-constexpr size_t kTcSmemBytes = (size_t)(2 * (kTcK / 4) * 128 + 2 * (kTcK / 4) * kTcN + kTcJW * 128) * 16;
+// cosine operand per block of modes, two stages of the row operand, coefficient window per block of modes
+constexpr size_t kTcSmemBytes = (size_t)(kTcMT * 2 * (kTcK / 4) * 128 + 2 * 2 * (kTcK / 4) * kTcN + kTcMT * kTcJW * 128) * 16;
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
@@ -56,6 +60,11 @@ __device__ __forceinline__ void tc_mma_tf32(uint32_t tmem_d, uint64_t da, uint64
         ::"r"(tmem_d), "l"(da), "l"(db), "r"(idesc), "r"(accumulate) : "memory");
 }
 
+__device__ __forceinline__ void tc_commit(uint64_t* bar)
+{
+    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+
 __device__ __forceinline__ void tc_ld16(uint32_t (&g)[16], uint32_t taddr)
 {
     asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
@@ -64,35 +73,69 @@ __device__ __forceinline__ void tc_ld16(uint32_t (&g)[16], uint32_t taddr)
                  : "r"(taddr));
 }
 
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar)
+{
+    asm volatile("{\n\t.reg .b64 st;\n\tmbarrier.arrive.shared::cta.b64 st, [%0];\n\t}" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity)
+{
+    uint32_t done = 0;
+    while (!done)
+        asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                     : "=r"(done) : "r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+
+// Plan-time tables of the tensor-core band kernel (no pointer chasing through the ring-pair table inside the kernel):
+// a run of rings, its tiles of up to TI output rings, per tile one word per accumulator column, and two words per ring.
+struct TcChunk { int i0, n, M, multi, tile0; };       // run of output rings i0 .. i0 + n - 1 with one grid length M; first tile
+struct TcItem { int chunk, bx; };                      // one thread block: run, block of 128 * kTcMT modes
+struct __align__(16) TcTile {                          // window of input rings, first output ring, output rings of the tile,
+    int jlo, jhi, i0, nti;                             // and per output ring its spectrum offsets (ring, mirror image) and N_i | shifted << 31
+    int offN[4], offS[4], n_sh[4];
+};
+struct TcRing { int offN, offS, n_sh; uint32_t magic; };   // spectrum offsets of ring j and of its mirror image, N_j | shifted << 31, ceil(2^32 / N_j)
+// column word: bits 0-24 first sample of the row in W (units of four floats), bits 25-30 samples, bit 31 half-step parity;
+// 0xffffffff: no such ring pair (zero row)
+constexpr uint32_t kTcNoPair = 0xffffffffu;
+
+// Warp-specialised: the producer warpgroup (threads 256 .. 383, thread = accumulator column) converts the rows of tile
+// k + 1 into the B operand (two stages) and its first thread issues the MMAs of both blocks of modes into TMEM stage
+// (k + 1) & 1, while the two consumer warpgroups (thread = mode) multiply-accumulate tile k out of TMEM stage k & 1.
+// mbarriers: full[s] (MMAs of the stage done), empty[s] (all eight consumer warps have read the stage), rows[s] (the MMAs
+// that read B-operand stage s are done).
 template <int KIND>
-__global__ void __launch_bounds__(kTcThreads, 2)
-band_mac_tc_kernel(const CapChunkItem* __restrict__ items, const CapChunk* __restrict__ chunks,
-                   const NorthRec* __restrict__ north, const PairRec* __restrict__ pairs, const float* __restrict__ W,
-                   const RingRec* __restrict__ rings, int R, const cx<float>* __restrict__ specIn,
-                   cx<float>* __restrict__ specOut, int64_t spec_stride)
+__global__ void __launch_bounds__(kTcThreads, 1)
+band_mac_tc_kernel(const TcItem* __restrict__ items, const TcChunk* __restrict__ chunks, const TcTile* __restrict__ tiles,
+                   const uint32_t* __restrict__ cols, const TcRing* __restrict__ ringtab, const float* __restrict__ W, int R,
+                   const cx<float>* __restrict__ specIn, cx<float>* __restrict__ specOut, int64_t spec_stride)
 {
     constexpr bool CAP = KIND >= 2, MULTI = KIND == 3, ALT = KIND == 0;
-    constexpr int TI = kTcTI, JW = kTcJW, N = kTcN, K = kTcK, KC = K / 4;
+    constexpr int TI = kTcTI, JW = kTcJW, N = kTcN, K = kTcK, KC = K / 4, MT = kTcMT;
     static_assert(TI == 4, "column = 4 * input ring + output ring");
     extern __shared__ __align__(128) unsigned char tc_smem[];
-    float4* sA = reinterpret_cast<float4*>(tc_smem);            // [hi / lo][KC][128 modes]: cos(pi m u s / M), u = 4 kc .. 4 kc + 3
-    float4* sB = sA + 2 * KC * 128;                              // [hi / lo][KC][N columns]: row samples of the tile's ring pairs
-    float4* sV = sB + 2 * KC * N;                                // [JW slots][128 threads]: (Bp_j[m], Bp_jS[m]) of window ring j
-    __shared__ __align__(8) uint64_t bar;
+    float4* sA = reinterpret_cast<float4*>(tc_smem);            // [block of modes][hi / lo][KC][128 modes]: cos(pi m u s / M), u = 4 kc .. 4 kc + 3
+    float4* sB = sA + MT * 2 * KC * 128;                         // [stage][hi / lo][KC][N columns]: row samples of the tile's ring pairs
+    float4* sV = sB + 2 * 2 * KC * N;                            // [block of modes][JW slots][128 threads]: (Bp_j[m], Bp_jS[m]) of window ring j
+    __shared__ __align__(8) uint64_t bar_full[2], bar_empty[2], bar_rows[2];
     __shared__ uint32_t s_tmem;
-    __shared__ int4 sJ[JW];                                      // window ring: spectrum offsets (N, S), N_j | shifted << 31, magic
-    __shared__ int sPlo[TI], sJ0[TI], sNp[TI], sUmax;
+    __shared__ int sUmax[2];
 
     const int t = (int)threadIdx.x, warp = t >> 5;
-    const CapChunkItem it = items[blockIdx.x];
-    const CapChunk ch = chunks[it.chunk];
+    const TcItem it = items[blockIdx.x];
+    const TcChunk ch = chunks[it.chunk];
     const int M = ch.M, Mh = M >> 1;
-    const int m_raw = it.bx * 128 + t, m = min(m_raw, Mh);
-    const cx<float>* __restrict__ in = specIn + (int64_t)blockIdx.y * spec_stride;
-    cx<float>* __restrict__ out = specOut + (int64_t)blockIdx.y * spec_stride;
+    const int ntiles = (ch.n + TI - 1) / TI;
+    const bool producer = t >= kTcConsumers;
+    const int wg = t >> 7, l128 = t & 127;                       // consumer: block of modes, lane within it
+    const int m_raw = (it.bx * MT + wg) * 128 + l128, m = min(m_raw, Mh);
 
-    // ---- A operand: the cosines of this block's 128 modes, split into TF32 hi + lo ------------------------------------
-    {
+    if (!producer) {
+        // ---- A operand: the cosines of this warpgroup's 128 modes, split into TF32 hi + lo ----------------------------
+        float4* sAw = sA + wg * 2 * KC * 128;
         const uint32_t twoM = 2u * (uint32_t)M, step = ALT ? 1u : 2u;
         const cx<float> rot = cispi_ratio<float>(((uint32_t)m * step) % twoM, (uint32_t)M);
         cx<float> c = mk<float>(1.f, 0.f);
@@ -104,186 +147,252 @@ band_mac_tc_kernel(const CapChunkItem* __restrict__ items, const CapChunk* __res
             hi[u & 3] = tf32_rn(c.x);
             lo[u & 3] = tf32_rn(c.x - hi[u & 3]);
             if ((u & 3) == 3) {
-                sA[(u >> 2) * 128 + t] = make_float4(hi[0], hi[1], hi[2], hi[3]);
-                sA[(KC + (u >> 2)) * 128 + t] = make_float4(lo[0], lo[1], lo[2], lo[3]);
+                sAw[(u >> 2) * 128 + l128] = make_float4(hi[0], hi[1], hi[2], hi[3]);
+                sAw[(KC + (u >> 2)) * 128 + l128] = make_float4(lo[0], lo[1], lo[2], lo[3]);
             }
         }
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        // the window starts out finite: accumulator columns past the tile's window are exact zeros, but 0 * garbage is not
+        for (int sl = 0; sl < JW; ++sl) sV[(wg * JW + sl) * 128 + l128] = make_float4(0.f, 0.f, 0.f, 0.f);
     }
-    for (int k = t; k < JW * 128; k += kTcThreads) sV[k] = make_float4(0.f, 0.f, 0.f, 0.f);
     if (t == 0) {
-        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(smem_u32(&bar)));
+#pragma unroll
+        for (int s = 0; s < 2; ++s) {
+            mbar_init(&bar_full[s], 1);
+            mbar_init(&bar_empty[s], kTcConsumers / 32);
+            mbar_init(&bar_rows[s], 1);
+            sUmax[s] = 1;
+        }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     if (warp == 0) {
-        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&s_tmem)), "r"(N));
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&s_tmem)), "r"(2 * MT * N));
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::);
     }
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     __syncthreads();
     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
     const uint32_t tmem = s_tmem;
-    // instruction descriptor: D = f32, A = B = tf32, both K-major, N >> 3 at bit 17, M >> 4 at bit 24
-    constexpr uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(N >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
 
-    // periodic extension of a stored half spectrum (reading R8): m = w N_j + r; above N_j/2 the conjugate of N_j - r
-    auto ext_index = [](int mm, int nj_sh, uint32_t magic) {
-        const int Nj = nj_sh & 0x7fffffff, w = MULTI ? (int)__umulhi((uint32_t)mm, magic) : 0, r = mm - w * Nj;
-        return 2 * r > Nj ? Nj - r : r;
-    };
-
-    uint32_t phase = 0;
-    int jhave = -1;                                              // highest ring whose coefficients sit in the window
-    for (int tile = 0; tile < ch.n; tile += TI) {
-        const int nti = min(TI, ch.n - tile), i0 = ch.i0 + tile;
-        const int p_first = north[i0].pair_lo, p_last = north[i0 + nti - 1].pair_hi;
-        const int jlo = pairs[p_first].j, jhi = pairs[p_last - 1].j, jw = jhi - jlo + 1;
-        const int jnew = max(jhave + 1, jlo);
-        __syncthreads();        // the previous tile is done with the accumulator, the B operand and the tile records
-        if (t < TI) {
-            const NorthRec nr = north[i0 + min(t, nti - 1)];
-            sPlo[t] = nr.pair_lo;
-            sJ0[t] = pairs[nr.pair_lo].j;
-            sNp[t] = t < nti ? nr.pair_hi - nr.pair_lo : 0;
-        }
-        if (t == 0) sUmax = 1;
-        for (int j = jnew + t; j <= jhi; j += kTcThreads) {
-            const RingRec rj = rings[j];
-            sJ[j & (JW - 1)] = make_int4((int)rj.spec_off, (int)rings[R - 1 - j].spec_off, rj.n | (rj.shifted ? (int)0x80000000 : 0),
-                                         MULTI ? (int)(uint32_t)((0x100000000ull + (uint64_t)rj.n - 1ull) / (uint64_t)rj.n) : 0);
-        }
-        __syncthreads();
-        // ---- B operand: one column per ring pair of the tile, TF32 hi + lo; missing pairs and the tails are zero ------
-        {
-            int umax = 0;
-            for (int idx = t; idx < N * KC; idx += kTcThreads) {
-                const int kc = idx / N, c = idx - kc * N, jj = c >> 2, ii = c & 3;
-                const int pj = jlo + jj - sJ0[ii];
-                float4 w = make_float4(0.f, 0.f, 0.f, 0.f);
-                if (pj >= 0 && pj < sNp[ii]) {
-                    const PairRec& pr = pairs[sPlo[ii] + pj];
-                    const int cnt = pr.cnt, cnt4 = (cnt + 3) & ~3;
-                    if (ALT) {
-                        const int par = pr.par;
-                        if (kc == 0) umax = max(umax, 2 * cnt - 1 + par);
-                        if (2 * kc < cnt4) {
-                            const float2 ww = *reinterpret_cast<const float2*>(W + pr.woff + 2 * kc);
-                            w = par ? make_float4(0.f, ww.x, 0.f, ww.y) : make_float4(ww.x, 0.f, ww.y, 0.f);
+    if (producer) {
+        // =================================== rows -> B operand -> MMAs =========================================
+        const int c = t - kTcConsumers;
+        // instruction descriptor: D = f32, A = B = tf32, both K-major, N >> 3 at bit 17, M >> 4 at bit 24
+        constexpr uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(N >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
+        float4 wrow[KC];
+        auto load_row = [&](uint32_t cw) {
+            const bool have = cw != kTcNoPair;
+            const int cnt4 = have ? (int)(((cw >> 25) & 63u) + 3u) & ~3 : 0;
+            const float* __restrict__ w = W + (size_t)(cw & 0x1ffffffu) * 4;
+#pragma unroll
+            for (int kc = 0; kc < KC; ++kc) {
+                wrow[kc] = make_float4(0.f, 0.f, 0.f, 0.f);
+                if (ALT) {                                       // u = 4 kc .. 4 kc + 3 holds samples 2 kc, 2 kc + 1 at parity par
+                    if (2 * kc < cnt4) {
+                        const float2 ww = *reinterpret_cast<const float2*>(w + 2 * kc);
+                        wrow[kc] = (cw >> 31) ? make_float4(0.f, ww.x, 0.f, ww.y) : make_float4(ww.x, 0.f, ww.y, 0.f);
+                    }
+                } else if (4 * kc < cnt4) wrow[kc] = *reinterpret_cast<const float4*>(w + 4 * kc);
+            }
+        };
+        const uint32_t* __restrict__ colp = cols + (size_t)ch.tile0 * N + c;
+        uint32_t colw = colp[0];
+        uint32_t colw_next = ntiles > 1 ? colp[N] : kTcNoPair;
+        load_row(colw);
+        for (int k = 0; k < ntiles; ++k) {
+            const int s = k & 1;
+            const uint32_t ph = (uint32_t)(k >> 1) & 1u;
+            mbar_wait(&bar_rows[s], ph ^ 1u);                    // the MMAs of tile k - 2 have read this stage
+            float4* sBs = sB + s * 2 * KC * N;
+            if (colw != kTcNoPair) {
+                const int cnt = (int)((colw >> 25) & 63u);
+                const int used = ALT ? 2 * cnt - 1 + (int)(colw >> 31) : cnt;      // sample positions u the row occupies
+                if (used > 8) atomicMax(&sUmax[s], used);
+            }
+#pragma unroll
+            for (int kc = 0; kc < KC; ++kc) {
+                const float4 w = wrow[kc];
+                const float4 h = make_float4(tf32_rn(w.x), tf32_rn(w.y), tf32_rn(w.z), tf32_rn(w.w));
+                sBs[kc * N + c] = h;
+                sBs[(KC + kc) * N + c] = make_float4(tf32_rn(w.x - h.x), tf32_rn(w.y - h.y), tf32_rn(w.z - h.z), tf32_rn(w.w - h.w));
+            }
+            if (k + 1 < ntiles) {                                // rows of the next tile, column word of the one after
+                colw = colw_next;
+                load_row(colw);
+                colw_next = k + 2 < ntiles ? colp[(size_t)(k + 2) * N] : kTcNoPair;
+            }
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+            asm volatile("bar.sync 1, %0;" ::"n"(kTcProducers) : "memory");
+            if (c == 0) {
+                mbar_wait(&bar_empty[s], ph ^ 1u);               // the consumers have read TMEM stage s (tile k - 2)
+                asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+                const int ksteps = min(K / 8, (sUmax[s] + 7) >> 3);
+                sUmax[s] = 1;
+                const uint32_t a0 = smem_u32(sA), b0 = smem_u32(sBs);
+#pragma unroll
+                for (int mt = 0; mt < MT; ++mt) {
+                    uint32_t acc_flag = 0;
+                    const uint32_t d = tmem + (uint32_t)((s * MT + mt) * N);
+#pragma unroll
+                    for (int sp = 0; sp < 3; ++sp) {             // (hi, lo), (lo, hi), then (hi, hi): small terms first
+                        const int ha = sp == 1 ? 1 : 0, hb = sp == 0 ? 1 : 0;
+                        for (int ks = 0; ks < ksteps; ++ks) {
+                            const uint64_t da = tc_smem_desc(a0 + (uint32_t)(((mt * 2 + ha) * KC + 2 * ks) * 128 * 16), 128 * 16, 128);
+                            const uint64_t db = tc_smem_desc(b0 + (uint32_t)((hb * KC + 2 * ks) * N * 16), N * 16, 128);
+                            tc_mma_tf32(d, da, db, idesc, acc_flag);
+                            acc_flag = 1;
                         }
-                    } else {
-                        if (kc == 0) umax = max(umax, cnt);
-                        if (4 * kc < cnt4) w = *reinterpret_cast<const float4*>(W + pr.woff + 4 * kc);
                     }
                 }
-                const float4 h = make_float4(tf32_rn(w.x), tf32_rn(w.y), tf32_rn(w.z), tf32_rn(w.w));
-                sB[kc * N + c] = h;
-                sB[(KC + kc) * N + c] = make_float4(tf32_rn(w.x - h.x), tf32_rn(w.y - h.y), tf32_rn(w.z - h.z), tf32_rn(w.w - h.w));
+                tc_commit(&bar_full[s]);
+                tc_commit(&bar_rows[s]);
             }
-            if (umax > 1) atomicMax(&sUmax, umax);
         }
-        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-        asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
-        __syncthreads();
-        if (t == 0) {
-            asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-            const int ksteps = min(K / 8, (sUmax + 7) >> 3);
-            const uint32_t a0 = smem_u32(sA), b0 = smem_u32(sB);
-            uint32_t acc_flag = 0;
+    } else {
+        // =================================== multiply-accumulate over input rings ==============================
+        const cx<float>* __restrict__ in = specIn + (int64_t)blockIdx.y * spec_stride;
+        cx<float>* __restrict__ out = specOut + (int64_t)blockIdx.y * spec_stride;
+        const uint32_t sv0 = smem_u32(sV + wg * JW * 128 + l128);      // this thread's slot 0; slot s at + 2048 s bytes
+        // periodic extension of a stored half spectrum (reading R8): m = w N_j + r; above N_j/2 the conjugate of N_j - r
+        auto ext_index = [](int mm, int nj_sh, uint32_t magic) {
+            const int Nj = nj_sh & 0x7fffffff, w = MULTI ? (int)__umulhi((uint32_t)mm, magic) : 0, r = mm - w * Nj;
+            return 2 * r > Nj ? Nj - r : r;
+        };
+        auto fetch_ring = [&](int j, const TcRing& rj) {
+            const int idx = CAP ? ext_index(m, rj.n_sh, rj.magic) : m;
+            const uint32_t dst = sv0 + 2048u * (uint32_t)(j & (JW - 1));
+            asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst), "l"(in + rj.offN + idx) : "memory");
+            asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst + 8u), "l"(in + rj.offS + idx) : "memory");
+        };
+        TcTile tl = tiles[ch.tile0];
+        // first tile: its whole window enters
+        for (int j0 = tl.jlo; j0 <= tl.jhi; j0 += 4) {
+            TcRing rr[4];
 #pragma unroll
-            for (int s = 0; s < 3; ++s) {                        // (hi, lo), (lo, hi), then (hi, hi): small terms first
-                const int ha = s == 1 ? 1 : 0, hb = s == 0 ? 1 : 0;
-                for (int ks = 0; ks < ksteps; ++ks) {
-                    const uint64_t da = tc_smem_desc(a0 + (uint32_t)((ha * KC + 2 * ks) * 128 * 16), 128 * 16, 128);
-                    const uint64_t db = tc_smem_desc(b0 + (uint32_t)((hb * KC + 2 * ks) * N * 16), N * 16, 128);
-                    tc_mma_tf32(tmem, da, db, idesc, acc_flag);
-                    acc_flag = 1;
-                }
-            }
-            asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(&bar)) : "memory");
-        }
-        // ---- window: coefficients of the rings that enter with this tile, fetched while the tensor core works ---------
-        for (int j = jnew; j <= jhi; ++j) {
-            const int4 rj = sJ[j & (JW - 1)];
-            const int idx = CAP ? ext_index(m, rj.z, (uint32_t)rj.w) : m;
-            float4* dst = sV + (j & (JW - 1)) * 128 + t;
-            cp_async8(dst, in + rj.x + idx);
-            cp_async8(reinterpret_cast<char*>(dst) + 8, in + rj.y + idx);
+            for (int q = 0; q < 4; ++q) rr[q] = ringtab[min(j0 + q, tl.jhi)];
+#pragma unroll
+            for (int q = 0; q < 4; ++q) if (j0 + q <= tl.jhi) fetch_ring(j0 + q, rr[q]);
         }
         cp_async_commit();
-        jhave = jhi;
-        {
-            uint32_t done = 0;
-            while (!done)
-                asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
-                             : "=r"(done) : "r"(smem_u32(&bar)), "r"(phase) : "memory");
-            phase ^= 1u;
-        }
-        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-        cp_async_wait<0>();
+        int jhave = tl.jhi;                                      // highest ring whose coefficients sit in (or travel to) the window
+        int nold = 0;                                            // rings of the tile's window that were there before this tile
+        for (int k = 0; k < ntiles; ++k) {
+            const int s = k & 1;
+            const uint32_t ph = (uint32_t)(k >> 1) & 1u;
+            const TcTile cur = tl;
+            const int jlo = cur.jlo, jw = cur.jhi - jlo + 1;
+            // records of the next tile and of the rings that enter the window with it: loaded now, used after this tile
+            TcRing nx[4];
+            if (k + 1 < ntiles) {
+                tl = tiles[ch.tile0 + k + 1];
+#pragma unroll
+                for (int q = 0; q < 4; ++q) nx[q] = ringtab[min(jhave + 1 + q, R - 1)];
+            }
+            bool landed = false;
+            mbar_wait(&bar_full[s], ph);
+            asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
 
-        // ---- multiply-accumulate over the window's input rings ---------------------------------------------------------
-        float2 acc[TI][2];
+            float2 acc[TI][2];
 #pragma unroll
-        for (int ii = 0; ii < TI; ++ii) acc[ii][0] = acc[ii][1] = make_float2(0.f, 0.f);
-        const uint32_t tbase = tmem + ((uint32_t)(warp * 32) << 16);
-        for (int jj0 = 0; jj0 < jw; jj0 += 4) {
-            uint32_t g[16];
-            tc_ld16(g, tbase + (uint32_t)(jj0 * TI));
-            asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+            for (int ii = 0; ii < TI; ++ii) acc[ii][0] = acc[ii][1] = make_float2(0.f, 0.f);
+            const uint32_t tbase = tmem + ((uint32_t)((warp & 3) * 32) << 16) + (uint32_t)((s * MT + wg) * N);
+            uint32_t soff = ((uint32_t)jlo & (JW - 1)) * 2048u;          // byte offset of the slot of ring jlo + jj
+            auto load_v = [&](float4 (&v)[4], int jj0) {
+                if (!landed && jj0 + 4 > nold) { cp_async_wait<0>(); landed = true; }
 #pragma unroll
-            for (int q = 0; q < 4; ++q) {
-                if (jj0 + q < jw) {
-                    const int slot = (jlo + jj0 + q) & (JW - 1);
-                    float4 v = sV[slot * 128 + t];
+                for (int q = 0; q < 4; ++q) {
+                    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v[q].x), "=f"(v[q].y), "=f"(v[q].z), "=f"(v[q].w) : "r"(sv0 + soff));
+                    soff = (soff + 2048u) & (JW * 2048u - 1u);
+                }
+            };
+            auto mac4 = [&](const uint32_t (&g)[16], float4 (&v)[4], int jj0) {
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
                     if (CAP) {
                         // reflection conjugates; a shifted ring changes sign on reflection and on every odd period
-                        const int4 rj = sJ[slot];
-                        const int Nj = rj.z & 0x7fffffff, w = MULTI ? (int)__umulhi((uint32_t)m, (uint32_t)rj.w) : 0, r = m - w * Nj;
+                        const TcRing rj = ringtab[min(jlo + jj0 + q, R - 1)];
+                        const int Nj = rj.n_sh & 0x7fffffff, w = MULTI ? (int)__umulhi((uint32_t)m, rj.magic) : 0, r = m - w * Nj;
                         const bool refl = 2 * r > Nj;
-                        const uint32_t sre = (rj.z < 0 && (refl != ((w & 1) != 0))) ? 0x80000000u : 0u;
+                        const uint32_t sre = (rj.n_sh < 0 && (refl != ((w & 1) != 0))) ? 0x80000000u : 0u;
                         const uint32_t sim = sre ^ (refl ? 0x80000000u : 0u);
-                        v.x = __uint_as_float(__float_as_uint(v.x) ^ sre); v.y = __uint_as_float(__float_as_uint(v.y) ^ sim);
-                        v.z = __uint_as_float(__float_as_uint(v.z) ^ sre); v.w = __uint_as_float(__float_as_uint(v.w) ^ sim);
+                        v[q].x = __uint_as_float(__float_as_uint(v[q].x) ^ sre); v[q].y = __uint_as_float(__float_as_uint(v[q].y) ^ sim);
+                        v[q].z = __uint_as_float(__float_as_uint(v[q].z) ^ sre); v[q].w = __uint_as_float(__float_as_uint(v[q].w) ^ sim);
                     }
 #pragma unroll
                     for (int ii = 0; ii < TI; ++ii) {
                         const float G = __uint_as_float(g[q * TI + ii]);
-                        acc[ii][0] = ffma2(make_float2(G, G), make_float2(v.x, v.y), acc[ii][0]);
-                        acc[ii][1] = ffma2(make_float2(G, G), make_float2(v.z, v.w), acc[ii][1]);
+                        acc[ii][0] = ffma2(make_float2(G, G), make_float2(v[q].x, v[q].y), acc[ii][0]);
+                        acc[ii][1] = ffma2(make_float2(G, G), make_float2(v[q].z, v[q].w), acc[ii][1]);
                     }
                 }
+            };
+            {
+                // groups of four input rings, the accumulator columns and coefficients of the next group in flight
+                uint32_t ga[16], gb[16];
+                float4 va[4], vb[4];
+                tc_ld16(ga, tbase);
+                load_v(va, 0);
+                for (int jj0 = 0; jj0 < jw; jj0 += 8) {
+                    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+                    tc_ld16(gb, tbase + (uint32_t)(min(jj0 + 4, JW - 4) * TI));
+                    load_v(vb, jj0 + 4);
+                    mac4(ga, va, jj0);
+                    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+                    tc_ld16(ga, tbase + (uint32_t)(min(jj0 + 8, JW - 4) * TI));
+                    load_v(va, jj0 + 8);
+                    if (jj0 + 4 < jw) mac4(gb, vb, jj0 + 4);
+                }
+                asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+                if (!landed) cp_async_wait<0>();
             }
-        }
-        asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+            asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+            __syncwarp();
+            if ((t & 31) == 0) mbar_arrive(&bar_empty[s]);       // this warp is done with TMEM stage s
 
-        // ---- output: class E stores its mode; cap runs fold onto the ring's own modes --------------------
+            // the rings that enter with the next tile take slots whose rings no later tile reads
+            if (k + 1 < ntiles) {
+                nold = jhave + 1 - tl.jlo;
 #pragma unroll
-        for (int ii = 0; ii < TI; ++ii) {
-            if (ii < nti) {
-                const int i = i0 + ii, iS = R - 1 - i;
-                const RingRec ri = rings[i];
-                const int64_t offS = rings[iS].spec_off;
-                if (!CAP) {
-                    out[ri.spec_off + m] = mk<float>(acc[ii][0].x, acc[ii][0].y);
-                    if (iS != i) out[offS + m] = mk<float>(acc[ii][1].x, acc[ii][1].y);
-                } else if (m_raw <= Mh) {
-                    const float hw = (2 * m == M) ? 0.5f : 1.f;          // the +-M/2 bins carry half the Nyquist term each
-                    const int w = MULTI ? m / ri.n : 0, r = m - w * ri.n;
-                    const float s0 = (ri.shifted && (w & 1)) ? -1.f : 1.f, s1 = ri.shifted ? -s0 : s0;
+                for (int q = 0; q < 4; ++q) if (jhave + 1 + q <= tl.jhi) fetch_ring(jhave + 1 + q, nx[q]);
+                for (int j = jhave + 5; j <= tl.jhi; ++j) fetch_ring(j, ringtab[j]);
+                cp_async_commit();
+                jhave = max(jhave, tl.jhi);
+            }
+
+            // ---- output: class E stores its mode; cap runs fold onto the ring's own modes ----------------
 #pragma unroll
-                    for (int h = 0; h < 2; ++h) {
-                        if (h == 1 && iS == i) continue;
-                        float2* dst = reinterpret_cast<float2*>(out + (h ? offS : ri.spec_off));
-                        const float tx = hw * acc[ii][h].x, ty = hw * acc[ii][h].y;
-                        if (2 * r <= ri.n) atomicAdd(dst + r, make_float2(s0 * tx, s0 * ty));
-                        if (2 * r >= ri.n) atomicAdd(dst + (ri.n - r), make_float2(s1 * tx, -s1 * ty));
-                        if (MULTI && r == 0 && w > 0) atomicAdd(dst, make_float2(s0 * tx, -s0 * ty));     // m = -w N_i folds onto 0 as well
+            for (int ii = 0; ii < TI; ++ii) {
+                if (ii < cur.nti) {
+                    const int i = cur.i0 + ii, iS = R - 1 - i;
+                    const int offN = cur.offN[ii], offS = cur.offS[ii];
+                    if (!CAP) {
+                        if (m_raw < Mh) {                                 // (the Nyquist bin of class-E rings is served elsewhere)
+                            out[offN + m] = mk<float>(acc[ii][0].x, acc[ii][0].y);
+                            if (iS != i) out[offS + m] = mk<float>(acc[ii][1].x, acc[ii][1].y);
+                        }
+                    } else if (m_raw <= Mh) {
+                        const int Ni = cur.n_sh[ii] & 0x7fffffff;
+                        const bool shifted = cur.n_sh[ii] < 0;
+                        const float hw = (2 * m == M) ? 0.5f : 1.f;      // the +-M/2 bins carry half the Nyquist term each
+                        const int w = MULTI ? m / Ni : 0, r = m - w * Ni;
+                        const float s0 = (shifted && (w & 1)) ? -1.f : 1.f, s1 = shifted ? -s0 : s0;
+#pragma unroll
+                        for (int h = 0; h < 2; ++h) {
+                            if (h == 1 && iS == i) continue;
+                            float2* dst = reinterpret_cast<float2*>(out + (h ? offS : offN));
+                            const float tx = hw * acc[ii][h].x, ty = hw * acc[ii][h].y;
+                            if (2 * r <= Ni) atomicAdd(dst + r, make_float2(s0 * tx, s0 * ty));
+                            if (2 * r >= Ni) atomicAdd(dst + (Ni - r), make_float2(s1 * tx, -s1 * ty));
+                            if (MULTI && r == 0 && w > 0) atomicAdd(dst, make_float2(s0 * tx, -s0 * ty));     // m = -w N_i folds onto 0 as well
+                        }
                     }
                 }
             }
         }
     }
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     __syncthreads();
-    if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"(N));
+    if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"(2 * MT * N));
 }
 
 }  // namespace arkcos

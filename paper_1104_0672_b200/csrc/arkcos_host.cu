@@ -163,8 +163,11 @@ struct HostTables {
     std::vector<EqChunk> eq_chunks;              // runs of consecutive class-E rings for band_mac_eq_kernel   // per band-kernel class (see band_class)
     int eq_alt = 0;
     bool use_tc = false;                         // tensor-core band kernels (arkcos_band_tc.cuh) serve the class-E and cap runs
-    std::vector<CapChunk> tc_eq_chunks;          // the class-E runs again, as (first ring, rings, M) for band_mac_tc_kernel
-    std::vector<CapChunkItem> tc_eq_items;       // (run, block of 128 modes)
+    std::vector<TcChunk> tc_chunks;              // runs of rings served by band_mac_tc_kernel, their tiles and column words
+    std::vector<TcTile> tc_tiles;
+    std::vector<uint32_t> tc_cols;
+    std::vector<TcItem> tc_items[3];             // thread blocks: 0 class-E runs, 1 cap runs (single period), 2 cap runs (several)
+    std::vector<TcRing> tc_rings;                // per ring: spectrum offsets (ring, mirror image), length | shifted, magic divisor
     std::vector<int> fft_order;          // rings of the shared-memory FFT kernels, sorted by decreasing transform size
     std::vector<FftJob> fft3_jobs[4];    // jobs of the register-resident FFT kernels, Q = 512 << k
     int64_t filt_total = 0, chirp_total = 0, ph_total = 0, nsamples = 0;
@@ -411,13 +414,48 @@ void build_pairs(HostGeometry& g, double theta_max, double ell_nyq, int fixed_mp
                 t.eq_chunks.push_back(EqChunk{i, 1});
         }
     }
-    if (use_tc)
-        for (const EqChunk& e : t.eq_chunks) {
-            const int M = g.n[e.i0];
-            if ((M / 2) % 128 != 0) continue;              // (such rings were not admitted with long rows, see above)
-            t.tc_eq_chunks.push_back(CapChunk{e.i0, e.n, M, 0});
-            for (int bx = 0; bx * 128 < M / 2; ++bx) t.tc_eq_items.push_back(CapChunkItem{(int)t.tc_eq_chunks.size() - 1, bx});
-        }
+    if (use_tc) {
+        // tables of band_mac_tc_kernel: per run its tiles of kTcTI output rings (window of input rings) and, per tile, one
+        // word per accumulator column = 4 * (input ring - window start) + output ring of the tile
+        auto add_run = [&](int i0, int n, int M, int multi, int cls, bool with_nyquist) {
+            TcChunk c{i0, n, M, multi, (int)t.tc_tiles.size()};
+            for (int tile = 0; tile < n; tile += kTcTI) {
+                const int nti = std::min(kTcTI, n - tile), ia = i0 + tile;
+                const int jlo = t.pairs[t.north[ia].pair_lo].j, jhi = t.pairs[t.north[ia + nti - 1].pair_hi - 1].j;
+                TcTile tile_rec{jlo, jhi, ia, nti, {0, 0, 0, 0}, {0, 0, 0, 0}, {0, 0, 0, 0}};
+                for (int ii = 0; ii < nti; ++ii) {
+                    tile_rec.offN[ii] = (int)g.spec_off[ia + ii];
+                    tile_rec.offS[ii] = (int)g.spec_off[R - 1 - ia - ii];
+                    tile_rec.n_sh[ii] = g.n[ia + ii] | (g.shifted[ia + ii] ? (int)0x80000000 : 0);
+                }
+                t.tc_tiles.push_back(tile_rec);
+                for (int col = 0; col < kTcN; ++col) {
+                    const int jj = col / kTcTI, ii = col % kTcTI;
+                    uint32_t word = kTcNoPair;
+                    if (ii < nti) {
+                        const NorthRec& nr = t.north[ia + ii];
+                        const int pj = jlo + jj - t.pairs[nr.pair_lo].j;
+                        if (pj >= 0 && pj < nr.pair_hi - nr.pair_lo) {
+                            const PairRec& pr = t.pairs[nr.pair_lo + pj];
+                            word = (uint32_t)(pr.woff / 4) | ((uint32_t)pr.cnt << 25) | ((uint32_t)pr.par << 31);
+                        }
+                    }
+                    t.tc_cols.push_back(word);
+                }
+            }
+            t.tc_chunks.push_back(c);
+            const int nmodes = with_nyquist ? M / 2 + 1 : M / 2;
+            for (int bx = 0; bx * 128 * kTcMT < nmodes; ++bx) t.tc_items[cls].push_back(TcItem{(int)t.tc_chunks.size() - 1, bx});
+        };
+        for (int j = 0; j < R; ++j)
+            t.tc_rings.push_back(TcRing{(int)g.spec_off[j], (int)g.spec_off[R - 1 - j], g.n[j] | (g.shifted[j] ? (int)0x80000000 : 0),
+                                        (uint32_t)((0x100000000ull + (uint64_t)g.n[j] - 1ull) / (uint64_t)g.n[j])});
+        for (const EqChunk& e : t.eq_chunks)
+            if ((g.n[e.i0] / 2) % 128 == 0) add_run(e.i0, e.n, g.n[e.i0], 0, 0, false);
+        // cap runs from the pole towards the equator: the longest (last) first
+        for (size_t c = t.cap_chunks.size(); c-- > 0;)
+            add_run(t.cap_chunks[c].i0, t.cap_chunks[c].n, t.cap_chunks[c].M, t.cap_chunks[c].multi, t.cap_chunks[c].multi ? 2 : 1, true);
+    }
     for (size_t c = 0; c < t.cap_chunks.size(); ++c) {
         const CapChunk& ch = t.cap_chunks[c];
         const int modes_per_block = use_tc ? 128 : kBandThreads * 2;
@@ -604,15 +642,15 @@ void launch_uniform(const arkcos_plan* pl, int nmaps, cudaStream_t st, bool seri
             band_mac_eq_cached_kernel<4, 1><<<dim3(gx, (unsigned)pl->neqchunks, 1), kBandThreads, 0, st>>>(
                 pl->d_eqchunks, pl->d_north, pl->d_pairs, pl->d_goff, pl->d_G, pl->d_rings, pl->g.R,
                 (const cx<float>*)pl->d_specIn, (cx<float>*)pl->d_specOut, pl->g.spec_total, nmaps);
-    } else if (pl->neqchunks > 0 && pl->use_tc && pl->ntc_eq_items > 0) {
-        const dim3 grid((unsigned)pl->ntc_eq_items, (unsigned)nmaps);
+    } else if (pl->neqchunks > 0 && pl->use_tc && pl->ntc_items[0] > 0) {
+        const dim3 grid((unsigned)pl->ntc_items[0], (unsigned)nmaps);
         if (pl->eq_alt)
             band_mac_tc_kernel<0><<<grid, kTcThreads, kTcSmemBytes, st>>>(
-                pl->d_tc_eq_items, pl->d_tc_eq_chunks, pl->d_north, pl->d_pairs, (const float*)pl->d_W, pl->d_rings, pl->g.R,
+                pl->d_tc_items[0], pl->d_tc_chunks, pl->d_tc_tiles, pl->d_tc_cols, pl->d_tc_rings, (const float*)pl->d_W, pl->g.R,
                 (const cx<float>*)pl->d_specIn, (cx<float>*)pl->d_specOut, pl->g.spec_total);
         else
             band_mac_tc_kernel<1><<<grid, kTcThreads, kTcSmemBytes, st>>>(
-                pl->d_tc_eq_items, pl->d_tc_eq_chunks, pl->d_north, pl->d_pairs, (const float*)pl->d_W, pl->d_rings, pl->g.R,
+                pl->d_tc_items[0], pl->d_tc_chunks, pl->d_tc_tiles, pl->d_tc_cols, pl->d_tc_rings, (const float*)pl->d_W, pl->g.R,
                 (const cx<float>*)pl->d_specIn, (cx<float>*)pl->d_specOut, pl->g.spec_total);
     } else if (pl->neqchunks > 0) {
         constexpr int TI = 4, MT = 2;
@@ -649,11 +687,12 @@ void launch_uniform(const arkcos_plan* pl, int nmaps, cudaStream_t st, bool seri
                 band_mac_capchunk_cached_kernel<4, 1, MULTI><<<dim3(n, 1), kBandThreads, 0, s1>>>(
                     items, pl->d_cap_chunks, pl->d_north, pl->d_pairs, pl->d_goff, pl->d_G, pl->d_rings, pl->g.R,
                     (const cx<float>*)pl->d_specIn, (cx<float>*)pl->d_specOut, pl->g.spec_total, nmaps);
-            else if (pl->use_tc)
-                band_mac_tc_kernel<MULTI ? 3 : 2><<<dim3(n, (unsigned)nmaps), kTcThreads, kTcSmemBytes, s1>>>(
-                    items, pl->d_cap_chunks, pl->d_north, pl->d_pairs, (const float*)pl->d_W, pl->d_rings, pl->g.R,
-                    (const cx<float>*)pl->d_specIn, (cx<float>*)pl->d_specOut, pl->g.spec_total);
-            else
+            else if (pl->use_tc) {
+                if (pl->ntc_items[MULTI ? 2 : 1] > 0)
+                    band_mac_tc_kernel<MULTI ? 3 : 2><<<dim3((unsigned)pl->ntc_items[MULTI ? 2 : 1], (unsigned)nmaps), kTcThreads, kTcSmemBytes, s1>>>(
+                        pl->d_tc_items[MULTI ? 2 : 1], pl->d_tc_chunks, pl->d_tc_tiles, pl->d_tc_cols, pl->d_tc_rings, (const float*)pl->d_W, pl->g.R,
+                        (const cx<float>*)pl->d_specIn, (cx<float>*)pl->d_specOut, pl->g.spec_total);
+            } else
                 band_mac_capchunk_kernel<4, 20, MULTI><<<dim3(n, (unsigned)nmaps), kBandThreads, 0, s1>>>(
                     items, pl->d_cap_chunks, pl->d_north, pl->d_pairs, (const float*)pl->d_W, pl->d_rings, pl->g.R,
                     (const cx<float>*)pl->d_specIn, (cx<float>*)pl->d_specOut, pl->g.spec_total);
@@ -901,7 +940,8 @@ static int plan_create_impl(arkcos_plan** out, const arkcos_pixelization* pix, c
     for (int c = 0; c < kBandClasses; ++c) pl->nitems[c] = (int)t.items[c].size();
     pl->neqchunks = (int)t.eq_chunks.size();
     pl->use_tc = t.use_tc;
-    pl->ntc_eq_items = (int)t.tc_eq_items.size();
+    for (int c = 0; c < 3; ++c) pl->ntc_items[c] = (int)t.tc_items[c].size();
+    if (t.nsamples / 4 >= (1 << 25)) return fail(ARKCOS_UNSUPPORTED, "too many kernel-row samples");
     pl->npole = (int)t.pole_rings.size();
     pl->pole_mh = t.pole_mh;
     pl->eq_alt = t.eq_alt;
@@ -945,12 +985,22 @@ static int plan_create_impl(arkcos_plan** out, const arkcos_pixelization* pix, c
         if (int rc = upload(&pl->d_direct_items, items, wsb)) return rc;
     }
     if (pl->use_tc) {
-        if (int rc = upload(&pl->d_tc_eq_chunks, t.tc_eq_chunks, wsb)) return rc;
-        if (int rc = upload(&pl->d_tc_eq_items, t.tc_eq_items, wsb)) return rc;
+        if (int rc = upload(&pl->d_tc_chunks, t.tc_chunks, wsb)) return rc;
+        if (int rc = upload(&pl->d_tc_tiles, t.tc_tiles, wsb)) return rc;
+        if (int rc = upload(&pl->d_tc_cols, t.tc_cols, wsb)) return rc;
+        if (int rc = upload(&pl->d_tc_rings, t.tc_rings, wsb)) return rc;
+        for (int c = 0; c < 3; ++c)
+            if (int rc = upload(&pl->d_tc_items[c], t.tc_items[c], wsb)) return rc;
         CUDA_TRY(cudaFuncSetAttribute(band_mac_tc_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kTcSmemBytes));
         CUDA_TRY(cudaFuncSetAttribute(band_mac_tc_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kTcSmemBytes));
         CUDA_TRY(cudaFuncSetAttribute(band_mac_tc_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kTcSmemBytes));
         CUDA_TRY(cudaFuncSetAttribute(band_mac_tc_kernel<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kTcSmemBytes));
+        // two blocks per SM need nearly all of its shared memory
+        CUDA_TRY(cudaFuncSetAttribute(band_mac_tc_kernel<0>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
+        CUDA_TRY(cudaFuncSetAttribute(band_mac_tc_kernel<1>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
+        CUDA_TRY(cudaFuncSetAttribute(band_mac_tc_kernel<2>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
+        CUDA_TRY(cudaFuncSetAttribute(band_mac_tc_kernel<3>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
+        CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&pl->tc_blocks_per_sm, band_mac_tc_kernel<0>, kTcThreads, kTcSmemBytes));
     }
     if (int rc = upload(&pl->d_cap_chunks, t.cap_chunks, wsb)) return rc;
     if (int rc = upload(&pl->d_cap_chunk_items, t.cap_chunk_items, wsb)) return rc;
@@ -1107,7 +1157,7 @@ int arkcos_plan_destroy(arkcos_plan* pl)
     void* ptrs[] = {pl->d_rings, pl->d_lens, pl->d_pairs, pl->d_north, pl->d_items[0], pl->d_items[1], pl->d_items[2], pl->d_items[3],
                     pl->d_items[4], pl->d_items[5], pl->d_eqchunks, pl->d_pole, pl->d_chirp, pl->d_phase, pl->d_fft_order, pl->d_table, pl->d_tw, pl->d_filt,
                     pl->d_W, pl->d_specIn, pl->d_specOut, pl->d_stage_in, pl->d_stage_out,
-                    pl->d_cap_chunks, pl->d_cap_chunk_items, pl->d_tc_eq_chunks, pl->d_tc_eq_items, pl->d_goff, pl->d_G, pl->d_direct_items, pl->d_tw3, pl->d_tw16, pl->d_fft3_jobs[0], pl->d_fft3_jobs[1], pl->d_fft3_jobs[2], pl->d_fft3_jobs[3]};
+                    pl->d_cap_chunks, pl->d_cap_chunk_items, pl->d_tc_chunks, pl->d_tc_tiles, pl->d_tc_cols, pl->d_tc_rings, pl->d_tc_items[0], pl->d_tc_items[1], pl->d_tc_items[2], pl->d_goff, pl->d_G, pl->d_direct_items, pl->d_tw3, pl->d_tw16, pl->d_fft3_jobs[0], pl->d_fft3_jobs[1], pl->d_fft3_jobs[2], pl->d_fft3_jobs[3]};
     for (void* p : ptrs) if (p) cudaFree(p);
     for (auto& e : pl->ev) if (e) cudaEventDestroy(e);
     for (auto& e : pl->ev_band) if (e) cudaEventDestroy(e);
@@ -1185,6 +1235,14 @@ int arkcos_plan_band_kernels(const arkcos_plan* pl, int* n, const char** names, 
         for (int k = 0; k < 8; ++k) CUDA_TRY(cudaEventElapsedTime(&last_ms[k], pl->ev_band[k], pl->ev_band[k + 1]));
     }
     return ARKCOS_OK;
+}
+
+int arkcos_plan_tensor_cores(const arkcos_plan* pl, int blocks[3], int* resident_per_sm)
+{
+    if (!pl) return fail(ARKCOS_INVALID_ARG, "NULL plan");
+    if (blocks) for (int c = 0; c < 3; ++c) blocks[c] = pl->use_tc ? pl->ntc_items[c] : 0;
+    if (resident_per_sm) *resident_per_sm = pl->use_tc ? pl->tc_blocks_per_sm : 0;
+    return pl->use_tc ? 1 : 0;
 }
 
 int arkcos_plan_launches_per_convolve(const arkcos_plan* pl)

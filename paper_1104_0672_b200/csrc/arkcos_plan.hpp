@@ -65,9 +65,13 @@ struct arkcos_plan {
     // tensor-core band kernels (arkcos_band_tc.cuh): class-E runs as (run, block of 128 modes) items; the cap runs use
     // d_cap_chunks / d_cap_chunk_items with blocks of 128 modes
     bool use_tc = false;
-    arkcos::CapChunk* d_tc_eq_chunks = nullptr;
-    arkcos::CapChunkItem* d_tc_eq_items = nullptr;
-    int ntc_eq_items = 0;
+    arkcos::TcChunk* d_tc_chunks = nullptr;
+    arkcos::TcTile* d_tc_tiles = nullptr;
+    uint32_t* d_tc_cols = nullptr;
+    arkcos::TcRing* d_tc_rings = nullptr;
+    arkcos::TcItem* d_tc_items[3] = {nullptr, nullptr, nullptr};    // 0 class-E runs, 1 cap runs (single period), 2 cap runs (several)
+    int ntc_items[3] = {0, 0, 0};
+    int tc_blocks_per_sm = 0;
     int* d_pole = nullptr;
     int npole = 0, pole_mh = 0;
     arkcos::BandItem* d_items[arkcos::kBandClasses] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
