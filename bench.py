@@ -178,6 +178,11 @@ def run_ours(args):
     for _ in range(max(args.warmup, 3)):
         step()
     barrier()
+    if args.profile:                    # launches only (for ncu): no end-to-end leg, no CPU oracle, no JSON line
+        for _ in range(args.steps):
+            step()
+        barrier()
+        return
     sampler = ClockSampler(local) if rank == 0 else None
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
@@ -325,6 +330,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--cfg", type=int, default=4)
+    ap.add_argument("--profile", action="store_true", help="warm-up + steps of arkcos_convolve only (the command ncu wraps)")
     ap.add_argument("--oracle-rings", type=int, default=2048, help="output rings in the CPU-oracle sample")
     args = ap.parse_args()
     if args.impl == "reference":
