@@ -13,7 +13,7 @@ convolution itself uses (oracle/direct.py kernel_lerp).
 
 The integral is written as the plain definition in theta,  K_l = 2 pi int K(theta) P_l(cos theta) sin(theta) dtheta,
 evaluated by a composite Gauss-Legendre rule (numpy leggauss nodes, scipy eval_legendre values) on panels short
-against the oscillation length pi / l of P_l; no recurrences, no blocking.
+against the oscillation length pi / l of P_l that end at the table nodes; no recurrences, no blocking.
 """
 from __future__ import annotations
 
@@ -22,14 +22,17 @@ from scipy.special import eval_legendre
 
 from .direct import kernel_lerp
 
-_GL_ORDER = 20
+_GL_ORDER = 8
 
 
 def _panels(theta_lo: float, theta_hi: float, lmax: int, ntab: int, theta_max: float) -> np.ndarray:
-    """Panel edges on [theta_lo, theta_hi]: at most a quarter of P_lmax's oscillation length each."""
+    """Panel edges on [theta_lo, theta_hi]: at most a quarter of P_lmax's oscillation length each, and every table node
+    in between is an edge (the interpolant's slope jumps there; a Gauss rule across a kink converges slowly)."""
     width = min(0.25 * np.pi / (lmax + 1), (theta_hi - theta_lo))
     npan = max(1, int(np.ceil((theta_hi - theta_lo) / width)))
-    return np.linspace(theta_lo, theta_hi, npan + 1)
+    nodes = np.arange(ntab) * (theta_max / (ntab - 1))
+    nodes = nodes[(nodes > theta_lo) & (nodes < theta_hi)]
+    return np.unique(np.concatenate([np.linspace(theta_lo, theta_hi, npan + 1), nodes]))
 
 
 def kernel_legendre(table: np.ndarray, theta_max: float, lmax: int, theta_lo: float = 0.0,

@@ -37,7 +37,7 @@ def test_gaussian_flat_sky_limit():
     fwhm = 2.0 * DEG
     sigma = fwhm * inputs.FWHM_TO_SIGMA
     tmax = 6 * sigma
-    tab = inputs.gaussian_table(fwhm, tmax)
+    tab = inputs.gaussian_table(fwhm, tmax, 2049)
     lmax = 150
     got = legendre.kernel_legendre(tab, tmax, lmax)
     ell = np.arange(lmax + 1)
@@ -51,7 +51,7 @@ def test_completeness_parseval():
     """sum_l (2l+1)/(4 pi) K_l^2 -> 2 pi int K(z)^2 dz for lmax beyond the profile's band (smooth profile)."""
     s = 4 * DEG
     tmax = 6 * s
-    tab = inputs.mexican_hat_table(s, tmax) * (1 - (inputs.table_thetas(tmax) / tmax) ** 2) ** 2    # smooth at the cut
+    tab = inputs.mexican_hat_table(s, tmax, 2049) * (1 - (inputs.table_thetas(tmax, 2049) / tmax) ** 2) ** 2    # smooth at the cut
     lmax = 160
     Kl = legendre.kernel_legendre(tab, tmax, lmax)
     ell = np.arange(lmax + 1)
