@@ -178,6 +178,32 @@ int arkcos_plan_launches_per_convolve(const arkcos_plan* plan);
  * "alu" roofline); result in TFLOP/s, best of `repeats` launches.  Synchronises the device. */
 int arkcos_probe_fp32_peak(double* tflops, int repeats);
 
+/* ---- truncation-error estimate (host side, no CUDA work, no plan) -----------------------------------------------------
+ * Eq. 2: K_l = 2 pi int_{-1}^{1} K(z) P_l(z) dz, z = cos(theta), of the tabulated profile (linear
+ * interpolation in theta between the nodes, as the convolution uses it) restricted to theta_lo <= theta < theta_hi,
+ * 0 <= theta_lo <= theta_hi <= kernel->theta_max; k_ell: caller's array of lmax + 1 doubles (l = 0 .. lmax), lmax <= 65536. */
+int arkcos_kernel_legendre(const arkcos_kernel* kernel, double theta_lo, double theta_hi, int lmax, double* k_ell);
+
+/* Eq. 7: mean quadratic error  sigma^2 = sum_{l=0}^{lmax} (2l+1)/(4 pi) dK_l^2 C_l  made by cutting the
+ * profile at theta_cut when the map is isotropic with power spectrum c_ell[0 .. lmax]; dK_l is the Legendre transform of
+ * "the difference of the exact and the truncated kernel" = the profile on [theta_cut, theta_max).  *signal2 = the same sum
+ * with the whole profile's K_l (variance of the exactly smoothed map).  theta_cut >= theta_max gives sigma2 = 0.
+ * sigma2 / signal2 may be NULL. */
+int arkcos_kernel_truncation_error(const arkcos_kernel* kernel, double theta_cut, const double* c_ell, int lmax,
+                                   double* sigma2, double* signal2);
+
+/* Support-radius chooser built on Eq. 7 ("it can be truncated at that radius without introducing significant
+ * errors"): among the candidate cuts g * theta_max / ngrid, moving inwards from theta_max, the smallest one up to which
+ * sigma(cut) <= rel_tol * sqrt(signal2) holds throughout.  *theta_cut = theta_max when even the outermost cell fails.
+ * A plan made from the table's first nodes up to *theta_cut then carries that relative truncation error. */
+int arkcos_kernel_choose_cut(const arkcos_kernel* kernel, const double* c_ell, int lmax, double rel_tol, int ngrid,
+                             double* theta_cut, double* sigma2, double* signal2);
+
+/* Companion for options.ell_nyquist (the phi grid of kernel rows that touch a polar-cap ring): the smallest wavenumber L
+ * such that the smoothed map's power beyond it, sum_{l > L} (2l+1)/(4 pi) K_l^2 C_l, is at most rel_tol^2 of the whole sum. */
+int arkcos_kernel_choose_ell_nyquist(const arkcos_kernel* kernel, const double* c_ell, int lmax, double rel_tol,
+                                     double* ell_nyquist);
+
 const char* arkcos_strerror(int status);
 const char* arkcos_last_error(void);             /* detail of the last failure on this thread ("" if none) */
 

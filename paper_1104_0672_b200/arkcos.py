@@ -67,6 +67,12 @@ SYMBOLS = {
     "arkcos_plan_tensor_cores": (c_int, [c_void_p, POINTER(c_int), POINTER(c_int)]),
     "arkcos_plan_launches_per_convolve": (c_int, [c_void_p]),
     "arkcos_probe_fp32_peak": (c_int, [POINTER(c_double), c_int]),
+    "arkcos_kernel_legendre": (c_int, [POINTER(Kernel), c_double, c_double, c_int, POINTER(c_double)]),
+    "arkcos_kernel_truncation_error": (c_int, [POINTER(Kernel), c_double, POINTER(c_double), c_int, POINTER(c_double),
+                                               POINTER(c_double)]),
+    "arkcos_kernel_choose_cut": (c_int, [POINTER(Kernel), POINTER(c_double), c_int, c_double, c_int, POINTER(c_double),
+                                         POINTER(c_double), POINTER(c_double)]),
+    "arkcos_kernel_choose_ell_nyquist": (c_int, [POINTER(Kernel), POINTER(c_double), c_int, c_double, POINTER(c_double)]),
     "arkcos_strerror": (c_char_p, [c_int]),
     "arkcos_last_error": (c_char_p, []),
 }
@@ -98,6 +104,48 @@ def arkcos_strerror(status: int) -> str:
 def arkcos_probe_fp32_peak(repeats: int = 10) -> float:
     v = c_double()
     _check(_lib().arkcos_probe_fp32_peak(byref(v), repeats), "arkcos_probe_fp32_peak")
+    return v.value
+
+
+def _kernel(table, theta_max):
+    tab = np.ascontiguousarray(table, dtype=np.float64)
+    return tab, Kernel(tab.ctypes.data_as(POINTER(c_double)), int(tab.shape[0]), float(theta_max))
+
+
+def arkcos_kernel_legendre(table, theta_max: float, lmax: int, theta_lo: float = 0.0, theta_hi=None) -> np.ndarray:
+    tab, k = _kernel(table, theta_max)
+    out = np.empty(lmax + 1)
+    _check(_lib().arkcos_kernel_legendre(byref(k), float(theta_lo), float(theta_max if theta_hi is None else theta_hi), int(lmax),
+                                         out.ctypes.data_as(POINTER(c_double))), "arkcos_kernel_legendre")
+    return out
+
+
+def arkcos_kernel_truncation_error(table, theta_max: float, theta_cut: float, c_ell):
+    """(sigma2, signal2) of Eq. 7 for lmax = len(c_ell) - 1."""
+    tab, k = _kernel(table, theta_max)
+    cl = np.ascontiguousarray(c_ell, dtype=np.float64)
+    s2, sig = c_double(), c_double()
+    _check(_lib().arkcos_kernel_truncation_error(byref(k), float(theta_cut), cl.ctypes.data_as(POINTER(c_double)), cl.shape[0] - 1,
+                                                 byref(s2), byref(sig)), "arkcos_kernel_truncation_error")
+    return s2.value, sig.value
+
+
+def arkcos_kernel_choose_cut(table, theta_max: float, c_ell, rel_tol: float, ngrid: int = 256):
+    """(theta_cut, sigma2, signal2)."""
+    tab, k = _kernel(table, theta_max)
+    cl = np.ascontiguousarray(c_ell, dtype=np.float64)
+    cut, s2, sig = c_double(), c_double(), c_double()
+    _check(_lib().arkcos_kernel_choose_cut(byref(k), cl.ctypes.data_as(POINTER(c_double)), cl.shape[0] - 1, float(rel_tol), int(ngrid),
+                                           byref(cut), byref(s2), byref(sig)), "arkcos_kernel_choose_cut")
+    return cut.value, s2.value, sig.value
+
+
+def arkcos_kernel_choose_ell_nyquist(table, theta_max: float, c_ell, rel_tol: float) -> float:
+    tab, k = _kernel(table, theta_max)
+    cl = np.ascontiguousarray(c_ell, dtype=np.float64)
+    v = c_double()
+    _check(_lib().arkcos_kernel_choose_ell_nyquist(byref(k), cl.ctypes.data_as(POINTER(c_double)), cl.shape[0] - 1, float(rel_tol),
+                                                   byref(v)), "arkcos_kernel_choose_ell_nyquist")
     return v.value
 
 

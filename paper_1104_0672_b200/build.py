@@ -1,4 +1,7 @@
-"""Builds libarkcos.so in-tree with nvcc for sm_100a (python -m paper_1104_0672_b200.build)."""
+"""Builds libarkcos.so in-tree with nvcc for sm_100a (python -m paper_1104_0672_b200.build).
+
+One object per translation unit under paper_1104_0672_b200/build/ (git-ignored), recompiled only when the source or a
+header it may include is newer; then one link step."""
 from __future__ import annotations
 
 import os
@@ -6,21 +9,35 @@ import subprocess
 import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
-SRC = [os.path.join(HERE, "csrc", "arkcos_host.cu")]
-DEPS = [os.path.join(HERE, "csrc", f) for f in os.listdir(os.path.join(HERE, "csrc"))] + \
-       [os.path.join(os.path.dirname(HERE), "include", "arkcos.h")]
+CSRC = os.path.join(HERE, "csrc")
+HEADERS = [os.path.join(CSRC, f) for f in os.listdir(CSRC) if f.endswith((".cuh", ".hpp", ".h"))] + \
+          [os.path.join(os.path.dirname(HERE), "include", "arkcos.h")]
+# translation unit -> headers it depends on (None = every header)
+UNITS = {"arkcos_host.cu": None, "arkcos_legendre.cpp": [HEADERS[-1]]}
+OBJ_DIR = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libarkcos.so")
 
 
+def _stale(target: str, deps) -> bool:
+    return not os.path.exists(target) or any(os.path.getmtime(target) < os.path.getmtime(d) for d in deps)
+
+
 def build(force: bool = False, verbose: bool = False) -> str:
-    if not force and os.path.exists(LIB) and all(os.path.getmtime(LIB) >= os.path.getmtime(d) for d in DEPS):
-        return LIB
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-    cmd = [nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
-           "-shared", "-Xcompiler", "-fPIC", "-o", LIB] + SRC
-    if verbose:
-        cmd.insert(1, "-Xptxas=-v")
-    subprocess.check_call(cmd)
+    os.makedirs(OBJ_DIR, exist_ok=True)
+    objs = []
+    for unit, hdrs in UNITS.items():
+        src = os.path.join(CSRC, unit)
+        obj = os.path.join(OBJ_DIR, os.path.splitext(unit)[0] + ".o")
+        objs.append(obj)
+        if force or _stale(obj, [src] + (HEADERS if hdrs is None else hdrs)):
+            cmd = [nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
+                   "-Xcompiler", "-fPIC", "-c", "-o", obj, src]
+            if verbose:
+                cmd.insert(1, "-Xptxas=-v")
+            subprocess.check_call(cmd)
+    if force or _stale(LIB, objs):
+        subprocess.check_call([nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-o", LIB] + objs)
     return LIB
 
 

@@ -23,6 +23,14 @@ int fail(int code, const std::string& msg)
     return code;
 }
 
+}  // namespace
+
+namespace arkcos {
+int set_last_error(int code, const std::string& msg) { return fail(code, msg); }      // for the other translation units
+}
+
+namespace {
+
 #define CUDA_TRY(expr)                                                                                        \
     do {                                                                                                      \
         cudaError_t e_ = (expr);                                                                              \
