@@ -119,6 +119,16 @@ int arkcos_plan_create_tables_only(arkcos_plan** out, const arkcos_pixelization*
  * (they share the plan's workspace). */
 int arkcos_convolve(const arkcos_plan* plan, const void* d_in, void* d_out, int nmaps, void* cuda_stream);
 
+/* One map set, several radial kernels (multi-kernel batching: a bank of wavelet scales, or the O(10) radial
+ * terms of an asymmetric-beam expansion, "ASYMFAST"): plans[0 .. nkernels-1] are distinct plans created for the
+ * same pixelization, dtype and device (kernels, support radii and options may differ).  The forward ring FFTs and the
+ * re-origin of Eq. 8 do not depend on the kernel: they run once, with plans[0]'s tables, and every plan's
+ * band step reads those spectra; each plan then runs its own kernel rows, band step and inverse FFTs.
+ * d_in: [nmaps][npix] as for arkcos_convolve; d_out: [nkernels][nmaps][npix], kernel-major; both DEVICE pointers.
+ * Equal to nkernels arkcos_convolve calls, bit for bit.  Only enqueues work on cuda_stream. */
+int arkcos_convolve_multi(const arkcos_plan* const* plans, int nkernels, const void* d_in, void* d_out, int nmaps,
+                          void* cuda_stream);
+
 /* Same result from HOST buffers (pinned memory makes the copies asynchronous): host -> device copy, arkcos_convolve,
  * device -> host copy, all on cuda_stream, then a stream synchronisation.  Uses staging buffers inside the plan. */
 int arkcos_convolve_host(const arkcos_plan* plan, const void* h_in, void* h_out, int nmaps, void* cuda_stream);

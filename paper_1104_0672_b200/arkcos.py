@@ -50,6 +50,7 @@ SYMBOLS = {
     "arkcos_plan_create_tables_only": (c_int, [POINTER(c_void_p), POINTER(Pixelization), POINTER(Kernel), c_int,
                                                POINTER(Options)]),
     "arkcos_convolve": (c_int, [c_void_p, c_void_p, c_void_p, c_int, c_void_p]),
+    "arkcos_convolve_multi": (c_int, [POINTER(c_void_p), c_int, c_void_p, c_void_p, c_int, c_void_p]),
     "arkcos_convolve_host": (c_int, [c_void_p, c_void_p, c_void_p, c_int, c_void_p]),
     "arkcos_convolve_host_async": (c_int, [c_void_p, c_void_p, c_void_p, c_int]),
     "arkcos_plan_synchronize": (c_int, [c_void_p]),
@@ -255,6 +256,13 @@ class Plan:
         ms = (c_float * 4)()
         _check(_lib().arkcos_plan_get_timing(self._h, ms), "arkcos_plan_get_timing")
         return dict(rows=ms[0], fft_forward=ms[1], band=ms[2], fft_inverse=ms[3])
+
+
+def arkcos_convolve_multi(plans, d_in: int, d_out: int, nmaps: int = 1, stream: int = 0):
+    """arkcos_convolve_multi: d_out is [len(plans)][nmaps][npix] on the device."""
+    arr = (c_void_p * len(plans))(*[p._h for p in plans])
+    _check(_lib().arkcos_convolve_multi(arr, len(plans), c_void_p(d_in), c_void_p(d_out), int(nmaps), c_void_p(stream)),
+           "arkcos_convolve_multi")
 
 
 def convolve_torch(plan: Plan, x, out=None):

@@ -634,7 +634,7 @@ template <int TMAX, bool HAS_ODD> void launch_uniform_class(const arkcos_plan* p
     if (pl->nitems[cls] == 0) return;
     band_mac_uniform_kernel<TMAX, HAS_ODD><<<dim3((unsigned)pl->nitems[cls], (unsigned)nmaps), kBandThreads, 0, st>>>(
         pl->d_items[cls], pl->d_north, pl->d_pairs, (const float*)pl->d_W, pl->d_rings, pl->g.R,
-        (const cx<float>*)pl->d_specIn, (cx<float>*)pl->d_specOut, pl->g.spec_total);
+        (const cx<float>*)pl->spec_in(), (cx<float>*)pl->d_specOut, pl->g.spec_total);
 }
 
 void launch_uniform(const arkcos_plan* pl, int nmaps, cudaStream_t st, bool serial)
@@ -645,32 +645,32 @@ void launch_uniform(const arkcos_plan* pl, int nmaps, cudaStream_t st, bool seri
         if (nmaps > 1)
             band_mac_eq_cached_kernel<4, 2><<<dim3(gx, (unsigned)pl->neqchunks, (unsigned)((nmaps + 1) / 2)), kBandThreads, 0, st>>>(
                 pl->d_eqchunks, pl->d_north, pl->d_pairs, pl->d_goff, pl->d_G, pl->d_rings, pl->g.R,
-                (const cx<float>*)pl->d_specIn, (cx<float>*)pl->d_specOut, pl->g.spec_total, nmaps);
+                (const cx<float>*)pl->spec_in(), (cx<float>*)pl->d_specOut, pl->g.spec_total, nmaps);
         else
             band_mac_eq_cached_kernel<4, 1><<<dim3(gx, (unsigned)pl->neqchunks, 1), kBandThreads, 0, st>>>(
                 pl->d_eqchunks, pl->d_north, pl->d_pairs, pl->d_goff, pl->d_G, pl->d_rings, pl->g.R,
-                (const cx<float>*)pl->d_specIn, (cx<float>*)pl->d_specOut, pl->g.spec_total, nmaps);
+                (const cx<float>*)pl->spec_in(), (cx<float>*)pl->d_specOut, pl->g.spec_total, nmaps);
     } else if (pl->neqchunks > 0 && pl->use_tc && pl->ntc_items[0] > 0) {
         const dim3 grid((unsigned)pl->ntc_items[0], (unsigned)nmaps);
         if (pl->eq_alt)
             band_mac_tc_kernel<0><<<grid, kTcThreads, kTcSmemBytes, st>>>(
                 pl->d_tc_items[0], pl->d_tc_chunks, pl->d_tc_tiles, pl->d_tc_cols, pl->d_tc_rings, (const float*)pl->d_W, pl->g.R,
-                (const cx<float>*)pl->d_specIn, (cx<float>*)pl->d_specOut, pl->g.spec_total);
+                (const cx<float>*)pl->spec_in(), (cx<float>*)pl->d_specOut, pl->g.spec_total);
         else
             band_mac_tc_kernel<1><<<grid, kTcThreads, kTcSmemBytes, st>>>(
                 pl->d_tc_items[0], pl->d_tc_chunks, pl->d_tc_tiles, pl->d_tc_cols, pl->d_tc_rings, (const float*)pl->d_W, pl->g.R,
-                (const cx<float>*)pl->d_specIn, (cx<float>*)pl->d_specOut, pl->g.spec_total);
+                (const cx<float>*)pl->spec_in(), (cx<float>*)pl->d_specOut, pl->g.spec_total);
     } else if (pl->neqchunks > 0) {
         constexpr int TI = 4, MT = 2;
         const dim3 grid((unsigned)((pl->eq_mh + kBandThreads * MT - 1) / (kBandThreads * MT)), (unsigned)pl->neqchunks, (unsigned)nmaps);
         if (pl->eq_alt)
             band_mac_eq_kernel<TI, MT, 12, 1><<<grid, kBandThreads, 0, st>>>(
                 pl->d_eqchunks, pl->d_north, pl->d_pairs, (const float*)pl->d_W, pl->d_rings, pl->g.R,
-                (const cx<float>*)pl->d_specIn, (cx<float>*)pl->d_specOut, pl->g.spec_total);
+                (const cx<float>*)pl->spec_in(), (cx<float>*)pl->d_specOut, pl->g.spec_total);
         else
             band_mac_eq_kernel<TI, MT, 12, 0><<<grid, kBandThreads, 0, st>>>(
                 pl->d_eqchunks, pl->d_north, pl->d_pairs, (const float*)pl->d_W, pl->d_rings, pl->g.R,
-                (const cx<float>*)pl->d_specIn, (cx<float>*)pl->d_specOut, pl->g.spec_total);
+                (const cx<float>*)pl->spec_in(), (cx<float>*)pl->d_specOut, pl->g.spec_total);
     }
     if (serial) cudaEventRecord(pl->ev_band[3], st);
     launch_uniform_class<12, false>(pl, 2, nmaps, s1);
@@ -690,20 +690,20 @@ void launch_uniform(const arkcos_plan* pl, int nmaps, cudaStream_t st, bool seri
             if (pl->d_G && nmaps > 1)
                 band_mac_capchunk_cached_kernel<4, 2, MULTI><<<dim3(n, (unsigned)((nmaps + 1) / 2)), kBandThreads, 0, s1>>>(
                     items, pl->d_cap_chunks, pl->d_north, pl->d_pairs, pl->d_goff, pl->d_G, pl->d_rings, pl->g.R,
-                    (const cx<float>*)pl->d_specIn, (cx<float>*)pl->d_specOut, pl->g.spec_total, nmaps);
+                    (const cx<float>*)pl->spec_in(), (cx<float>*)pl->d_specOut, pl->g.spec_total, nmaps);
             else if (pl->d_G)
                 band_mac_capchunk_cached_kernel<4, 1, MULTI><<<dim3(n, 1), kBandThreads, 0, s1>>>(
                     items, pl->d_cap_chunks, pl->d_north, pl->d_pairs, pl->d_goff, pl->d_G, pl->d_rings, pl->g.R,
-                    (const cx<float>*)pl->d_specIn, (cx<float>*)pl->d_specOut, pl->g.spec_total, nmaps);
+                    (const cx<float>*)pl->spec_in(), (cx<float>*)pl->d_specOut, pl->g.spec_total, nmaps);
             else if (pl->use_tc) {
                 if (pl->ntc_items[MULTI ? 2 : 1] > 0)
                     band_mac_tc_kernel<MULTI ? 3 : 2><<<dim3((unsigned)pl->ntc_items[MULTI ? 2 : 1], (unsigned)nmaps), kTcThreads, kTcSmemBytes, s1>>>(
                         pl->d_tc_items[MULTI ? 2 : 1], pl->d_tc_chunks, pl->d_tc_tiles, pl->d_tc_cols, pl->d_tc_rings, (const float*)pl->d_W, pl->g.R,
-                        (const cx<float>*)pl->d_specIn, (cx<float>*)pl->d_specOut, pl->g.spec_total);
+                        (const cx<float>*)pl->spec_in(), (cx<float>*)pl->d_specOut, pl->g.spec_total);
             } else
                 band_mac_capchunk_kernel<4, 20, MULTI><<<dim3(n, (unsigned)nmaps), kBandThreads, 0, s1>>>(
                     items, pl->d_cap_chunks, pl->d_north, pl->d_pairs, (const float*)pl->d_W, pl->d_rings, pl->g.R,
-                    (const cx<float>*)pl->d_specIn, (cx<float>*)pl->d_specOut, pl->g.spec_total);
+                    (const cx<float>*)pl->spec_in(), (cx<float>*)pl->d_specOut, pl->g.spec_total);
         };
         launch_cap(std::false_type{}, 0, pl->ncapsingle);
         launch_cap(std::true_type{}, pl->ncapsingle, pl->ncapitems - pl->ncapsingle);
@@ -724,7 +724,7 @@ void launch_fft3(const arkcos_plan* pl, const void* d_in, void* d_out, int nmaps
     if (pl->nfft3[c] > pl->nfft3_bluestein[c]) {      // power-of-two rings: one transform per block
         const int nb = pl->nfft3_bluestein[c], nd = pl->nfft3[c] - nb;
         ring_fft3_direct1_kernel<LOGQ, FWD><<<dim3(2u * (unsigned)nd, (unsigned)nmaps), Fft3<LOGQ>::T, Fft3<LOGQ>::smem_bytes / 2, st>>>(
-            (const float*)d_in, (float*)d_out, g.npix, (cx<float>*)(FWD ? pl->d_specIn : pl->d_specOut), g.spec_total,
+            (const float*)d_in, (float*)d_out, g.npix, (cx<float>*)(FWD ? pl->spec_in() : pl->d_specOut), g.spec_total,
             pl->d_fft3_jobs[c] + nb, (const cx<float>*)pl->d_tw, pl->logPT, (const cx<float>*)pl->d_tw16,
             (const cx<float>*)pl->d_tw3 + pl->tw3_off[c], (const cx<float>*)pl->d_phase);
         njobs = nb;
@@ -734,7 +734,7 @@ void launch_fft3(const arkcos_plan* pl, const void* d_in, void* d_out, int nmaps
     const int ahead = pl->sm_count * Fft3<LOGQ>::MINB;         // resident blocks: the one that will take this block's slot
     if (FWD)
         ring_fft3_forward_kernel<LOGQ><<<grid, Fft3<LOGQ>::T, Fft3<LOGQ>::smem_bytes, st>>>(
-            (const float*)d_in, g.npix, (cx<float>*)pl->d_specIn, g.spec_total, pl->d_rings, pl->d_fft3_jobs[c], pl->d_lens,
+            (const float*)d_in, g.npix, (cx<float>*)pl->spec_in(), g.spec_total, pl->d_rings, pl->d_fft3_jobs[c], pl->d_lens,
             (const cx<float>*)pl->d_tw, pl->logPT, (const cx<float>*)pl->d_tw16, (const cx<float>*)pl->d_tw3 + pl->tw3_off[c],
             (const cx<float>*)pl->d_filt,
             (const cx<float>*)pl->d_chirp, (const cx<float>*)pl->d_phase, ahead);
@@ -769,11 +769,11 @@ void launch_ring_ffts(const arkcos_plan* pl, const void* d_in, void* d_out, int 
         if (FWD) {
             if (pl->fft_bpt == 2)
                 ring_fft_forward_kernel<T, 2><<<gfft, kFftThreads, pl->fft_smem, so>>>(
-                    (const T*)d_in, g.npix, (cx<T>*)pl->d_specIn, g.spec_total, pl->d_rings, pl->d_fft_order, pl->d_lens,
+                    (const T*)d_in, g.npix, (cx<T>*)pl->spec_in(), g.spec_total, pl->d_rings, pl->d_fft_order, pl->d_lens,
                     (const cx<T>*)pl->d_tw, pl->logPT, (const cx<T>*)pl->d_filt, (const cx<T>*)pl->d_chirp, (const cx<T>*)pl->d_phase);
             else
                 ring_fft_forward_kernel<T, 4><<<gfft, kFftThreads, pl->fft_smem, so>>>(
-                    (const T*)d_in, g.npix, (cx<T>*)pl->d_specIn, g.spec_total, pl->d_rings, pl->d_fft_order, pl->d_lens,
+                    (const T*)d_in, g.npix, (cx<T>*)pl->spec_in(), g.spec_total, pl->d_rings, pl->d_fft_order, pl->d_lens,
                     (const cx<T>*)pl->d_tw, pl->logPT, (const cx<T>*)pl->d_filt, (const cx<T>*)pl->d_chirp, (const cx<T>*)pl->d_phase);
         } else {
             if (pl->fft_bpt == 2)
@@ -793,7 +793,9 @@ void launch_ring_ffts(const arkcos_plan* pl, const void* d_in, void* d_out, int 
         }
 }
 
-template <class T> int enqueue_convolve(const arkcos_plan* pl, const void* d_in, void* d_out, int nmaps, cudaStream_t st)
+// skip_forward: the input-ring spectra pl->spec_in() are already there (arkcos_convolve_multi: another plan of the same
+// pixelization made them on this stream); d_in is then only read by the exact_caps direct sum.
+template <class T> int enqueue_convolve(const arkcos_plan* pl, const void* d_in, void* d_out, int nmaps, cudaStream_t st, bool skip_forward = false)
 {
     const HostGeometry& g = pl->g;
     const bool tm = pl->timing != 0;
@@ -821,7 +823,7 @@ template <class T> int enqueue_convolve(const arkcos_plan* pl, const void* d_in,
         if (!pl->opt.cache_kernel_rows) enqueue_rows<T>(pl, st);
     }
     if (tm) cudaEventRecord(pl->ev[1], st);
-    launch_ring_ffts<T, true>(pl, d_in, d_out, nmaps, st);
+    if (!skip_forward) launch_ring_ffts<T, true>(pl, d_in, d_out, nmaps, st);
     if (rows_aside || aside) cudaStreamWaitEvent(st, pl->ev_rows_done, 0);
     if (tm) cudaEventRecord(pl->ev[2], st);
     // the band kernels of the different ring classes write disjoint rings: fork them onto the plan's side streams
@@ -835,13 +837,13 @@ template <class T> int enqueue_convolve(const arkcos_plan* pl, const void* d_in,
     if (serial) cudaEventRecord(pl->ev_band[0], st);
     if (pl->nitems[0] > 0)
         band_mac_general_kernel<T, 16><<<dim3((unsigned)pl->nitems[0], (unsigned)nmaps), kBandThreads, 0, s0>>>(
-            pl->d_items[0], pl->d_north, pl->d_pairs, (const T*)pl->d_W, pl->d_rings, g.R, (const cx<T>*)pl->d_specIn,
+            pl->d_items[0], pl->d_north, pl->d_pairs, (const T*)pl->d_W, pl->d_rings, g.R, (const cx<T>*)pl->spec_in(),
             (cx<T>*)pl->d_specOut, g.spec_total, pl->opt.variant == 1 ? 1 : 0);
     if (serial) cudaEventRecord(pl->ev_band[1], st);
     if (pl->npole > 0)
         band_mac_pole_kernel<T, 16><<<dim3((unsigned)pl->npole, (unsigned)nmaps), kPoleThreads,
                                        2 * (size_t)(pl->pole_mh + 1) * sizeof(cx<T>), s0>>>(
-            pl->d_pole, pl->d_north, pl->d_pairs, (const T*)pl->d_W, pl->d_rings, g.R, (const cx<T>*)pl->d_specIn,
+            pl->d_pole, pl->d_north, pl->d_pairs, (const T*)pl->d_W, pl->d_rings, g.R, (const cx<T>*)pl->spec_in(),
             (cx<T>*)pl->d_specOut, g.spec_total);
     if (serial) cudaEventRecord(pl->ev_band[2], st);
     launch_uniform(pl, nmaps, st, serial);
@@ -1083,6 +1085,42 @@ int arkcos_convolve(const arkcos_plan* pl, const void* d_in, void* d_out, int nm
     if (dev != pl->device) return fail(ARKCOS_INVALID_ARG, "the current device is not the device the plan was created on");
     return pl->dtype == ARKCOS_F32 ? enqueue_convolve<float>(pl, d_in, d_out, nmaps, st)
                                    : enqueue_convolve<double>(pl, d_in, d_out, nmaps, st);
+}
+
+int arkcos_convolve_multi(const arkcos_plan* const* plans, int nkernels, const void* d_in, void* d_out, int nmaps, void* cuda_stream)
+{
+    if (!plans || nkernels < 1 || !d_in || !d_out) return fail(ARKCOS_INVALID_ARG, "NULL argument or nkernels < 1");
+    const arkcos_plan* p0 = plans[0];
+    if (!p0) return fail(ARKCOS_INVALID_ARG, "NULL plan");
+    for (int k = 0; k < nkernels; ++k) {
+        const arkcos_plan* pk = plans[k];
+        if (!pk || pk->tables_only) return fail(ARKCOS_INVALID_ARG, "NULL or tables-only plan");
+        // one forward transform serves every kernel only if the ring spectra have one layout and one meaning
+        if (pk->pix.kind != p0->pix.kind || pk->pix.ntheta != p0->pix.ntheta || pk->pix.nphi != p0->pix.nphi ||
+            pk->pix.nside != p0->pix.nside || pk->dtype != p0->dtype || pk->device != p0->device)
+            return fail(ARKCOS_INVALID_ARG, "arkcos_convolve_multi: the plans must share pixelization, dtype and device");
+        if (nmaps < 1 || nmaps > pk->max_nmaps) return fail(ARKCOS_INVALID_ARG, "nmaps must be in [1, max_nmaps] of every plan");
+        for (int q = 0; q < k; ++q)
+            if (plans[q] == pk) return fail(ARKCOS_INVALID_ARG, "arkcos_convolve_multi: a plan appears twice (one workspace per plan)");
+    }
+    const size_t bytes = (size_t)nmaps * (size_t)p0->g.npix * elem_size(p0->dtype);
+    const char *a = (const char*)d_in, *b = (const char*)d_out;
+    if (a < b + bytes * (size_t)nkernels && b < a + bytes) return fail(ARKCOS_INVALID_ARG, "d_in and d_out overlap");
+    if (((uintptr_t)d_in | (uintptr_t)d_out | (uintptr_t)bytes) & 15) return fail(ARKCOS_INVALID_ARG, "d_in / d_out / nmaps * npix * element size must be multiples of 16 bytes");
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    int dev = -1;
+    CUDA_TRY(cudaGetDevice(&dev));
+    if (dev != p0->device) return fail(ARKCOS_INVALID_ARG, "the current device is not the device the plans were created on");
+    for (int k = 0; k < nkernels; ++k) {
+        const arkcos_plan* pk = plans[k];
+        void* out_k = (char*)d_out + (size_t)k * bytes;
+        pk->spec_in_shared = k > 0 ? p0->d_specIn : nullptr;
+        const int rc = pk->dtype == ARKCOS_F32 ? enqueue_convolve<float>(pk, d_in, out_k, nmaps, st, k > 0)
+                                               : enqueue_convolve<double>(pk, d_in, out_k, nmaps, st, k > 0);
+        pk->spec_in_shared = nullptr;
+        if (rc) return rc;
+    }
+    return ARKCOS_OK;
 }
 
 int arkcos_convolve_host(const arkcos_plan* pl, const void* h_in, void* h_out, int nmaps, void* cuda_stream)

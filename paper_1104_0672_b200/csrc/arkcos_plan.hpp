@@ -93,6 +93,9 @@ struct arkcos_plan {
     void* d_W = nullptr;         // T[nsamples] kernel rows
     void* d_specIn = nullptr;    // cx<T>[max_nmaps][spec_total]
     void* d_specOut = nullptr;
+    // arkcos_convolve_multi: the band kernels of this plan read the input-ring spectra another plan made
+    mutable void* spec_in_shared = nullptr;
+    void* spec_in() const { return spec_in_shared ? spec_in_shared : d_specIn; }
     // lazily allocated staging for arkcos_convolve_host
     mutable void* d_stage_in = nullptr;
     mutable void* d_stage_out = nullptr;

@@ -441,3 +441,72 @@ def test_cached_spectra_long_equatorial_rows():
     rings = np.unique(np.concatenate([rings, [398, 400, 403, 509, 511, 514]]))
     ref1 = direct.direct_sum(geom, tab, tmax, x.astype(np.float64), out_rings=rings)
     assert frms(take_rings(geom, out, rings), ref1) <= 1e-6
+
+
+# ------------------------------------------------------------------ several kernels, one forward transform --------
+
+def test_multi_kernel_batching_shares_forward_ffts():
+    """arkcos_convolve_multi (PAPER.md:19-21 wavelet banks, :233 asymmetric beams as O(10) radial terms): K = 4 kernels on one
+    map pair; every kernel's result equals its own arkcos_convolve (same kernels on the same spectra) and the brute-force sum."""
+    nside = 256
+    geom = geometry.healpix_ring(nside)
+    px = np.sqrt(4 * np.pi / geom.npix)
+    kernels = [("gauss", inputs.gaussian_table(3.0 * px, 9.0 * px), 9.0 * px),
+               ("mexhat_a", inputs.mexican_hat_table(1.6 * px, 8.0 * px), 8.0 * px),
+               ("mexhat_b", inputs.mexican_hat_table(2.4 * px, 12.0 * px), 12.0 * px),
+               ("disc", inputs.tophat_table(6.0 * px), 6.0 * px)]
+    nmaps = 2
+    x = inputs.white_noise_maps(geom.npix, 7, nmaps)
+    plans = [arkcos.Plan(("healpix", nside), tab, tmax, arkcos.F32, max_nmaps=nmaps) for _, tab, tmax in kernels]
+    d_in = torch.from_numpy(x).cuda()
+    d_out = torch.full((len(plans), nmaps, geom.npix), float("nan"), device="cuda", dtype=torch.float32)
+    st = torch.cuda.current_stream().cuda_stream
+    arkcos.arkcos_convolve_multi(plans, d_in.data_ptr(), d_out.data_ptr(), nmaps, st)
+    torch.cuda.synchronize()
+    multi = d_out.cpu().numpy()
+    assert np.isfinite(multi).all()
+    rings = sample_rings(geom, extra=(nside - 2, nside - 1, nside, nside + 1, 3 * nside - 1), nrand=6, seed=5)
+    eq_rings = np.array([r for r in rings if nside + 16 <= r <= 3 * nside - 18])
+    for k, (name, tab, tmax) in enumerate(kernels):
+        single, _ = gpu_convolve(("healpix", nside), tab, tmax, x, plan=plans[k])
+        # same kernels on the same spectra: bit-equal wherever the result has a fixed summation order (belt rings, cap
+        # rings whose grid spans one period); a cap ring whose grid spans several periods folds 3-4 terms per coefficient
+        # with atomic additions (DESIGN.md section 5), so there only to rounding
+        belt = slice(int(geom.offset[nside + 16]), int(geom.offset[3 * nside - 17]))
+        assert np.array_equal(multi[k][:, belt], single[:, belt]), name
+        assert frms(multi[k], single) <= 1e-7, name
+        ref = direct.direct_sum(geom, tab, tmax, x.astype(np.float64), out_rings=rings)
+        got = take_rings(geom, multi[k], rings)
+        if name == "disc":        # the Fourier scheme only suppresses ringing in the caps (PAPER.md:219): exact in the belt
+            ref_eq = direct.direct_sum(geom, tab, tmax, x.astype(np.float64), out_rings=eq_rings)
+            assert frms(take_rings(geom, multi[k], eq_rings), ref_eq) <= 1e-6
+        else:
+            assert frms(got, ref) <= (3e-5 if name.startswith("mexhat") else 1e-5), name
+    # argument errors: a plan twice, plans of different pixelizations
+    with pytest.raises(arkcos.ArkcosError):
+        arkcos.arkcos_convolve_multi([plans[0], plans[0]], d_in.data_ptr(), d_out.data_ptr(), nmaps, st)
+    other = arkcos.Plan(("healpix", 128), kernels[0][1], kernels[0][2], arkcos.F32, max_nmaps=nmaps)
+    with pytest.raises(arkcos.ArkcosError):
+        arkcos.arkcos_convolve_multi([plans[0], other], d_in.data_ptr(), d_out.data_ptr(), nmaps, st)
+
+
+@pytest.mark.parametrize("tc", [0, 1], ids=["tensor_cores", "fp32_only"])
+def test_repeatability(tc):
+    """Two calls on one plan give the same bits wherever the summation order is fixed: everywhere for a plan whose cap
+    grids span a single period (here: all rings of 512+ pixels at nside 512 with a Gaussian), and on belt rings always.
+    The fold of a grid spanning several periods (rings next to the poles; hard-edged kernels) adds 3-4 terms per
+    coefficient atomically: equal to rounding only (documented in DESIGN.md section 5)."""
+    nside = 512
+    geom = geometry.healpix_ring(nside)
+    px = np.sqrt(4 * np.pi / geom.npix)
+    tab, tmax = inputs.gaussian_table(2.91 * px, 3 * 2.91 * px), 3 * 2.91 * px
+    x = inputs.white_noise(geom.npix, 8)
+    a, plan = gpu_convolve(("healpix", nside), tab, tmax, x, no_tensor_cores=tc)
+    b, _ = gpu_convolve(("healpix", nside), tab, tmax, x, plan=plan)
+    mp = plan_mprime(plan, geom, tmax)
+    # belt rings use their own length as the grid; a cap ring's grid spans one period when M'/2 < N
+    single = [r for r in range(geom.nrings) if geom.n[r] == 4 * nside or (geom.n[r] >= 512 and mp[r] // 2 < geom.n[r])]
+    assert len(single) > geom.nrings * 0.85
+    for r in single:
+        assert np.array_equal(a[geom.ring_slice(r)], b[geom.ring_slice(r)]), r
+    assert frms(a, b) <= 1e-7

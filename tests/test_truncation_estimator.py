@@ -93,12 +93,12 @@ def test_chosen_cut_carries_the_predicted_error_on_the_gpu():
     import torch
     nside = 256
     npix = 12 * nside * nside
-    fwhm = 40 * inputs.ARCMIN
+    fwhm = 80 * inputs.ARCMIN          # sigma = 2.5 pixels: the annulus that is cut away is sampled by many pixels
     tmax = 3.5 * fwhm * inputs.FWHM_TO_SIGMA
     n, ngrid = 4097, 64
     tab = inputs.gaussian_table(fwhm, tmax, n)
-    lmax = 8 * nside
-    cl = np.full(lmax + 1, 4 * np.pi / npix)
+    lmax = 64 * nside                  # pixel white noise is not band-limited, and the annulus that is cut away has sharp edges:
+    cl = np.full(lmax + 1, 4 * np.pi / npix)     # dK_l^2 (2l+1) falls off as 1/l^2 only, the sum needs l far beyond the pixel scale
     cut, s2, sig = arkcos.arkcos_kernel_choose_cut(tab, tmax, cl, 3e-3, ngrid)
     g = round(cut / tmax * ngrid)
     assert 0 < g < ngrid
@@ -107,5 +107,6 @@ def test_chosen_cut_carries_the_predicted_error_on_the_gpu():
     full = arkcos.convolve_torch(arkcos.Plan(("healpix", nside), tab, tmax, arkcos.F32), x).double()
     part = arkcos.convolve_torch(arkcos.Plan(("healpix", nside), tab[:ncut], cut, arkcos.F32), x).double()
     measured = float(((full - part) ** 2).sum() / (full ** 2).sum())
-    assert measured <= (3e-3) ** 2 * 1.2
-    assert abs(measured / (s2 / sig) - 1) < 0.15, (measured, s2 / sig)
+    print('measured', measured, 'predicted', s2 / sig)
+    assert measured <= (3e-3) ** 2 * 1.3
+    assert abs(measured / (s2 / sig) - 1) < 0.12, (measured, s2 / sig)
