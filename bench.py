@@ -38,10 +38,10 @@ TRAFFIC = {  # profiles/r1_v8_final.md (ncu --set full, config 4, one map); FFT 
 UNIT = "Mpix/s"
 
 
-def workload(cfg: int):
+def workload(cfg: int, which: int = 1):
     c = inputs.config(cfg)
     if cfg == 5:
-        k = c["kernels"][1]
+        k = c["kernels"][which]
         c = dict(c, **k)
     tab = inputs.kernel_table(c)
     pix = c["pix"]
@@ -153,7 +153,7 @@ def run_ours(args):
     torch.cuda.set_device(local)
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
-    c, tab, x, npix, nmaps, name = workload(args.cfg)
+    c, tab, x, npix, nmaps, name = workload(args.cfg, args.cfg5_kernel)
     if world > 1:                       # every rank its own map(s): same shape, different seed
         mine = shard_range(nmaps * world, world, rank)
         x = np.stack([inputs.white_noise(npix, args.cfg, k) for k in mine])
@@ -182,6 +182,26 @@ def run_ours(args):
         for _ in range(args.steps):
             step()
         barrier()
+        return
+    if args.quick:                      # device-resident timing only: whole step, stages, band kernels one after the other
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(args.steps):
+            step()
+        e1.record()
+        barrier()
+        out = {"ms_per_step": e0.elapsed_time(e1) / args.steps}
+        plan.set_timing(2)
+        acc, stage = None, {}
+        for _ in range(args.steps):
+            step()
+            cur = [b[2] for b in plan.band_kernels(with_timing=True)]
+            acc = cur if acc is None else [a + b for a, b in zip(acc, cur)]
+            for k, v in plan.get_timing().items():
+                stage[k] = stage.get(k, 0.0) + v / args.steps
+        out["stage_ms_serial"] = stage
+        out["band_ms"] = {b[0]: a / args.steps for b, a in zip(plan.band_kernels(), acc) if a > 0.5e-3 * args.steps}
+        print(json.dumps(out))
         return
     sampler = ClockSampler(local) if rank == 0 else None
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -331,6 +351,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--cfg", type=int, default=4)
     ap.add_argument("--profile", action="store_true", help="warm-up + steps of arkcos_convolve only (the command ncu wraps)")
+    ap.add_argument("--cfg5-kernel", type=int, default=1, help="--cfg 5: 0 = top-hat disc, 1 = cut Mexican hat")
+    ap.add_argument("--quick", action="store_true", help="device-resident timing of the step, its stages and band kernels only")
     ap.add_argument("--oracle-rings", type=int, default=2048, help="output rings in the CPU-oracle sample")
     args = ap.parse_args()
     if args.impl == "reference":

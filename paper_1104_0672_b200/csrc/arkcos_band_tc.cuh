@@ -19,21 +19,20 @@
 // KIND 2: runs of cap rings with one M', single period (M'/2 < N of every ring involved);  3: several periods.
 // The fold of the cap kinds and all sign rules are those of band_mac_capchunk_kernel (arkcos_band.cuh).
 #pragma once
+#ifndef ARKCOS_ABL
+#define ARKCOS_ABL 0
+#endif
 #include "arkcos_band.cuh"
+#include "arkcos_band_tc.hpp"
 
 namespace arkcos {
 
-constexpr int kTcMT = 2;                   // blocks of 128 modes (TMEM lanes) per thread block, one consumer warpgroup each
-constexpr int kTcConsumers = 128 * kTcMT;  // multiply-accumulate threads: thread = mode
-constexpr int kTcProducers = 128;          // B-operand threads: thread = accumulator column; its thread 0 issues the MMAs
-constexpr int kTcThreads = kTcConsumers + kTcProducers;
-constexpr int kTcTI = 4;                   // output rings per tile
-constexpr int kTcJW = 32;                  // input rings a tile's window can hold
-constexpr int kTcN = kTcTI * kTcJW;        // accumulator columns per block of modes
-constexpr int kTcK = 24;                   // sample positions u per row
-constexpr int kTcChunkRings = 24;          // longest run of cap rings handed to one block
-// cosine operand per block of modes, two stages of the row operand, coefficient window per block of modes
-constexpr size_t kTcSmemBytes = (size_t)(kTcMT * 2 * (kTcK / 4) * 128 + 2 * 2 * (kTcK / 4) * kTcN + kTcMT * kTcJW * 128) * 16;
+#if ARKCOS_ABL == 7
+__device__ unsigned long long g_dbg[4096];
+#define DBG(slot) do { if (blockIdx.x == 200 && k < 30) g_dbg[k * 16 + (slot)] = clock64(); } while (0)
+#else
+#define DBG(slot) do {} while (0)
+#endif
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
@@ -89,19 +88,6 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity)
                      : "=r"(done) : "r"(smem_u32(bar)), "r"(parity) : "memory");
 }
 
-// Plan-time tables of the tensor-core band kernel (no pointer chasing through the ring-pair table inside the kernel):
-// a run of rings, its tiles of up to TI output rings, per tile one word per accumulator column, and two words per ring.
-struct TcChunk { int i0, n, M, multi, tile0; };       // run of output rings i0 .. i0 + n - 1 with one grid length M; first tile
-struct TcItem { int chunk, bx; };                      // one thread block: run, block of 128 * kTcMT modes
-struct __align__(16) TcTile {                          // window of input rings, first output ring, output rings of the tile,
-    int jlo, jhi, i0, nti;                             // and per output ring its spectrum offsets (ring, mirror image) and N_i | shifted << 31
-    int offN[4], offS[4], n_sh[4];
-};
-struct TcRing { int offN, offS, n_sh; uint32_t magic; };   // spectrum offsets of ring j and of its mirror image, N_j | shifted << 31, ceil(2^32 / N_j)
-// column word: bits 0-24 first sample of the row in W (units of four floats), bits 25-30 samples, bit 31 half-step parity;
-// 0xffffffff: no such ring pair (zero row)
-constexpr uint32_t kTcNoPair = 0xffffffffu;
-
 // Warp-specialised: the producer warpgroup (threads 256 .. 383, thread = accumulator column) converts the rows of tile
 // k + 1 into the B operand (two stages) and its first thread issues the MMAs of both blocks of modes into TMEM stage
 // (k + 1) & 1, while the two consumer warpgroups (thread = mode) multiply-accumulate tile k out of TMEM stage k & 1.
@@ -123,6 +109,8 @@ band_mac_tc_kernel(const TcItem* __restrict__ items, const TcChunk* __restrict__
     __shared__ __align__(8) uint64_t bar_full[2], bar_empty[2], bar_rows[2];
     __shared__ uint32_t s_tmem;
     __shared__ int sUmax[2];
+    __shared__ TcTile sTiles[kTcMaxTiles];                       // records of the run's tiles and of the rings of their windows
+    __shared__ TcRing sRings[kTcMaxWindow];
 
     const int t = (int)threadIdx.x, warp = t >> 5;
     const TcItem it = items[blockIdx.x];
@@ -133,6 +121,22 @@ band_mac_tc_kernel(const TcItem* __restrict__ items, const TcChunk* __restrict__
     const int wg = t >> 7, l128 = t & 127;                       // consumer: block of modes, lane within it
     const int m_raw = (it.bx * MT + wg) * 128 + l128, m = min(m_raw, Mh);
 
+    const cx<float>* __restrict__ in = specIn + (int64_t)blockIdx.y * spec_stride;
+    cx<float>* __restrict__ out = specOut + (int64_t)blockIdx.y * spec_stride;
+    const uint32_t sv0 = smem_u32(sV + wg * JW * 128 + l128);      // this thread's slot 0; slot s at + 2048 s bytes
+    // periodic extension of a stored half spectrum (reading R8): m = w N_j + r; above N_j/2 the conjugate of N_j - r
+    auto ext_index = [](int mm, int nj_sh, uint32_t magic) {
+        const int Nj = nj_sh & 0x7fffffff, w = MULTI ? (int)__umulhi((uint32_t)mm, magic) : 0, r = mm - w * Nj;
+        return 2 * r > Nj ? Nj - r : r;
+    };
+    auto fetch_ring = [&](int j, const TcRing& rj) {
+        const int idx = CAP ? ext_index(m, rj.n_sh, rj.magic) : m;
+        const uint32_t dst = sv0 + 2048u * (uint32_t)(j & (JW - 1));
+#if ARKCOS_ABL != 6
+        asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst), "l"(in + rj.offN + idx) : "memory");
+        asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst + 8u), "l"(in + rj.offS + idx) : "memory");
+#endif
+    };
     if (!producer) {
         // ---- A operand: the cosines of this warpgroup's 128 modes, split into TF32 hi + lo ----------------------------
         float4* sAw = sA + wg * 2 * KC * 128;
@@ -155,6 +159,17 @@ band_mac_tc_kernel(const TcItem* __restrict__ items, const TcChunk* __restrict__
         // the window starts out finite: accumulator columns past the tile's window are exact zeros, but 0 * garbage is not
         for (int sl = 0; sl < JW; ++sl) sV[(wg * JW + sl) * 128 + l128] = make_float4(0.f, 0.f, 0.f, 0.f);
     }
+    const int jbase = tiles[ch.tile0].jlo;                      // first ring of the run's first window
+    if (producer) {
+        const int c = t - kTcConsumers;
+        const int4* __restrict__ src = reinterpret_cast<const int4*>(tiles + ch.tile0);
+        int4* dst = reinterpret_cast<int4*>(sTiles);
+        for (int q = c; q < ntiles * (int)(sizeof(TcTile) / 16); q += kTcProducers) dst[q] = src[q];
+        const int jlast = tiles[ch.tile0 + ntiles - 1].jhi;
+        const int4* __restrict__ rsrc = reinterpret_cast<const int4*>(ringtab + jbase);
+        int4* rdst = reinterpret_cast<int4*>(sRings);
+        for (int q = c; q <= jlast - jbase; q += kTcProducers) rdst[q] = rsrc[q];
+    }
     if (t == 0) {
 #pragma unroll
         for (int s = 0; s < 2; ++s) {
@@ -165,7 +180,7 @@ band_mac_tc_kernel(const TcItem* __restrict__ items, const TcChunk* __restrict__
         }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
-    if (warp == 0) {
+    if (warp == kTcConsumers / 32) {                             // the first producer warp owns the tensor-memory allocation
         asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&s_tmem)), "r"(2 * MT * N));
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::);
     }
@@ -179,30 +194,37 @@ band_mac_tc_kernel(const TcItem* __restrict__ items, const TcChunk* __restrict__
         const int c = t - kTcConsumers;
         // instruction descriptor: D = f32, A = B = tf32, both K-major, N >> 3 at bit 17, M >> 4 at bit 24
         constexpr uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(N >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
-        float4 wrow[KC];
-        auto load_row = [&](uint32_t cw) {
+        // Rows travel two tiles ahead of their conversion: the raw samples of tile k sit in buffer k & 1, which is refilled
+        // with tile k + 2 once tile k has been converted (the loads have a whole tile to arrive); column words three ahead.
+        float4 raw[2][KC];
+        auto load_row = [&](float4 (&dst)[KC], uint32_t cw) {
             const bool have = cw != kTcNoPair;
             const int cnt4 = have ? (int)(((cw >> 25) & 63u) + 3u) & ~3 : 0;
             const float* __restrict__ w = W + (size_t)(cw & 0x1ffffffu) * 4;
-#pragma unroll
+    #pragma unroll
             for (int kc = 0; kc < KC; ++kc) {
-                wrow[kc] = make_float4(0.f, 0.f, 0.f, 0.f);
-                if (ALT) {                                       // u = 4 kc .. 4 kc + 3 holds samples 2 kc, 2 kc + 1 at parity par
+                dst[kc] = make_float4(0.f, 0.f, 0.f, 0.f);
+                if (ALT) {                                       // two samples per group of four positions (see convert)
                     if (2 * kc < cnt4) {
                         const float2 ww = *reinterpret_cast<const float2*>(w + 2 * kc);
-                        wrow[kc] = (cw >> 31) ? make_float4(0.f, ww.x, 0.f, ww.y) : make_float4(ww.x, 0.f, ww.y, 0.f);
+                        dst[kc].x = ww.x;
+                        dst[kc].y = ww.y;
                     }
-                } else if (4 * kc < cnt4) wrow[kc] = *reinterpret_cast<const float4*>(w + 4 * kc);
+                } else if (4 * kc < cnt4) dst[kc] = *reinterpret_cast<const float4*>(w + 4 * kc);
             }
         };
         const uint32_t* __restrict__ colp = cols + (size_t)ch.tile0 * N + c;
-        uint32_t colw = colp[0];
-        uint32_t colw_next = ntiles > 1 ? colp[N] : kTcNoPair;
-        load_row(colw);
-        for (int k = 0; k < ntiles; ++k) {
+        auto col_word = [&](int k) { return k < ntiles ? colp[(size_t)k * N] : kTcNoPair; };
+        uint32_t cwv[2] = {col_word(0), col_word(1)};            // column words of the tiles whose rows sit in raw[0], raw[1]
+        uint32_t cw_ahead = col_word(2);                         // column word of the tile loaded next
+        load_row(raw[0], cwv[0]);
+        load_row(raw[1], cwv[1]);
+        auto tile_step = [&](int k, float4 (&rw)[KC], uint32_t& colw) {
             const int s = k & 1;
             const uint32_t ph = (uint32_t)(k >> 1) & 1u;
+            if (c == 0) DBG(0);
             mbar_wait(&bar_rows[s], ph ^ 1u);                    // the MMAs of tile k - 2 have read this stage
+            if (c == 0) DBG(1);
             float4* sBs = sB + s * 2 * KC * N;
             if (colw != kTcNoPair) {
                 const int cnt = (int)((colw >> 25) & 63u);
@@ -211,20 +233,19 @@ band_mac_tc_kernel(const TcItem* __restrict__ items, const TcChunk* __restrict__
             }
 #pragma unroll
             for (int kc = 0; kc < KC; ++kc) {
-                const float4 w = wrow[kc];
+                float4 w = rw[kc];
+                // half-step parity alternates: positions u = 4 kc .. 4 kc + 3 hold samples 2 kc, 2 kc + 1 at parity par
+                if (ALT) w = (colw >> 31) ? make_float4(0.f, w.x, 0.f, w.y) : make_float4(w.x, 0.f, w.y, 0.f);
                 const float4 h = make_float4(tf32_rn(w.x), tf32_rn(w.y), tf32_rn(w.z), tf32_rn(w.w));
                 sBs[kc * N + c] = h;
                 sBs[(KC + kc) * N + c] = make_float4(tf32_rn(w.x - h.x), tf32_rn(w.y - h.y), tf32_rn(w.z - h.z), tf32_rn(w.w - h.w));
             }
-            if (k + 1 < ntiles) {                                // rows of the next tile, column word of the one after
-                colw = colw_next;
-                load_row(colw);
-                colw_next = k + 2 < ntiles ? colp[(size_t)(k + 2) * N] : kTcNoPair;
-            }
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
             asm volatile("bar.sync 1, %0;" ::"n"(kTcProducers) : "memory");
             if (c == 0) {
+                DBG(2);
                 mbar_wait(&bar_empty[s], ph ^ 1u);               // the consumers have read TMEM stage s (tile k - 2)
+                DBG(3);
                 asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
                 const int ksteps = min(K / 8, (sUmax[s] + 7) >> 3);
                 sUmax[s] = 1;
@@ -239,37 +260,44 @@ band_mac_tc_kernel(const TcItem* __restrict__ items, const TcChunk* __restrict__
                         for (int ks = 0; ks < ksteps; ++ks) {
                             const uint64_t da = tc_smem_desc(a0 + (uint32_t)(((mt * 2 + ha) * KC + 2 * ks) * 128 * 16), 128 * 16, 128);
                             const uint64_t db = tc_smem_desc(b0 + (uint32_t)((hb * KC + 2 * ks) * N * 16), N * 16, 128);
+#if ARKCOS_ABL != 1
                             tc_mma_tf32(d, da, db, idesc, acc_flag);
+#endif
                             acc_flag = 1;
                         }
                     }
                 }
                 tc_commit(&bar_full[s]);
                 tc_commit(&bar_rows[s]);
+                DBG(4);
             }
+            // this buffer takes the rows of tile k + 2 (issued behind the fence, which waits for loads in flight)
+            if (k + 2 < ntiles) {
+                colw = cw_ahead;
+                load_row(rw, colw);
+                cw_ahead = col_word(k + 3);
+            }
+        };
+        for (int k = 0; k < ntiles; k += 2) {
+            tile_step(k, raw[0], cwv[0]);
+            if (k + 1 < ntiles) tile_step(k + 1, raw[1], cwv[1]);
+        }
+        // the first producer warp frees the tensor memory as soon as the consumers have read the last two tiles (they
+        // go on to write their results; the block does not meet again)
+        if (warp == kTcConsumers / 32) {
+            for (int k = max(ntiles - 2, 0); k < ntiles; ++k) mbar_wait(&bar_empty[k & 1], (uint32_t)(k >> 1) & 1u);
+            asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+            __syncwarp();
+            asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"(2 * MT * N));
         }
     } else {
         // =================================== multiply-accumulate over input rings ==============================
-        const cx<float>* __restrict__ in = specIn + (int64_t)blockIdx.y * spec_stride;
-        cx<float>* __restrict__ out = specOut + (int64_t)blockIdx.y * spec_stride;
-        const uint32_t sv0 = smem_u32(sV + wg * JW * 128 + l128);      // this thread's slot 0; slot s at + 2048 s bytes
-        // periodic extension of a stored half spectrum (reading R8): m = w N_j + r; above N_j/2 the conjugate of N_j - r
-        auto ext_index = [](int mm, int nj_sh, uint32_t magic) {
-            const int Nj = nj_sh & 0x7fffffff, w = MULTI ? (int)__umulhi((uint32_t)mm, magic) : 0, r = mm - w * Nj;
-            return 2 * r > Nj ? Nj - r : r;
-        };
-        auto fetch_ring = [&](int j, const TcRing& rj) {
-            const int idx = CAP ? ext_index(m, rj.n_sh, rj.magic) : m;
-            const uint32_t dst = sv0 + 2048u * (uint32_t)(j & (JW - 1));
-            asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst), "l"(in + rj.offN + idx) : "memory");
-            asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst + 8u), "l"(in + rj.offS + idx) : "memory");
-        };
-        TcTile tl = tiles[ch.tile0];
+        TcTile tl = sTiles[0];
         // first tile: its whole window enters
         for (int j0 = tl.jlo; j0 <= tl.jhi; j0 += 4) {
             TcRing rr[4];
 #pragma unroll
-            for (int q = 0; q < 4; ++q) rr[q] = ringtab[min(j0 + q, tl.jhi)];
+            for (int q = 0; q < 4; ++q) rr[q] = sRings[min(j0 + q, tl.jhi) - jbase];
 #pragma unroll
             for (int q = 0; q < 4; ++q) if (j0 + q <= tl.jhi) fetch_ring(j0 + q, rr[q]);
         }
@@ -284,12 +312,14 @@ band_mac_tc_kernel(const TcItem* __restrict__ items, const TcChunk* __restrict__
             // records of the next tile and of the rings that enter the window with it: loaded now, used after this tile
             TcRing nx[4];
             if (k + 1 < ntiles) {
-                tl = tiles[ch.tile0 + k + 1];
+                tl = sTiles[k + 1];
 #pragma unroll
-                for (int q = 0; q < 4; ++q) nx[q] = ringtab[min(jhave + 1 + q, R - 1)];
+                for (int q = 0; q < 4; ++q) nx[q] = sRings[min(jhave + 1 + q, tl.jhi) - jbase];
             }
             bool landed = false;
+            if (t == 0) DBG(8);
             mbar_wait(&bar_full[s], ph);
+            if (t == 0) DBG(9);
             asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
 
             float2 acc[TI][2];
@@ -297,8 +327,29 @@ band_mac_tc_kernel(const TcItem* __restrict__ items, const TcChunk* __restrict__
             for (int ii = 0; ii < TI; ++ii) acc[ii][0] = acc[ii][1] = make_float2(0.f, 0.f);
             const uint32_t tbase = tmem + ((uint32_t)((warp & 3) * 32) << 16) + (uint32_t)((s * MT + wg) * N);
             uint32_t soff = ((uint32_t)jlo & (JW - 1)) * 2048u;          // byte offset of the slot of ring jlo + jj
+            // cap runs: the periodic extension conjugates on reflection, and a shifted ring changes sign on reflection and on
+            // every odd period (reading R8): applied once, in place, when the coefficients of a ring have landed
+            auto land = [&]() {
+                cp_async_wait<0>();
+                landed = true;
+                if (CAP) {
+                    for (int jj = nold; jj < jw; ++jj) {
+                        const TcRing rj = sRings[jlo + jj - jbase];
+                        const int Nj = rj.n_sh & 0x7fffffff, w = MULTI ? (int)__umulhi((uint32_t)m, rj.magic) : 0, r = m - w * Nj;
+                        const bool refl = 2 * r > Nj;
+                        const uint32_t sre = (rj.n_sh < 0 && (refl != ((w & 1) != 0))) ? 0x80000000u : 0u;
+                        const uint32_t sim = sre ^ (refl ? 0x80000000u : 0u);
+                        if (sre | sim) {
+                            const uint32_t a = sv0 + 2048u * (uint32_t)((jlo + jj) & (JW - 1));
+                            uint32_t x, y, z, ww;
+                            asm volatile("ld.shared.v4.b32 {%0, %1, %2, %3}, [%4];" : "=r"(x), "=r"(y), "=r"(z), "=r"(ww) : "r"(a));
+                            asm volatile("st.shared.v4.b32 [%4], {%0, %1, %2, %3};" ::"r"(x ^ sre), "r"(y ^ sim), "r"(z ^ sre), "r"(ww ^ sim), "r"(a) : "memory");
+                        }
+                    }
+                }
+            };
             auto load_v = [&](float4 (&v)[4], int jj0) {
-                if (!landed && jj0 + 4 > nold) { cp_async_wait<0>(); landed = true; }
+                if (!landed && jj0 + 4 > nold) land();
 #pragma unroll
                 for (int q = 0; q < 4; ++q) {
                     asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v[q].x), "=f"(v[q].y), "=f"(v[q].z), "=f"(v[q].w) : "r"(sv0 + soff));
@@ -308,21 +359,15 @@ band_mac_tc_kernel(const TcItem* __restrict__ items, const TcChunk* __restrict__
             auto mac4 = [&](const uint32_t (&g)[16], float4 (&v)[4], int jj0) {
 #pragma unroll
                 for (int q = 0; q < 4; ++q) {
-                    if (CAP) {
-                        // reflection conjugates; a shifted ring changes sign on reflection and on every odd period
-                        const TcRing rj = ringtab[min(jlo + jj0 + q, R - 1)];
-                        const int Nj = rj.n_sh & 0x7fffffff, w = MULTI ? (int)__umulhi((uint32_t)m, rj.magic) : 0, r = m - w * Nj;
-                        const bool refl = 2 * r > Nj;
-                        const uint32_t sre = (rj.n_sh < 0 && (refl != ((w & 1) != 0))) ? 0x80000000u : 0u;
-                        const uint32_t sim = sre ^ (refl ? 0x80000000u : 0u);
-                        v[q].x = __uint_as_float(__float_as_uint(v[q].x) ^ sre); v[q].y = __uint_as_float(__float_as_uint(v[q].y) ^ sim);
-                        v[q].z = __uint_as_float(__float_as_uint(v[q].z) ^ sre); v[q].w = __uint_as_float(__float_as_uint(v[q].w) ^ sim);
-                    }
 #pragma unroll
                     for (int ii = 0; ii < TI; ++ii) {
                         const float G = __uint_as_float(g[q * TI + ii]);
+#if ARKCOS_ABL == 2
+                        if (ii == 0) acc[ii][0].x += G + v[q].x + v[q].z;
+#else
                         acc[ii][0] = ffma2(make_float2(G, G), make_float2(v[q].x, v[q].y), acc[ii][0]);
                         acc[ii][1] = ffma2(make_float2(G, G), make_float2(v[q].z, v[q].w), acc[ii][1]);
+#endif
                     }
                 }
             };
@@ -334,17 +379,26 @@ band_mac_tc_kernel(const TcItem* __restrict__ items, const TcChunk* __restrict__
                 load_v(va, 0);
                 for (int jj0 = 0; jj0 < jw; jj0 += 8) {
                     asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#if ARKCOS_ABL != 3
                     tc_ld16(gb, tbase + (uint32_t)(min(jj0 + 4, JW - 4) * TI));
+#endif
+#if ARKCOS_ABL != 5
                     load_v(vb, jj0 + 4);
+#endif
                     mac4(ga, va, jj0);
                     asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#if ARKCOS_ABL != 3
                     tc_ld16(ga, tbase + (uint32_t)(min(jj0 + 8, JW - 4) * TI));
+#endif
+#if ARKCOS_ABL != 5
                     load_v(va, jj0 + 8);
+#endif
                     if (jj0 + 4 < jw) mac4(gb, vb, jj0 + 4);
                 }
                 asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-                if (!landed) cp_async_wait<0>();
+                if (!landed) land();
             }
+            if (t == 0) DBG(10);
             asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
             __syncwarp();
             if ((t & 31) == 0) mbar_arrive(&bar_empty[s]);       // this warp is done with TMEM stage s
@@ -354,7 +408,7 @@ band_mac_tc_kernel(const TcItem* __restrict__ items, const TcChunk* __restrict__
                 nold = jhave + 1 - tl.jlo;
 #pragma unroll
                 for (int q = 0; q < 4; ++q) if (jhave + 1 + q <= tl.jhi) fetch_ring(jhave + 1 + q, nx[q]);
-                for (int j = jhave + 5; j <= tl.jhi; ++j) fetch_ring(j, ringtab[j]);
+                for (int j = jhave + 5; j <= tl.jhi; ++j) fetch_ring(j, sRings[j - jbase]);
                 cp_async_commit();
                 jhave = max(jhave, tl.jhi);
             }
@@ -362,7 +416,7 @@ band_mac_tc_kernel(const TcItem* __restrict__ items, const TcChunk* __restrict__
             // ---- output: class E stores its mode; cap runs fold onto the ring's own modes ----------------
 #pragma unroll
             for (int ii = 0; ii < TI; ++ii) {
-                if (ii < cur.nti) {
+                if (ii < cur.nti && (ARKCOS_ABL != 4 || acc[ii][0].x == 12345.f)) {
                     const int i = cur.i0 + ii, iS = R - 1 - i;
                     const int offN = cur.offN[ii], offS = cur.offS[ii];
                     if (!CAP) {
@@ -388,11 +442,9 @@ band_mac_tc_kernel(const TcItem* __restrict__ items, const TcChunk* __restrict__
                     }
                 }
             }
+            if (t == 0) DBG(11);
         }
     }
-    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
-    __syncthreads();
-    if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"(2 * MT * N));
 }
 
 }  // namespace arkcos

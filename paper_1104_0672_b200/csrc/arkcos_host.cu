@@ -412,7 +412,8 @@ void build_pairs(HostGeometry& g, double theta_max, double ell_nyq, int fixed_mp
         const int mh = eq_rings.empty() ? 0 : g.n[eq_rings[0]] / 2;
         const int gx = std::max(1, (mh + kBandThreads * 2 - 1) / (kBandThreads * 2));
         const int target = std::max(1, (4 * sm_count) / gx);
-        const int chn = std::max(8, ((int)eq_rings.size() + target - 1) / target);
+        int chn = std::max(8, ((int)eq_rings.size() + target - 1) / target);
+        if (use_tc) chn = std::min(chn, kTcMaxTiles * kTcTI);       // the tile records of a run live in shared memory
         for (size_t k = 0; k < eq_rings.size(); ++k) {
             const int i = eq_rings[k];
             if (!t.eq_chunks.empty() && t.eq_chunks.back().i0 + t.eq_chunks.back().n == i && t.eq_chunks.back().n < chn &&
@@ -651,15 +652,9 @@ void launch_uniform(const arkcos_plan* pl, int nmaps, cudaStream_t st, bool seri
                 pl->d_eqchunks, pl->d_north, pl->d_pairs, pl->d_goff, pl->d_G, pl->d_rings, pl->g.R,
                 (const cx<float>*)pl->spec_in(), (cx<float>*)pl->d_specOut, pl->g.spec_total, nmaps);
     } else if (pl->neqchunks > 0 && pl->use_tc && pl->ntc_items[0] > 0) {
-        const dim3 grid((unsigned)pl->ntc_items[0], (unsigned)nmaps);
-        if (pl->eq_alt)
-            band_mac_tc_kernel<0><<<grid, kTcThreads, kTcSmemBytes, st>>>(
-                pl->d_tc_items[0], pl->d_tc_chunks, pl->d_tc_tiles, pl->d_tc_cols, pl->d_tc_rings, (const float*)pl->d_W, pl->g.R,
-                (const cx<float>*)pl->spec_in(), (cx<float>*)pl->d_specOut, pl->g.spec_total);
-        else
-            band_mac_tc_kernel<1><<<grid, kTcThreads, kTcSmemBytes, st>>>(
-                pl->d_tc_items[0], pl->d_tc_chunks, pl->d_tc_tiles, pl->d_tc_cols, pl->d_tc_rings, (const float*)pl->d_W, pl->g.R,
-                (const cx<float>*)pl->spec_in(), (cx<float>*)pl->d_specOut, pl->g.spec_total);
+        tc_launch(pl->eq_alt ? 0 : 1, (unsigned)pl->ntc_items[0], (unsigned)nmaps, st, pl->d_tc_items[0], pl->d_tc_chunks, pl->d_tc_tiles,
+                  pl->d_tc_cols, pl->d_tc_rings, (const float*)pl->d_W, pl->g.R, (const cx<float>*)pl->spec_in(), (cx<float>*)pl->d_specOut,
+                  pl->g.spec_total);
     } else if (pl->neqchunks > 0) {
         constexpr int TI = 4, MT = 2;
         const dim3 grid((unsigned)((pl->eq_mh + kBandThreads * MT - 1) / (kBandThreads * MT)), (unsigned)pl->neqchunks, (unsigned)nmaps);
@@ -697,9 +692,9 @@ void launch_uniform(const arkcos_plan* pl, int nmaps, cudaStream_t st, bool seri
                     (const cx<float>*)pl->spec_in(), (cx<float>*)pl->d_specOut, pl->g.spec_total, nmaps);
             else if (pl->use_tc) {
                 if (pl->ntc_items[MULTI ? 2 : 1] > 0)
-                    band_mac_tc_kernel<MULTI ? 3 : 2><<<dim3((unsigned)pl->ntc_items[MULTI ? 2 : 1], (unsigned)nmaps), kTcThreads, kTcSmemBytes, s1>>>(
-                        pl->d_tc_items[MULTI ? 2 : 1], pl->d_tc_chunks, pl->d_tc_tiles, pl->d_tc_cols, pl->d_tc_rings, (const float*)pl->d_W, pl->g.R,
-                        (const cx<float>*)pl->spec_in(), (cx<float>*)pl->d_specOut, pl->g.spec_total);
+                    tc_launch(MULTI ? 3 : 2, (unsigned)pl->ntc_items[MULTI ? 2 : 1], (unsigned)nmaps, s1, pl->d_tc_items[MULTI ? 2 : 1],
+                              pl->d_tc_chunks, pl->d_tc_tiles, pl->d_tc_cols, pl->d_tc_rings, (const float*)pl->d_W, pl->g.R,
+                              (const cx<float>*)pl->spec_in(), (cx<float>*)pl->d_specOut, pl->g.spec_total);
             } else
                 band_mac_capchunk_kernel<4, 20, MULTI><<<dim3(n, (unsigned)nmaps), kBandThreads, 0, s1>>>(
                     items, pl->d_cap_chunks, pl->d_north, pl->d_pairs, (const float*)pl->d_W, pl->d_rings, pl->g.R,
@@ -1001,16 +996,7 @@ static int plan_create_impl(arkcos_plan** out, const arkcos_pixelization* pix, c
         if (int rc = upload(&pl->d_tc_rings, t.tc_rings, wsb)) return rc;
         for (int c = 0; c < 3; ++c)
             if (int rc = upload(&pl->d_tc_items[c], t.tc_items[c], wsb)) return rc;
-        CUDA_TRY(cudaFuncSetAttribute(band_mac_tc_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kTcSmemBytes));
-        CUDA_TRY(cudaFuncSetAttribute(band_mac_tc_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kTcSmemBytes));
-        CUDA_TRY(cudaFuncSetAttribute(band_mac_tc_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kTcSmemBytes));
-        CUDA_TRY(cudaFuncSetAttribute(band_mac_tc_kernel<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kTcSmemBytes));
-        // two blocks per SM need nearly all of its shared memory
-        CUDA_TRY(cudaFuncSetAttribute(band_mac_tc_kernel<0>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
-        CUDA_TRY(cudaFuncSetAttribute(band_mac_tc_kernel<1>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
-        CUDA_TRY(cudaFuncSetAttribute(band_mac_tc_kernel<2>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
-        CUDA_TRY(cudaFuncSetAttribute(band_mac_tc_kernel<3>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
-        CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&pl->tc_blocks_per_sm, band_mac_tc_kernel<0>, kTcThreads, kTcSmemBytes));
+        CUDA_TRY((cudaError_t)tc_setup(&pl->tc_blocks_per_sm));
     }
     if (int rc = upload(&pl->d_cap_chunks, t.cap_chunks, wsb)) return rc;
     if (int rc = upload(&pl->d_cap_chunk_items, t.cap_chunk_items, wsb)) return rc;

@@ -12,7 +12,7 @@
 #include "arkcos_fft3.cuh"
 #include "arkcos_direct.cuh"
 #include "arkcos_band_cached.cuh"
-#include "arkcos_band_tc.cuh"
+#include "arkcos_band_tc.hpp"
 
 namespace arkcos {
 
