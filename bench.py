@@ -27,14 +27,25 @@ from paper_1104_0672_b200 import inputs  # noqa: E402
 from paper_1104_0672_b200.sharding import shard_range  # noqa: E402
 
 METRIC = "output Mpix/s per map at HEALPix Nside=2048"
-# dram__bytes_read.sum + dram__bytes_write.sum per launch (bytes) from the ncu --set full captures summarised in
-# profiles/ (config 4, one map); None where no capture exists
-TRAFFIC = {  # profiles/r1_v8_final.md (ncu --set full, config 4, one map); FFT entries = sum over the size classes
-    "band_mac_eq_kernel": 224e6 + 111e6,
-    "band_mac_capchunk_kernel<4,20>": 138e6 + 30e6,
-    "ring_fft3_forward_kernel (all transform sizes)": 306e6 + 149e6 + 42e6 + 1e6 + 11e6 + 3e6,
-    "ring_fft3_inverse_kernel (all transform sizes)": 309e6 + 149e6 + 42e6 + 1e6 + 11e6 + 3e6,
-}
+
+
+def ncu_table(which: str) -> dict:
+    """Numbers taken from the ncu captures summarised under profiles/ (text files; absent -> empty):
+    dram_bytes: kernel -> dram__bytes_read.sum + dram__bytes_write.sum per launch; fp32_thread_inst: step totals."""
+    path = os.path.join(ROOT, "profiles", "r2_final_ncu.csv")
+    out = {}
+    try:
+        import csv
+        for row in csv.DictReader(open(path)):
+            if which == "dram_bytes" and row.get("dram_bytes"):
+                out[row["kernel"]] = float(row["dram_bytes"])
+            if which == "fp32_thread_inst" and row["kernel"] == "STEP TOTAL" and row.get("fp32_gflop"):
+                out["step_gflop"] = float(row["fp32_gflop"])
+    except OSError:
+        pass
+    return out
+
+
 UNIT = "Mpix/s"
 
 
@@ -268,19 +279,20 @@ def run_ours(args):
             dist.destroy_process_group()
         return
 
-    # per-kernel durations: the band kernels normally overlap on side streams; timing mode 2 runs them one after the
-    # other with events in between (same launches, same stream torch handed us)
+    # per-launch durations: the band kernels and the ring-FFT launches normally overlap on side streams; timing mode 2
+    # runs them one after the other with events in between (same launches, same stream torch handed us)
     plan.set_timing(2)
-    band_ms = None
+    band_ms, fwd_ms, inv_ms = None, None, None
+    add = lambda acc, cur: cur if acc is None else [x + y for x, y in zip(acc, cur)]   # noqa: E731
     for _ in range(args.steps):
         step()
-        cur = [b[2] for b in plan.band_kernels(with_timing=True)]
-        band_ms = cur if band_ms is None else [a + b for a, b in zip(band_ms, cur)]
-    band_info = plan.band_kernels()
+        band_ms = add(band_ms, [b[2] for b in plan.band_kernels(with_timing=True)])
+        fk = plan.fft_kernels(with_timing=True)
+        fwd_ms, inv_ms = add(fwd_ms, [f[2] for f in fk]), add(inv_ms, [f[3] for f in fk])
+    band_info, fft_info = plan.band_kernels(), plan.fft_kernels()
     plan.set_timing(False)
-    band_ms = [v / args.steps for v in band_ms]
+    band_ms, fwd_ms, inv_ms = ([v / args.steps for v in lst] for lst in (band_ms, fwd_ms, inv_ms))
 
-    # roofline of the dominant kernel (largest measured duration)
     peaks = {}
     try:
         peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
@@ -289,55 +301,135 @@ def run_ours(args):
     fp32_peak = arkcos.arkcos_probe_fp32_peak(10)
     hbm = float(peaks.get("hbm_gbs", 6650.0))
     hbm_src = "MEASURED_PEAKS.json hbm_gbs" if "hbm_gbs" in peaks else "fallback 6650 GB/s (B200_PROFILING.md)"
-    alu_src = "FFMA chain measured in this run (arkcos_probe_fp32_peak); nominal 148*128*2*1.965 GHz = 74.4"
+    alu_src = ("FFMA chain measured in this run (arkcos_probe_fp32_peak); nominal 148*128*2*1.965 GHz = 74.4.  achieved = "
+               "work-model flops of the kernel's rings (cosine transform of the rows + multiply-accumulate, DESIGN.md "
+               "section 5) / duration; the tensor-core kernels run the cosine transform as 3xTF32 products, their FP32 pipe "
+               "only the multiply-accumulate")
+    tc = plan.tensor_cores()
+    traffic = ncu_table("dram_bytes")
     kernels = []
+    sass_name = {"band_mac_eq_kernel": "band_mac_tc_kernel<0>", "band_mac_capchunk_kernel<4,20>": "band_mac_tc_kernel<2>"} if tc["used"] else {}
     for (kname, flops, _), ms_k in zip(band_info, band_ms):
-        if flops > 0:
+        if flops > 0 and ms_k > 0:
             ach = flops * nmaps / (ms_k * 1e-3) / 1e12
-            kernels.append({"kernel": kname, "ms": ms_k, "bound": "alu", "achieved": ach, "peak": fp32_peak,
-                            "unit": "TFLOP/s", "frac": ach / fp32_peak, "traffic": TRAFFIC.get(kname), "peak_source": alu_src})
-    for kname, key in (("ring_fft3_forward_kernel (all transform sizes)", "fft_forward"),
-                       ("ring_fft3_inverse_kernel (all transform sizes)", "fft_inverse")):
-        byts = 2.0 * 4.0 * npix * nmaps           # a ring FFT reads and writes every map element once (4 B each way)
-        ach = byts / (stage[key] * 1e-3) / 1e9
-        kernels.append({"kernel": kname, "ms": stage[key], "bound": "hbm", "achieved": ach, "peak": hbm, "unit": "GB/s",
-                        "frac": ach / hbm, "traffic": TRAFFIC.get(kname), "peak_source": hbm_src})
-    roof = dict(max(kernels, key=lambda k: k["ms"]))
+            launch = sass_name.get(kname, kname)
+            kernels.append({"kernel": launch, "ring_class": kname, "ms": ms_k, "bound": "alu", "achieved": ach, "peak": fp32_peak,
+                            "unit": "TFLOP/s", "frac": ach / fp32_peak, "traffic": traffic.get(launch), "peak_source": alu_src})
+    for direction, mss in (("forward", fwd_ms), ("inverse", inv_ms)):
+        for (kname, px, _, _), ms_k in zip(fft_info, mss):
+            if px > 0 and ms_k > 0:
+                byts = 2.0 * 4.0 * px * nmaps      # a ring FFT reads and writes every map element once (4 B each way)
+                ach = byts / (ms_k * 1e-3) / 1e9
+                launch = f"{kname} {direction}"
+                kernels.append({"kernel": launch, "ms": ms_k, "bound": "hbm", "achieved": ach, "peak": hbm, "unit": "GB/s",
+                                "frac": ach / hbm, "traffic": traffic.get(launch), "peak_source": hbm_src})
+    roof = dict(max(kernels, key=lambda k: k["ms"]))      # the longest single launch of the step
     roof["stage_ms"] = stage
     roof["all_kernels"] = [{k: v for k, v in kk.items() if k != "peak_source"} for kk in kernels]
     launches_per_step = plan.launches_per_convolve
+    wm = plan.work_model()
+
+    # whole-step fractions (SURVEY.md section 8d reporting rule): the work model as executed and as the method needs it
+    t_s = ms_step * 1e-3
+    gf_exec = (stats["mac_flops"] + stats["fft_flops"]) * nmaps / 1e9
+    gf_alg = (stats["mac_flops"] + wm["fft_flops_min"]) * nmaps / 1e9
+    inst = ncu_table("fp32_thread_inst")
+    step_roof = {"model_gflop_executed": gf_exec, "model_gflop_algorithmic": gf_alg,
+                 "frac_fp32_executed": gf_exec / t_s / 1e3 / fp32_peak, "frac_fp32_algorithmic": gf_alg / t_s / 1e3 / fp32_peak,
+                 "tensor_gflop_issued": wm["tensor_flops"] * nmaps / 1e9,
+                 "hbm_bytes_unfused": 6 * 4 * npix * nmaps, "frac_hbm_unfused": 6 * 4 * npix * nmaps / t_s / 1e9 / hbm,
+                 "fp32_peak_tflops": fp32_peak, "hbm_peak_gbs": hbm,
+                 "ncu_fp32_gflop_executed": inst.get("step_gflop"),
+                 "note": "model_gflop_executed counts the Bluestein transforms as run and the rows' cosine transforms as FP32 "
+                         "flops although the tensor-core kernels issue them as 3xTF32 products (tensor_gflop_issued, padded "
+                         "tiles); ncu_fp32_gflop_executed = 2 FFMA + FMUL + FADD thread instructions of one step from "
+                         "profiles/ (null until that capture exists)"}
 
     # beside the headline (kernel rows regenerated every step, Table 1): the plan-cached mode for many maps
     # with one kernel, rows and their transforms computed once at plan time
+    def timed(p, n_maps, d_i, d_o, reps):
+        for _ in range(2):
+            p.convolve(d_i.data_ptr(), d_o.data_ptr(), n_maps, stream)
+        torch.cuda.synchronize()
+        e0.record()
+        for _ in range(reps):
+            p.convolve(d_i.data_ptr(), d_o.data_ptr(), n_maps, stream)
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / reps
+
     plan_c = arkcos.Plan(c["pix"], tab, c["theta_max"], dtype, max_nmaps=nmaps, cache_kernel_spectra=1)
-    for _ in range(3):
-        plan_c.convolve(d_in.data_ptr(), d_out.data_ptr(), nmaps, stream)
-    torch.cuda.synchronize()
-    e0.record()
-    for _ in range(args.steps):
-        plan_c.convolve(d_in.data_ptr(), d_out.data_ptr(), nmaps, stream)
-    e1.record()
-    torch.cuda.synchronize()
-    cached_ms = e0.elapsed_time(e1) / args.steps
+    cached_ms = timed(plan_c, nmaps, d_in, d_out, args.steps)
     cached = {"ms_per_step": cached_ms, "value": npix * nmaps / (cached_ms * 1e-3) / 1e6, "unit": UNIT,
               "workspace_gb": plan_c.stats()["workspace_bytes"] / 1e9, "note": "options.cache_kernel_spectra = 1; not the headline"}
     del plan_c
 
+    # several kernels on one map (arkcos_convolve_multi): K Gaussians of different widths
+    extra = {}
+    if args.cfg == 4 and not args.no_extras:
+        K = 8
+        fw = [c["fwhm"] * (0.7 + 0.1 * k) for k in range(K)]
+        plans = [arkcos.Plan(c["pix"], inputs.gaussian_table(f, 3.0 * f), 3.0 * f, dtype) for f in fw]
+        d_multi = torch.empty((K, npix), device="cuda", dtype=torch.float32)
+        run_multi = lambda: arkcos.arkcos_convolve_multi(plans, d_in.data_ptr(), d_multi.data_ptr(), 1, stream)   # noqa: E731
+        run_sep = lambda: [p.convolve(d_in.data_ptr(), d_multi[k].data_ptr(), 1, stream) for k, p in enumerate(plans)]   # noqa: E731
+        res = {}
+        for name, fn in (("multi", run_multi), ("separate", run_sep)):
+            fn()
+            torch.cuda.synchronize()
+            e0.record()
+            for _ in range(5):
+                fn()
+            e1.record()
+            torch.cuda.synchronize()
+            res[name] = e0.elapsed_time(e1) / 5
+        extra["multi_kernel"] = {"kernels": K, "workload": "cfg4 map, Gaussians FWHM 3.5' .. 7', cut at 3 FWHM",
+                                 "ms_arkcos_convolve_multi": res["multi"], "ms_separate_calls": res["separate"]}
+        del plans, d_multi
+        torch.cuda.empty_cache()
+        # config 5 (BASELINE.json configs[4]): 16 maps, hard-edged kernels; kernel spectra computed per call, cached, exact caps
+        c5 = inputs.config(5)
+        x5 = torch.from_numpy(inputs.white_noise_maps(npix, 5, c5["nmaps"])).cuda()
+        o5 = torch.empty_like(x5)
+        blk = {}
+        for kspec in c5["kernels"]:
+            tab5 = inputs.kernel_table(kspec)
+            row = {}
+            for mode, opts in (("computed", {}), ("cached_spectra", {"cache_kernel_spectra": 1}), ("computed_exact_caps", {"exact_caps": 1})):
+                p5 = arkcos.Plan(c5["pix"], tab5, kspec["theta_max"], dtype, max_nmaps=c5["nmaps"], **opts)
+                ms5 = timed(p5, c5["nmaps"], x5, o5, 3)
+                row[mode] = {"ms_per_16_maps": ms5, "gpix_per_s": npix * c5["nmaps"] / (ms5 * 1e-3) / 1e9,
+                             "workspace_gb": p5.stats()["workspace_bytes"] / 1e9, "tensor_cores": p5.tensor_cores()["used"]}
+                del p5
+                torch.cuda.empty_cache()
+            blk[kspec["kernel"]] = row
+        extra["cfg5"] = blk
+        del x5, o5
+
     cpu = time_oracle(c, tab, x, args.oracle_rings)
     cpu_val = cpu["pixels"] * cpu["maps"] / cpu["seconds"] / 1e6
+    cpu1 = time_oracle(c, tab, x, max(16, args.oracle_rings // 32), nthreads=1)
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
             "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
             "data": "synthetic",
             "config": {"workload": name, "l2": "input map 201 MB + spectra 403 MB per step exceed the 126 MB L2; no flush",
                        "kernel_rows": "regenerated every step", "ell_nyquist": plan.ell_nyquist,
                        "plan_create_s": plan_s, "ring_pairs": stats["ring_pairs"], "row_samples": stats["row_samples"],
-                       "model_gflop": {"band": stats["mac_flops"] / 1e9, "fft": stats["fft_flops"] / 1e9}},
-            "roofline": roof,
+                       "model_gflop": {"band": stats["mac_flops"] / 1e9, "fft": stats["fft_flops"] / 1e9,
+                                       "fft_own_lengths": wm["fft_flops_min"] / 1e9},
+                       "band_kernels": "tcgen05 3xTF32 row transform + FP32 multiply-accumulate" if tc["used"] else "FP32 only",
+                       "tensor_core_blocks": tc["blocks"]},
+            "roofline": roof, "step_roofline": step_roof,
             "cpu_baseline": {"value": cpu_val, "unit": UNIT, "cores": cpu["threads"], "kind": "oracle",
                              "sample": f"{cpu['rings']} of {cpu['nrings']} output rings evenly spaced in ring index, "
-                                       f"{cpu['pixels']} pixels, {cpu['seconds']:.1f} s"},
-            "cached_spectra_mode": cached, "e2e": e2e, "gpu_launches": launches_per_step * args.steps, "clocks": clocks,
-            "paper_context": "2.2 s on a GTX 480 incl. PCIe copies = 22.9 Mpix/s (PAPER.md:195)"}
+                                       f"{cpu['pixels']} pixels, {cpu['seconds']:.1f} s",
+                             "one_thread": {"value": cpu1["pixels"] * cpu1["maps"] / cpu1["seconds"] / 1e6, "unit": UNIT,
+                                            "sample": f"{cpu1['rings']} rings, {cpu1['pixels']} pixels, {cpu1['seconds']:.1f} s"}},
+            "cached_spectra_mode": cached, "e2e": e2e, "gpu_launches": launches_per_step * args.steps,
+            "gpu_launches_note": "kernels only; plus %d cudaMemsetAsync per step that clear the ranges the cap fold accumulates into"
+                                 % (wm["memsets_per_map"] * nmaps),
+            "clocks": clocks, "paper_context": "2.2 s on a GTX 480 incl. PCIe copies = 22.9 Mpix/s (PAPER.md:195)"}
+    line.update(extra)
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
@@ -352,6 +444,7 @@ def main():
     ap.add_argument("--cfg", type=int, default=4)
     ap.add_argument("--profile", action="store_true", help="warm-up + steps of arkcos_convolve only (the command ncu wraps)")
     ap.add_argument("--cfg5-kernel", type=int, default=1, help="--cfg 5: 0 = top-hat disc, 1 = cut Mexican hat")
+    ap.add_argument("--no-extras", action="store_true", help="skip the multi-kernel and config-5 blocks")
     ap.add_argument("--quick", action="store_true", help="device-resident timing of the step, its stages and band kernels only")
     ap.add_argument("--oracle-rings", type=int, default=2048, help="output rings in the CPU-oracle sample")
     args = ap.parse_args()

@@ -174,6 +174,22 @@ int arkcos_plan_get_timing(const arkcos_plan* plan, float* ms4);
  * names / model_flops / last_ms: arrays of 8, any may be NULL. */
 int arkcos_plan_band_kernels(const arkcos_plan* plan, int* n, const char** names, double* model_flops, float* last_ms);
 
+/* The ring FFTs of one direction are up to nine launches: per transform size Q = 4096, 2048, 1024, 512 the power-of-two rings
+ * (one transform per block) and the Bluestein rings, then the shared-memory kernel for very short or very long rings.
+ * Returns their number (*n = 9), names, the pixels each serves (algorithmic bytes of a launch = 8 bytes per pixel and map:
+ * every map element is read or written once and so is its half spectrum) and -- only after a call made in timing mode 2,
+ * which runs them one after the other -- their last durations in milliseconds per direction.  Arrays of 9; any may be NULL. */
+int arkcos_plan_fft_kernels(const arkcos_plan* plan, int* n, const char** names, double* pixels, float* last_ms_forward,
+                            float* last_ms_inverse);
+
+/* Further terms of the work model of one arkcos_convolve with nmaps = 1; any pointer may be NULL.
+ *  band_pair_modes   sum over northern ring pairs of (M/2 + 1): products G_ij[m] B_j[m] per hemisphere
+ *  fft_flops_min     flops of the forward + inverse ring FFTs at the rings' own lengths (no Bluestein padding)
+ *  tensor_flops      tensor-core flops issued by band_mac_tc_kernel (3 x TF32 terms, zero-padded tiles; upper bound); 0 if unused
+ *  memsets_per_map   cudaMemsetAsync calls per map that clear the output-spectrum ranges the cap fold accumulates into */
+int arkcos_plan_work_model(const arkcos_plan* plan, double* band_pair_modes, double* fft_flops_min, double* tensor_flops,
+                           int* memsets_per_map);
+
 /* Whether the plan's band step runs on the tensor cores (options.no_tensor_cores = 0, a float plan with computed spectra,
  * band windows that fit): *blocks = blocks of band_mac_tc_kernel launched per arkcos_convolve and map (class-E runs, cap
  * runs single period, cap runs several periods), *resident_per_sm = how many of them one SM holds.  Pointers may be NULL.

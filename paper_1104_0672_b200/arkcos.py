@@ -65,6 +65,9 @@ SYMBOLS = {
     "arkcos_plan_set_timing": (c_int, [c_void_p, c_int]),
     "arkcos_plan_get_timing": (c_int, [c_void_p, POINTER(c_float)]),
     "arkcos_plan_band_kernels": (c_int, [c_void_p, POINTER(c_int), POINTER(c_char_p), POINTER(c_double), POINTER(c_float)]),
+    "arkcos_plan_fft_kernels": (c_int, [c_void_p, POINTER(c_int), POINTER(c_char_p), POINTER(c_double), POINTER(c_float),
+                                        POINTER(c_float)]),
+    "arkcos_plan_work_model": (c_int, [c_void_p, POINTER(c_double), POINTER(c_double), POINTER(c_double), POINTER(c_int)]),
     "arkcos_plan_tensor_cores": (c_int, [c_void_p, POINTER(c_int), POINTER(c_int)]),
     "arkcos_plan_launches_per_convolve": (c_int, [c_void_p]),
     "arkcos_probe_fp32_peak": (c_int, [POINTER(c_double), c_int]),
@@ -251,6 +254,21 @@ class Plan:
         _check(_lib().arkcos_plan_band_kernels(self._h, byref(n), names, fl, ms if with_timing else None),
                "arkcos_plan_band_kernels")
         return [(names[k].decode(), fl[k], ms[k] if with_timing else None) for k in range(n.value)]
+
+    def fft_kernels(self, with_timing: bool = False):
+        """[(name, pixels, forward_ms or None, inverse_ms or None)] of the ring-FFT launches (timing needs set_timing(2))."""
+        n = c_int()
+        names = (c_char_p * 9)()
+        px = (c_double * 9)()
+        f, i = (c_float * 9)(), (c_float * 9)()
+        _check(_lib().arkcos_plan_fft_kernels(self._h, byref(n), names, px, f if with_timing else None, i if with_timing else None),
+               "arkcos_plan_fft_kernels")
+        return [(names[k].decode(), px[k], f[k] if with_timing else None, i[k] if with_timing else None) for k in range(n.value)]
+
+    def work_model(self) -> dict:
+        a, b, c, m = c_double(), c_double(), c_double(), c_int()
+        _check(_lib().arkcos_plan_work_model(self._h, byref(a), byref(b), byref(c), byref(m)), "arkcos_plan_work_model")
+        return dict(band_pair_modes=a.value, fft_flops_min=b.value, tensor_flops=c.value, memsets_per_map=m.value)
 
     def get_timing(self):
         ms = (c_float * 4)()

@@ -11,7 +11,7 @@ import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
-UNITS = ["arkcos_host.cu", "arkcos_band_tc.cu", "arkcos_legendre.cpp"]
+UNITS = ["arkcos_host.cu", "arkcos_band_tc.cu", "arkcos_fft3.cu", "arkcos_legendre.cpp"]
 OBJ_DIR = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libarkcos.so")
 

@@ -15,19 +15,9 @@
 //     even and the odd half, the filter product needs no exchange (the output layout of one transform is the input
 //     layout of the next) and chirp, filter and half-bin phases are fused into the loads and stores.
 #pragma once
-#include "arkcos_fft.cuh"
+#include "arkcos_fft3.hpp"
 
 namespace arkcos {
-
-// One job, self-contained (copies of the ring and length records, so a block needs a single table read):
-// power-of-two rings: two rings, served by two blocks (has1 = 0: only r0); Bluestein: r0 only.
-struct FftJob { RingRec r0, r1; FftLen f; int has1, pad; };
-
-template <int LOGQ> struct Fft3 {
-    static constexpr int Q = 1 << LOGQ, T = Q / 16, RL = Q / 256, NC = 16 / RL, SQ = Q + Q / 16;
-    static constexpr int MINB = 512 / T;
-    static constexpr size_t smem_bytes = 2 * (size_t)SQ * sizeof(cx<float>);
-};
 
 // Forward complex DFT of size Q of NB sequences held in registers: in  u[b][r] = x_b[t + T r],  out u[b][q] = X_b[t + T q].
 // s: NB arrays of SQ complex numbers (padded indexing e + e/16).  Twiddle tables laid out so that a warp reads whole

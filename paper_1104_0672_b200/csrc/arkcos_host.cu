@@ -221,6 +221,7 @@ void build_fft_lens(const HostGeometry& g, HostTables& t, Stats& st, bool use_ff
         const double P = (double)(1 << f.logP);
         // forward + inverse: complex FFT(s) + O(N) split / chirps
         st.fft_flops += 2.0 * (f.pow2 ? 5.0 * P * f.logP + 20.0 * L : 2.0 * 5.0 * P * f.logP + 6.0 * P + 32.0 * L);
+        st.fft_flops_min += 2.0 * (5.0 * L * log2((double)std::max(L, 2)) + 20.0 * L);
     }
     // Rings whose transform size Q (L for a power of two, half the Bluestein convolution length otherwise) is 512 .. 4096
     // go to the register-resident kernels: Bluestein rings first, a ring next to its mirror image (same tables), then
@@ -260,6 +261,13 @@ void build_fft_lens(const HostGeometry& g, HostTables& t, Stats& st, bool use_ff
         }
     for (int i = 0; i < g.R; ++i)
         if (!taken[i]) t.fft_order.push_back(i);
+    // launch order of one direction: Q = 4096 power-of-two, Bluestein, then 2048, 1024, 512 alike, then the shared-memory kernel
+    for (int c = 0; c < 4; ++c)
+        for (const FftJob& j : t.fft3_jobs[c]) {
+            const int slot = 2 * (3 - c) + (j.f.pow2 ? 0 : 1);
+            st.fft_pixels[slot] += j.r0.n + (j.has1 ? j.r1.n : 0);
+        }
+    for (int i : t.fft_order) st.fft_pixels[8] += g.n[i];
     std::stable_sort(t.fft_order.begin(), t.fft_order.end(), [&](int a, int b) {
         const FftLen &fa = t.lens[t.rings[a].len_id], &fb = t.lens[t.rings[b].len_id];
         const int wa = (fa.pow2 ? 1 : 2) << fa.logP, wb = (fb.pow2 ? 1 : 2) << fb.logP;
@@ -332,6 +340,7 @@ void build_pairs(HostGeometry& g, double theta_max, double ell_nyq, int fixed_mp
             const double modes = p.M / 2 + 1;
             ring_flops += modes * (2.0 * p.cnt + (has_mirror ? 8.0 : 4.0));
             st.mac_flops += modes * (2.0 * p.cnt + (has_mirror ? 8.0 : 4.0));
+            st.mac_pairs_modes += modes;
             st.ring_pairs += has_mirror ? 2 : 1;
         }
         t.north[i].pair_hi = (int)t.pairs.size();
@@ -454,7 +463,11 @@ void build_pairs(HostGeometry& g, double theta_max, double ell_nyq, int fixed_mp
             }
             t.tc_chunks.push_back(c);
             const int nmodes = with_nyquist ? M / 2 + 1 : M / 2;
-            for (int bx = 0; bx * 128 * kTcMT < nmodes; ++bx) t.tc_items[cls].push_back(TcItem{(int)t.tc_chunks.size() - 1, bx});
+            for (int bx = 0; bx * 128 * kTcMT < nmodes; ++bx) {
+                t.tc_items[cls].push_back(TcItem{(int)t.tc_chunks.size() - 1, bx});
+                // upper bound: the kernel issues fewer K steps for tiles whose rows are short
+                st.tc_flops += (double)((n + kTcTI - 1) / kTcTI) * kTcMT * 3.0 * (kTcK / 8) * 2.0 * 128.0 * kTcN * 8.0;
+            }
         };
         for (int j = 0; j < R; ++j)
             t.tc_rings.push_back(TcRing{(int)g.spec_off[j], (int)g.spec_off[R - 1 - j], g.n[j] | (g.shifted[j] ? (int)0x80000000 : 0),
@@ -516,15 +529,6 @@ template <class T, int BPT> int set_fft_smem(size_t bytes)
     return 0;
 }
 
-template <int LOGQ> int set_fft3_smem()
-{
-    CUDA_TRY(cudaFuncSetAttribute(ring_fft3_forward_kernel<LOGQ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Fft3<LOGQ>::smem_bytes));
-    CUDA_TRY(cudaFuncSetAttribute(ring_fft3_inverse_kernel<LOGQ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Fft3<LOGQ>::smem_bytes));
-    CUDA_TRY(cudaFuncSetAttribute(ring_fft3_direct1_kernel<LOGQ, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Fft3<LOGQ>::smem_bytes / 2));
-    CUDA_TRY(cudaFuncSetAttribute(ring_fft3_direct1_kernel<LOGQ, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Fft3<LOGQ>::smem_bytes / 2));
-    return 0;
-}
-
 // job lists and the 16 x 16 twiddle table of the register-resident FFT kernels (float plans only)
 template <class T> int setup_fft3(arkcos_plan* pl, const HostTables& t)
 {
@@ -552,10 +556,7 @@ template <class T> int setup_fft3(arkcos_plan* pl, const HostTables& t)
     cx<float>* d3 = nullptr;
     if (int rc = upload(&d3, tw3, &pl->stats.workspace_bytes)) return rc;
     pl->d_tw3 = d3;
-    if (int rc = set_fft3_smem<9>()) return rc;
-    if (int rc = set_fft3_smem<10>()) return rc;
-    if (int rc = set_fft3_smem<11>()) return rc;
-    if (int rc = set_fft3_smem<12>()) return rc;
+    CUDA_TRY((cudaError_t)fft3_setup());
     }
     return 0;
 }
@@ -712,33 +713,32 @@ void launch_uniform(const arkcos_plan* pl, int nmaps, cudaStream_t st, bool seri
 template <int LOGQ, bool FWD>
 void launch_fft3(const arkcos_plan* pl, const void* d_in, void* d_out, int nmaps, cudaStream_t st)
 {
-    const int c = LOGQ - 9;
-    if (pl->nfft3[c] == 0) return;
-    const HostGeometry& g = pl->g;
-    int njobs = pl->nfft3[c];
-    if (pl->nfft3[c] > pl->nfft3_bluestein[c]) {      // power-of-two rings: one transform per block
-        const int nb = pl->nfft3_bluestein[c], nd = pl->nfft3[c] - nb;
-        ring_fft3_direct1_kernel<LOGQ, FWD><<<dim3(2u * (unsigned)nd, (unsigned)nmaps), Fft3<LOGQ>::T, Fft3<LOGQ>::smem_bytes / 2, st>>>(
-            (const float*)d_in, (float*)d_out, g.npix, (cx<float>*)(FWD ? pl->spec_in() : pl->d_specOut), g.spec_total,
-            pl->d_fft3_jobs[c] + nb, (const cx<float>*)pl->d_tw, pl->logPT, (const cx<float>*)pl->d_tw16,
-            (const cx<float>*)pl->d_tw3 + pl->tw3_off[c], (const cx<float>*)pl->d_phase);
-        njobs = nb;
-        if (njobs == 0) return;
+    const int c = LOGQ - 9, dir = FWD ? 0 : 1, slot = 2 * (3 - c);
+    if (pl->nfft3[c] == 0) {
+        if (pl->timing == 2) { cudaEventRecord(pl->ev_fft[dir][slot], st); cudaEventRecord(pl->ev_fft[dir][slot + 1], st); }
+        return;
     }
-    const dim3 grid((unsigned)njobs, (unsigned)nmaps);
-    const int ahead = pl->sm_count * Fft3<LOGQ>::MINB;         // resident blocks: the one that will take this block's slot
-    if (FWD)
-        ring_fft3_forward_kernel<LOGQ><<<grid, Fft3<LOGQ>::T, Fft3<LOGQ>::smem_bytes, st>>>(
-            (const float*)d_in, g.npix, (cx<float>*)pl->spec_in(), g.spec_total, pl->d_rings, pl->d_fft3_jobs[c], pl->d_lens,
-            (const cx<float>*)pl->d_tw, pl->logPT, (const cx<float>*)pl->d_tw16, (const cx<float>*)pl->d_tw3 + pl->tw3_off[c],
-            (const cx<float>*)pl->d_filt,
-            (const cx<float>*)pl->d_chirp, (const cx<float>*)pl->d_phase, ahead);
-    else
-        ring_fft3_inverse_kernel<LOGQ><<<grid, Fft3<LOGQ>::T, Fft3<LOGQ>::smem_bytes, st>>>(
-            (const cx<float>*)pl->d_specOut, g.spec_total, (float*)d_out, g.npix, pl->d_rings, pl->d_fft3_jobs[c], pl->d_lens,
-            (const cx<float>*)pl->d_tw, pl->logPT, (const cx<float>*)pl->d_tw16, (const cx<float>*)pl->d_tw3 + pl->tw3_off[c],
-            (const cx<float>*)pl->d_filt,
-            (const cx<float>*)pl->d_chirp, (const cx<float>*)pl->d_phase, ahead);
+    const HostGeometry& g = pl->g;
+    Fft3Args a{};
+    a.in = (const float*)d_in;
+    a.outmap = (float*)d_out;
+    a.npix = g.npix;
+    a.spec = (cx<float>*)(FWD ? pl->spec_in() : pl->d_specOut);
+    a.spec_stride = g.spec_total;
+    a.tw = (const cx<float>*)pl->d_tw;
+    a.tw16 = (const cx<float>*)pl->d_tw16;
+    a.tw3 = (const cx<float>*)pl->d_tw3 + pl->tw3_off[c];
+    a.filt = (const cx<float>*)pl->d_filt;
+    a.chirp = (const cx<float>*)pl->d_chirp;
+    a.phase = (const cx<float>*)pl->d_phase;
+    a.logPT = pl->logPT;
+    const int nb = pl->nfft3_bluestein[c], nd = pl->nfft3[c] - nb;
+    if (pl->timing == 2) cudaEventRecord(pl->ev_fft[dir][slot], st);
+    if (nd > 0)                                       // power-of-two rings: one transform per block
+        fft3_launch_direct(LOGQ, FWD, pl->d_fft3_jobs[c] + nb, (unsigned)nd, (unsigned)nmaps, st, a);
+    if (pl->timing == 2) cudaEventRecord(pl->ev_fft[dir][slot + 1], st);
+    if (nb > 0)
+        fft3_launch_bluestein(LOGQ, FWD, pl->d_fft3_jobs[c], (unsigned)nb, (unsigned)nmaps, st, a, pl->sm_count);
 }
 
 template <class T, bool FWD>
@@ -757,7 +757,9 @@ void launch_ring_ffts(const arkcos_plan* pl, const void* d_in, void* d_out, int 
         launch_fft3<11, FWD>(pl, d_in, d_out, nmaps, forked ? pl->side[0] : st);
         launch_fft3<10, FWD>(pl, d_in, d_out, nmaps, forked ? pl->side[1] : st);
         launch_fft3<9, FWD>(pl, d_in, d_out, nmaps, forked ? pl->side[1] : st);
-    }
+    } else if (pl->timing == 2)
+        for (int k = 0; k < 8; ++k) cudaEventRecord(pl->ev_fft[FWD ? 0 : 1][k], st);
+    if (pl->timing == 2) cudaEventRecord(pl->ev_fft[FWD ? 0 : 1][8], st);
     if (pl->nfft_old > 0) {
         cudaStream_t so = forked ? pl->side[2] : st;
         const dim3 gfft((unsigned)pl->nfft_old, (unsigned)nmaps);
@@ -781,6 +783,7 @@ void launch_ring_ffts(const arkcos_plan* pl, const void* d_in, void* d_out, int 
                     (const cx<T>*)pl->d_tw, pl->logPT, (const cx<T>*)pl->d_filt, (const cx<T>*)pl->d_chirp, (const cx<T>*)pl->d_phase);
         }
     }
+    if (pl->timing == 2) cudaEventRecord(pl->ev_fft[FWD ? 0 : 1][9], st);
     if (forked)
         for (int k = 0; k < 3; ++k) {
             cudaEventRecord(pl->ev_join[k], pl->side[k]);
@@ -1008,6 +1011,7 @@ static int plan_create_impl(arkcos_plan** out, const arkcos_pixelization* pix, c
     if (int rc = dtype == ARKCOS_F32 ? build_device_numeric<float>(pl, t) : build_device_numeric<double>(pl, t)) return rc;
     for (auto& e : pl->ev) CUDA_TRY(cudaEventCreate(&e));
     for (auto& e : pl->ev_band) CUDA_TRY(cudaEventCreate(&e));
+    for (auto& d : pl->ev_fft) for (auto& e : d) CUDA_TRY(cudaEventCreate(&e));
     CUDA_TRY(cudaEventCreateWithFlags(&pl->ev_fork, cudaEventDisableTiming));
     for (auto& e : pl->ev_join) CUDA_TRY(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
     for (auto& q : pl->side) CUDA_TRY(cudaStreamCreateWithFlags(&q, cudaStreamNonBlocking));
@@ -1193,6 +1197,7 @@ int arkcos_plan_destroy(arkcos_plan* pl)
     for (void* p : ptrs) if (p) cudaFree(p);
     for (auto& e : pl->ev) if (e) cudaEventDestroy(e);
     for (auto& e : pl->ev_band) if (e) cudaEventDestroy(e);
+    for (auto& d : pl->ev_fft) for (auto& e : d) if (e) cudaEventDestroy(e);
     if (pl->ev_fork) cudaEventDestroy(pl->ev_fork);
     for (auto& e : pl->ev_join) if (e) cudaEventDestroy(e);
     for (auto& q : pl->side) if (q) cudaStreamDestroy(q);
@@ -1266,6 +1271,40 @@ int arkcos_plan_band_kernels(const arkcos_plan* pl, int* n, const char** names, 
         CUDA_TRY(cudaEventSynchronize(pl->ev_band[8]));
         for (int k = 0; k < 8; ++k) CUDA_TRY(cudaEventElapsedTime(&last_ms[k], pl->ev_band[k], pl->ev_band[k + 1]));
     }
+    return ARKCOS_OK;
+}
+
+int arkcos_plan_fft_kernels(const arkcos_plan* pl, int* n, const char** names, double* pixels, float* last_ms_forward,
+                            float* last_ms_inverse)
+{
+    static const char* kNames[9] = {"ring_fft3_direct1_kernel<12>", "ring_fft3_bluestein<12>", "ring_fft3_direct1_kernel<11>",
+                                    "ring_fft3_bluestein<11>", "ring_fft3_direct1_kernel<10>", "ring_fft3_bluestein<10>",
+                                    "ring_fft3_direct1_kernel<9>", "ring_fft3_bluestein<9>", "ring_fft_kernel (shared memory)"};
+    if (!pl || !n) return fail(ARKCOS_INVALID_ARG, "NULL argument");
+    *n = 9;
+    for (int k = 0; k < 9; ++k) {
+        if (names) names[k] = kNames[k];
+        if (pixels) pixels[k] = pl->stats.fft_pixels[k];
+    }
+    if (last_ms_forward || last_ms_inverse) {
+        if (pl->timing != 2) return fail(ARKCOS_INVALID_ARG, "per-kernel timing needs arkcos_plan_set_timing(plan, 2)");
+        CUDA_TRY(cudaEventSynchronize(pl->ev_fft[1][9]));
+        for (int k = 0; k < 9; ++k) {
+            if (last_ms_forward) CUDA_TRY(cudaEventElapsedTime(&last_ms_forward[k], pl->ev_fft[0][k], pl->ev_fft[0][k + 1]));
+            if (last_ms_inverse) CUDA_TRY(cudaEventElapsedTime(&last_ms_inverse[k], pl->ev_fft[1][k], pl->ev_fft[1][k + 1]));
+        }
+    }
+    return ARKCOS_OK;
+}
+
+int arkcos_plan_work_model(const arkcos_plan* pl, double* band_pair_modes, double* fft_flops_min, double* tensor_flops,
+                           int* memsets_per_map)
+{
+    if (!pl) return fail(ARKCOS_INVALID_ARG, "NULL plan");
+    if (band_pair_modes) *band_pair_modes = pl->stats.mac_pairs_modes;
+    if (fft_flops_min) *fft_flops_min = pl->stats.fft_flops_min;
+    if (tensor_flops) *tensor_flops = pl->use_tc ? pl->stats.tc_flops : 0.0;
+    if (memsets_per_map) *memsets_per_map = pl->ncapitems > 0 ? (int)pl->cap_zero.size() : 0;
     return ARKCOS_OK;
 }
 

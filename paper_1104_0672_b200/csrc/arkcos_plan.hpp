@@ -9,7 +9,7 @@
 #include "../../include/arkcos.h"
 #include "arkcos_band.cuh"
 #include "arkcos_fft.cuh"
-#include "arkcos_fft3.cuh"
+#include "arkcos_fft3.hpp"
 #include "arkcos_direct.cuh"
 #include "arkcos_band_cached.cuh"
 #include "arkcos_band_tc.hpp"
@@ -27,6 +27,10 @@ struct HostGeometry {
 struct Stats {
     int64_t ring_pairs = 0, row_samples = 0, workspace_bytes = 0;
     double mac_flops = 0, fft_flops = 0;
+    double fft_flops_min = 0;        // ring FFTs of the rings' own lengths (no Bluestein padding), both directions
+    double mac_pairs_modes = 0;      // sum over northern ring pairs of (M/2 + 1): products G_ij[m] B_j[m] per hemisphere
+    double tc_flops = 0;             // tensor-core flops issued per map by band_mac_tc_kernel (3 x TF32, padded tiles)
+    double fft_pixels[10] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0};   // pixels served by each ring-FFT launch, see arkcos_plan_fft_kernels
     double band_flops[8] = {0, 0, 0, 0, 0, 0, 0, 0};   // per band kernel, see arkcos_plan_band_kernels
 };
 
@@ -109,6 +113,7 @@ struct arkcos_plan {
     mutable int timing = 0;
     mutable cudaEvent_t ev[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
     mutable cudaEvent_t ev_band[9] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+    mutable cudaEvent_t ev_fft[2][10] = {};      // timing mode 2: before each ring-FFT launch of a direction and after the last
     // fork/join of the band kernels of the different ring classes
     cudaStream_t side[3] = {nullptr, nullptr, nullptr}, side_rows = nullptr;
     cudaEvent_t ev_fork = nullptr, ev_join[3] = {nullptr, nullptr, nullptr};
