@@ -91,8 +91,10 @@ template <class T> __device__ __forceinline__ cx<T> ext_mode(const cx<T>* __rest
     return v;
 }
 
-// Reference band kernel: one thread per folded output mode m', cosines by rotation re-seeded every RESEED samples.
-// grid = (items, nmaps).
+// Reference band kernel: kGeneralSplit threads per folded output mode m', each taking every kGeneralSplit-th ring pair of
+// the band (the sums meet by warp shuffles), cosines by rotation re-seeded every RESEED samples.  grid = (items, nmaps);
+// an item is a ring and a first mode, kBandThreads / kGeneralSplit modes per block.
+constexpr int kGeneralSplit = 4;
 template <class T, int RESEED>
 __global__ void band_mac_general_kernel(const BandItem* __restrict__ items, const NorthRec* __restrict__ north,
                                         const PairRec* __restrict__ pairs, const T* __restrict__ W,
@@ -102,12 +104,14 @@ __global__ void band_mac_general_kernel(const BandItem* __restrict__ items, cons
     const BandItem it = items[blockIdx.x];
     const int i = it.ring, iS = R - 1 - i;
     const RingRec ri = rings[i];
-    const int Ni = ri.n, mp = it.m0 + (int)threadIdx.x;
-    if (2 * mp > Ni) return;
+    const int slice = (int)threadIdx.x % kGeneralSplit;
+    const int Ni = ri.n, mp_raw = it.m0 + (int)threadIdx.x / kGeneralSplit;
+    const bool live = 2 * mp_raw <= Ni;
+    const int mp = live ? mp_raw : 0;                           // idle threads follow along (the shuffles need whole warps)
     const cx<T>* __restrict__ in = specIn + (int64_t)blockIdx.y * spec_stride;
     cx<T> accN = mk<T>(0, 0), accS = mk<T>(0, 0);
     const NorthRec nr = north[i];
-    for (int p = nr.pair_lo; p < nr.pair_hi; ++p) {
+    for (int p = nr.pair_lo + slice; p < nr.pair_hi; p += kGeneralSplit) {
         const PairRec pr = pairs[p];
         const RingRec rj = rings[pr.j], rjS = rings[R - 1 - pr.j];
         const cx<T>* __restrict__ bN = in + rj.spec_off;
@@ -145,6 +149,12 @@ __global__ void band_mac_general_kernel(const BandItem* __restrict__ items, cons
             }
         }
     }
+#pragma unroll
+    for (int d = 1; d < kGeneralSplit; d <<= 1) {
+        accN.x += __shfl_xor_sync(0xffffffffu, accN.x, d); accN.y += __shfl_xor_sync(0xffffffffu, accN.y, d);
+        accS.x += __shfl_xor_sync(0xffffffffu, accS.x, d); accS.y += __shfl_xor_sync(0xffffffffu, accS.y, d);
+    }
+    if (!live || slice != 0) return;
     cx<T>* __restrict__ out = specOut + (int64_t)blockIdx.y * spec_stride;
     out[ri.spec_off + mp] = accN;
     if (iS != i) out[rings[iS].spec_off + mp] = accS;
@@ -465,51 +475,68 @@ namespace arkcos {
 
 // ---- band kernel for short rings with long rows (the rings next to the poles) ----------------------------------------------
 // There a row covers the whole circle (cnt ~ M/2) and many unfolded modes fold onto each of the few output modes, so the
-// work is spread over the UNFOLDED modes: phase 1, one thread per m in [0, M/2]: T(m) = sum_j G_ij[m] Bp_j[m] into
-// shared memory; phase 2, one thread per folded mode m': the signed sum of T over m = m' + w N_i and w N_i - m'.
-// One block per output ring (and its mirror image); every pair of the ring has the same M.
+// work is spread over the UNFOLDED modes: phase 1, one warp per m in [0, M/2]: T(m) = sum_j G_ij[m] Bp_j[m] into a
+// scratch array; phase 2 (a second, small launch), one thread per folded mode m': the signed sum of T over
+// m = m' + w N_i and w N_i - m'.  Every pair of the ring has the same M.
 constexpr int kPoleThreads = 256;
+constexpr int kPoleWarps = kPoleThreads / 32;
 
-template <class T, int RESEED>
+// Phase 1.  grid = (rings of the list x blocks_per_ring, nmaps); a warp owns one unfolded mode m, its lanes share the
+// samples of a row (stride 32, cosines by rotation with exp(i 64 pi m / M): at most 32 steps) and meet by shuffles.
+// T[m] of the ring and of its mirror image go to scratch[((map * nlist + k) * 2 + hemisphere) * tstride + m].
+template <class T>
 __global__ void __launch_bounds__(kPoleThreads)
-band_mac_pole_kernel(const int* __restrict__ ring_list, const NorthRec* __restrict__ north,
+band_mac_pole_kernel(const int* __restrict__ ring_list, int blocks_per_ring, const NorthRec* __restrict__ north,
                      const PairRec* __restrict__ pairs, const T* __restrict__ W, const RingRec* __restrict__ rings,
-                     int R, const cx<T>* __restrict__ specIn, cx<T>* __restrict__ specOut, int64_t spec_stride)
+                     int R, const cx<T>* __restrict__ specIn, int64_t spec_stride, cx<T>* __restrict__ scratch, int tstride)
 {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    cx<T>* sT = reinterpret_cast<cx<T>*>(smem_raw);             // [2][Mh + 1]
+    const int k = (int)blockIdx.x / blocks_per_ring, lane = (int)threadIdx.x & 31;
+    const int m = ((int)blockIdx.x % blocks_per_ring) * kPoleWarps + ((int)threadIdx.x >> 5);
+    const int i = ring_list[k];
+    const NorthRec nr = north[i];
+    const int M = pairs[nr.pair_lo].M, Mh = M >> 1;
+    if (m > Mh) return;
+    const cx<T>* __restrict__ in = specIn + (int64_t)blockIdx.y * spec_stride;
+    const cx<T> rot = cispi_ratio<T>((64u * (uint32_t)m) % (2u * (uint32_t)M), (uint32_t)M);
+    cx<T> tN = mk<T>(0, 0), tS = mk<T>(0, 0);
+    for (int p = nr.pair_lo; p < nr.pair_hi; ++p) {
+        const PairRec pr = pairs[p];
+        const T* __restrict__ w = W + pr.woff;
+        // G_ij[m] = sum_t w[t] cos(m (2t + par) pi / M)
+        cx<T> c = cispi_ratio<T>(((uint32_t)m * (uint32_t)(2 * lane + pr.par)) % (2u * (uint32_t)M), (uint32_t)M);
+        T G = 0;
+        for (int t = lane; t < pr.cnt; t += 32) {
+            G += w[t] * c.x;
+            c = cmul(c, rot);
+        }
+#pragma unroll
+        for (int d = 16; d > 0; d >>= 1) G += __shfl_xor_sync(0xffffffffu, G, d);
+        const RingRec rj = rings[pr.j], rjS = rings[R - 1 - pr.j];
+        const cx<T> vN = ext_mode(in + rj.spec_off, m, rj.n, rj.shifted);
+        const cx<T> vS = ext_mode(in + rjS.spec_off, m, rjS.n, rjS.shifted);
+        tN.x += G * vN.x; tN.y += G * vN.y;
+        tS.x += G * vS.x; tS.y += G * vS.y;
+    }
+    if (2 * m == M) { tN = cscale(tN, (T)0.5); tS = cscale(tS, (T)0.5); }   // +-M/2 bins: half the Nyquist term each
+    if (lane == 0) {
+        cx<T>* __restrict__ dst = scratch + ((int64_t)blockIdx.y * (gridDim.x / blocks_per_ring) + k) * 2 * tstride;
+        dst[m] = tN;
+        dst[tstride + m] = tS;
+    }
+}
+
+// Phase 2.  grid = (rings of the list, nmaps): one thread per folded mode m', the signed sum of T over m = m' + w N_i and
+// w N_i - m' in a fixed order.
+template <class T>
+__global__ void __launch_bounds__(kPoleThreads)
+band_mac_pole_fold_kernel(const int* __restrict__ ring_list, const NorthRec* __restrict__ north, const PairRec* __restrict__ pairs,
+                          const RingRec* __restrict__ rings, int R, const cx<T>* __restrict__ scratch, int tstride,
+                          cx<T>* __restrict__ specOut, int64_t spec_stride)
+{
     const int i = ring_list[blockIdx.x], iS = R - 1 - i;
     const RingRec ri = rings[i];
-    const NorthRec nr = north[i];
-    const int M = pairs[nr.pair_lo].M, Mh = M >> 1, Ni = ri.n;
-    const cx<T>* __restrict__ in = specIn + (int64_t)blockIdx.y * spec_stride;
-    for (int m = threadIdx.x; m <= Mh; m += kPoleThreads) {
-        const cx<T> rot = cispi_ratio<T>((2u * (uint32_t)m) % (2u * (uint32_t)M), (uint32_t)M);
-        cx<T> tN = mk<T>(0, 0), tS = mk<T>(0, 0);
-        for (int p = nr.pair_lo; p < nr.pair_hi; ++p) {
-            const PairRec pr = pairs[p];
-            const T* __restrict__ w = W + pr.woff;
-            T G = 0;
-            for (int t0 = 0; t0 < pr.cnt; t0 += RESEED) {
-                const uint64_t q = ((uint64_t)m * (uint64_t)(2 * t0 + pr.par)) % (uint64_t)(2 * M);
-                cx<T> c = cispi_ratio<T>((uint32_t)q, (uint32_t)M);
-                const int t1 = min(pr.cnt, t0 + RESEED);
-                for (int t = t0; t < t1; ++t) {
-                    G += w[t] * c.x;
-                    c = cmul(c, rot);
-                }
-            }
-            const RingRec rj = rings[pr.j], rjS = rings[R - 1 - pr.j];
-            const cx<T> vN = ext_mode(in + rj.spec_off, m, rj.n, rj.shifted);
-            const cx<T> vS = ext_mode(in + rjS.spec_off, m, rjS.n, rjS.shifted);
-            tN.x += G * vN.x; tN.y += G * vN.y;
-            tS.x += G * vS.x; tS.y += G * vS.y;
-        }
-        if (2 * m == M) { tN = cscale(tN, (T)0.5); tS = cscale(tS, (T)0.5); }   // +-M/2 bins: half the Nyquist term each
-        sT[m] = tN;
-        sT[Mh + 1 + m] = tS;
-    }
-    __syncthreads();
+    const int M = pairs[north[i].pair_lo].M, Mh = M >> 1, Ni = ri.n;
+    const cx<T>* __restrict__ sT = scratch + ((int64_t)blockIdx.y * gridDim.x + blockIdx.x) * 2 * tstride;
     cx<T>* __restrict__ out = specOut + (int64_t)blockIdx.y * spec_stride;
     for (int mp = threadIdx.x; 2 * mp <= Ni; mp += kPoleThreads) {
         cx<T> aN = mk<T>(0, 0), aS = mk<T>(0, 0);
@@ -517,7 +544,7 @@ band_mac_pole_kernel(const int* __restrict__ ring_list, const NorthRec* __restri
             int wi = fam;
             for (int m = fam ? Ni - mp : mp; m <= Mh; m += Ni, ++wi) {
                 const T sg = (ri.shifted && (wi & 1)) ? (T)-1 : (T)1;        // exp(i m phi0_i) = (-1)^w exp(+-i m' phi0_i)
-                const cx<T> tN = sT[m], tS = sT[Mh + 1 + m];
+                const cx<T> tN = sT[m], tS = sT[tstride + m];
                 aN.x += sg * tN.x; aN.y += (fam ? -sg : sg) * tN.y;
                 aS.x += sg * tS.x; aS.y += (fam ? -sg : sg) * tS.y;
             }

@@ -32,9 +32,3 @@ void tc_launch(int kind, unsigned nitems, unsigned nmaps, cudaStream_t st, const
 
 }  // namespace arkcos
 
-#if ARKCOS_ABL == 7
-extern "C" int arkcos_dbg_read(unsigned long long* out, int n)
-{
-    return (int)cudaMemcpyFromSymbol(out, arkcos::g_dbg, sizeof(unsigned long long) * n);
-}
-#endif

@@ -19,20 +19,10 @@
 // KIND 2: runs of cap rings with one M', single period (M'/2 < N of every ring involved);  3: several periods.
 // The fold of the cap kinds and all sign rules are those of band_mac_capchunk_kernel (arkcos_band.cuh).
 #pragma once
-#ifndef ARKCOS_ABL
-#define ARKCOS_ABL 0
-#endif
 #include "arkcos_band.cuh"
 #include "arkcos_band_tc.hpp"
 
 namespace arkcos {
-
-#if ARKCOS_ABL == 7
-__device__ unsigned long long g_dbg[4096];
-#define DBG(slot) do { if (blockIdx.x == 200 && k < 30) g_dbg[k * 16 + (slot)] = clock64(); } while (0)
-#else
-#define DBG(slot) do {} while (0)
-#endif
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
@@ -132,10 +122,8 @@ band_mac_tc_kernel(const TcItem* __restrict__ items, const TcChunk* __restrict__
     auto fetch_ring = [&](int j, const TcRing& rj) {
         const int idx = CAP ? ext_index(m, rj.n_sh, rj.magic) : m;
         const uint32_t dst = sv0 + 2048u * (uint32_t)(j & (JW - 1));
-#if ARKCOS_ABL != 6
         asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst), "l"(in + rj.offN + idx) : "memory");
         asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst + 8u), "l"(in + rj.offS + idx) : "memory");
-#endif
     };
     if (!producer) {
         // ---- A operand: the cosines of this warpgroup's 128 modes, split into TF32 hi + lo ----------------------------
@@ -222,9 +210,7 @@ band_mac_tc_kernel(const TcItem* __restrict__ items, const TcChunk* __restrict__
         auto tile_step = [&](int k, float4 (&rw)[KC], uint32_t& colw) {
             const int s = k & 1;
             const uint32_t ph = (uint32_t)(k >> 1) & 1u;
-            if (c == 0) DBG(0);
             mbar_wait(&bar_rows[s], ph ^ 1u);                    // the MMAs of tile k - 2 have read this stage
-            if (c == 0) DBG(1);
             float4* sBs = sB + s * 2 * KC * N;
             if (colw != kTcNoPair) {
                 const int cnt = (int)((colw >> 25) & 63u);
@@ -243,13 +229,13 @@ band_mac_tc_kernel(const TcItem* __restrict__ items, const TcChunk* __restrict__
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
             asm volatile("bar.sync 1, %0;" ::"n"(kTcProducers) : "memory");
             if (c == 0) {
-                DBG(2);
                 mbar_wait(&bar_empty[s], ph ^ 1u);               // the consumers have read TMEM stage s (tile k - 2)
-                DBG(3);
                 asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
                 const int ksteps = min(K / 8, (sUmax[s] + 7) >> 3);
                 sUmax[s] = 1;
-                const uint32_t a0 = smem_u32(sA), b0 = smem_u32(sBs);
+                // descriptors differ by the start address only (bits 0-13, in units of 16 bytes; shared memory is < 256 KB,
+                // so adding an offset never carries out of the field): one add per operand and product
+                const uint64_t da0 = tc_smem_desc(smem_u32(sA), 128 * 16, 128), db0 = tc_smem_desc(smem_u32(sBs), N * 16, 128);
 #pragma unroll
                 for (int mt = 0; mt < MT; ++mt) {
                     uint32_t acc_flag = 0;
@@ -257,19 +243,19 @@ band_mac_tc_kernel(const TcItem* __restrict__ items, const TcChunk* __restrict__
 #pragma unroll
                     for (int sp = 0; sp < 3; ++sp) {             // (hi, lo), (lo, hi), then (hi, hi): small terms first
                         const int ha = sp == 1 ? 1 : 0, hb = sp == 0 ? 1 : 0;
-                        for (int ks = 0; ks < ksteps; ++ks) {
-                            const uint64_t da = tc_smem_desc(a0 + (uint32_t)(((mt * 2 + ha) * KC + 2 * ks) * 128 * 16), 128 * 16, 128);
-                            const uint64_t db = tc_smem_desc(b0 + (uint32_t)((hb * KC + 2 * ks) * N * 16), N * 16, 128);
-#if ARKCOS_ABL != 1
-                            tc_mma_tf32(d, da, db, idesc, acc_flag);
-#endif
-                            acc_flag = 1;
+#pragma unroll
+                        for (int ks = 0; ks < K / 8; ++ks) {
+                            if (ks < ksteps) {
+                                const uint64_t da = da0 + (uint64_t)((((mt * 2 + ha) * KC + 2 * ks) * 128 * 16) >> 4);
+                                const uint64_t db = db0 + (uint64_t)((((hb * KC + 2 * ks) * N * 16)) >> 4);
+                                tc_mma_tf32(d, da, db, idesc, acc_flag);
+                                acc_flag = 1;
+                            }
                         }
                     }
                 }
                 tc_commit(&bar_full[s]);
                 tc_commit(&bar_rows[s]);
-                DBG(4);
             }
             // this buffer takes the rows of tile k + 2 (issued behind the fence, which waits for loads in flight)
             if (k + 2 < ntiles) {
@@ -317,9 +303,7 @@ band_mac_tc_kernel(const TcItem* __restrict__ items, const TcChunk* __restrict__
                 for (int q = 0; q < 4; ++q) nx[q] = sRings[min(jhave + 1 + q, tl.jhi) - jbase];
             }
             bool landed = false;
-            if (t == 0) DBG(8);
             mbar_wait(&bar_full[s], ph);
-            if (t == 0) DBG(9);
             asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
 
             float2 acc[TI][2];
@@ -356,18 +340,14 @@ band_mac_tc_kernel(const TcItem* __restrict__ items, const TcChunk* __restrict__
                     soff = (soff + 2048u) & (JW * 2048u - 1u);
                 }
             };
-            auto mac4 = [&](const uint32_t (&g)[16], float4 (&v)[4], int jj0) {
+            auto mac4 = [&](const uint32_t (&g)[16], const float4 (&v)[4]) {
 #pragma unroll
                 for (int q = 0; q < 4; ++q) {
 #pragma unroll
                     for (int ii = 0; ii < TI; ++ii) {
                         const float G = __uint_as_float(g[q * TI + ii]);
-#if ARKCOS_ABL == 2
-                        if (ii == 0) acc[ii][0].x += G + v[q].x + v[q].z;
-#else
                         acc[ii][0] = ffma2(make_float2(G, G), make_float2(v[q].x, v[q].y), acc[ii][0]);
                         acc[ii][1] = ffma2(make_float2(G, G), make_float2(v[q].z, v[q].w), acc[ii][1]);
-#endif
                     }
                 }
             };
@@ -379,26 +359,17 @@ band_mac_tc_kernel(const TcItem* __restrict__ items, const TcChunk* __restrict__
                 load_v(va, 0);
                 for (int jj0 = 0; jj0 < jw; jj0 += 8) {
                     asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-#if ARKCOS_ABL != 3
                     tc_ld16(gb, tbase + (uint32_t)(min(jj0 + 4, JW - 4) * TI));
-#endif
-#if ARKCOS_ABL != 5
                     load_v(vb, jj0 + 4);
-#endif
-                    mac4(ga, va, jj0);
+                    mac4(ga, va);
                     asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-#if ARKCOS_ABL != 3
                     tc_ld16(ga, tbase + (uint32_t)(min(jj0 + 8, JW - 4) * TI));
-#endif
-#if ARKCOS_ABL != 5
                     load_v(va, jj0 + 8);
-#endif
-                    if (jj0 + 4 < jw) mac4(gb, vb, jj0 + 4);
+                    if (jj0 + 4 < jw) mac4(gb, vb);
                 }
                 asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
                 if (!landed) land();
             }
-            if (t == 0) DBG(10);
             asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
             __syncwarp();
             if ((t & 31) == 0) mbar_arrive(&bar_empty[s]);       // this warp is done with TMEM stage s
@@ -416,7 +387,7 @@ band_mac_tc_kernel(const TcItem* __restrict__ items, const TcChunk* __restrict__
             // ---- output: class E stores its mode; cap runs fold onto the ring's own modes ----------------
 #pragma unroll
             for (int ii = 0; ii < TI; ++ii) {
-                if (ii < cur.nti && (ARKCOS_ABL != 4 || acc[ii][0].x == 12345.f)) {
+                if (ii < cur.nti) {
                     const int i = cur.i0 + ii, iS = R - 1 - i;
                     const int offN = cur.offN[ii], offS = cur.offS[ii];
                     if (!CAP) {
@@ -442,7 +413,6 @@ band_mac_tc_kernel(const TcItem* __restrict__ items, const TcChunk* __restrict__
                     }
                 }
             }
-            if (t == 0) DBG(11);
         }
     }
 }

@@ -414,7 +414,9 @@ void build_pairs(HostGeometry& g, double theta_max, double ell_nyq, int fixed_mp
                 t.cap_chunks.push_back(CapChunk{i, 1, M, multi});
             continue;
         }
-        for (int m0 = 0; m0 <= g.n[i] / 2; m0 += band_threads) t.items[cls].push_back(BandItem{i, m0});
+        // the general kernel spends kGeneralSplit threads per mode
+        const int modes_per_block = cls == 0 ? band_threads / kGeneralSplit : band_threads;
+        for (int m0 = 0; m0 <= g.n[i] / 2; m0 += modes_per_block) t.items[cls].push_back(BandItem{i, m0});
     }
     // chunks of consecutive class-E rings: about one block per resident slot of the device (4 blocks per SM)
     {
@@ -838,11 +840,15 @@ template <class T> int enqueue_convolve(const arkcos_plan* pl, const void* d_in,
             pl->d_items[0], pl->d_north, pl->d_pairs, (const T*)pl->d_W, pl->d_rings, g.R, (const cx<T>*)pl->spec_in(),
             (cx<T>*)pl->d_specOut, g.spec_total, pl->opt.variant == 1 ? 1 : 0);
     if (serial) cudaEventRecord(pl->ev_band[1], st);
-    if (pl->npole > 0)
-        band_mac_pole_kernel<T, 16><<<dim3((unsigned)pl->npole, (unsigned)nmaps), kPoleThreads,
-                                       2 * (size_t)(pl->pole_mh + 1) * sizeof(cx<T>), s0>>>(
-            pl->d_pole, pl->d_north, pl->d_pairs, (const T*)pl->d_W, pl->d_rings, g.R, (const cx<T>*)pl->spec_in(),
-            (cx<T>*)pl->d_specOut, g.spec_total);
+    if (pl->npole > 0) {
+        const int tstride = pl->pole_mh + 1, bpr = (tstride + kPoleWarps - 1) / kPoleWarps;
+        band_mac_pole_kernel<T><<<dim3((unsigned)(pl->npole * bpr), (unsigned)nmaps), kPoleThreads, 0, s0>>>(
+            pl->d_pole, bpr, pl->d_north, pl->d_pairs, (const T*)pl->d_W, pl->d_rings, g.R, (const cx<T>*)pl->spec_in(), g.spec_total,
+            (cx<T>*)pl->d_pole_scratch, tstride);
+        band_mac_pole_fold_kernel<T><<<dim3((unsigned)pl->npole, (unsigned)nmaps), kPoleThreads, 0, s0>>>(
+            pl->d_pole, pl->d_north, pl->d_pairs, pl->d_rings, g.R, (const cx<T>*)pl->d_pole_scratch, tstride, (cx<T>*)pl->d_specOut,
+            g.spec_total);
+    }
     if (serial) cudaEventRecord(pl->ev_band[2], st);
     launch_uniform(pl, nmaps, st, serial);
     if (!serial)
@@ -978,6 +984,11 @@ static int plan_create_impl(arkcos_plan** out, const arkcos_pixelization* pix, c
         if (int rc = upload(&pl->d_items[c], t.items[c], wsb)) return rc;
     if (int rc = upload(&pl->d_eqchunks, t.eq_chunks, wsb)) return rc;
     if (int rc = upload(&pl->d_pole, t.pole_rings, wsb)) return rc;
+    if (!t.pole_rings.empty()) {                // unfolded spectra T[m] of the pole kernel, ring and mirror image, per map
+        const size_t nb = (size_t)pl->max_nmaps * t.pole_rings.size() * 2 * (size_t)(t.pole_mh + 1) * 2 * elem_size(dtype);
+        CUDA_TRY(cudaMalloc(&pl->d_pole_scratch, nb));
+        *wsb += (int64_t)nb;
+    }
     if (opt.exact_caps && pix->kind == ARKCOS_HEALPIX_RING) {
         // rings whose band contains a ring shorter than the longest one: caps + the equatorial rings next to them
         const HostGeometry& g = pl->g;
@@ -1193,7 +1204,7 @@ int arkcos_plan_destroy(arkcos_plan* pl)
     void* ptrs[] = {pl->d_rings, pl->d_lens, pl->d_pairs, pl->d_north, pl->d_items[0], pl->d_items[1], pl->d_items[2], pl->d_items[3],
                     pl->d_items[4], pl->d_items[5], pl->d_eqchunks, pl->d_pole, pl->d_chirp, pl->d_phase, pl->d_fft_order, pl->d_table, pl->d_tw, pl->d_filt,
                     pl->d_W, pl->d_specIn, pl->d_specOut, pl->d_stage_in, pl->d_stage_out,
-                    pl->d_cap_chunks, pl->d_cap_chunk_items, pl->d_tc_chunks, pl->d_tc_tiles, pl->d_tc_cols, pl->d_tc_rings, pl->d_tc_items[0], pl->d_tc_items[1], pl->d_tc_items[2], pl->d_goff, pl->d_G, pl->d_direct_items, pl->d_tw3, pl->d_tw16, pl->d_fft3_jobs[0], pl->d_fft3_jobs[1], pl->d_fft3_jobs[2], pl->d_fft3_jobs[3]};
+                    pl->d_cap_chunks, pl->d_cap_chunk_items, pl->d_tc_chunks, pl->d_tc_tiles, pl->d_tc_cols, pl->d_tc_rings, pl->d_tc_items[0], pl->d_tc_items[1], pl->d_tc_items[2], pl->d_goff, pl->d_G, pl->d_pole_scratch, pl->d_direct_items, pl->d_tw3, pl->d_tw16, pl->d_fft3_jobs[0], pl->d_fft3_jobs[1], pl->d_fft3_jobs[2], pl->d_fft3_jobs[3]};
     for (void* p : ptrs) if (p) cudaFree(p);
     for (auto& e : pl->ev) if (e) cudaEventDestroy(e);
     for (auto& e : pl->ev_band) if (e) cudaEventDestroy(e);
@@ -1323,7 +1334,7 @@ int arkcos_plan_launches_per_convolve(const arkcos_plan* pl)
     int fft = pl->nfft_old > 0 ? 1 : 0;
     for (int c = 0; c < 4; ++c) fft += (pl->nfft3_bluestein[c] > 0 ? 1 : 0) + (pl->nfft3[c] > pl->nfft3_bluestein[c] ? 1 : 0);
     n += 2 * fft;
-    n += (pl->nitems[0] > 0) + (pl->npole > 0) + (pl->neqchunks > 0);
+    n += (pl->nitems[0] > 0) + 2 * (pl->npole > 0) + (pl->neqchunks > 0);
     for (int c = 1; c < kBandClasses; ++c) n += pl->nitems[c] > 0 ? 1 : 0;
     n += pl->ndirect > 0 ? 1 : 0;
     n += (pl->ncapsingle > 0 ? 1 : 0) + (pl->ncapitems > pl->ncapsingle ? 1 : 0);

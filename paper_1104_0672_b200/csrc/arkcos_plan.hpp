@@ -77,6 +77,7 @@ struct arkcos_plan {
     int ntc_items[3] = {0, 0, 0};
     int tc_blocks_per_sm = 0;
     int* d_pole = nullptr;
+    void* d_pole_scratch = nullptr;   // cx<T>[max_nmaps][npole][2][pole_mh + 1]: unfolded spectra between the two pole launches
     int npole = 0, pole_mh = 0;
     arkcos::BandItem* d_items[arkcos::kBandClasses] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
     double* d_table = nullptr;
