@@ -28,7 +28,7 @@ def test_launches_per_convolve():
     tab = inputs.gaussian_table(5 * inputs.ARCMIN, 15 * inputs.ARCMIN)
     p = arkcos.Plan(("healpix", 2048), tab, 15 * inputs.ARCMIN, tables_only=True)
     n = p.launches_per_convolve
-    assert n == 25        # rows + 2 x (4 Bluestein size classes + 4 power-of-two classes + shortest rings) + 6 band kernels
+    assert n == 26        # rows + 2 x (4 Bluestein size classes + 4 power-of-two classes + shortest rings) + 7 band launches (the pole kernel is two)
     assert arkcos.Plan(("healpix", 2048), tab, 15 * inputs.ARCMIN, cache_kernel_rows=1,
                        tables_only=True).launches_per_convolve == n - 1
     assert arkcos.Plan(("ecp", 64, 128), inputs.gaussian_table(0.1, 0.2, 64), 0.2, arkcos.F64,
