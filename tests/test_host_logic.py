@@ -32,7 +32,7 @@ def test_launches_per_convolve():
     assert arkcos.Plan(("healpix", 2048), tab, 15 * inputs.ARCMIN, cache_kernel_rows=1,
                        tables_only=True).launches_per_convolve == n - 1
     assert arkcos.Plan(("ecp", 64, 128), inputs.gaussian_table(0.1, 0.2, 64), 0.2, arkcos.F64,
-                       tables_only=True).launches_per_convolve == 4      # rows, forward FFT, one band kernel, inverse FFT (fp64: shared-memory FFT)
+                       tables_only=True).launches_per_convolve == 5      # rows, forward FFT, band (pole kernel: two launches), inverse FFT (fp64: shared-memory FFT)
 
 
 def test_strerror_and_bad_args():
