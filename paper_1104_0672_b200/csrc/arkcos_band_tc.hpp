@@ -16,7 +16,7 @@ constexpr int kTcTI = 4;                   // output rings per tile
 constexpr int kTcJW = 32;                  // input rings a tile's window can hold
 constexpr int kTcN = kTcTI * kTcJW;        // accumulator columns per block of modes
 constexpr int kTcK = 24;                   // sample positions u per row
-constexpr int kTcChunkRings = 24;          // longest run of cap rings handed to one block
+constexpr int kTcChunkRings = 48;          // longest run of cap rings handed to one block
 constexpr int kTcMaxTiles = 16;            // tiles of the longest run (class-E runs: 64 rings); their records live in shared memory
 constexpr int kTcMaxWindow = kTcMaxTiles * kTcTI + kTcJW;   // input rings the tiles of one run can touch
 // cosine operand per block of modes, two stages of the row operand, coefficient window per block of modes

@@ -297,7 +297,9 @@ void build_pairs(HostGeometry& g, double theta_max, double ell_nyq, int fixed_mp
         g.mprime[i] = fixed_mprime > 0 ? fixed_mprime : std::max(8, 2 * (int)ceil(ell_nyq * smax));
         // grids of 512 points and more are rounded up to a multiple of 128 so that runs of consecutive cap rings share one
         // grid length (reading R10; band_mac_capchunk_kernel)
-        if (fixed_mprime <= 0 && g.mprime[i] >= 512) g.mprime[i] = (g.mprime[i] + 127) / 128 * 128;
+        // (multiples of 256 from 2048 on when the tensor-core kernel serves the runs: twice as many rings per block)
+        const int step = use_tc && g.mprime[i] >= 2048 ? 256 : 128;
+        if (fixed_mprime <= 0 && g.mprime[i] >= 512) g.mprime[i] = (g.mprime[i] + step - 1) / step * step;
     }
     for (int i = 0; i < R; ++i) any_odd = any_odd || (g.n[i] == nmax && g.shifted[i] != g.shifted[std::min(i + 1, R - 1)] && g.n[std::min(i + 1, R - 1)] == nmax);
     const int eq_alt = any_odd ? 1 : 0;
