@@ -93,9 +93,9 @@ template <class T> __device__ __forceinline__ cx<T> ext_mode(const cx<T>* __rest
 
 // Reference band kernel: kGeneralSplit threads per folded output mode m', each taking every kGeneralSplit-th ring pair of
 // the band (the sums meet by warp shuffles), cosines by rotation re-seeded every RESEED samples.  grid = (items, nmaps);
-// an item is a ring and a first mode, kBandThreads / kGeneralSplit modes per block.
-constexpr int kGeneralSplit = 4;
-template <class T, int RESEED>
+// an item is a ring and a first mode, kBandThreads / kGeneralSplit modes per block.  The plan picks kGeneralSplit = 4 when
+// the kernel has too few blocks to fill the device (it is latency-bound then), 1 otherwise (coalesced coefficient loads).
+template <class T, int RESEED, int kGeneralSplit>
 __global__ void band_mac_general_kernel(const BandItem* __restrict__ items, const NorthRec* __restrict__ north,
                                         const PairRec* __restrict__ pairs, const T* __restrict__ W,
                                         const RingRec* __restrict__ rings, int R, const cx<T>* __restrict__ specIn,
@@ -481,6 +481,67 @@ namespace arkcos {
 constexpr int kPoleThreads = 256;
 constexpr int kPoleWarps = kPoleThreads / 32;
 
+// Many such rings (a hard-edged kernel with a fine grid: > 100 rings per cap): one block per output ring, a thread per
+// unfolded mode walks the samples of a row itself; T through shared memory, both phases in one launch.
+template <class T, int RESEED>
+__global__ void __launch_bounds__(kPoleThreads)
+band_mac_pole1_kernel(const int* __restrict__ ring_list, const NorthRec* __restrict__ north,
+                     const PairRec* __restrict__ pairs, const T* __restrict__ W, const RingRec* __restrict__ rings,
+                     int R, const cx<T>* __restrict__ specIn, cx<T>* __restrict__ specOut, int64_t spec_stride)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cx<T>* sT = reinterpret_cast<cx<T>*>(smem_raw);             // [2][Mh + 1]
+    const int i = ring_list[blockIdx.x], iS = R - 1 - i;
+    const RingRec ri = rings[i];
+    const NorthRec nr = north[i];
+    const int M = pairs[nr.pair_lo].M, Mh = M >> 1, Ni = ri.n;
+    const cx<T>* __restrict__ in = specIn + (int64_t)blockIdx.y * spec_stride;
+    for (int m = threadIdx.x; m <= Mh; m += kPoleThreads) {
+        const cx<T> rot = cispi_ratio<T>((2u * (uint32_t)m) % (2u * (uint32_t)M), (uint32_t)M);
+        cx<T> tN = mk<T>(0, 0), tS = mk<T>(0, 0);
+        for (int p = nr.pair_lo; p < nr.pair_hi; ++p) {
+            const PairRec pr = pairs[p];
+            const T* __restrict__ w = W + pr.woff;
+            T G = 0;
+            for (int t0 = 0; t0 < pr.cnt; t0 += RESEED) {
+                const uint64_t q = ((uint64_t)m * (uint64_t)(2 * t0 + pr.par)) % (uint64_t)(2 * M);
+                cx<T> c = cispi_ratio<T>((uint32_t)q, (uint32_t)M);
+                const int t1 = min(pr.cnt, t0 + RESEED);
+                for (int t = t0; t < t1; ++t) {
+                    G += w[t] * c.x;
+                    c = cmul(c, rot);
+                }
+            }
+            const RingRec rj = rings[pr.j], rjS = rings[R - 1 - pr.j];
+            const cx<T> vN = ext_mode(in + rj.spec_off, m, rj.n, rj.shifted);
+            const cx<T> vS = ext_mode(in + rjS.spec_off, m, rjS.n, rjS.shifted);
+            tN.x += G * vN.x; tN.y += G * vN.y;
+            tS.x += G * vS.x; tS.y += G * vS.y;
+        }
+        if (2 * m == M) { tN = cscale(tN, (T)0.5); tS = cscale(tS, (T)0.5); }   // +-M/2 bins: half the Nyquist term each
+        sT[m] = tN;
+        sT[Mh + 1 + m] = tS;
+    }
+    __syncthreads();
+    cx<T>* __restrict__ out = specOut + (int64_t)blockIdx.y * spec_stride;
+    for (int mp = threadIdx.x; 2 * mp <= Ni; mp += kPoleThreads) {
+        cx<T> aN = mk<T>(0, 0), aS = mk<T>(0, 0);
+        for (int fam = 0; fam < 2; ++fam) {
+            int wi = fam;
+            for (int m = fam ? Ni - mp : mp; m <= Mh; m += Ni, ++wi) {
+                const T sg = (ri.shifted && (wi & 1)) ? (T)-1 : (T)1;        // exp(i m phi0_i) = (-1)^w exp(+-i m' phi0_i)
+                const cx<T> tN = sT[m], tS = sT[Mh + 1 + m];
+                aN.x += sg * tN.x; aN.y += (fam ? -sg : sg) * tN.y;
+                aS.x += sg * tS.x; aS.y += (fam ? -sg : sg) * tS.y;
+            }
+        }
+        out[ri.spec_off + mp] = aN;
+        if (iS != i) out[rings[iS].spec_off + mp] = aS;
+    }
+}
+
+
+// Few such rings (a smooth kernel: ~10 per cap, too few blocks to fill the device): two launches.
 // Phase 1.  grid = (rings of the list x blocks_per_ring, nmaps); a warp owns one unfolded mode m, its lanes share the
 // samples of a row (stride 32, cosines by rotation with exp(i 64 pi m / M): at most 32 steps) and meet by shuffles.
 // T[m] of the ring and of its mirror image go to scratch[((map * nlist + k) * 2 + hemisphere) * tstride + m].

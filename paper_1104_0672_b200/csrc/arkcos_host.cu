@@ -168,6 +168,8 @@ struct HostTables {
     std::vector<std::pair<int64_t, int64_t>> cap_zero;   // (first coefficient, count) ranges of the output spectrum to clear
     std::vector<int> pole_rings;                 // rings for band_mac_pole_kernel
     int pole_mh = 0;
+    int general_split = 1;                       // threads per mode of band_mac_general_kernel
+    bool pole_warp_per_mode = false;             // long rows: band_mac_pole_kernel + fold; short rows: band_mac_pole1_kernel
     std::vector<EqChunk> eq_chunks;              // runs of consecutive class-E rings for band_mac_eq_kernel   // per band-kernel class (see band_class)
     int eq_alt = 0;
     bool use_tc = false;                         // tensor-core band kernels (arkcos_band_tc.cuh) serve the class-E and cap runs
@@ -176,14 +178,16 @@ struct HostTables {
     std::vector<uint32_t> tc_cols;
     std::vector<TcItem> tc_items[3];             // thread blocks: 0 class-E runs, 1 cap runs (single period), 2 cap runs (several)
     std::vector<TcRing> tc_rings;                // per ring: spectrum offsets (ring, mirror image), length | shifted, magic divisor
-    std::vector<int> fft_order;          // rings of the shared-memory FFT kernels, sorted by decreasing transform size
-    std::vector<FftJob> fft3_jobs[4];    // jobs of the register-resident FFT kernels, Q = 512 << k
+    // per direction (0 forward, 1 inverse): exact_caps plans transform only the rings the hybrid pass needs
+    std::vector<int> fft_order[2];       // rings of the shared-memory FFT kernels, sorted by decreasing transform size
+    std::vector<FftJob> fft3_jobs[2][4]; // jobs of the register-resident FFT kernels, Q = 512 << k
     int64_t filt_total = 0, chirp_total = 0, ph_total = 0, nsamples = 0;
     int logPT = 1;
 };
 
 // FFT length table: one entry per distinct ring length
-void build_fft_lens(const HostGeometry& g, HostTables& t, Stats& st, bool use_fft3)
+// need[d][i]: ring i is transformed in direction d (0 forward, 1 inverse)
+void build_fft_lens(const HostGeometry& g, HostTables& t, Stats& st, bool use_fft3, const std::vector<char> (&need)[2])
 {
     std::map<int, int> id_of;
     t.rings.resize(g.R);
@@ -220,59 +224,64 @@ void build_fft_lens(const HostGeometry& g, HostTables& t, Stats& st, bool use_ff
         const FftLen& f = t.lens[r.len_id];
         const double P = (double)(1 << f.logP);
         // forward + inverse: complex FFT(s) + O(N) split / chirps
-        st.fft_flops += 2.0 * (f.pow2 ? 5.0 * P * f.logP + 20.0 * L : 2.0 * 5.0 * P * f.logP + 6.0 * P + 32.0 * L);
-        st.fft_flops_min += 2.0 * (5.0 * L * log2((double)std::max(L, 2)) + 20.0 * L);
+        const double ndir = (need[0][i] ? 1.0 : 0.0) + (need[1][i] ? 1.0 : 0.0);
+        st.fft_flops += ndir * (f.pow2 ? 5.0 * P * f.logP + 20.0 * L : 2.0 * 5.0 * P * f.logP + 6.0 * P + 32.0 * L);
+        st.fft_flops_min += ndir * (5.0 * L * log2((double)std::max(L, 2)) + 20.0 * L);
     }
     // Rings whose transform size Q (L for a power of two, half the Bluestein convolution length otherwise) is 512 .. 4096
     // go to the register-resident kernels: Bluestein rings first, a ring next to its mirror image (same tables), then
     // the power-of-two rings two per block.  Everything else stays with the shared-memory kernels.
-    std::vector<int> direct[4];
-    std::vector<char> taken(g.R, 0);
     auto cls_of = [&](int i) {
         const FftLen& f = t.lens[t.rings[i].len_id];
         const int logq = f.pow2 ? f.logP : f.logP - 1;
         return (use_fft3 && logq >= 9 && logq <= 12) ? logq - 9 : -1;
     };
-    for (int i = g.R / 2; i >= 0; --i) {                 // longest rings first
-        const int twin[2] = {i, g.R - 1 - i};
-        for (int h = 0; h < 2; ++h) {
-            const int r = twin[h];
-            const int c = cls_of(r);
-            if (c < 0 || taken[r]) continue;
-            taken[r] = 1;
-            if (t.lens[t.rings[r].len_id].pow2) direct[c].push_back(r);
-            else {
-                FftJob j{};
-                j.r0 = t.rings[r];
-                j.f = t.lens[t.rings[r].len_id];
-                t.fft3_jobs[c].push_back(j);
+    for (int d = 0; d < 2; ++d) {
+        std::vector<int> direct[4];
+        std::vector<char> taken(g.R, 0);
+        for (int i = g.R / 2; i >= 0; --i) {                 // longest rings first
+            const int twin[2] = {i, g.R - 1 - i};
+            for (int h = 0; h < 2; ++h) {
+                const int r = twin[h];
+                const int c = cls_of(r);
+                if (c < 0 || taken[r]) continue;
+                taken[r] = 1;
+                if (!need[d][r]) continue;
+                if (t.lens[t.rings[r].len_id].pow2) direct[c].push_back(r);
+                else {
+                    FftJob j{};
+                    j.r0 = t.rings[r];
+                    j.f = t.lens[t.rings[r].len_id];
+                    t.fft3_jobs[d][c].push_back(j);
+                }
             }
         }
+        for (int c = 0; c < 4; ++c)
+            for (size_t k = 0; k < direct[c].size(); k += 2)
+            {
+                FftJob j{};
+                j.r0 = t.rings[direct[c][k]];
+                j.f = t.lens[j.r0.len_id];
+                j.has1 = k + 1 < direct[c].size() ? 1 : 0;
+                if (j.has1) j.r1 = t.rings[direct[c][k + 1]];
+                t.fft3_jobs[d][c].push_back(j);
+            }
+        for (int i = 0; i < g.R; ++i)
+            if (!taken[i] && need[d][i]) t.fft_order[d].push_back(i);
+        std::stable_sort(t.fft_order[d].begin(), t.fft_order[d].end(), [&](int a, int b) {
+            const FftLen &fa = t.lens[t.rings[a].len_id], &fb = t.lens[t.rings[b].len_id];
+            const int wa = (fa.pow2 ? 1 : 2) << fa.logP, wb = (fb.pow2 ? 1 : 2) << fb.logP;
+            return wa > wb;
+        });
     }
+    // launch order of one direction: Q = 4096 power-of-two, Bluestein, then 2048, 1024, 512 alike, then the shared-memory
+    // kernel (pixel counts of the forward direction; the inverse differs only for exact_caps plans)
     for (int c = 0; c < 4; ++c)
-        for (size_t k = 0; k < direct[c].size(); k += 2)
-        {
-            FftJob j{};
-            j.r0 = t.rings[direct[c][k]];
-            j.f = t.lens[j.r0.len_id];
-            j.has1 = k + 1 < direct[c].size() ? 1 : 0;
-            if (j.has1) j.r1 = t.rings[direct[c][k + 1]];
-            t.fft3_jobs[c].push_back(j);
-        }
-    for (int i = 0; i < g.R; ++i)
-        if (!taken[i]) t.fft_order.push_back(i);
-    // launch order of one direction: Q = 4096 power-of-two, Bluestein, then 2048, 1024, 512 alike, then the shared-memory kernel
-    for (int c = 0; c < 4; ++c)
-        for (const FftJob& j : t.fft3_jobs[c]) {
+        for (const FftJob& j : t.fft3_jobs[0][c]) {
             const int slot = 2 * (3 - c) + (j.f.pow2 ? 0 : 1);
             st.fft_pixels[slot] += j.r0.n + (j.has1 ? j.r1.n : 0);
         }
-    for (int i : t.fft_order) st.fft_pixels[8] += g.n[i];
-    std::stable_sort(t.fft_order.begin(), t.fft_order.end(), [&](int a, int b) {
-        const FftLen &fa = t.lens[t.rings[a].len_id], &fb = t.lens[t.rings[b].len_id];
-        const int wa = (fa.pow2 ? 1 : 2) << fa.logP, wb = (fb.pow2 ? 1 : 2) << fb.logP;
-        return wa > wb;
-    });
+    for (int i : t.fft_order[0]) st.fft_pixels[8] += g.n[i];
 }
 
 // Ring-pair table for the northern output rings (the southern ones reuse the rows of their mirror images).
@@ -286,7 +295,7 @@ void build_pairs(HostGeometry& g, double theta_max, double ell_nyq, int fixed_mp
     for (int i = 0; i < nnorth && use_tc; ++i)
         use_tc = g.band_hi[std::min(i + kTcTI - 1, nnorth - 1)] - g.band_lo[i] + 1 <= kTcJW;
     t.use_tc = use_tc;
-    std::vector<int> eq_rings;
+    std::vector<int> eq_rings, general_rings;
     bool any_odd = false;
     const double shm = sin(0.5 * theta_max), xmax = 4.0 * shm * shm;
     g.mprime.assign(R, 0);
@@ -339,13 +348,15 @@ void build_pairs(HostGeometry& g, double theta_max, double ell_nyq, int fixed_mp
             p.woff = t.nsamples;
             t.nsamples += (p.cnt + 3) & ~3;          // rows are stored zero-padded to a multiple of four samples
             t.pairs.push_back(p);
+            st.ring_pairs += has_mirror ? 2 : 1;
+            if (g.direct[i]) continue;               // (the direct-space sum uses the pair record, the hybrid pass skips the ring)
             const double modes = p.M / 2 + 1;
             ring_flops += modes * (2.0 * p.cnt + (has_mirror ? 8.0 : 4.0));
             st.mac_flops += modes * (2.0 * p.cnt + (has_mirror ? 8.0 : 4.0));
             st.mac_pairs_modes += modes;
-            st.ring_pairs += has_mirror ? 2 : 1;
         }
         t.north[i].pair_hi = (int)t.pairs.size();
+        if (g.direct[i]) continue;
         // which band kernel serves this ring: the fast ones need one grid length M for the whole ring, short rows
         // and few pairs (rows and pair records live in shared memory)
         int cls = 0;
@@ -416,9 +427,21 @@ void build_pairs(HostGeometry& g, double theta_max, double ell_nyq, int fixed_mp
                 t.cap_chunks.push_back(CapChunk{i, 1, M, multi});
             continue;
         }
-        // the general kernel spends kGeneralSplit threads per mode
-        const int modes_per_block = cls == 0 ? band_threads / kGeneralSplit : band_threads;
-        for (int m0 = 0; m0 <= g.n[i] / 2; m0 += modes_per_block) t.items[cls].push_back(BandItem{i, m0});
+        if (cls == 0) { general_rings.push_back(i); continue; }      // items once the split is known
+        for (int m0 = 0; m0 <= g.n[i] / 2; m0 += band_threads) t.items[cls].push_back(BandItem{i, m0});
+    }
+    // general kernel: four threads per mode when it would have too few blocks to fill the device
+    {
+        int64_t blocks1 = 0;
+        for (int i : general_rings) blocks1 += (g.n[i] / 2 + band_threads) / band_threads;
+        t.general_split = blocks1 < 8 * (int64_t)sm_count ? 4 : 1;
+        std::vector<BandItem> nyq = t.items[0];                  // (Nyquist bins of cached-spectra plans were added above)
+        t.items[0].clear();
+        for (int i : general_rings)
+            for (int m0 = 0; m0 <= g.n[i] / 2; m0 += band_threads / t.general_split) t.items[0].push_back(BandItem{i, m0});
+        t.items[0].insert(t.items[0].end(), nyq.begin(), nyq.end());
+        // pole kernel: one block per ring leaves the device idle when the rings are few; then a warp per mode, two launches
+        t.pole_warp_per_mode = !t.pole_rings.empty() && 4 * (int)t.pole_rings.size() <= sm_count;
     }
     // chunks of consecutive class-E rings: about one block per resident slot of the device (4 blocks per SM)
     {
@@ -537,10 +560,11 @@ template <class T, int BPT> int set_fft_smem(size_t bytes)
 template <class T> int setup_fft3(arkcos_plan* pl, const HostTables& t)
 {
     if constexpr (sizeof(T) == 4) {
-    for (int c = 0; c < 4; ++c) {
-        pl->nfft3[c] = (int)t.fft3_jobs[c].size();
-        if (int rc = upload(&pl->d_fft3_jobs[c], t.fft3_jobs[c], &pl->stats.workspace_bytes)) return rc;
-    }
+    for (int d = 0; d < 2; ++d)
+        for (int c = 0; c < 4; ++c) {
+            pl->nfft3[d][c] = (int)t.fft3_jobs[d][c].size();
+            if (int rc = upload(&pl->d_fft3_jobs[d][c], t.fft3_jobs[d][c], &pl->stats.workspace_bytes)) return rc;
+        }
     std::vector<cx<float>> tw16(256);
     for (int k = 0; k < 16; ++k)
         for (int r = 0; r < 16; ++r)
@@ -590,8 +614,10 @@ template <class T> int build_device_numeric(arkcos_plan* pl, const HostTables& t
     pl->d_chirp = d_chirp;
     if (int rc = upload(&d_phase, phase, &pl->stats.workspace_bytes)) return rc;
     pl->d_phase = d_phase;
-    if (int rc = upload(&pl->d_fft_order, t.fft_order, &pl->stats.workspace_bytes)) return rc;
-    pl->nfft_old = (int)t.fft_order.size();
+    for (int d = 0; d < 2; ++d) {
+        if (int rc = upload(&pl->d_fft_order[d], t.fft_order[d], &pl->stats.workspace_bytes)) return rc;
+        pl->nfft_old[d] = (int)t.fft_order[d].size();
+    }
     if (int rc = setup_fft3<T>(pl, t)) return rc;
     pl->fft_smem = fft_smem_elems(PT) * sizeof(cx<T>);
     pl->fft_bpt = PT <= 8 * kFftThreads * 2 ? 2 : 4;
@@ -718,7 +744,7 @@ template <int LOGQ, bool FWD>
 void launch_fft3(const arkcos_plan* pl, const void* d_in, void* d_out, int nmaps, cudaStream_t st)
 {
     const int c = LOGQ - 9, dir = FWD ? 0 : 1, slot = 2 * (3 - c);
-    if (pl->nfft3[c] == 0) {
+    if (pl->nfft3[dir][c] == 0) {
         if (pl->timing == 2) { cudaEventRecord(pl->ev_fft[dir][slot], st); cudaEventRecord(pl->ev_fft[dir][slot + 1], st); }
         return;
     }
@@ -736,13 +762,13 @@ void launch_fft3(const arkcos_plan* pl, const void* d_in, void* d_out, int nmaps
     a.chirp = (const cx<float>*)pl->d_chirp;
     a.phase = (const cx<float>*)pl->d_phase;
     a.logPT = pl->logPT;
-    const int nb = pl->nfft3_bluestein[c], nd = pl->nfft3[c] - nb;
+    const int nb = pl->nfft3_bluestein[dir][c], nd = pl->nfft3[dir][c] - nb;
     if (pl->timing == 2) cudaEventRecord(pl->ev_fft[dir][slot], st);
     if (nd > 0)                                       // power-of-two rings: one transform per block
-        fft3_launch_direct(LOGQ, FWD, pl->d_fft3_jobs[c] + nb, (unsigned)nd, (unsigned)nmaps, st, a);
+        fft3_launch_direct(LOGQ, FWD, pl->d_fft3_jobs[dir][c] + nb, (unsigned)nd, (unsigned)nmaps, st, a);
     if (pl->timing == 2) cudaEventRecord(pl->ev_fft[dir][slot + 1], st);
     if (nb > 0)
-        fft3_launch_bluestein(LOGQ, FWD, pl->d_fft3_jobs[c], (unsigned)nb, (unsigned)nmaps, st, a, pl->sm_count);
+        fft3_launch_bluestein(LOGQ, FWD, pl->d_fft3_jobs[dir][c], (unsigned)nb, (unsigned)nmaps, st, a, pl->sm_count);
 }
 
 template <class T, bool FWD>
@@ -751,8 +777,9 @@ void launch_ring_ffts(const arkcos_plan* pl, const void* d_in, void* d_out, int 
     const HostGeometry& g = pl->g;
     bool forked = false;
     if constexpr (sizeof(T) == 4) {
-        const int nside_launches = (pl->nfft3[2] > 0) + (pl->nfft3[1] + pl->nfft3[0] > 0) + (pl->nfft_old > 0);
-        forked = pl->nfft3[3] > 0 && nside_launches > 0 && pl->timing != 2;
+        const int dir = FWD ? 0 : 1;
+        const int nside_launches = (pl->nfft3[dir][2] > 0) + (pl->nfft3[dir][1] + pl->nfft3[dir][0] > 0) + (pl->nfft_old[dir] > 0);
+        forked = pl->nfft3[dir][3] > 0 && nside_launches > 0 && pl->timing != 2;
         if (forked) {
             cudaEventRecord(pl->ev_fork, st);
             for (int k = 0; k < 3; ++k) cudaStreamWaitEvent(pl->side[k], pl->ev_fork, 0);
@@ -764,26 +791,26 @@ void launch_ring_ffts(const arkcos_plan* pl, const void* d_in, void* d_out, int 
     } else if (pl->timing == 2)
         for (int k = 0; k < 8; ++k) cudaEventRecord(pl->ev_fft[FWD ? 0 : 1][k], st);
     if (pl->timing == 2) cudaEventRecord(pl->ev_fft[FWD ? 0 : 1][8], st);
-    if (pl->nfft_old > 0) {
+    if (pl->nfft_old[FWD ? 0 : 1] > 0) {
         cudaStream_t so = forked ? pl->side[2] : st;
-        const dim3 gfft((unsigned)pl->nfft_old, (unsigned)nmaps);
+        const dim3 gfft((unsigned)pl->nfft_old[FWD ? 0 : 1], (unsigned)nmaps);
         if (FWD) {
             if (pl->fft_bpt == 2)
                 ring_fft_forward_kernel<T, 2><<<gfft, kFftThreads, pl->fft_smem, so>>>(
-                    (const T*)d_in, g.npix, (cx<T>*)pl->spec_in(), g.spec_total, pl->d_rings, pl->d_fft_order, pl->d_lens,
+                    (const T*)d_in, g.npix, (cx<T>*)pl->spec_in(), g.spec_total, pl->d_rings, pl->d_fft_order[FWD ? 0 : 1], pl->d_lens,
                     (const cx<T>*)pl->d_tw, pl->logPT, (const cx<T>*)pl->d_filt, (const cx<T>*)pl->d_chirp, (const cx<T>*)pl->d_phase);
             else
                 ring_fft_forward_kernel<T, 4><<<gfft, kFftThreads, pl->fft_smem, so>>>(
-                    (const T*)d_in, g.npix, (cx<T>*)pl->spec_in(), g.spec_total, pl->d_rings, pl->d_fft_order, pl->d_lens,
+                    (const T*)d_in, g.npix, (cx<T>*)pl->spec_in(), g.spec_total, pl->d_rings, pl->d_fft_order[FWD ? 0 : 1], pl->d_lens,
                     (const cx<T>*)pl->d_tw, pl->logPT, (const cx<T>*)pl->d_filt, (const cx<T>*)pl->d_chirp, (const cx<T>*)pl->d_phase);
         } else {
             if (pl->fft_bpt == 2)
                 ring_fft_inverse_kernel<T, 2><<<gfft, kFftThreads, pl->fft_smem, so>>>(
-                    (const cx<T>*)pl->d_specOut, g.spec_total, (T*)d_out, g.npix, pl->d_rings, pl->d_fft_order, pl->d_lens,
+                    (const cx<T>*)pl->d_specOut, g.spec_total, (T*)d_out, g.npix, pl->d_rings, pl->d_fft_order[FWD ? 0 : 1], pl->d_lens,
                     (const cx<T>*)pl->d_tw, pl->logPT, (const cx<T>*)pl->d_filt, (const cx<T>*)pl->d_chirp, (const cx<T>*)pl->d_phase);
             else
                 ring_fft_inverse_kernel<T, 4><<<gfft, kFftThreads, pl->fft_smem, so>>>(
-                    (const cx<T>*)pl->d_specOut, g.spec_total, (T*)d_out, g.npix, pl->d_rings, pl->d_fft_order, pl->d_lens,
+                    (const cx<T>*)pl->d_specOut, g.spec_total, (T*)d_out, g.npix, pl->d_rings, pl->d_fft_order[FWD ? 0 : 1], pl->d_lens,
                     (const cx<T>*)pl->d_tw, pl->logPT, (const cx<T>*)pl->d_filt, (const cx<T>*)pl->d_chirp, (const cx<T>*)pl->d_phase);
         }
     }
@@ -837,12 +864,24 @@ template <class T> int enqueue_convolve(const arkcos_plan* pl, const void* d_in,
         for (int k = 0; k < 3; ++k) cudaStreamWaitEvent(pl->side[k], pl->ev_fork, 0);
     }
     if (serial) cudaEventRecord(pl->ev_band[0], st);
-    if (pl->nitems[0] > 0)
-        band_mac_general_kernel<T, 16><<<dim3((unsigned)pl->nitems[0], (unsigned)nmaps), kBandThreads, 0, s0>>>(
-            pl->d_items[0], pl->d_north, pl->d_pairs, (const T*)pl->d_W, pl->d_rings, g.R, (const cx<T>*)pl->spec_in(),
-            (cx<T>*)pl->d_specOut, g.spec_total, pl->opt.variant == 1 ? 1 : 0);
+    if (pl->nitems[0] > 0) {
+        const dim3 gg((unsigned)pl->nitems[0], (unsigned)nmaps);
+        if (pl->general_split == 4)
+            band_mac_general_kernel<T, 16, 4><<<gg, kBandThreads, 0, s0>>>(
+                pl->d_items[0], pl->d_north, pl->d_pairs, (const T*)pl->d_W, pl->d_rings, g.R, (const cx<T>*)pl->spec_in(),
+                (cx<T>*)pl->d_specOut, g.spec_total, pl->opt.variant == 1 ? 1 : 0);
+        else
+            band_mac_general_kernel<T, 16, 1><<<gg, kBandThreads, 0, s0>>>(
+                pl->d_items[0], pl->d_north, pl->d_pairs, (const T*)pl->d_W, pl->d_rings, g.R, (const cx<T>*)pl->spec_in(),
+                (cx<T>*)pl->d_specOut, g.spec_total, pl->opt.variant == 1 ? 1 : 0);
+    }
     if (serial) cudaEventRecord(pl->ev_band[1], st);
-    if (pl->npole > 0) {
+    if (pl->npole > 0 && !pl->pole_warp_per_mode)
+        band_mac_pole1_kernel<T, 16><<<dim3((unsigned)pl->npole, (unsigned)nmaps), kPoleThreads,
+                                        2 * (size_t)(pl->pole_mh + 1) * sizeof(cx<T>), s0>>>(
+            pl->d_pole, pl->d_north, pl->d_pairs, (const T*)pl->d_W, pl->d_rings, g.R, (const cx<T>*)pl->spec_in(),
+            (cx<T>*)pl->d_specOut, g.spec_total);
+    else if (pl->npole > 0) {
         const int tstride = pl->pole_mh + 1, bpr = (tstride + kPoleWarps - 1) / kPoleWarps;
         band_mac_pole_kernel<T><<<dim3((unsigned)(pl->npole * bpr), (unsigned)nmaps), kPoleThreads, 0, s0>>>(
             pl->d_pole, bpr, pl->d_north, pl->d_pairs, (const T*)pl->d_W, pl->d_rings, g.R, (const cx<T>*)pl->spec_in(), g.spec_total,
@@ -948,7 +987,23 @@ static int plan_create_impl(arkcos_plan** out, const arkcos_pixelization* pix, c
     if (!tables_only) CUDA_TRY(cudaDeviceGetAttribute(&sm_count, cudaDevAttrMultiProcessorCount, pl->device));
     pl->sm_count = sm_count;
     HostTables t;
-    build_fft_lens(pl->g, t, pl->stats, dtype == ARKCOS_F32);
+    // exact_caps: every output ring whose band contains a ring shorter than the longest one (the caps and the equatorial
+    // rings next to them) comes from the direct-space sum; the hybrid pass then needs forward transforms of the full-length
+    // rings only (the bands of the rings it still serves hold nothing else) and inverse transforms of those rings alone
+    std::vector<char> need[2] = {std::vector<char>(pl->g.R, 1), std::vector<char>(pl->g.R, 1)};
+    pl->g.direct.assign(pl->g.R, 0);
+    if (opt.exact_caps && pix->kind == ARKCOS_HEALPIX_RING) {
+        HostGeometry& g = pl->g;
+        const int nmax = *std::max_element(g.n.begin(), g.n.end());
+        for (int i = 0; i < g.R; ++i) {
+            bool all_full = true;
+            for (int j = g.band_lo[i]; j <= g.band_hi[i]; ++j) all_full = all_full && g.n[j] == nmax;
+            g.direct[i] = all_full ? 0 : 1;
+            need[0][i] = g.n[i] == nmax;
+            need[1][i] = all_full;
+        }
+    }
+    build_fft_lens(pl->g, t, pl->stats, dtype == ARKCOS_F32, need);
     build_pairs(pl->g, pl->theta_max, pl->ell_nyquist, fixed_mprime, kBandThreads, dtype == ARKCOS_F32 && opt.variant == 0, opt.variant == 0, opt.cache_kernel_spectra != 0, opt.no_tensor_cores == 0, sm_count, t, pl->stats);
     if (t.pairs.size() > (size_t)INT32_MAX) return fail(ARKCOS_UNSUPPORTED, "too many ring pairs");
     pl->nnorth = (int)t.north.size();
@@ -960,16 +1015,20 @@ static int plan_create_impl(arkcos_plan** out, const arkcos_pixelization* pix, c
     if (t.nsamples / 4 >= (1 << 25)) return fail(ARKCOS_UNSUPPORTED, "too many kernel-row samples");
     pl->npole = (int)t.pole_rings.size();
     pl->pole_mh = t.pole_mh;
+    pl->general_split = t.general_split;
+    pl->pole_warp_per_mode = t.pole_warp_per_mode;
     pl->eq_alt = t.eq_alt;
     pl->eq_mh = t.eq_chunks.empty() ? 0 : pl->g.n[t.eq_chunks[0].i0] / 2;
     for (const EqChunk& c : t.eq_chunks) pl->eq_mh = std::max(pl->eq_mh, pl->g.n[c.i0] / 2);
     pl->nsamples = t.nsamples;
     pl->logPT = t.logPT;
-    pl->nfft_old = (int)t.fft_order.size();
-    for (int c = 0; c < 4; ++c) {
-        pl->nfft3[c] = (int)t.fft3_jobs[c].size();
-        pl->nfft3_bluestein[c] = 0;
-        for (const FftJob& j : t.fft3_jobs[c]) pl->nfft3_bluestein[c] += j.f.pow2 ? 0 : 1;
+    for (int d = 0; d < 2; ++d) {
+        pl->nfft_old[d] = (int)t.fft_order[d].size();
+        for (int c = 0; c < 4; ++c) {
+            pl->nfft3[d][c] = (int)t.fft3_jobs[d][c].size();
+            pl->nfft3_bluestein[d][c] = 0;
+            for (const FftJob& j : t.fft3_jobs[d][c]) pl->nfft3_bluestein[d][c] += j.f.pow2 ? 0 : 1;
+        }
     }
 
     if (tables_only) {
@@ -992,14 +1051,10 @@ static int plan_create_impl(arkcos_plan** out, const arkcos_pixelization* pix, c
         *wsb += (int64_t)nb;
     }
     if (opt.exact_caps && pix->kind == ARKCOS_HEALPIX_RING) {
-        // rings whose band contains a ring shorter than the longest one: caps + the equatorial rings next to them
         const HostGeometry& g = pl->g;
-        const int nmax = *std::max_element(g.n.begin(), g.n.end());
         std::vector<BandItem> items;
         for (int i = 0; i < (g.R + 1) / 2; ++i) {
-            bool all_full = true;
-            for (int j = g.band_lo[i]; j <= g.band_hi[i]; ++j) all_full = all_full && g.n[j] == nmax;
-            if (all_full) continue;
+            if (!g.direct[i]) continue;
             for (int k0 = 0; k0 < g.n[i]; k0 += kDirectThreads) items.push_back(BandItem{i, k0});
         }
         pl->ndirect = (int)items.size();
@@ -1204,9 +1259,10 @@ int arkcos_plan_destroy(arkcos_plan* pl)
     }
     for (cudaStream_t q : {pl->s_h2d, pl->s_comp, pl->s_d2h}) if (q) cudaStreamDestroy(q);
     void* ptrs[] = {pl->d_rings, pl->d_lens, pl->d_pairs, pl->d_north, pl->d_items[0], pl->d_items[1], pl->d_items[2], pl->d_items[3],
-                    pl->d_items[4], pl->d_items[5], pl->d_eqchunks, pl->d_pole, pl->d_chirp, pl->d_phase, pl->d_fft_order, pl->d_table, pl->d_tw, pl->d_filt,
+                    pl->d_items[4], pl->d_items[5], pl->d_eqchunks, pl->d_pole, pl->d_chirp, pl->d_phase, pl->d_fft_order[0], pl->d_fft_order[1], pl->d_table, pl->d_tw, pl->d_filt,
                     pl->d_W, pl->d_specIn, pl->d_specOut, pl->d_stage_in, pl->d_stage_out,
-                    pl->d_cap_chunks, pl->d_cap_chunk_items, pl->d_tc_chunks, pl->d_tc_tiles, pl->d_tc_cols, pl->d_tc_rings, pl->d_tc_items[0], pl->d_tc_items[1], pl->d_tc_items[2], pl->d_goff, pl->d_G, pl->d_pole_scratch, pl->d_direct_items, pl->d_tw3, pl->d_tw16, pl->d_fft3_jobs[0], pl->d_fft3_jobs[1], pl->d_fft3_jobs[2], pl->d_fft3_jobs[3]};
+                    pl->d_cap_chunks, pl->d_cap_chunk_items, pl->d_tc_chunks, pl->d_tc_tiles, pl->d_tc_cols, pl->d_tc_rings, pl->d_tc_items[0], pl->d_tc_items[1], pl->d_tc_items[2], pl->d_goff, pl->d_G, pl->d_pole_scratch, pl->d_direct_items, pl->d_tw3, pl->d_tw16, pl->d_fft3_jobs[0][0], pl->d_fft3_jobs[0][1], pl->d_fft3_jobs[0][2], pl->d_fft3_jobs[0][3],
+                    pl->d_fft3_jobs[1][0], pl->d_fft3_jobs[1][1], pl->d_fft3_jobs[1][2], pl->d_fft3_jobs[1][3]};
     for (void* p : ptrs) if (p) cudaFree(p);
     for (auto& e : pl->ev) if (e) cudaEventDestroy(e);
     for (auto& e : pl->ev_band) if (e) cudaEventDestroy(e);
@@ -1333,10 +1389,11 @@ int arkcos_plan_launches_per_convolve(const arkcos_plan* pl)
 {
     if (!pl) return -1;
     int n = (pl->opt.cache_kernel_rows || pl->npairs == 0) ? 0 : 1;
-    int fft = pl->nfft_old > 0 ? 1 : 0;
-    for (int c = 0; c < 4; ++c) fft += (pl->nfft3_bluestein[c] > 0 ? 1 : 0) + (pl->nfft3[c] > pl->nfft3_bluestein[c] ? 1 : 0);
-    n += 2 * fft;
-    n += (pl->nitems[0] > 0) + 2 * (pl->npole > 0) + (pl->neqchunks > 0);
+    for (int d = 0; d < 2; ++d) {
+        n += pl->nfft_old[d] > 0 ? 1 : 0;
+        for (int c = 0; c < 4; ++c) n += (pl->nfft3_bluestein[d][c] > 0 ? 1 : 0) + (pl->nfft3[d][c] > pl->nfft3_bluestein[d][c] ? 1 : 0);
+    }
+    n += (pl->nitems[0] > 0) + (pl->pole_warp_per_mode ? 2 : 1) * (pl->npole > 0) + (pl->neqchunks > 0);
     for (int c = 1; c < kBandClasses; ++c) n += pl->nitems[c] > 0 ? 1 : 0;
     n += pl->ndirect > 0 ? 1 : 0;
     n += (pl->ncapsingle > 0 ? 1 : 0) + (pl->ncapitems > pl->ncapsingle ? 1 : 0);

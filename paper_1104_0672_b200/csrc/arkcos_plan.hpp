@@ -21,6 +21,7 @@ struct HostGeometry {
     int64_t npix = 0, spec_total = 0;
     std::vector<double> theta, phi0, omega;
     std::vector<int> n, shifted, band_lo, band_hi, mprime;
+    std::vector<char> direct;        // exact_caps: output ring is recomputed by the direct-space sum (and skipped by the hybrid pass)
     std::vector<int64_t> pix_off, spec_off;
 };
 
@@ -78,19 +79,21 @@ struct arkcos_plan {
     int tc_blocks_per_sm = 0;
     int* d_pole = nullptr;
     void* d_pole_scratch = nullptr;   // cx<T>[max_nmaps][npole][2][pole_mh + 1]: unfolded spectra between the two pole launches
-    int npole = 0, pole_mh = 0;
+    int npole = 0, pole_mh = 0, general_split = 1;
+    bool pole_warp_per_mode = false;
     arkcos::BandItem* d_items[arkcos::kBandClasses] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
     double* d_table = nullptr;
     void* d_tw = nullptr;        // cx<T>[PT/2]
     void* d_filt = nullptr;      // cx<T>[...] Bluestein filter spectra
     void* d_chirp = nullptr;     // cx<T>[...] Bluestein chirps
     void* d_phase = nullptr;     // cx<T>[...] exp(-i pi k / N) per ring length
-    int* d_fft_order = nullptr;  // rings served by the shared-memory FFT kernels (arkcos_fft.cuh), longest transform first
-    int nfft_old = 0;
+    // per direction (0 forward, 1 inverse; the lists differ only for exact_caps plans)
+    int* d_fft_order[2] = {nullptr, nullptr};  // rings served by the shared-memory FFT kernels (arkcos_fft.cuh), longest transform first
+    int nfft_old[2] = {0, 0};
     // register-resident FFT kernels (arkcos_fft3.cuh): job lists for transform sizes Q = 512, 1024, 2048, 4096
-    arkcos::FftJob* d_fft3_jobs[4] = {nullptr, nullptr, nullptr, nullptr};
-    int nfft3[4] = {0, 0, 0, 0};
-    int nfft3_bluestein[4] = {0, 0, 0, 0};   // the first jobs of each list are the Bluestein rings, the rest pairs of power-of-two rings
+    arkcos::FftJob* d_fft3_jobs[2][4] = {};
+    int nfft3[2][4] = {};
+    int nfft3_bluestein[2][4] = {};   // the first jobs of each list are the Bluestein rings, the rest pairs of power-of-two rings
     void* d_tw3 = nullptr;       // cx<float>: pass-3 twiddles of the four transform sizes, see arkcos_fft3.cuh
     int tw3_off[4] = {0, 0, 0, 0};
     void* d_tw16 = nullptr;      // cx<float>[256]: exp(-2 pi i r k / 256) at [16 r + k]
