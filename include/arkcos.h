@@ -169,9 +169,9 @@ int arkcos_plan_set_timing(const arkcos_plan* plan, int enable /* 0 off, 1 stage
 int arkcos_plan_get_timing(const arkcos_plan* plan, float* ms4);
 
 /* The band step is split over several kernels by ring class; normally they run concurrently on
- * plan-owned side streams.  Returns their number (*n = 8), names, the work model's flops of each (nmaps = 1) and -- only
+ * plan-owned side streams.  Returns their number (*n = 9), names (of the launches the plan uses: tensor-core, FP32 or cached-spectra kernels), the work model's flops of each (nmaps = 1) and -- only
  * after a call made in timing mode 2, which runs them one after the other -- their last durations in milliseconds.
- * names / model_flops / last_ms: arrays of 8, any may be NULL. */
+ * names / model_flops / last_ms: arrays of 9, any may be NULL. */
 int arkcos_plan_band_kernels(const arkcos_plan* plan, int* n, const char** names, double* model_flops, float* last_ms);
 
 /* The ring FFTs of one direction are up to nine launches: per transform size Q = 4096, 2048, 1024, 512 the power-of-two rings

@@ -248,9 +248,9 @@ class Plan:
     def band_kernels(self, with_timing: bool = False):
         """[(name, model_flops, last_ms or None)] of the band kernels (timing needs set_timing(2) before the call)."""
         n = c_int()
-        names = (c_char_p * 8)()
-        fl = (c_double * 8)()
-        ms = (c_float * 8)()
+        names = (c_char_p * 9)()
+        fl = (c_double * 9)()
+        ms = (c_float * 9)()
         _check(_lib().arkcos_plan_band_kernels(self._h, byref(n), names, fl, ms if with_timing else None),
                "arkcos_plan_band_kernels")
         return [(names[k].decode(), fl[k], ms[k] if with_timing else None) for k in range(n.value)]

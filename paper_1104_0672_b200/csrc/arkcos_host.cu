@@ -413,13 +413,14 @@ void build_pairs(HostGeometry& g, double theta_max, double ell_nyq, int fixed_mp
         }
         // band-kernel slots: 0 general, 1 pole, 2 eq, 3 uniform<12>, 4 uniform<20>, 5 uniform<32,odd>, 6 uniform<12,odd>
         static const int slot_of_cls[kBandClasses] = {0, 6, 3, 4, 5, 7};
-        st.band_flops[slot_of_cls[cls]] += ring_flops;
+        if (cls != 5) st.band_flops[slot_of_cls[cls]] += ring_flops;
         if (cls == 5) {
             const int M = t.pairs[t.north[i].pair_lo].M;
             // single-period ring: M/2 below the length of ring i and of every ring of its band (a run is homogeneous)
             bool single = M / 2 < g.n[i] && g.n[i] <= M;
             for (int p = t.north[i].pair_lo; p < t.north[i].pair_hi; ++p) single = single && M / 2 < g.n[t.pairs[p].j];
             const int multi = single ? 0 : 1;
+            st.band_flops[7 + multi] += ring_flops;          // slot 7: runs of a single period, 8: of several
             if (!t.cap_chunks.empty() && t.cap_chunks.back().i0 + t.cap_chunks.back().n == i && t.cap_chunks.back().M == M &&
                 t.cap_chunks.back().multi == multi && t.cap_chunks.back().n < (use_tc ? kTcChunkRings : kCapChunkRings))
                 ++t.cap_chunks.back().n;
@@ -732,9 +733,10 @@ void launch_uniform(const arkcos_plan* pl, int nmaps, cudaStream_t st, bool seri
                     (const cx<float>*)pl->spec_in(), (cx<float>*)pl->d_specOut, pl->g.spec_total);
         };
         launch_cap(std::false_type{}, 0, pl->ncapsingle);
+        if (serial) cudaEventRecord(pl->ev_band[8], st);
         launch_cap(std::true_type{}, pl->ncapsingle, pl->ncapitems - pl->ncapsingle);
-    }
-    if (serial) cudaEventRecord(pl->ev_band[8], st);
+    } else if (serial) cudaEventRecord(pl->ev_band[8], st);
+    if (serial) cudaEventRecord(pl->ev_band[9], st);
 }
 
 // Ring FFTs of one direction (FWD: map -> specIn, else specOut -> map).  Float plans: one launch per transform size of the
@@ -1326,19 +1328,33 @@ int arkcos_plan_get_timing(const arkcos_plan* pl, float* ms4)
 
 int arkcos_plan_band_kernels(const arkcos_plan* pl, int* n, const char** names, double* model_flops, float* last_ms)
 {
-    static const char* kNames[8] = {"band_mac_general_kernel", "band_mac_pole_kernel", "band_mac_eq_kernel",
-                                    "band_mac_uniform_kernel<12,0>", "band_mac_uniform_kernel<20,0>",
-                                    "band_mac_uniform_kernel<32,1>", "band_mac_uniform_kernel<12,1>", "band_mac_capchunk_kernel<4,20>"};
+    // launch names: the class-E and cap runs are band_mac_tc_kernel<KIND> when the plan uses the tensor cores
+    static const char* kFp32[9] = {"band_mac_general_kernel", "band_mac_pole_kernel", "band_mac_eq_kernel",
+                                   "band_mac_uniform_kernel<12,0>", "band_mac_uniform_kernel<20,0>",
+                                   "band_mac_uniform_kernel<32,1>", "band_mac_uniform_kernel<12,1>", "band_mac_capchunk_kernel<4,20,0>",
+                                   "band_mac_capchunk_kernel<4,20,1>"};
     if (!pl || !n) return fail(ARKCOS_INVALID_ARG, "NULL argument");
-    *n = 8;
-    for (int k = 0; k < 8; ++k) {
+    const char* kNames[9];
+    for (int k = 0; k < 9; ++k) kNames[k] = kFp32[k];
+    if (pl->use_tc) {
+        kNames[2] = pl->eq_alt ? "band_mac_tc_kernel<0>" : "band_mac_tc_kernel<1>";
+        kNames[7] = "band_mac_tc_kernel<2>";
+        kNames[8] = "band_mac_tc_kernel<3>";
+    } else if (pl->d_G) {
+        kNames[2] = "band_mac_eq_cached_kernel";
+        kNames[7] = "band_mac_capchunk_cached_kernel<0>";
+        kNames[8] = "band_mac_capchunk_cached_kernel<1>";
+    }
+    if (pl->npole > 0 && pl->pole_warp_per_mode) kNames[1] = "band_mac_pole_kernel + band_mac_pole_fold_kernel";
+    *n = 9;
+    for (int k = 0; k < 9; ++k) {
         if (names) names[k] = kNames[k];
         if (model_flops) model_flops[k] = pl->stats.band_flops[k];
     }
     if (last_ms) {
         if (pl->timing != 2) return fail(ARKCOS_INVALID_ARG, "per-kernel timing needs arkcos_plan_set_timing(plan, 2)");
-        CUDA_TRY(cudaEventSynchronize(pl->ev_band[8]));
-        for (int k = 0; k < 8; ++k) CUDA_TRY(cudaEventElapsedTime(&last_ms[k], pl->ev_band[k], pl->ev_band[k + 1]));
+        CUDA_TRY(cudaEventSynchronize(pl->ev_band[9]));
+        for (int k = 0; k < 9; ++k) CUDA_TRY(cudaEventElapsedTime(&last_ms[k], pl->ev_band[k], pl->ev_band[k + 1]));
     }
     return ARKCOS_OK;
 }

@@ -32,7 +32,7 @@ struct Stats {
     double mac_pairs_modes = 0;      // sum over northern ring pairs of (M/2 + 1): products G_ij[m] B_j[m] per hemisphere
     double tc_flops = 0;             // tensor-core flops issued per map by band_mac_tc_kernel (3 x TF32, padded tiles)
     double fft_pixels[10] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0};   // pixels served by each ring-FFT launch, see arkcos_plan_fft_kernels
-    double band_flops[8] = {0, 0, 0, 0, 0, 0, 0, 0};   // per band kernel, see arkcos_plan_band_kernels
+    double band_flops[9] = {0, 0, 0, 0, 0, 0, 0, 0, 0};   // per band kernel, see arkcos_plan_band_kernels
 };
 
 }  // namespace arkcos
@@ -116,7 +116,7 @@ struct arkcos_plan {
     // optional per-stage timing
     mutable int timing = 0;
     mutable cudaEvent_t ev[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
-    mutable cudaEvent_t ev_band[9] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+    mutable cudaEvent_t ev_band[10] = {};
     mutable cudaEvent_t ev_fft[2][10] = {};      // timing mode 2: before each ring-FFT launch of a direction and after the last
     // fork/join of the band kernels of the different ring classes
     cudaStream_t side[3] = {nullptr, nullptr, nullptr}, side_rows = nullptr;
