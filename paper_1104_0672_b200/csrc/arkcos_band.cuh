@@ -45,24 +45,7 @@ template <class T> __global__ void __launch_bounds__(128) kernel_rows_kernel(con
         const int u = 2 * t + pr.par;
         const double sh = sinpi((double)u * inv2M);                    // sin(psi/2), psi = u pi / M
         const double x = pr.A + pr.B * sh * sh;
-        double hx = 0.5 * sqrt(x);
-        if (hx > 1.0) hx = 1.0;
-        // gamma = 2 asin(hx); compact kernels only see small hx: Maclaurin series (10 terms, truncation < 1e-18 relative
-        // for hx < 1/8) instead of the library asin
-        double gamma;
-        if (hx < 0.125) {
-            const double q = hx * hx;
-            double p = 34459425.0 / 3530096640.0;
-            p = p * q + 2027025.0 / 175472640.0;
-            p = p * q + 135135.0 / 9676800.0;
-            p = p * q + 10395.0 / 599040.0;
-            p = p * q + 945.0 / 42240.0;
-            p = p * q + 105.0 / 3456.0;
-            p = p * q + 15.0 / 336.0;
-            p = p * q + 3.0 / 40.0;
-            p = p * q + 1.0 / 6.0;
-            gamma = 2.0 * (hx + hx * q * p);
-        } else gamma = 2.0 * asin(hx);
+        const double gamma = gamma_of_chord2(x);
         double val = 0.0;
         if (gamma < theta_max) {
             const double uu = gamma * tscale;

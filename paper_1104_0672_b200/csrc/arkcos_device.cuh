@@ -69,4 +69,26 @@ __device__ __forceinline__ void cp_async16(void* smem_dst, const void* gsrc)
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 
+// gamma = 2 asin(sqrt(x) / 2) from the squared chord x = 2 - 2 cos(gamma) (Eq. 9).  Compact kernels only see small
+// arguments: Maclaurin series of asin (10 terms, truncation < 1e-18 relative for sqrt(x)/2 < 1/8) instead of the library asin.
+__device__ __forceinline__ double gamma_of_chord2(double x)
+{
+    double hx = 0.5 * sqrt(x);
+    if (hx > 1.0) hx = 1.0;
+    if (hx < 0.125) {
+        const double q = hx * hx;
+        double p = 34459425.0 / 3530096640.0;
+        p = p * q + 2027025.0 / 175472640.0;
+        p = p * q + 135135.0 / 9676800.0;
+        p = p * q + 10395.0 / 599040.0;
+        p = p * q + 945.0 / 42240.0;
+        p = p * q + 105.0 / 3456.0;
+        p = p * q + 15.0 / 336.0;
+        p = p * q + 3.0 / 40.0;
+        p = p * q + 1.0 / 6.0;
+        return 2.0 * (hx + hx * q * p);
+    }
+    return 2.0 * asin(hx);
+}
+
 }  // namespace arkcos

@@ -16,27 +16,6 @@ namespace arkcos {
 
 constexpr int kDirectThreads = 128;
 
-// gamma from the squared chord x (shared with kernel_rows_kernel's arithmetic: series for small arguments)
-__device__ __forceinline__ double gamma_of_chord2(double x)
-{
-    double hx = 0.5 * sqrt(x);
-    if (hx > 1.0) hx = 1.0;
-    if (hx < 0.125) {
-        const double q = hx * hx;
-        double p = 34459425.0 / 3530096640.0;
-        p = p * q + 2027025.0 / 175472640.0;
-        p = p * q + 135135.0 / 9676800.0;
-        p = p * q + 10395.0 / 599040.0;
-        p = p * q + 945.0 / 42240.0;
-        p = p * q + 105.0 / 3456.0;
-        p = p * q + 15.0 / 336.0;
-        p = p * q + 3.0 / 40.0;
-        p = p * q + 1.0 / 6.0;
-        return 2.0 * (hx + hx * q * p);
-    }
-    return 2.0 * asin(hx);
-}
-
 // grid = (blocks of kDirectThreads pixels over the listed rings, map chunks); items: {index into ring_list, first pixel}
 template <class T, int NM>
 __global__ void __launch_bounds__(kDirectThreads)

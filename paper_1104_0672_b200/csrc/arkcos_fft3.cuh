@@ -251,6 +251,7 @@ ring_fft3_inverse_kernel(const cx<float>* __restrict__ spec, int64_t spec_stride
         prefetch_l2(D + nx.r0.spec_off, (uint32_t)(nx.r0.n / 2 + 1) * 8u);
         if (nx.has1) prefetch_l2(D + nx.r1.spec_off, (uint32_t)(nx.r1.n / 2 + 1) * 8u);
         if (!nx.f.pow2) prefetch_l2(chirp + nx.f.chirp_off, (uint32_t)nx.f.L * 8u);
+        prefetch_l2(phase + nx.f.ph_off, (uint32_t)(nx.f.L + 1) * 8u);      // the inverse needs the phases with its first loads
     }
     const cx<float>* __restrict__ ph = phase + f.ph_off;
     cx<float> u[2][16];

@@ -674,15 +674,18 @@ void launch_uniform(const arkcos_plan* pl, int nmaps, cudaStream_t st, bool seri
 {
     cudaStream_t s1 = serial ? st : pl->side[1], s2 = serial ? st : pl->side[2];
     if (pl->neqchunks > 0 && pl->d_G) {
-        const unsigned gx = (unsigned)((pl->eq_mh + kBandThreads * 2 - 1) / (kBandThreads * 2));
-        if (nmaps > 1)
-            band_mac_eq_cached_kernel<4, 2><<<dim3(gx, (unsigned)pl->neqchunks, (unsigned)((nmaps + 1) / 2)), kBandThreads, 0, st>>>(
+        const unsigned gx = (unsigned)((pl->eq_mh + 255) / 256);
+        auto launch_eq = [&](auto nm_tag, auto mt_tag) {
+            constexpr int NM = decltype(nm_tag)::value, MT = decltype(mt_tag)::value;
+            band_mac_eq_cached_kernel<4, NM, MT><<<dim3(gx, (unsigned)pl->neqchunks, (unsigned)((nmaps + NM - 1) / NM)), 256 / MT,
+                                                   cached_smem_bytes<NM>(), st>>>(
                 pl->d_eqchunks, pl->d_north, pl->d_pairs, pl->d_goff, pl->d_G, pl->d_rings, pl->g.R,
                 (const cx<float>*)pl->spec_in(), (cx<float>*)pl->d_specOut, pl->g.spec_total, nmaps);
-        else
-            band_mac_eq_cached_kernel<4, 1><<<dim3(gx, (unsigned)pl->neqchunks, 1), kBandThreads, 0, st>>>(
-                pl->d_eqchunks, pl->d_north, pl->d_pairs, pl->d_goff, pl->d_G, pl->d_rings, pl->g.R,
-                (const cx<float>*)pl->spec_in(), (cx<float>*)pl->d_specOut, pl->g.spec_total, nmaps);
+        };
+        // G is read once per group of maps: four maps per read (one mode per thread) from four maps on
+        if (nmaps >= 4) launch_eq(std::integral_constant<int, 4>{}, std::integral_constant<int, 1>{});
+        else if (nmaps > 1) launch_eq(std::integral_constant<int, 2>{}, std::integral_constant<int, 2>{});
+        else launch_eq(std::integral_constant<int, 1>{}, std::integral_constant<int, 2>{});
     } else if (pl->neqchunks > 0 && pl->use_tc && pl->ntc_items[0] > 0) {
         tc_launch(pl->eq_alt ? 0 : 1, (unsigned)pl->ntc_items[0], (unsigned)nmaps, st, pl->d_tc_items[0], pl->d_tc_chunks, pl->d_tc_tiles,
                   pl->d_tc_cols, pl->d_tc_rings, (const float*)pl->d_W, pl->g.R, (const cx<float>*)pl->spec_in(), (cx<float>*)pl->d_specOut,
@@ -714,12 +717,16 @@ void launch_uniform(const arkcos_plan* pl, int nmaps, cudaStream_t st, bool seri
             if (count <= 0) return;
             const unsigned n = (unsigned)count;
             const CapChunkItem* items = pl->d_cap_chunk_items + first;
-            if (pl->d_G && nmaps > 1)
-                band_mac_capchunk_cached_kernel<4, 2, MULTI><<<dim3(n, (unsigned)((nmaps + 1) / 2)), kBandThreads, 0, s1>>>(
+            if (pl->d_G && nmaps >= 4)
+                band_mac_capchunk_cached_kernel<4, 4, MULTI, 1><<<dim3(n, (unsigned)((nmaps + 3) / 4)), 256, 0, s1>>>(
+                    items, pl->d_cap_chunks, pl->d_north, pl->d_pairs, pl->d_goff, pl->d_G, pl->d_rings, pl->g.R,
+                    (const cx<float>*)pl->spec_in(), (cx<float>*)pl->d_specOut, pl->g.spec_total, nmaps);
+            else if (pl->d_G && nmaps > 1)
+                band_mac_capchunk_cached_kernel<4, 2, MULTI, 2><<<dim3(n, (unsigned)((nmaps + 1) / 2)), kBandThreads, 0, s1>>>(
                     items, pl->d_cap_chunks, pl->d_north, pl->d_pairs, pl->d_goff, pl->d_G, pl->d_rings, pl->g.R,
                     (const cx<float>*)pl->spec_in(), (cx<float>*)pl->d_specOut, pl->g.spec_total, nmaps);
             else if (pl->d_G)
-                band_mac_capchunk_cached_kernel<4, 1, MULTI><<<dim3(n, 1), kBandThreads, 0, s1>>>(
+                band_mac_capchunk_cached_kernel<4, 1, MULTI, 2><<<dim3(n, 1), kBandThreads, 0, s1>>>(
                     items, pl->d_cap_chunks, pl->d_north, pl->d_pairs, pl->d_goff, pl->d_G, pl->d_rings, pl->g.R,
                     (const cx<float>*)pl->spec_in(), (cx<float>*)pl->d_specOut, pl->g.spec_total, nmaps);
             else if (pl->use_tc) {
@@ -1093,6 +1100,7 @@ static int plan_create_impl(arkcos_plan** out, const arkcos_pixelization* pix, c
         CUDA_TRY(cudaDeviceSynchronize());
     }
     if (opt.cache_kernel_spectra && pl->npairs > 0) {
+        CUDA_TRY(cudaFuncSetAttribute(band_mac_eq_cached_kernel<4, 4, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cached_smem_bytes<4>()));
         // one row of M/2 + 1 floats per northern ring pair, padded to a multiple of four
         std::vector<uint32_t> goff(t.pairs.size());
         uint64_t n4 = 0;

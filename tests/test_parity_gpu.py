@@ -131,12 +131,13 @@ def test_healpix_mid_size_all_kernel_classes(nside, fwhm_px, nmaps):
     assert frms(take_rings(geom, out, rings), ref1) <= 1e-5
 
 
-@pytest.mark.parametrize("cache", [0, 1], ids=["computed", "cached_spectra"])
+@pytest.mark.parametrize("cache,nmaps", [(0, 3), (1, 3), (1, 5)], ids=["computed", "cached_spectra", "cached_spectra_5maps"])
 @pytest.mark.parametrize("kernel", ["gauss", "tophat", "mexhat"])
-def test_healpix_256_cap_runs_and_cached_spectra(kernel, cache):
-    """nside 256, 3 maps: single-period cap runs (Gaussian), multi-period ones (hard-edged kernels: M' up to 3 N_i) and
-    the cached-spectra kernels (options.cache_kernel_spectra, two maps per read of G) against oracle #2 at the plan's M'."""
-    nside, nmaps = 256, 3
+def test_healpix_256_cap_runs_and_cached_spectra(kernel, cache, nmaps):
+    """nside 256, 3 or 5 maps: single-period cap runs (Gaussian), multi-period ones (hard-edged kernels: M' up to 3 N_i) and
+    the cached-spectra kernels (options.cache_kernel_spectra: two maps per read of G, four from four maps on) against
+    oracle #2 at the plan's M'."""
+    nside = 256
     geom = geometry.healpix_ring(nside)
     px = np.sqrt(4 * np.pi / geom.npix)
     tab, tmax = {"gauss": (inputs.gaussian_table(2.5 * px, 7.5 * px), 7.5 * px),
