@@ -283,6 +283,16 @@ ring_fft3_inverse_kernel(const cx<float>* __restrict__ spec, int64_t spec_stride
 
 namespace arkcos {
 
+// exp(-i pi q / 32), q = 0 .. 15 (an immediate once the loop over q is unrolled).  A power-of-two ring has N = 32 T, so the
+// half-angle phase of the split at k = t + T q is exp(-i pi k / N) = exp(-i pi t / N) exp(-i pi q / 32): one table load per thread.
+__device__ __forceinline__ cx<float> phase_step(int q)
+{
+    constexpr float c[16] = {1.000000000e+00f, 9.951847267e-01f, 9.807852804e-01f, 9.569403357e-01f, 9.238795325e-01f, 8.819212643e-01f,
+                             8.314696123e-01f, 7.730104534e-01f, 7.071067812e-01f, 6.343932842e-01f, 5.555702330e-01f, 4.713967368e-01f,
+                             3.826834324e-01f, 2.902846773e-01f, 1.950903220e-01f, 9.801714033e-02f};
+    return mk<float>(c[q], q == 0 ? 0.f : -c[16 - q]);      // sin(pi q / 32) = cos(pi (16 - q) / 32)
+}
+
 // Power-of-two rings, ONE transform per block (block b works on ring b & 1 of direct job b >> 1): twice as many resident
 // blocks at half the registers, so that the load / store phases of some blocks overlap the butterflies of the others.
 template <int LOGQ, bool FWD>
@@ -303,6 +313,7 @@ ring_fft3_direct1_kernel(const float* __restrict__ in, float* __restrict__ outma
     const int L = job.f.L;
     const cx<float>* __restrict__ ph = phase + job.f.ph_off;
     cx<float>* __restrict__ sp = spec + (int64_t)blockIdx.y * spec_stride + rr.spec_off;
+    const cx<float> pht = ph[t];                                               // exp(-i pi t / N)
     cx<float> u[1][16];
     if (FWD) {
         const cx<float>* __restrict__ x0 = reinterpret_cast<const cx<float>*>(in + (int64_t)blockIdx.y * npix + rr.pix_off);
@@ -317,14 +328,14 @@ ring_fft3_direct1_kernel(const float* __restrict__ in, float* __restrict__ outma
         for (int q = 0; q < 16; ++q) {
             const int k = t + T * q;
             const cx<float> zc = cconj(s[phys(k == 0 ? 0 : L - k)]);
-            sp[k] = split_fwd(u[0][q], zc, ph[k], rr.shifted);
+            sp[k] = split_fwd(u[0][q], zc, cmul(pht, phase_step(q)), rr.shifted);
         }
         if (t == 0) sp[L] = split_fwd(u[0][0], cconj(u[0][0]), ph[L], rr.shifted);
     } else {
 #pragma unroll
         for (int r = 0; r < 16; ++r) {
             const int k = t + T * r;
-            const cx<float> hk = cconj(ph[k]);                                 // exp(+i pi k / N)
+            const cx<float> hk = cconj(cmul(pht, phase_step(r)));              // exp(+i pi k / N)
             u[0][r] = pack_inv(sp[k], sp[L - k], hk, mk<float>(hk.y, hk.x), rr.shifted);   // exp(i pi (L-k)/N) = i conj(hk)
         }
         fft3<LOGQ, 1>(u, s, tw, logPT, tw16, tw3);
