@@ -83,14 +83,16 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity)
 // (k + 1) & 1, while the two consumer warpgroups (thread = mode) multiply-accumulate tile k out of TMEM stage k & 1.
 // mbarriers: full[s] (MMAs of the stage done), empty[s] (all eight consumer warps have read the stage), rows[s] (the MMAs
 // that read B-operand stage s are done).
-template <int KIND>
-__global__ void __launch_bounds__(kTcThreads, 1)
+template <int KIND, class CFG>
+__global__ void __launch_bounds__(CFG::threads, 1)
 band_mac_tc_kernel(const TcItem* __restrict__ items, const TcChunk* __restrict__ chunks, const TcTile* __restrict__ tiles,
                    const uint32_t* __restrict__ cols, const TcRing* __restrict__ ringtab, const float* __restrict__ W, int R,
                    const cx<float>* __restrict__ specIn, cx<float>* __restrict__ specOut, int64_t spec_stride)
 {
     constexpr bool CAP = KIND >= 2, MULTI = KIND == 3, ALT = KIND == 0;
-    constexpr int TI = kTcTI, JW = kTcJW, N = kTcN, K = kTcK, KC = K / 4, MT = kTcMT;
+    constexpr int TI = CFG::TI, JW = CFG::JW, N = CFG::N, K = CFG::K, KC = K / 4, MT = CFG::MT;
+    constexpr int kTcConsumers = CFG::consumers, kTcProducers = CFG::producers;
+    constexpr int kTmemCols = 2 * MT * N <= 256 ? 256 : 512;       // two stages of MT x N accumulator columns (a power of two)
     static_assert(TI == 4, "column = 4 * input ring + output ring");
     extern __shared__ __align__(128) unsigned char tc_smem[];
     float4* sA = reinterpret_cast<float4*>(tc_smem);            // [block of modes][hi / lo][KC][128 modes]: cos(pi m u s / M), u = 4 kc .. 4 kc + 3
@@ -121,7 +123,7 @@ band_mac_tc_kernel(const TcItem* __restrict__ items, const TcChunk* __restrict__
     };
     auto fetch_ring = [&](int j, const TcRing& rj) {
         const int idx = CAP ? ext_index(m, rj.n_sh, rj.magic) : m;
-        const uint32_t dst = sv0 + 2048u * (uint32_t)(j & (JW - 1));
+        const uint32_t dst = sv0 + 2048u * (uint32_t)(j % JW);
         asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst), "l"(in + rj.offN + idx) : "memory");
         asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst + 8u), "l"(in + rj.offS + idx) : "memory");
     };
@@ -169,7 +171,7 @@ band_mac_tc_kernel(const TcItem* __restrict__ items, const TcChunk* __restrict__
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     if (warp == kTcConsumers / 32) {                             // the first producer warp owns the tensor-memory allocation
-        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&s_tmem)), "r"(2 * MT * N));
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&s_tmem)), "r"(kTmemCols));
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::);
     }
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
@@ -274,7 +276,7 @@ band_mac_tc_kernel(const TcItem* __restrict__ items, const TcChunk* __restrict__
             for (int k = max(ntiles - 2, 0); k < ntiles; ++k) mbar_wait(&bar_empty[k & 1], (uint32_t)(k >> 1) & 1u);
             asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
             __syncwarp();
-            asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"(2 * MT * N));
+            asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"(kTmemCols));
         }
     } else {
         // =================================== multiply-accumulate over input rings ==============================
@@ -310,7 +312,7 @@ band_mac_tc_kernel(const TcItem* __restrict__ items, const TcChunk* __restrict__
 #pragma unroll
             for (int ii = 0; ii < TI; ++ii) acc[ii][0] = acc[ii][1] = make_float2(0.f, 0.f);
             const uint32_t tbase = tmem + ((uint32_t)((warp & 3) * 32) << 16) + (uint32_t)((s * MT + wg) * N);
-            uint32_t soff = ((uint32_t)jlo & (JW - 1)) * 2048u;          // byte offset of the slot of ring jlo + jj
+            uint32_t soff = (uint32_t)(jlo % JW) * 2048u;                // byte offset of the slot of ring jlo + jj
             // cap runs: the periodic extension conjugates on reflection, and a shifted ring changes sign on reflection and on
             // every odd period (reading R8): applied once, in place, when the coefficients of a ring have landed
             auto land = [&]() {
@@ -324,7 +326,7 @@ band_mac_tc_kernel(const TcItem* __restrict__ items, const TcChunk* __restrict__
                         const uint32_t sre = (rj.n_sh < 0 && (refl != ((w & 1) != 0))) ? 0x80000000u : 0u;
                         const uint32_t sim = sre ^ (refl ? 0x80000000u : 0u);
                         if (sre | sim) {
-                            const uint32_t a = sv0 + 2048u * (uint32_t)((jlo + jj) & (JW - 1));
+                            const uint32_t a = sv0 + 2048u * (uint32_t)((jlo + jj) % JW);
                             uint32_t x, y, z, ww;
                             asm volatile("ld.shared.v4.b32 {%0, %1, %2, %3}, [%4];" : "=r"(x), "=r"(y), "=r"(z), "=r"(ww) : "r"(a));
                             asm volatile("st.shared.v4.b32 [%4], {%0, %1, %2, %3};" ::"r"(x ^ sre), "r"(y ^ sim), "r"(z ^ sre), "r"(ww ^ sim), "r"(a) : "memory");
@@ -337,7 +339,8 @@ band_mac_tc_kernel(const TcItem* __restrict__ items, const TcChunk* __restrict__
 #pragma unroll
                 for (int q = 0; q < 4; ++q) {
                     asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v[q].x), "=f"(v[q].y), "=f"(v[q].z), "=f"(v[q].w) : "r"(sv0 + soff));
-                    soff = (soff + 2048u) & (JW * 2048u - 1u);
+                    soff += 2048u;
+                    if (soff == JW * 2048u) soff = 0u;
                 }
             };
             auto mac4 = [&](const uint32_t (&g)[16], const float4 (&v)[4]) {

@@ -8,24 +8,35 @@
 
 namespace arkcos {
 
-constexpr int kTcMT = 2;                   // blocks of 128 modes (TMEM lanes) per thread block, one consumer warpgroup each
-constexpr int kTcConsumers = 128 * kTcMT;  // multiply-accumulate threads: thread = mode
-constexpr int kTcProducers = 128;          // B-operand threads: thread = accumulator column; its thread 0 issues the MMAs
-constexpr int kTcThreads = kTcConsumers + kTcProducers;
+// Tile geometry.  A block owns MT blocks of 128 modes (TMEM lanes), a tile is TI = 4 output rings whose window of input
+// rings has at most JW rings (accumulator column = 4 * input ring + output ring), a row has at most K sample positions.
+// Two instantiations: narrow windows (two blocks of modes per thread block) and wide windows / long rows (one).
+template <int MT_, int JW_, int K_> struct TcCfgT {
+    static constexpr int MT = MT_, JW = JW_, K = K_, TI = 4, N = TI * JW_, KC = K_ / 4;
+    static constexpr int consumers = 128 * MT_;        // multiply-accumulate threads: thread = mode
+    static constexpr int producers = N;                // B-operand threads: thread = accumulator column; its thread 0 issues the MMAs
+    static constexpr int threads = consumers + producers;
+    // cosine operand per block of modes, two stages of the row operand, coefficient window per block of modes
+    static constexpr size_t smem_bytes = (size_t)(MT_ * 2 * KC * 128 + 2 * 2 * KC * N + MT_ * JW_ * 128) * 16;
+    static_assert(N % 32 == 0 && N <= 256 && K_ % 8 == 0 && 2 * MT_ * N <= 512, "tile geometry");
+};
+using TcCfgNarrow = TcCfgT<2, 32, 24>;     // windows of up to 32 rings, rows of up to 24 positions (Gaussian-like kernels)
+using TcCfgWide = TcCfgT<1, 40, 40>;       // windows of up to 40 rings, rows of up to 40 positions (wide hard-cut kernels)
+struct TcGeom { int mt, jw, k, n, threads; size_t smem_bytes; };       // the chosen instantiation, for the host
+inline TcGeom tc_geom(int cfg)
+{
+    return cfg == 0 ? TcGeom{TcCfgNarrow::MT, TcCfgNarrow::JW, TcCfgNarrow::K, TcCfgNarrow::N, TcCfgNarrow::threads, TcCfgNarrow::smem_bytes}
+                    : TcGeom{TcCfgWide::MT, TcCfgWide::JW, TcCfgWide::K, TcCfgWide::N, TcCfgWide::threads, TcCfgWide::smem_bytes};
+}
 constexpr int kTcTI = 4;                   // output rings per tile
-constexpr int kTcJW = 32;                  // input rings a tile's window can hold
-constexpr int kTcN = kTcTI * kTcJW;        // accumulator columns per block of modes
-constexpr int kTcK = 24;                   // sample positions u per row
 constexpr int kTcChunkRings = 48;          // longest run of cap rings handed to one block
 constexpr int kTcMaxTiles = 16;            // tiles of the longest run (class-E runs: 64 rings); their records live in shared memory
-constexpr int kTcMaxWindow = kTcMaxTiles * kTcTI + kTcJW;   // input rings the tiles of one run can touch
-// cosine operand per block of modes, two stages of the row operand, coefficient window per block of modes
-constexpr size_t kTcSmemBytes = (size_t)(kTcMT * 2 * (kTcK / 4) * 128 + 2 * 2 * (kTcK / 4) * kTcN + kTcMT * kTcJW * 128) * 16;
+constexpr int kTcMaxWindow = kTcMaxTiles * kTcTI + TcCfgWide::JW;   // input rings the tiles of one run can touch
 
 // Plan-time tables of the tensor-core band kernel (no pointer chasing through the ring-pair table inside the kernel):
 // a run of rings, its tiles of up to TI output rings, per tile one word per accumulator column, and two words per ring.
 struct TcChunk { int i0, n, M, multi, tile0; };       // run of output rings i0 .. i0 + n - 1 with one grid length M; first tile
-struct TcItem { int chunk, bx; };                      // one thread block: run, block of 128 * kTcMT modes
+struct TcItem { int chunk, bx; };                      // one thread block: run, block of 128 * MT modes
 struct __align__(16) TcTile {                          // window of input rings, first output ring, output rings of the tile,
     int jlo, jhi, i0, nti;                             // and per output ring its spectrum offsets (ring, mirror image) and N_i | shifted << 31
     int offN[4], offS[4], n_sh[4];
@@ -35,11 +46,12 @@ struct TcRing { int offN, offS, n_sh; uint32_t magic; };   // spectrum offsets o
 // 0xffffffff: no such ring pair (zero row)
 constexpr uint32_t kTcNoPair = 0xffffffffu;
 
-// Shared-memory limit and carve-out of the four instantiations; *blocks_per_sm = resident blocks per SM.  Returns a cudaError_t.
-int tc_setup(int* blocks_per_sm);
+// Shared-memory limit and carve-out of the instantiations of geometry cfg (0 narrow, 1 wide); *blocks_per_sm = resident blocks
+// per SM.  Returns a cudaError_t.
+int tc_setup(int cfg, int* blocks_per_sm);
 
 // KIND as in arkcos_band_tc.cuh (0 class-E alternating parity, 1 class-E integer grid, 2 cap runs single period, 3 several).
-void tc_launch(int kind, unsigned nitems, unsigned nmaps, cudaStream_t st, const TcItem* items, const TcChunk* chunks,
+void tc_launch(int cfg, int kind, unsigned nitems, unsigned nmaps, cudaStream_t st, const TcItem* items, const TcChunk* chunks,
                const TcTile* tiles, const uint32_t* cols, const TcRing* ringtab, const float* W, int R,
                const cx<float>* specIn, cx<float>* specOut, int64_t spec_stride);
 

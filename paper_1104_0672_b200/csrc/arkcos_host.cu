@@ -173,6 +173,7 @@ struct HostTables {
     std::vector<EqChunk> eq_chunks;              // runs of consecutive class-E rings for band_mac_eq_kernel   // per band-kernel class (see band_class)
     int eq_alt = 0;
     bool use_tc = false;                         // tensor-core band kernels (arkcos_band_tc.cuh) serve the class-E and cap runs
+    int tc_cfg = 0;                              // their tile geometry: 0 narrow windows, 1 wide windows / long rows
     std::vector<TcChunk> tc_chunks;              // runs of rings served by band_mac_tc_kernel, their tiles and column words
     std::vector<TcTile> tc_tiles;
     std::vector<uint32_t> tc_cols;
@@ -290,10 +291,17 @@ void build_pairs(HostGeometry& g, double theta_max, double ell_nyq, int fixed_mp
 {
     const int R = g.R, nnorth = (R + 1) / 2;
     // tensor-core band kernels: float plans with computed spectra; the window of a tile of kTcTI consecutive output rings
-    // must fit the kernel's kTcJW slots for every tile the plan could form
+    // must fit the kernel's slots for every tile the plan could form: the narrow geometry if it does, else the wide one
     bool use_tc = allow_tc && allow_fast && !cached;
-    for (int i = 0; i < nnorth && use_tc; ++i)
-        use_tc = g.band_hi[std::min(i + kTcTI - 1, nnorth - 1)] - g.band_lo[i] + 1 <= kTcJW;
+    int tc_cfg = 0;
+    if (use_tc) {
+        int wmax = 0;
+        for (int i = 0; i < nnorth; ++i) wmax = std::max(wmax, g.band_hi[std::min(i + kTcTI - 1, nnorth - 1)] - g.band_lo[i] + 1);
+        tc_cfg = wmax <= tc_geom(0).jw ? 0 : 1;
+        use_tc = wmax <= tc_geom(tc_cfg).jw;
+    }
+    const TcGeom tg = tc_geom(tc_cfg);
+    t.tc_cfg = tc_cfg;
     t.use_tc = use_tc;
     std::vector<int> eq_rings, general_rings;
     bool any_odd = false;
@@ -374,9 +382,9 @@ void build_pairs(HostGeometry& g, double theta_max, double ell_nyq, int fixed_mp
                 all_e = t.pairs[p].M == g.n[i] && g.n[t.pairs[p].j] == g.n[i];
                 alt_ok = alt_ok && t.pairs[p].par == (eq_alt ? ((i ^ t.pairs[p].j) & 1) : 0);
             }
-            // rows of the tensor-core kernel hold kTcK sample positions: 12 samples with half-step positions, 24 without
+            // rows of the tensor-core kernel hold K sample positions: K/2 samples with half-step positions, K without
             const bool tc_eq = use_tc && (g.n[i] / 2) % 128 == 0;
-            if (all_e && alt_ok && hi > lo && (maxcnt <= (tc_eq && !eq_alt ? kTcK : 12) || cached) && g.n[i] >= 8 && g.spec_total < (int64_t)INT32_MAX) {
+            if (all_e && alt_ok && hi > lo && (maxcnt <= (tc_eq ? (eq_alt ? tg.k / 2 : tg.k) : 12) || cached) && g.n[i] >= 8 && g.spec_total < (int64_t)INT32_MAX) {
                 eq_rings.push_back(i);
                 st.band_flops[2] += ring_flops;
                 // the Nyquist bin m = M/2 goes to a per-mode kernel that holds the whole row (cached plans admit long rows)
@@ -389,8 +397,8 @@ void build_pairs(HostGeometry& g, double theta_max, double ell_nyq, int fixed_mp
                 else if (maxcnt <= 32) cls = 4;
                 // runs of band_mac_capchunk_kernel: one grid length, integer grid, rings long enough for 256-mode blocks
                 if (use_tc) {
-                    // tensor-core run kernel: integer grid, rows of at most kTcK samples, any number of periods
-                    if (!odd && maxcnt <= kTcK && g.n[i] >= 256 && g.n[i] < nmax && t.pairs[lo].M / 2 < (1 << 15)) cls = 5;
+                    // tensor-core run kernel: integer grid, rows of at most K samples, any number of periods
+                    if (!odd && maxcnt <= tg.k && g.n[i] >= 256 && g.n[i] < nmax && t.pairs[lo].M / 2 < (1 << 15)) cls = 5;
                 } else if ((cls == 2 || cls == 3 || (cached && !odd))) {
                     bool single_period = t.pairs[lo].M / 2 < g.n[i] && g.n[i] <= t.pairs[lo].M;
                     for (int p = lo; p < hi; ++p) single_period = single_period && t.pairs[lo].M / 2 < g.n[t.pairs[p].j];
@@ -475,7 +483,7 @@ void build_pairs(HostGeometry& g, double theta_max, double ell_nyq, int fixed_mp
                     tile_rec.n_sh[ii] = g.n[ia + ii] | (g.shifted[ia + ii] ? (int)0x80000000 : 0);
                 }
                 t.tc_tiles.push_back(tile_rec);
-                for (int col = 0; col < kTcN; ++col) {
+                for (int col = 0; col < tg.n; ++col) {
                     const int jj = col / kTcTI, ii = col % kTcTI;
                     uint32_t word = kTcNoPair;
                     if (ii < nti) {
@@ -491,10 +499,10 @@ void build_pairs(HostGeometry& g, double theta_max, double ell_nyq, int fixed_mp
             }
             t.tc_chunks.push_back(c);
             const int nmodes = with_nyquist ? M / 2 + 1 : M / 2;
-            for (int bx = 0; bx * 128 * kTcMT < nmodes; ++bx) {
+            for (int bx = 0; bx * 128 * tg.mt < nmodes; ++bx) {
                 t.tc_items[cls].push_back(TcItem{(int)t.tc_chunks.size() - 1, bx});
                 // upper bound: the kernel issues fewer K steps for tiles whose rows are short
-                st.tc_flops += (double)((n + kTcTI - 1) / kTcTI) * kTcMT * 3.0 * (kTcK / 8) * 2.0 * 128.0 * kTcN * 8.0;
+                st.tc_flops += (double)((n + kTcTI - 1) / kTcTI) * tg.mt * 3.0 * (tg.k / 8) * 2.0 * 128.0 * tg.n * 8.0;
             }
         };
         for (int j = 0; j < R; ++j)
@@ -687,7 +695,7 @@ void launch_uniform(const arkcos_plan* pl, int nmaps, cudaStream_t st, bool seri
         else if (nmaps > 1) launch_eq(std::integral_constant<int, 2>{}, std::integral_constant<int, 2>{});
         else launch_eq(std::integral_constant<int, 1>{}, std::integral_constant<int, 2>{});
     } else if (pl->neqchunks > 0 && pl->use_tc && pl->ntc_items[0] > 0) {
-        tc_launch(pl->eq_alt ? 0 : 1, (unsigned)pl->ntc_items[0], (unsigned)nmaps, st, pl->d_tc_items[0], pl->d_tc_chunks, pl->d_tc_tiles,
+        tc_launch(pl->tc_cfg, pl->eq_alt ? 0 : 1, (unsigned)pl->ntc_items[0], (unsigned)nmaps, st, pl->d_tc_items[0], pl->d_tc_chunks, pl->d_tc_tiles,
                   pl->d_tc_cols, pl->d_tc_rings, (const float*)pl->d_W, pl->g.R, (const cx<float>*)pl->spec_in(), (cx<float>*)pl->d_specOut,
                   pl->g.spec_total);
     } else if (pl->neqchunks > 0) {
@@ -731,7 +739,7 @@ void launch_uniform(const arkcos_plan* pl, int nmaps, cudaStream_t st, bool seri
                     (const cx<float>*)pl->spec_in(), (cx<float>*)pl->d_specOut, pl->g.spec_total, nmaps);
             else if (pl->use_tc) {
                 if (pl->ntc_items[MULTI ? 2 : 1] > 0)
-                    tc_launch(MULTI ? 3 : 2, (unsigned)pl->ntc_items[MULTI ? 2 : 1], (unsigned)nmaps, s1, pl->d_tc_items[MULTI ? 2 : 1],
+                    tc_launch(pl->tc_cfg, MULTI ? 3 : 2, (unsigned)pl->ntc_items[MULTI ? 2 : 1], (unsigned)nmaps, s1, pl->d_tc_items[MULTI ? 2 : 1],
                               pl->d_tc_chunks, pl->d_tc_tiles, pl->d_tc_cols, pl->d_tc_rings, (const float*)pl->d_W, pl->g.R,
                               (const cx<float>*)pl->spec_in(), (cx<float>*)pl->d_specOut, pl->g.spec_total);
             } else
@@ -1020,6 +1028,7 @@ static int plan_create_impl(arkcos_plan** out, const arkcos_pixelization* pix, c
     for (int c = 0; c < kBandClasses; ++c) pl->nitems[c] = (int)t.items[c].size();
     pl->neqchunks = (int)t.eq_chunks.size();
     pl->use_tc = t.use_tc;
+    pl->tc_cfg = t.tc_cfg;
     for (int c = 0; c < 3; ++c) pl->ntc_items[c] = (int)t.tc_items[c].size();
     if (t.nsamples / 4 >= (1 << 25)) return fail(ARKCOS_UNSUPPORTED, "too many kernel-row samples");
     pl->npole = (int)t.pole_rings.size();
@@ -1076,7 +1085,7 @@ static int plan_create_impl(arkcos_plan** out, const arkcos_pixelization* pix, c
         if (int rc = upload(&pl->d_tc_rings, t.tc_rings, wsb)) return rc;
         for (int c = 0; c < 3; ++c)
             if (int rc = upload(&pl->d_tc_items[c], t.tc_items[c], wsb)) return rc;
-        CUDA_TRY((cudaError_t)tc_setup(&pl->tc_blocks_per_sm));
+        CUDA_TRY((cudaError_t)tc_setup(pl->tc_cfg, &pl->tc_blocks_per_sm));
     }
     if (int rc = upload(&pl->d_cap_chunks, t.cap_chunks, wsb)) return rc;
     if (int rc = upload(&pl->d_cap_chunk_items, t.cap_chunk_items, wsb)) return rc;

@@ -70,6 +70,7 @@ struct arkcos_plan {
     // tensor-core band kernels (arkcos_band_tc.cuh): class-E runs as (run, block of 128 modes) items; the cap runs use
     // d_cap_chunks / d_cap_chunk_items with blocks of 128 modes
     bool use_tc = false;
+    int tc_cfg = 0;                   // tile geometry of band_mac_tc_kernel: 0 narrow (TcCfgNarrow), 1 wide (TcCfgWide)
     arkcos::TcChunk* d_tc_chunks = nullptr;
     arkcos::TcTile* d_tc_tiles = nullptr;
     uint32_t* d_tc_cols = nullptr;
