@@ -678,10 +678,13 @@ template <int TMAX, bool HAS_ODD> void launch_uniform_class(const arkcos_plan* p
         (const cx<float>*)pl->spec_in(), (cx<float>*)pl->d_specOut, pl->g.spec_total);
 }
 
-void launch_uniform(const arkcos_plan* pl, int nmaps, cudaStream_t st, bool serial)
+// which: 1 = the big launches (class-E runs on st, cap runs on side stream 0), 2 = the small uniform classes (side stream 2),
+// 3 = both in the order of the timing slots (serial timing mode).
+void launch_uniform(const arkcos_plan* pl, int nmaps, cudaStream_t st, bool serial, int which)
 {
-    cudaStream_t s1 = serial ? st : pl->side[1], s2 = serial ? st : pl->side[2];
-    if (pl->neqchunks > 0 && pl->d_G) {
+    cudaStream_t s1 = serial ? st : pl->side[2], s2 = serial ? st : pl->side[2], sc = serial ? st : pl->side[0];
+    if (!(which & 1)) {
+    } else if (pl->neqchunks > 0 && pl->d_G) {
         const unsigned gx = (unsigned)((pl->eq_mh + 255) / 256);
         auto launch_eq = [&](auto nm_tag, auto mt_tag) {
             constexpr int NM = decltype(nm_tag)::value, MT = decltype(mt_tag)::value;
@@ -711,39 +714,39 @@ void launch_uniform(const arkcos_plan* pl, int nmaps, cudaStream_t st, bool seri
                 (const cx<float>*)pl->spec_in(), (cx<float>*)pl->d_specOut, pl->g.spec_total);
     }
     if (serial) cudaEventRecord(pl->ev_band[3], st);
-    launch_uniform_class<12, false>(pl, 2, nmaps, s1);
+    if (which & 2) launch_uniform_class<12, false>(pl, 2, nmaps, s1);
     if (serial) cudaEventRecord(pl->ev_band[4], st);
-    launch_uniform_class<20, false>(pl, 3, nmaps, s1);
+    if (which & 2) launch_uniform_class<20, false>(pl, 3, nmaps, s1);
     if (serial) cudaEventRecord(pl->ev_band[5], st);
-    launch_uniform_class<32, true>(pl, 4, nmaps, s2);
+    if (which & 2) launch_uniform_class<32, true>(pl, 4, nmaps, s2);
     if (serial) cudaEventRecord(pl->ev_band[6], st);
-    launch_uniform_class<12, true>(pl, 1, nmaps, s2);
+    if (which & 2) launch_uniform_class<12, true>(pl, 1, nmaps, s2);
     if (serial) cudaEventRecord(pl->ev_band[7], st);
-    if (pl->ncapitems > 0) {
+    if (pl->ncapitems > 0 && (which & 1)) {
         auto launch_cap = [&](auto multi_tag, int first, int count) {
             constexpr bool MULTI = decltype(multi_tag)::value;
             if (count <= 0) return;
             const unsigned n = (unsigned)count;
             const CapChunkItem* items = pl->d_cap_chunk_items + first;
             if (pl->d_G && nmaps >= 4)
-                band_mac_capchunk_cached_kernel<4, 4, MULTI, 1><<<dim3(n, (unsigned)((nmaps + 3) / 4)), 256, 0, s1>>>(
+                band_mac_capchunk_cached_kernel<4, 4, MULTI, 1><<<dim3(n, (unsigned)((nmaps + 3) / 4)), 256, 0, sc>>>(
                     items, pl->d_cap_chunks, pl->d_north, pl->d_pairs, pl->d_goff, pl->d_G, pl->d_rings, pl->g.R,
                     (const cx<float>*)pl->spec_in(), (cx<float>*)pl->d_specOut, pl->g.spec_total, nmaps);
             else if (pl->d_G && nmaps > 1)
-                band_mac_capchunk_cached_kernel<4, 2, MULTI, 2><<<dim3(n, (unsigned)((nmaps + 1) / 2)), kBandThreads, 0, s1>>>(
+                band_mac_capchunk_cached_kernel<4, 2, MULTI, 2><<<dim3(n, (unsigned)((nmaps + 1) / 2)), kBandThreads, 0, sc>>>(
                     items, pl->d_cap_chunks, pl->d_north, pl->d_pairs, pl->d_goff, pl->d_G, pl->d_rings, pl->g.R,
                     (const cx<float>*)pl->spec_in(), (cx<float>*)pl->d_specOut, pl->g.spec_total, nmaps);
             else if (pl->d_G)
-                band_mac_capchunk_cached_kernel<4, 1, MULTI, 2><<<dim3(n, 1), kBandThreads, 0, s1>>>(
+                band_mac_capchunk_cached_kernel<4, 1, MULTI, 2><<<dim3(n, 1), kBandThreads, 0, sc>>>(
                     items, pl->d_cap_chunks, pl->d_north, pl->d_pairs, pl->d_goff, pl->d_G, pl->d_rings, pl->g.R,
                     (const cx<float>*)pl->spec_in(), (cx<float>*)pl->d_specOut, pl->g.spec_total, nmaps);
             else if (pl->use_tc) {
                 if (pl->ntc_items[MULTI ? 2 : 1] > 0)
-                    tc_launch(pl->tc_cfg, MULTI ? 3 : 2, (unsigned)pl->ntc_items[MULTI ? 2 : 1], (unsigned)nmaps, s1, pl->d_tc_items[MULTI ? 2 : 1],
+                    tc_launch(pl->tc_cfg, MULTI ? 3 : 2, (unsigned)pl->ntc_items[MULTI ? 2 : 1], (unsigned)nmaps, sc, pl->d_tc_items[MULTI ? 2 : 1],
                               pl->d_tc_chunks, pl->d_tc_tiles, pl->d_tc_cols, pl->d_tc_rings, (const float*)pl->d_W, pl->g.R,
                               (const cx<float>*)pl->spec_in(), (cx<float>*)pl->d_specOut, pl->g.spec_total);
             } else
-                band_mac_capchunk_kernel<4, 20, MULTI><<<dim3(n, (unsigned)nmaps), kBandThreads, 0, s1>>>(
+                band_mac_capchunk_kernel<4, 20, MULTI><<<dim3(n, (unsigned)nmaps), kBandThreads, 0, sc>>>(
                     items, pl->d_cap_chunks, pl->d_north, pl->d_pairs, (const float*)pl->d_W, pl->d_rings, pl->g.R,
                     (const cx<float>*)pl->spec_in(), (cx<float>*)pl->d_specOut, pl->g.spec_total);
         };
@@ -875,10 +878,14 @@ template <class T> int enqueue_convolve(const arkcos_plan* pl, const void* d_in,
     // the band kernels of the different ring classes write disjoint rings: fork them onto the plan's side streams
     // (timing mode 2: one after the other on the caller's stream with an event between them)
     const bool serial = pl->timing == 2;
-    cudaStream_t s0 = serial ? st : pl->side[0];
+    // The big launches (tensor-core / run kernels) go first: each of their blocks takes a whole SM, and a small latency-bound
+    // kernel that got there before them would hold every SM for its whole duration; issued behind them the small ones run in
+    // the gaps of the big launches' last waves.
+    cudaStream_t s0 = serial ? st : pl->side[1];
     if (!serial) {
         cudaEventRecord(pl->ev_fork, st);
         for (int k = 0; k < 3; ++k) cudaStreamWaitEvent(pl->side[k], pl->ev_fork, 0);
+        launch_uniform(pl, nmaps, st, false, 1);
     }
     if (serial) cudaEventRecord(pl->ev_band[0], st);
     if (pl->nitems[0] > 0) {
@@ -908,7 +915,7 @@ template <class T> int enqueue_convolve(const arkcos_plan* pl, const void* d_in,
             g.spec_total);
     }
     if (serial) cudaEventRecord(pl->ev_band[2], st);
-    launch_uniform(pl, nmaps, st, serial);
+    launch_uniform(pl, nmaps, st, serial, serial ? 3 : 2);
     if (!serial)
         for (int k = 0; k < 3; ++k) {
             cudaEventRecord(pl->ev_join[k], pl->side[k]);
