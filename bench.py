@@ -162,6 +162,8 @@ def run_ours(args):
     rank = int(os.environ.get("RANK", "0"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
     torch.cuda.set_device(local)
+    # a stream of our own (events and launches on the same, non-default stream; the library replays a CUDA graph there)
+    torch.cuda.set_stream(torch.cuda.Stream())
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     c, tab, x, npix, nmaps, name = workload(args.cfg, args.cfg5_kernel)

@@ -89,7 +89,12 @@ typedef struct {
  *                       fp64 distances per pixel pair, weights shared by the maps of a call.
  *  no_tensor_cores   0: float plans run the kernel-row phi-transform of the class-E and cap-ring runs as
  *                       3xTF32 tcgen05 matrix products (FP32-level accuracy); 1: every band kernel
- *                       uses FP32 FMAs only (the round-1 kernels; also what small grids and cached-spectra plans use). */
+ *                       uses FP32 FMAs only (the round-1 kernels; also what small grids and cached-spectra plans use).
+ *  no_cuda_graph     0: arkcos_convolve captures the launches of a call (about 30 kernels on the caller's stream and six plan-owned
+ *                       streams, with their event dependencies) into a CUDA graph the first time it sees a combination of
+ *                       (d_in, d_out, nmaps, stream) and replays that graph afterwards (the four most recent combinations are
+ *                       kept); not on the NULL / legacy default stream, not while the stream is being captured by the caller
+ *                       (then the launches simply join the caller's capture), not in the timing modes.  1: always launch directly. */
 typedef struct {
     int variant;
     double ell_nyquist;
@@ -99,7 +104,8 @@ typedef struct {
     int exact_caps;
     int cache_kernel_spectra;
     int no_tensor_cores;
-    int reserved[5];               /* must be zero */
+    int no_cuda_graph;
+    int reserved[4];               /* must be zero */
 } arkcos_options;
 
 /* Builds the ring-geometry table (theta, N, phi0, offset per ring), the band and ring-pair tables, FFT twiddles,

@@ -31,7 +31,7 @@ class Kernel(Structure):
 class Options(Structure):
     _fields_ = [("variant", c_int), ("ell_nyquist", c_double), ("polar_oversample", c_int), ("max_nmaps", c_int),
                 ("cache_kernel_rows", c_int), ("exact_caps", c_int), ("cache_kernel_spectra", c_int), ("no_tensor_cores", c_int),
-                ("reserved", c_int * 5)]
+                ("no_cuda_graph", c_int), ("reserved", c_int * 4)]
 
 
 class ArkcosError(RuntimeError):
@@ -157,7 +157,7 @@ class Plan:
     """Owns an ``arkcos_plan*``.  ``pix`` is ("ecp", ntheta, nphi) or ("healpix", nside)."""
 
     def __init__(self, pix, table, theta_max: float, dtype=F32, *, variant=0, ell_nyquist=0.0, polar_oversample=0,
-                 max_nmaps=1, cache_kernel_rows=0, exact_caps=0, cache_kernel_spectra=0, no_tensor_cores=0, tables_only=False):
+                 max_nmaps=1, cache_kernel_rows=0, exact_caps=0, cache_kernel_spectra=0, no_tensor_cores=0, no_cuda_graph=0, tables_only=False):
         lib = _lib()
         if pix[0] == "ecp":
             p = Pixelization(ECP, int(pix[1]), int(pix[2]), 0)
@@ -168,7 +168,7 @@ class Plan:
         tab = np.ascontiguousarray(table, dtype=np.float64)
         k = Kernel(tab.ctypes.data_as(POINTER(c_double)), int(tab.shape[0]), float(theta_max))
         o = Options(int(variant), float(ell_nyquist), int(polar_oversample), int(max_nmaps), int(cache_kernel_rows),
-                    int(exact_caps), int(cache_kernel_spectra), int(no_tensor_cores))
+                    int(exact_caps), int(cache_kernel_spectra), int(no_tensor_cores), int(no_cuda_graph))
         self._h = c_void_p()
         self.dtype = dtype
         self.max_nmaps = max(1, int(max_nmaps))

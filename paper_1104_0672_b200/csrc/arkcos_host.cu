@@ -682,7 +682,8 @@ template <int TMAX, bool HAS_ODD> void launch_uniform_class(const arkcos_plan* p
 // 3 = both in the order of the timing slots (serial timing mode).
 void launch_uniform(const arkcos_plan* pl, int nmaps, cudaStream_t st, bool serial, int which)
 {
-    cudaStream_t s1 = serial ? st : pl->side[2], s2 = serial ? st : pl->side[2], sc = serial ? st : pl->side[0];
+    // every small class on a stream of its own: they are latency-bound, tiny grids
+    cudaStream_t s1 = serial ? st : pl->side[2], s2 = serial ? st : pl->side[3], s3 = serial ? st : pl->side[4], sc = serial ? st : pl->side[0];
     if (!(which & 1)) {
     } else if (pl->neqchunks > 0 && pl->d_G) {
         const unsigned gx = (unsigned)((pl->eq_mh + 255) / 256);
@@ -720,7 +721,7 @@ void launch_uniform(const arkcos_plan* pl, int nmaps, cudaStream_t st, bool seri
     if (serial) cudaEventRecord(pl->ev_band[5], st);
     if (which & 2) launch_uniform_class<32, true>(pl, 4, nmaps, s2);
     if (serial) cudaEventRecord(pl->ev_band[6], st);
-    if (which & 2) launch_uniform_class<12, true>(pl, 1, nmaps, s2);
+    if (which & 2) launch_uniform_class<12, true>(pl, 1, nmaps, s3);
     if (serial) cudaEventRecord(pl->ev_band[7], st);
     if (pl->ncapitems > 0 && (which & 1)) {
         auto launch_cap = [&](auto multi_tag, int first, int count) {
@@ -881,10 +882,10 @@ template <class T> int enqueue_convolve(const arkcos_plan* pl, const void* d_in,
     // The big launches (tensor-core / run kernels) go first: each of their blocks takes a whole SM, and a small latency-bound
     // kernel that got there before them would hold every SM for its whole duration; issued behind them the small ones run in
     // the gaps of the big launches' last waves.
-    cudaStream_t s0 = serial ? st : pl->side[1];
+    cudaStream_t s0 = serial ? st : pl->side[1], sp = serial ? st : pl->side[5];
     if (!serial) {
         cudaEventRecord(pl->ev_fork, st);
-        for (int k = 0; k < 3; ++k) cudaStreamWaitEvent(pl->side[k], pl->ev_fork, 0);
+        for (int k = 0; k < 6; ++k) cudaStreamWaitEvent(pl->side[k], pl->ev_fork, 0);
         launch_uniform(pl, nmaps, st, false, 1);
     }
     if (serial) cudaEventRecord(pl->ev_band[0], st);
@@ -902,22 +903,22 @@ template <class T> int enqueue_convolve(const arkcos_plan* pl, const void* d_in,
     if (serial) cudaEventRecord(pl->ev_band[1], st);
     if (pl->npole > 0 && !pl->pole_warp_per_mode)
         band_mac_pole1_kernel<T, 16><<<dim3((unsigned)pl->npole, (unsigned)nmaps), kPoleThreads,
-                                        2 * (size_t)(pl->pole_mh + 1) * sizeof(cx<T>), s0>>>(
+                                        2 * (size_t)(pl->pole_mh + 1) * sizeof(cx<T>), sp>>>(
             pl->d_pole, pl->d_north, pl->d_pairs, (const T*)pl->d_W, pl->d_rings, g.R, (const cx<T>*)pl->spec_in(),
             (cx<T>*)pl->d_specOut, g.spec_total);
     else if (pl->npole > 0) {
         const int tstride = pl->pole_mh + 1, bpr = (tstride + kPoleWarps - 1) / kPoleWarps;
-        band_mac_pole_kernel<T><<<dim3((unsigned)(pl->npole * bpr), (unsigned)nmaps), kPoleThreads, 0, s0>>>(
+        band_mac_pole_kernel<T><<<dim3((unsigned)(pl->npole * bpr), (unsigned)nmaps), kPoleThreads, 0, sp>>>(
             pl->d_pole, bpr, pl->d_north, pl->d_pairs, (const T*)pl->d_W, pl->d_rings, g.R, (const cx<T>*)pl->spec_in(), g.spec_total,
             (cx<T>*)pl->d_pole_scratch, tstride);
-        band_mac_pole_fold_kernel<T><<<dim3((unsigned)pl->npole, (unsigned)nmaps), kPoleThreads, 0, s0>>>(
+        band_mac_pole_fold_kernel<T><<<dim3((unsigned)pl->npole, (unsigned)nmaps), kPoleThreads, 0, sp>>>(
             pl->d_pole, pl->d_north, pl->d_pairs, pl->d_rings, g.R, (const cx<T>*)pl->d_pole_scratch, tstride, (cx<T>*)pl->d_specOut,
             g.spec_total);
     }
     if (serial) cudaEventRecord(pl->ev_band[2], st);
     launch_uniform(pl, nmaps, st, serial, serial ? 3 : 2);
     if (!serial)
-        for (int k = 0; k < 3; ++k) {
+        for (int k = 0; k < 6; ++k) {
             cudaEventRecord(pl->ev_join[k], pl->side[k]);
             cudaStreamWaitEvent(st, pl->ev_join[k], 0);
         }
@@ -971,6 +972,7 @@ static int plan_create_impl(arkcos_plan** out, const arkcos_pixelization* pix, c
     if (opt.cache_kernel_spectra != 0 && opt.cache_kernel_spectra != 1)
         return fail(ARKCOS_INVALID_ARG, "options.cache_kernel_spectra must be 0 or 1");
     if (opt.no_tensor_cores != 0 && opt.no_tensor_cores != 1) return fail(ARKCOS_INVALID_ARG, "options.no_tensor_cores must be 0 or 1");
+    if (opt.no_cuda_graph != 0 && opt.no_cuda_graph != 1) return fail(ARKCOS_INVALID_ARG, "options.no_cuda_graph must be 0 or 1");
     if (opt.cache_kernel_spectra && (dtype != ARKCOS_F32 || opt.variant != 0))
         return fail(ARKCOS_UNSUPPORTED, "cache_kernel_spectra needs a float plan of variant 0");
     if (opt.cache_kernel_spectra) opt.cache_kernel_rows = 1;     // the spectra are made from the rows, once
@@ -1167,8 +1169,41 @@ int arkcos_convolve(const arkcos_plan* pl, const void* d_in, void* d_out, int nm
     int dev = -1;
     CUDA_TRY(cudaGetDevice(&dev));
     if (dev != pl->device) return fail(ARKCOS_INVALID_ARG, "the current device is not the device the plan was created on");
-    return pl->dtype == ARKCOS_F32 ? enqueue_convolve<float>(pl, d_in, d_out, nmaps, st)
-                                   : enqueue_convolve<double>(pl, d_in, d_out, nmaps, st);
+    auto enqueue = [&]() {
+        return pl->dtype == ARKCOS_F32 ? enqueue_convolve<float>(pl, d_in, d_out, nmaps, st)
+                                       : enqueue_convolve<double>(pl, d_in, d_out, nmaps, st);
+    };
+    // One graph launch instead of ~30 kernel launches and their cross-stream events (options.no_cuda_graph).
+    cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+    const bool graph_ok = !pl->opt.no_cuda_graph && pl->timing == 0 && st != nullptr && st != cudaStreamLegacy &&
+                          st != cudaStreamPerThread && cudaStreamIsCapturing(st, &cap) == cudaSuccess && cap == cudaStreamCaptureStatusNone;
+    if (!graph_ok) return enqueue();
+    for (size_t k = 0; k < pl->graphs.size(); ++k) {
+        const arkcos_plan::GraphEntry e = pl->graphs[k];
+        if (e.in == d_in && e.out == d_out && e.nmaps == nmaps && e.st == st) {
+            if (k > 0) { pl->graphs.erase(pl->graphs.begin() + k); pl->graphs.insert(pl->graphs.begin(), e); }
+            CUDA_TRY(cudaGraphLaunch(e.exec, st));
+            return ARKCOS_OK;
+        }
+    }
+    if (cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal) != cudaSuccess) {
+        cudaGetLastError();
+        return enqueue();
+    }
+    const int rc = enqueue();
+    cudaGraph_t graph = nullptr;
+    const cudaError_t ce = cudaStreamEndCapture(st, &graph);
+    cudaGraphExec_t exec = nullptr;
+    if (rc != ARKCOS_OK || ce != cudaSuccess || !graph || cudaGraphInstantiate(&exec, graph, 0) != cudaSuccess) {
+        if (graph) cudaGraphDestroy(graph);
+        cudaGetLastError();
+        return rc != ARKCOS_OK ? rc : enqueue();                // capture refused: launch directly
+    }
+    cudaGraphDestroy(graph);
+    if (pl->graphs.size() >= 4) { cudaGraphExecDestroy(pl->graphs.back().exec); pl->graphs.pop_back(); }
+    pl->graphs.insert(pl->graphs.begin(), arkcos_plan::GraphEntry{d_in, d_out, nmaps, st, exec});
+    CUDA_TRY(cudaGraphLaunch(exec, st));
+    return ARKCOS_OK;
 }
 
 int arkcos_convolve_multi(const arkcos_plan* const* plans, int nkernels, const void* d_in, void* d_out, int nmaps, void* cuda_stream)
@@ -1276,6 +1311,8 @@ int arkcos_plan_synchronize(const arkcos_plan* pl)
 int arkcos_plan_destroy(arkcos_plan* pl)
 {
     if (!pl) return ARKCOS_OK;
+    for (const auto& e : pl->graphs) cudaGraphExecDestroy(e.exec);
+    pl->graphs.clear();
     for (int b = 0; b < 2; ++b) {
         if (pl->d_pipe_in[b]) cudaFree(pl->d_pipe_in[b]);
         if (pl->d_pipe_out[b]) cudaFree(pl->d_pipe_out[b]);

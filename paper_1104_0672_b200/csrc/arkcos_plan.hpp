@@ -114,13 +114,17 @@ struct arkcos_plan {
     mutable cudaStream_t s_h2d = nullptr, s_comp = nullptr, s_d2h = nullptr;
     mutable cudaEvent_t ev_h2d[2] = {nullptr, nullptr}, ev_comp[2] = {nullptr, nullptr}, ev_d2h[2] = {nullptr, nullptr};
     mutable uint64_t pipe_calls = 0;
+    // CUDA graphs of whole calls, keyed by the call's arguments (most recent first)
+    struct GraphEntry { const void* in; void* out; int nmaps; cudaStream_t st; cudaGraphExec_t exec; };
+    mutable std::vector<GraphEntry> graphs;
     // optional per-stage timing
     mutable int timing = 0;
     mutable cudaEvent_t ev[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
     mutable cudaEvent_t ev_band[10] = {};
     mutable cudaEvent_t ev_fft[2][10] = {};      // timing mode 2: before each ring-FFT launch of a direction and after the last
     // fork/join of the band kernels of the different ring classes
-    cudaStream_t side[3] = {nullptr, nullptr, nullptr}, side_rows = nullptr;
-    cudaEvent_t ev_fork = nullptr, ev_join[3] = {nullptr, nullptr, nullptr};
+    // side streams 0-2: ring-FFT size classes and the big band launches; 0-5: the band kernels of the ring classes
+    cudaStream_t side[6] = {}, side_rows = nullptr;
+    cudaEvent_t ev_fork = nullptr, ev_join[6] = {};
     cudaEvent_t ev_rows_fork = nullptr, ev_rows_done = nullptr;   // kernel-row generator beside the forward FFTs
 };

@@ -511,3 +511,43 @@ def test_repeatability(tc):
     for r in single:
         assert np.array_equal(a[geom.ring_slice(r)], b[geom.ring_slice(r)]), r
     assert frms(a, b) <= 1e-7
+
+
+def test_cuda_graph_replay_equals_direct_launches():
+    """arkcos_convolve on a non-default stream captures the launches of the first call with a given (d_in, d_out, nmaps,
+    stream) into a CUDA graph and replays it afterwards (options.no_cuda_graph = 0).  Replays, re-captures for new buffers
+    (more than the four combinations the plan keeps) and a plan that launches directly must agree: bit-equal on the belt,
+    to rounding elsewhere (multi-period fold); the first call's own result included."""
+    nside, nmaps = 256, 2
+    geom = geometry.healpix_ring(nside)
+    px = np.sqrt(4 * np.pi / geom.npix)
+    tab, tmax = inputs.gaussian_table(2.91 * px, 3 * 2.91 * px), 3 * 2.91 * px
+    plan_g = arkcos.Plan(("healpix", nside), tab, tmax, arkcos.F32, max_nmaps=nmaps)
+    plan_d = arkcos.Plan(("healpix", nside), tab, tmax, arkcos.F32, max_nmaps=nmaps, no_cuda_graph=1)
+    belt = slice(int(geom.offset[nside + 16]), int(geom.offset[3 * nside - 17]))
+    s = torch.cuda.Stream()
+    outs = []
+    with torch.cuda.stream(s):
+        xs = [torch.from_numpy(inputs.white_noise_maps(geom.npix, 20 + k, nmaps)).cuda() for k in range(6)]
+        os_ = [torch.full_like(x, float("nan")) for x in xs]
+        ref = [torch.empty_like(x) for x in xs]
+        for rep in range(3):                       # capture, replay, replay; six buffer pairs > four cached graphs
+            for x, o in zip(xs, os_):
+                plan_g.convolve(x.data_ptr(), o.data_ptr(), nmaps, s.cuda_stream)
+            s.synchronize()
+            outs.append([o.cpu().numpy() for o in os_])
+        for x, r in zip(xs, ref):
+            plan_d.convolve(x.data_ptr(), r.data_ptr(), nmaps, s.cuda_stream)
+        s.synchronize()
+    for k in range(6):
+        r = ref[k].cpu().numpy()
+        for rep in range(3):
+            assert np.array_equal(outs[rep][k][:, belt], r[:, belt]), (rep, k)
+            assert frms(outs[rep][k], r) <= 1e-7, (rep, k)
+    # one map of a two-map plan through the same stream: another graph
+    with torch.cuda.stream(s):
+        o1 = torch.empty_like(xs[0][0])
+        plan_g.convolve(xs[0][0].data_ptr(), o1.data_ptr(), 1, s.cuda_stream)
+        plan_g.convolve(xs[0][0].data_ptr(), o1.data_ptr(), 1, s.cuda_stream)
+        s.synchronize()
+    assert frms(o1.cpu().numpy(), ref[0][0].cpu().numpy()) <= 1e-7
