@@ -94,9 +94,18 @@ __global__ void band_mac_general_kernel(const BandItem* __restrict__ items, cons
     const cx<T>* __restrict__ in = specIn + (int64_t)blockIdx.y * spec_stride;
     cx<T> accN = mk<T>(0, 0), accS = mk<T>(0, 0);
     const NorthRec nr = north[i];
+    // the records of the next pair travel while this one is worked on (pair record -> ring records -> coefficients is a
+    // chain of dependent loads; the kernel is latency-bound)
+    int pnx = min(nr.pair_lo + slice, nr.pair_hi - 1);
+    PairRec prn = pairs[pnx];
+    RingRec rjn = rings[prn.j], rjSn = rings[R - 1 - prn.j];
     for (int p = nr.pair_lo + slice; p < nr.pair_hi; p += kGeneralSplit) {
-        const PairRec pr = pairs[p];
-        const RingRec rj = rings[pr.j], rjS = rings[R - 1 - pr.j];
+        const PairRec pr = prn;
+        const RingRec rj = rjn, rjS = rjSn;
+        pnx = min(p + kGeneralSplit, nr.pair_hi - 1);
+        prn = pairs[pnx];
+        rjn = rings[prn.j];
+        rjSn = rings[R - 1 - prn.j];
         const cx<T>* __restrict__ bN = in + rj.spec_off;
         const cx<T>* __restrict__ bS = in + rjS.spec_off;
         const T* __restrict__ w = W + pr.woff;
@@ -543,8 +552,30 @@ band_mac_pole_kernel(const int* __restrict__ ring_list, int blocks_per_ring, con
     const cx<T>* __restrict__ in = specIn + (int64_t)blockIdx.y * spec_stride;
     const cx<T> rot = cispi_ratio<T>((64u * (uint32_t)m) % (2u * (uint32_t)M), (uint32_t)M);
     cx<T> tN = mk<T>(0, 0), tS = mk<T>(0, 0);
+    // lane l keeps the records of pair pair_lo + l and its two coefficients (all pairs' loads in flight at once: the chain
+    // pair record -> ring records -> coefficients is what the warp would otherwise wait for, pair after pair)
+    const int npairs = nr.pair_hi - nr.pair_lo;
+    PairRec prl = pairs[nr.pair_lo + min(lane, npairs - 1)];
+    cx<T> vNl, vSl;
+    {
+        const RingRec rj = rings[prl.j], rjS = rings[R - 1 - prl.j];
+        vNl = ext_mode(in + rj.spec_off, m, rj.n, rj.shifted);
+        vSl = ext_mode(in + rjS.spec_off, m, rjS.n, rjS.shifted);
+    }
     for (int p = nr.pair_lo; p < nr.pair_hi; ++p) {
-        const PairRec pr = pairs[p];
+        const int src = (p - nr.pair_lo) & 31;
+        if (p > nr.pair_lo && src == 0) {                       // more than 32 pairs: the next batch
+            prl = pairs[min(p + lane, nr.pair_hi - 1)];
+            const RingRec rj = rings[prl.j], rjS = rings[R - 1 - prl.j];
+            vNl = ext_mode(in + rj.spec_off, m, rj.n, rj.shifted);
+            vSl = ext_mode(in + rjS.spec_off, m, rjS.n, rjS.shifted);
+        }
+        PairRec pr;
+        pr.woff = __shfl_sync(0xffffffffu, prl.woff, src);
+        pr.cnt = __shfl_sync(0xffffffffu, prl.cnt, src);
+        pr.par = __shfl_sync(0xffffffffu, prl.par, src);
+        const cx<T> vN = mk<T>(__shfl_sync(0xffffffffu, vNl.x, src), __shfl_sync(0xffffffffu, vNl.y, src));
+        const cx<T> vS = mk<T>(__shfl_sync(0xffffffffu, vSl.x, src), __shfl_sync(0xffffffffu, vSl.y, src));
         const T* __restrict__ w = W + pr.woff;
         // G_ij[m] = sum_t w[t] cos(m (2t + par) pi / M)
         cx<T> c = cispi_ratio<T>(((uint32_t)m * (uint32_t)(2 * lane + pr.par)) % (2u * (uint32_t)M), (uint32_t)M);
@@ -555,9 +586,6 @@ band_mac_pole_kernel(const int* __restrict__ ring_list, int blocks_per_ring, con
         }
 #pragma unroll
         for (int d = 16; d > 0; d >>= 1) G += __shfl_xor_sync(0xffffffffu, G, d);
-        const RingRec rj = rings[pr.j], rjS = rings[R - 1 - pr.j];
-        const cx<T> vN = ext_mode(in + rj.spec_off, m, rj.n, rj.shifted);
-        const cx<T> vS = ext_mode(in + rjS.spec_off, m, rjS.n, rjS.shifted);
         tN.x += G * vN.x; tN.y += G * vN.y;
         tS.x += G * vS.x; tS.y += G * vS.y;
     }
