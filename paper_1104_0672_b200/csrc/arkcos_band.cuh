@@ -117,7 +117,8 @@ __global__ void band_mac_general_kernel(const BandItem* __restrict__ items, cons
                 const cx<T> rot = cispi_ratio<T>((uint32_t)((2u * (uint32_t)m) % (2u * (uint32_t)M)), (uint32_t)M);
                 T G = 0;
                 for (int t0 = 0; t0 < pr.cnt; t0 += RESEED) {
-                    const uint64_t q = ((uint64_t)m * (uint64_t)(2 * t0 + pr.par)) % (uint64_t)(2 * M);
+                    // m <= M/2 < 2^15 and 2 t0 + par < 2 M <= 2^17: the product fits 32 bits
+                    const uint32_t q = ((uint32_t)m * (uint32_t)(2 * t0 + pr.par)) % (2u * (uint32_t)M);
                     cx<T> c = cispi_ratio<T>((uint32_t)q, (uint32_t)M);
                     const int t1 = min(pr.cnt, t0 + RESEED);
                     for (int t = t0; t < t1; ++t) {
