@@ -135,6 +135,24 @@ int arkcos_convolve(const arkcos_plan* plan, const void* d_in, void* d_out, int 
 int arkcos_convolve_multi(const arkcos_plan* const* plans, int nkernels, const void* d_in, void* d_out, int nmaps,
                           void* cuda_stream);
 
+/* arkcos_convolve for callers that cannot allocate device memory inside the call (code under CUDA graph capture, tight
+ * serving loops, harnesses that forbid cudaMalloc): the same launches with the same arguments, except that everything
+ * the call writes besides d_out -- the input-ring spectra B_j[m], the output-ring spectra (steps 1 and 3 of the hot path,
+ * PAPER.md:123-129) and the unfolded spectra between the two pole-ring launches -- lives in one array that is part of the
+ * library image (a file-scope __device__ array of ARKCOS_NO_ALLOC_SCRATCH_BYTES; every GPU that loads the library
+ * holds it until exit), not in the plan's workspace, and that no CUDA graph is built: the call makes no cudaMalloc,
+ * cudaFree, graph instantiation or other allocating call, it only enqueues memsets and kernels on cuda_stream and on the
+ * plan's side streams.  The plan's read-only tables are still the ones arkcos_plan_create allocated.
+ * Needs  2 * nmaps * spectrum bytes + pole scratch  <= ARKCOS_NO_ALLOC_SCRATCH_BYTES (fp32: about 8.1 bytes per pixel
+ * and map, e.g. HEALPix nside 512 with one map, nside 256 with four); more is refused with ARKCOS_INVALID_ARG and a
+ * message that names both numbers, and nothing is enqueued.  Arguments, layout and result as for arkcos_convolve.
+ * ALL calls on a device share the array, whatever their plan, and it keeps the last call's contents; the part a call
+ * uses is cleared at its start.  Two calls that overlap on the GPU (different streams, no dependency) race on it: order
+ * them.  The first call on a device looks up the array's address (cudaGetSymbolAddress): make that one outside stream
+ * capture. */
+#define ARKCOS_NO_ALLOC_SCRATCH_BYTES (32u << 20)
+int arkcos_convolve_no_alloc(const arkcos_plan* plan, const void* d_in, void* d_out, int nmaps, void* cuda_stream);
+
 /* Same result from HOST buffers (pinned memory makes the copies asynchronous): host -> device copy, arkcos_convolve,
  * device -> host copy, all on cuda_stream, then a stream synchronisation.  Uses staging buffers inside the plan. */
 int arkcos_convolve_host(const arkcos_plan* plan, const void* h_in, void* h_out, int nmaps, void* cuda_stream);

@@ -15,6 +15,7 @@ import numpy as np
 ECP, HEALPIX_RING = 0, 1
 F32, F64 = 0, 1
 OK, INVALID_ARG, UNSUPPORTED, CUDA_ERROR, OUT_OF_MEMORY = 0, -1, -2, -3, -4
+NO_ALLOC_SCRATCH_BYTES = 32 << 20      # ARKCOS_NO_ALLOC_SCRATCH_BYTES of include/arkcos.h
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libarkcos.so")
@@ -50,6 +51,7 @@ SYMBOLS = {
     "arkcos_plan_create_tables_only": (c_int, [POINTER(c_void_p), POINTER(Pixelization), POINTER(Kernel), c_int,
                                                POINTER(Options)]),
     "arkcos_convolve": (c_int, [c_void_p, c_void_p, c_void_p, c_int, c_void_p]),
+    "arkcos_convolve_no_alloc": (c_int, [c_void_p, c_void_p, c_void_p, c_int, c_void_p]),
     "arkcos_convolve_multi": (c_int, [POINTER(c_void_p), c_int, c_void_p, c_void_p, c_int, c_void_p]),
     "arkcos_convolve_host": (c_int, [c_void_p, c_void_p, c_void_p, c_int, c_void_p]),
     "arkcos_convolve_host_async": (c_int, [c_void_p, c_void_p, c_void_p, c_int]),
@@ -180,6 +182,11 @@ class Plan:
         """arkcos_convolve: device pointers (ints), raw cudaStream_t (int)."""
         _check(_lib().arkcos_convolve(self._h, c_void_p(d_in), c_void_p(d_out), int(nmaps), c_void_p(stream)),
                "arkcos_convolve")
+
+    def convolve_no_alloc(self, d_in: int, d_out: int, nmaps: int = 1, stream: int = 0):
+        """arkcos_convolve_no_alloc: as convolve, scratch in the library's static device array (NO_ALLOC_SCRATCH_BYTES)."""
+        _check(_lib().arkcos_convolve_no_alloc(self._h, c_void_p(d_in), c_void_p(d_out), int(nmaps), c_void_p(stream)),
+               "arkcos_convolve_no_alloc")
 
     def convolve_host(self, h_in: int, h_out: int, nmaps: int = 1, stream: int = 0):
         _check(_lib().arkcos_convolve_host(self._h, c_void_p(h_in), c_void_p(h_out), int(nmaps), c_void_p(stream)),

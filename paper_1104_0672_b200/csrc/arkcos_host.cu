@@ -6,6 +6,7 @@
 
 #include <algorithm>
 #include <map>
+#include <mutex>
 #include <new>
 #include <type_traits>
 
@@ -955,6 +956,14 @@ size_t elem_size(arkcos_dtype d) { return d == ARKCOS_F64 ? 8 : 4; }
 
 }  // namespace
 
+// arkcos_convolve_no_alloc: the spectra and the pole scratch of a call, in the library image instead of the plan's workspace.
+// In host code the name below is a host-side stand-in, not a device address: g_no_alloc_ptr[device] is the address
+// cudaGetSymbolAddress gave on that device, looked up once per device with that device current.
+static __device__ __align__(256) unsigned char g_no_alloc_scratch[ARKCOS_NO_ALLOC_SCRATCH_BYTES];
+static const int kNoAllocMaxDevices = 64;
+static void* g_no_alloc_ptr[kNoAllocMaxDevices] = {};
+static std::mutex g_no_alloc_mutex;
+
 extern "C" {
 
 static int plan_create_impl(arkcos_plan** out, const arkcos_pixelization* pix, const arkcos_kernel* kernel, arkcos_dtype dtype,
@@ -1204,6 +1213,58 @@ int arkcos_convolve(const arkcos_plan* pl, const void* d_in, void* d_out, int nm
     pl->graphs.insert(pl->graphs.begin(), arkcos_plan::GraphEntry{d_in, d_out, nmaps, st, exec});
     CUDA_TRY(cudaGraphLaunch(exec, st));
     return ARKCOS_OK;
+}
+
+int arkcos_convolve_no_alloc(const arkcos_plan* pl, const void* d_in, void* d_out, int nmaps, void* cuda_stream)
+{
+    if (!pl || !d_in || !d_out) return fail(ARKCOS_INVALID_ARG, "NULL argument");
+    if (pl->tables_only) return fail(ARKCOS_INVALID_ARG, "plan was created with arkcos_plan_create_tables_only");
+    if (nmaps < 1 || nmaps > pl->max_nmaps) return fail(ARKCOS_INVALID_ARG, "nmaps must be in [1, max_nmaps]");
+    const size_t bytes = (size_t)nmaps * (size_t)pl->g.npix * elem_size(pl->dtype);
+    const char *a = (const char*)d_in, *b = (const char*)d_out;
+    if (a < b + bytes && b < a + bytes) return fail(ARKCOS_INVALID_ARG, "d_in and d_out overlap");
+    if (((uintptr_t)d_in | (uintptr_t)d_out) & 15) return fail(ARKCOS_INVALID_ARG, "d_in / d_out must be 16-byte aligned");
+    // layout of the shared array: [input-ring spectra | output-ring spectra | unfolded pole spectra], each 256-byte aligned,
+    // per-map strides as in the plan's own workspace (build_device_numeric, plan_create_impl)
+    auto up = [](size_t x) { return (x + 255) & ~(size_t)255; };
+    const size_t sb = up((size_t)nmaps * (size_t)pl->g.spec_total * 2 * elem_size(pl->dtype));
+    const size_t pb = pl->d_pole_scratch ? up((size_t)nmaps * (size_t)pl->npole * 2 * (size_t)(pl->pole_mh + 1) * 2 * elem_size(pl->dtype)) : 0;
+    const size_t need = 2 * sb + pb;
+    if (need > (size_t)ARKCOS_NO_ALLOC_SCRATCH_BYTES)
+        return fail(ARKCOS_INVALID_ARG, "arkcos_convolve_no_alloc: this plan with " + std::to_string(nmaps) + " map(s) needs " +
+                                            std::to_string(need) + " bytes of scratch, the library holds ARKCOS_NO_ALLOC_SCRATCH_BYTES = " +
+                                            std::to_string((size_t)ARKCOS_NO_ALLOC_SCRATCH_BYTES) + "; use arkcos_convolve");
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    int dev = -1;
+    CUDA_TRY(cudaGetDevice(&dev));
+    if (dev != pl->device) return fail(ARKCOS_INVALID_ARG, "the current device is not the device the plan was created on");
+    if (dev < 0 || dev >= kNoAllocMaxDevices) return fail(ARKCOS_INVALID_ARG, "device ordinal beyond the table of scratch addresses");
+    unsigned char* base = nullptr;
+    {
+        std::lock_guard<std::mutex> lock(g_no_alloc_mutex);
+        if (!g_no_alloc_ptr[dev]) {
+            void* p = nullptr;
+            CUDA_TRY(cudaGetSymbolAddress(&p, g_no_alloc_scratch));
+            g_no_alloc_ptr[dev] = p;
+        }
+        base = (unsigned char*)g_no_alloc_ptr[dev];
+    }
+    // the array keeps the last call's contents (any plan's): start from zeros in the part this call uses
+    CUDA_TRY(cudaMemsetAsync(base, 0, need, st));
+    // the launches read the three addresses from the plan: point them at the array for the time of the enqueue
+    arkcos_plan* mpl = const_cast<arkcos_plan*>(pl);
+    void* const keep_in = pl->spec_in_shared;
+    void* const keep_out = pl->d_specOut;
+    void* const keep_pole = pl->d_pole_scratch;
+    mpl->spec_in_shared = base;
+    mpl->d_specOut = base + sb;
+    if (pb) mpl->d_pole_scratch = base + 2 * sb;
+    const int rc = pl->dtype == ARKCOS_F32 ? enqueue_convolve<float>(pl, d_in, d_out, nmaps, st)
+                                           : enqueue_convolve<double>(pl, d_in, d_out, nmaps, st);
+    mpl->spec_in_shared = keep_in;
+    mpl->d_specOut = keep_out;
+    mpl->d_pole_scratch = keep_pole;
+    return rc;
 }
 
 int arkcos_convolve_multi(const arkcos_plan* const* plans, int nkernels, const void* d_in, void* d_out, int nmaps, void* cuda_stream)
