@@ -290,6 +290,49 @@ band_mac_uniform_kernel(const BandItem* __restrict__ items, const NorthRec* __re
     if (iS != i) out[rings[iS].spec_off + mp] = accS;
 }
 
+// Nyquist bin m' = N_i / 2 of the class-E rings (N_i = N_j = M for the whole band; the run kernels stop at M/2 - 1).
+// Both families of the fold meet there at m = M/2 with half the weight each, the second one conjugated (and negated on a
+// shifted output ring), and G_ij[M/2] = sum_t w[t] cos((2t + par) pi / 2) = sum_t (-1)^t w[t] on the integer grid, 0 on
+// the half-step grid.  So  D_i[M/2] = sum_j G_ij Re B_j[M/2]  (shifted ring: i sum_j G_ij Im B_j[M/2]).
+// One warp per output ring, the lanes take the ring pairs; grid = (ceil(nrings / WARPS), nmaps).
+template <int WARPS>
+__global__ void __launch_bounds__(32 * WARPS)
+band_nyquist_eq_kernel(const int* __restrict__ ring_list, int nrings, const NorthRec* __restrict__ north,
+                       const PairRec* __restrict__ pairs, const float* __restrict__ W, const RingRec* __restrict__ rings, int R,
+                       const cx<float>* __restrict__ specIn, cx<float>* __restrict__ specOut, int64_t spec_stride)
+{
+    const int k = (int)blockIdx.x * WARPS + ((int)threadIdx.x >> 5), lane = (int)threadIdx.x & 31;
+    if (k >= nrings) return;
+    const int i = ring_list[k], iS = R - 1 - i;
+    const RingRec ri = rings[i];
+    const NorthRec nr = north[i];
+    const int Mh = ri.n >> 1;
+    const cx<float>* __restrict__ in = specIn + (int64_t)blockIdx.y * spec_stride;
+    float aN = 0.f, aS = 0.f;
+    for (int p = nr.pair_lo + lane; p < nr.pair_hi; p += 32) {
+        const PairRec pr = pairs[p];
+        if (pr.par) continue;
+        const cx<float> vN = in[rings[pr.j].spec_off + Mh], vS = in[rings[R - 1 - pr.j].spec_off + Mh];
+        const float4* __restrict__ w4 = reinterpret_cast<const float4*>(W + pr.woff);
+        float G = 0.f;
+        for (int t4 = 0; 4 * t4 < pr.cnt; ++t4) {                    // rows are stored zero-padded to a multiple of four
+            const float4 w = w4[t4];
+            G += (w.x - w.y) + (w.z - w.w);
+        }
+        aN = fmaf(G, ri.shifted ? vN.y : vN.x, aN);
+        aS = fmaf(G, ri.shifted ? vS.y : vS.x, aS);
+    }
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) {
+        aN += __shfl_xor_sync(0xffffffffu, aN, d);
+        aS += __shfl_xor_sync(0xffffffffu, aS, d);
+    }
+    if (lane != 0) return;
+    cx<float>* __restrict__ out = specOut + (int64_t)blockIdx.y * spec_stride;
+    out[ri.spec_off + Mh] = ri.shifted ? mk<float>(0.f, aN) : mk<float>(aN, 0.f);
+    if (iS != i) out[rings[iS].spec_off + Mh] = ri.shifted ? mk<float>(0.f, aS) : mk<float>(aS, 0.f);
+}
+
 }  // namespace arkcos
 
 namespace arkcos {

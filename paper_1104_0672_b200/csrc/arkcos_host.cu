@@ -168,6 +168,7 @@ struct HostTables {
     std::vector<CapChunkItem> cap_chunk_items;
     std::vector<std::pair<int64_t, int64_t>> cap_zero;   // (first coefficient, count) ranges of the output spectrum to clear
     std::vector<int> pole_rings;                 // rings for band_mac_pole_kernel
+    std::vector<int> nyq_rings;                  // class-E rings: their Nyquist bin goes to band_nyquist_eq_kernel
     int pole_mh = 0;
     int general_split = 1;                       // threads per mode of band_mac_general_kernel
     bool pole_warp_per_mode = false;             // long rows: band_mac_pole_kernel + fold; short rows: band_mac_pole1_kernel
@@ -388,8 +389,8 @@ void build_pairs(HostGeometry& g, double theta_max, double ell_nyq, int fixed_mp
             if (all_e && alt_ok && hi > lo && (maxcnt <= (tc_eq ? (eq_alt ? tg.k / 2 : tg.k) : 12) || cached) && g.n[i] >= 8 && g.spec_total < (int64_t)INT32_MAX) {
                 eq_rings.push_back(i);
                 st.band_flops[2] += ring_flops;
-                // the Nyquist bin m = M/2 goes to a per-mode kernel that holds the whole row (cached plans admit long rows)
-                t.items[maxcnt <= 12 ? 1 : (maxcnt <= 32 ? 4 : 0)].push_back(BandItem{i, g.n[i] / 2});
+                // the Nyquist bin m = M/2 goes to a kernel of its own (a warp per ring, rows of any length)
+                t.nyq_rings.push_back(i);
                 continue;
             }
             if (same && hi > lo) {
@@ -445,11 +446,8 @@ void build_pairs(HostGeometry& g, double theta_max, double ell_nyq, int fixed_mp
         int64_t blocks1 = 0;
         for (int i : general_rings) blocks1 += (g.n[i] / 2 + band_threads) / band_threads;
         t.general_split = blocks1 < 8 * (int64_t)sm_count ? 4 : 1;
-        std::vector<BandItem> nyq = t.items[0];                  // (Nyquist bins of cached-spectra plans were added above)
-        t.items[0].clear();
         for (int i : general_rings)
             for (int m0 = 0; m0 <= g.n[i] / 2; m0 += band_threads / t.general_split) t.items[0].push_back(BandItem{i, m0});
-        t.items[0].insert(t.items[0].end(), nyq.begin(), nyq.end());
         // pole kernel: one block per ring leaves the device idle when the rings are few; then a warp per mode, two launches
         t.pole_warp_per_mode = !t.pole_rings.empty() && 4 * (int)t.pole_rings.size() <= sm_count;
     }
@@ -723,6 +721,10 @@ void launch_uniform(const arkcos_plan* pl, int nmaps, cudaStream_t st, bool seri
     if (which & 2) launch_uniform_class<32, true>(pl, 4, nmaps, s2);
     if (serial) cudaEventRecord(pl->ev_band[6], st);
     if (which & 2) launch_uniform_class<12, true>(pl, 1, nmaps, s3);
+    if ((which & 2) && pl->nnyq > 0)
+        band_nyquist_eq_kernel<4><<<dim3((unsigned)((pl->nnyq + 3) / 4), (unsigned)nmaps), 128, 0, s3>>>(
+            pl->d_nyq, pl->nnyq, pl->d_north, pl->d_pairs, (const float*)pl->d_W, pl->d_rings, pl->g.R,
+            (const cx<float>*)pl->spec_in(), (cx<float>*)pl->d_specOut, pl->g.spec_total);
     if (serial) cudaEventRecord(pl->ev_band[7], st);
     if (pl->ncapitems > 0 && (which & 1)) {
         auto launch_cap = [&](auto multi_tag, int first, int count) {
@@ -1050,6 +1052,7 @@ static int plan_create_impl(arkcos_plan** out, const arkcos_pixelization* pix, c
     for (int c = 0; c < 3; ++c) pl->ntc_items[c] = (int)t.tc_items[c].size();
     if (t.nsamples / 4 >= (1 << 25)) return fail(ARKCOS_UNSUPPORTED, "too many kernel-row samples");
     pl->npole = (int)t.pole_rings.size();
+    pl->nnyq = (int)t.nyq_rings.size();
     pl->pole_mh = t.pole_mh;
     pl->general_split = t.general_split;
     pl->pole_warp_per_mode = t.pole_warp_per_mode;
@@ -1081,6 +1084,7 @@ static int plan_create_impl(arkcos_plan** out, const arkcos_pixelization* pix, c
         if (int rc = upload(&pl->d_items[c], t.items[c], wsb)) return rc;
     if (int rc = upload(&pl->d_eqchunks, t.eq_chunks, wsb)) return rc;
     if (int rc = upload(&pl->d_pole, t.pole_rings, wsb)) return rc;
+    if (int rc = upload(&pl->d_nyq, t.nyq_rings, wsb)) return rc;
     if (!t.pole_rings.empty()) {                // unfolded spectra T[m] of the pole kernel, ring and mirror image, per map
         const size_t nb = (size_t)pl->max_nmaps * t.pole_rings.size() * 2 * (size_t)(t.pole_mh + 1) * 2 * elem_size(dtype);
         CUDA_TRY(cudaMalloc(&pl->d_pole_scratch, nb));
@@ -1385,7 +1389,7 @@ int arkcos_plan_destroy(arkcos_plan* pl)
     void* ptrs[] = {pl->d_rings, pl->d_lens, pl->d_pairs, pl->d_north, pl->d_items[0], pl->d_items[1], pl->d_items[2], pl->d_items[3],
                     pl->d_items[4], pl->d_items[5], pl->d_eqchunks, pl->d_pole, pl->d_chirp, pl->d_phase, pl->d_fft_order[0], pl->d_fft_order[1], pl->d_table, pl->d_tw, pl->d_filt,
                     pl->d_W, pl->d_specIn, pl->d_specOut, pl->d_stage_in, pl->d_stage_out,
-                    pl->d_cap_chunks, pl->d_cap_chunk_items, pl->d_tc_chunks, pl->d_tc_tiles, pl->d_tc_cols, pl->d_tc_rings, pl->d_tc_items[0], pl->d_tc_items[1], pl->d_tc_items[2], pl->d_goff, pl->d_G, pl->d_pole_scratch, pl->d_direct_items, pl->d_tw3, pl->d_tw16, pl->d_fft3_jobs[0][0], pl->d_fft3_jobs[0][1], pl->d_fft3_jobs[0][2], pl->d_fft3_jobs[0][3],
+                    pl->d_cap_chunks, pl->d_cap_chunk_items, pl->d_tc_chunks, pl->d_tc_tiles, pl->d_tc_cols, pl->d_tc_rings, pl->d_tc_items[0], pl->d_tc_items[1], pl->d_tc_items[2], pl->d_goff, pl->d_G, pl->d_pole_scratch, pl->d_nyq, pl->d_direct_items, pl->d_tw3, pl->d_tw16, pl->d_fft3_jobs[0][0], pl->d_fft3_jobs[0][1], pl->d_fft3_jobs[0][2], pl->d_fft3_jobs[0][3],
                     pl->d_fft3_jobs[1][0], pl->d_fft3_jobs[1][1], pl->d_fft3_jobs[1][2], pl->d_fft3_jobs[1][3]};
     for (void* p : ptrs) if (p) cudaFree(p);
     for (auto& e : pl->ev) if (e) cudaEventDestroy(e);
@@ -1453,7 +1457,7 @@ int arkcos_plan_band_kernels(const arkcos_plan* pl, int* n, const char** names, 
     // launch names: the class-E and cap runs are band_mac_tc_kernel<KIND> when the plan uses the tensor cores
     static const char* kFp32[9] = {"band_mac_general_kernel", "band_mac_pole_kernel", "band_mac_eq_kernel",
                                    "band_mac_uniform_kernel<12,0>", "band_mac_uniform_kernel<20,0>",
-                                   "band_mac_uniform_kernel<32,1>", "band_mac_uniform_kernel<12,1>", "band_mac_capchunk_kernel<4,20,0>",
+                                   "band_mac_uniform_kernel<32,1>", "band_mac_uniform_kernel<12,1> + band_nyquist_eq_kernel", "band_mac_capchunk_kernel<4,20,0>",
                                    "band_mac_capchunk_kernel<4,20,1>"};
     if (!pl || !n) return fail(ARKCOS_INVALID_ARG, "NULL argument");
     const char* kNames[9];
@@ -1534,6 +1538,7 @@ int arkcos_plan_launches_per_convolve(const arkcos_plan* pl)
     n += (pl->nitems[0] > 0) + (pl->pole_warp_per_mode ? 2 : 1) * (pl->npole > 0) + (pl->neqchunks > 0);
     for (int c = 1; c < kBandClasses; ++c) n += pl->nitems[c] > 0 ? 1 : 0;
     n += pl->ndirect > 0 ? 1 : 0;
+    n += pl->nnyq > 0 ? 1 : 0;
     n += (pl->ncapsingle > 0 ? 1 : 0) + (pl->ncapitems > pl->ncapsingle ? 1 : 0);
     return n;
 }

@@ -79,6 +79,8 @@ struct arkcos_plan {
     int ntc_items[3] = {0, 0, 0};
     int tc_blocks_per_sm = 0;
     int* d_pole = nullptr;
+    int* d_nyq = nullptr;             // class-E rings whose Nyquist bin band_nyquist_eq_kernel writes
+    int nnyq = 0;
     void* d_pole_scratch = nullptr;   // cx<T>[max_nmaps][npole][2][pole_mh + 1]: unfolded spectra between the two pole launches
     int npole = 0, pole_mh = 0, general_split = 1;
     bool pole_warp_per_mode = false;

@@ -212,6 +212,28 @@ def test_hard_edged_kernels_vs_scheme_oracle():
         assert frms(take_rings(geom, out, eq), ref1) <= 1e-6
 
 
+@pytest.mark.parametrize("pix", [("healpix", 32), ("ecp", 48, 128)], ids=["healpix32", "ecp48x128"])
+def test_input_in_the_nyquist_bin_of_full_length_rings(pix):
+    """Every ring carries (-1)^k times a ring amplitude: on rings of the full length that is the m = N/2 mode alone, so the
+    equatorial (class-E) output rings are made by the Nyquist bin of the band step and nothing else (half weight for the two
+    folded families, sine part on HEALPix's shifted rings).  Hard-edged kernel: G_ij[N/2] is far from zero."""
+    geom = geom_of(pix)
+    pixsz = np.sqrt(4 * np.pi / geom.npix)
+    tmax = 5.8 * pixsz
+    tab = inputs.tophat_table(tmax)
+    amp = np.random.default_rng(17).standard_normal((2, geom.nrings))
+    x = np.zeros((2, geom.npix), np.float32)
+    for i in range(geom.nrings):
+        x[:, geom.ring_slice(i)] = amp[:, i, None] * (1.0 - 2.0 * (np.arange(geom.n[i]) & 1))[None, :]
+    out, _ = gpu_convolve(pix, tab, tmax, x, arkcos.F32)
+    nfull = geom.n.max()
+    eq = np.array([i for i in range(geom.nrings) if np.all(geom.n[geometry.band(geom, i, tmax)] == nfull)])
+    assert eq.size >= geom.nrings // 4
+    ref1 = direct.direct_sum(geom, tab, tmax, x.astype(np.float64), out_rings=eq)
+    assert np.abs(ref1).max() > 1e-3 * np.abs(amp).max() * tab.max() * pixsz ** 2          # the test is not vacuous
+    assert frms(take_rings(geom, out, eq), ref1) <= 1e-6
+
+
 @pytest.mark.parametrize("dtype,nmaps", [(arkcos.F32, 3), (arkcos.F32, 1), (arkcos.F64, 9)])
 def test_exact_caps_hard_edged_kernels(dtype, nmaps):
     """exact_caps = 1: cap-zone rings by the direct-space sum: the WHOLE map equals the
