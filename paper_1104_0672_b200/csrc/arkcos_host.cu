@@ -929,15 +929,18 @@ template <class T> int enqueue_convolve(const arkcos_plan* pl, const void* d_in,
     launch_ring_ffts<T, false>(pl, d_in, d_out, nmaps, st);
     if (pl->ndirect > 0) {                      // exact_caps: overwrite the cap-zone rings with the direct-space sum
         const double sh = sin(0.5 * pl->theta_max), xmax = 4.0 * sh * sh;
-        auto launch = [&](auto nm_tag, int chunks) {
+        auto launch = [&](auto nm_tag) {
             constexpr int NM = decltype(nm_tag)::value;
-            direct_rings_kernel<T, NM><<<dim3((unsigned)pl->ndirect, (unsigned)chunks), kDirectThreads, 0, st>>>(
-                pl->d_direct_items, pl->d_north, pl->d_pairs, pl->d_rings, g.R, pl->d_table, pl->ntab, pl->theta_max, xmax,
+            direct_rings_kernel<T, NM, 4><<<dim3((unsigned)pl->ndirect, (unsigned)((nmaps + NM - 1) / NM)), kDirectThreads, DirectCfg<T, NM>::smem, st>>>(
+                pl->d_direct_items, pl->d_north, pl->d_pairs, pl->d_rings, g.R, (const double2*)pl->d_table2, pl->ntab, pl->theta_max, xmax,
                 (const T*)d_in, (T*)d_out, g.npix, nmaps);
         };
-        if (nmaps >= 8) launch(std::integral_constant<int, 16>{}, (nmaps + 15) / 16);
-        else if (nmaps >= 2) launch(std::integral_constant<int, 4>{}, (nmaps + 3) / 4);
-        else launch(std::integral_constant<int, 1>{}, 1);
+        // a thread holds 8 accumulators per map (four quadrants, two hemispheres)
+        constexpr int kMaxNM = sizeof(T) == 4 ? 8 : 4;
+        if (nmaps >= 5 && kMaxNM >= 8) launch(std::integral_constant<int, kMaxNM>{});
+        else if (nmaps >= 3) launch(std::integral_constant<int, 4>{});
+        else if (nmaps == 2) launch(std::integral_constant<int, 2>{});
+        else launch(std::integral_constant<int, 1>{});
     }
     if (tm) cudaEventRecord(pl->ev[4], st);
     CUDA_TRY(cudaGetLastError());
@@ -1095,10 +1098,24 @@ static int plan_create_impl(arkcos_plan** out, const arkcos_pixelization* pix, c
         std::vector<BandItem> items;
         for (int i = 0; i < (g.R + 1) / 2; ++i) {
             if (!g.direct[i]) continue;
-            for (int k0 = 0; k0 < g.n[i]; k0 += kDirectThreads) items.push_back(BandItem{i, k0});
+            if (g.n[i] % 4 != 0) return fail(ARKCOS_UNSUPPORTED, "exact_caps needs rings of a multiple of four pixels");
+            for (int k0 = 0; k0 < g.n[i] / 4; k0 += kDirectThreads) items.push_back(BandItem{i, k0});     // first quadrant
         }
         pl->ndirect = (int)items.size();
         if (int rc = upload(&pl->d_direct_items, items, wsb)) return rc;
+        // profile table as (K[t], K[t+1] - K[t]): one 16-byte load per interpolation
+        std::vector<double> tab2(2 * (size_t)(kernel->n - 1));
+        for (int tt = 0; tt + 1 < kernel->n; ++tt) {
+            tab2[2 * (size_t)tt] = kernel->table[tt];
+            tab2[2 * (size_t)tt + 1] = kernel->table[tt + 1] - kernel->table[tt];
+        }
+        if (int rc = upload(&pl->d_table2, tab2, wsb)) return rc;
+        // the instantiations that stage input windows use more than 48 KB of dynamic shared memory
+        if (dtype == ARKCOS_F32) {
+            CUDA_TRY(cudaFuncSetAttribute(direct_rings_kernel<float, 8, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)DirectCfg<float, 8>::smem));
+            CUDA_TRY(cudaFuncSetAttribute(direct_rings_kernel<float, 4, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)DirectCfg<float, 4>::smem));
+        } else
+            CUDA_TRY(cudaFuncSetAttribute(direct_rings_kernel<double, 4, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)DirectCfg<double, 4>::smem));
     }
     if (pl->use_tc) {
         if (int rc = upload(&pl->d_tc_chunks, t.tc_chunks, wsb)) return rc;
@@ -1387,7 +1404,7 @@ int arkcos_plan_destroy(arkcos_plan* pl)
     }
     for (cudaStream_t q : {pl->s_h2d, pl->s_comp, pl->s_d2h}) if (q) cudaStreamDestroy(q);
     void* ptrs[] = {pl->d_rings, pl->d_lens, pl->d_pairs, pl->d_north, pl->d_items[0], pl->d_items[1], pl->d_items[2], pl->d_items[3],
-                    pl->d_items[4], pl->d_items[5], pl->d_eqchunks, pl->d_pole, pl->d_chirp, pl->d_phase, pl->d_fft_order[0], pl->d_fft_order[1], pl->d_table, pl->d_tw, pl->d_filt,
+                    pl->d_items[4], pl->d_items[5], pl->d_eqchunks, pl->d_pole, pl->d_chirp, pl->d_phase, pl->d_fft_order[0], pl->d_fft_order[1], pl->d_table, pl->d_table2, pl->d_tw, pl->d_filt,
                     pl->d_W, pl->d_specIn, pl->d_specOut, pl->d_stage_in, pl->d_stage_out,
                     pl->d_cap_chunks, pl->d_cap_chunk_items, pl->d_tc_chunks, pl->d_tc_tiles, pl->d_tc_cols, pl->d_tc_rings, pl->d_tc_items[0], pl->d_tc_items[1], pl->d_tc_items[2], pl->d_goff, pl->d_G, pl->d_pole_scratch, pl->d_nyq, pl->d_direct_items, pl->d_tw3, pl->d_tw16, pl->d_fft3_jobs[0][0], pl->d_fft3_jobs[0][1], pl->d_fft3_jobs[0][2], pl->d_fft3_jobs[0][3],
                     pl->d_fft3_jobs[1][0], pl->d_fft3_jobs[1][1], pl->d_fft3_jobs[1][2], pl->d_fft3_jobs[1][3]};
