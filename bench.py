@@ -172,7 +172,7 @@ def run_ours(args):
         x = np.stack([inputs.white_noise(npix, args.cfg, k) for k in mine])
     dtype = arkcos.F32
     t0 = time.perf_counter()
-    plan = arkcos.Plan(c["pix"], tab, c["theta_max"], dtype, max_nmaps=nmaps)
+    plan = arkcos.Plan(c["pix"], tab, c["theta_max"], dtype, max_nmaps=nmaps, exact_caps=int(args.exact_caps))
     torch.cuda.synchronize()
     plan_s = time.perf_counter() - t0
     stats = plan.stats()
@@ -460,6 +460,7 @@ def main():
     ap.add_argument("--cfg", type=int, default=4)
     ap.add_argument("--profile", action="store_true", help="warm-up + steps of arkcos_convolve only (the command ncu wraps)")
     ap.add_argument("--cfg5-kernel", type=int, default=1, help="--cfg 5: 0 = top-hat disc, 1 = cut Mexican hat")
+    ap.add_argument("--exact-caps", action="store_true", help="plan with options.exact_caps = 1 (with --profile / --quick: the direct-space kernel)")
     ap.add_argument("--no-extras", action="store_true", help="skip the multi-kernel and config-5 blocks")
     ap.add_argument("--quick", action="store_true", help="device-resident timing of the step, its stages and band kernels only")
     ap.add_argument("--oracle-rings", type=int, default=2048, help="output rings in the CPU-oracle sample")

@@ -78,13 +78,19 @@ template <class T> __device__ __forceinline__ cx<T> ext_mode(const cx<T>* __rest
 // the band (the sums meet by warp shuffles), cosines by rotation re-seeded every RESEED samples.  grid = (items, nmaps);
 // an item is a ring and a first mode, kBandThreads / kGeneralSplit modes per block.  The plan picks kGeneralSplit = 4 when
 // the kernel has too few blocks to fill the device (it is latency-bound then), 1 otherwise (coalesced coefficient loads).
+constexpr int kBandThreads = 128;
+constexpr int kGeneralPack = 6;              // items per block of the four-threads-per-mode form
 template <class T, int RESEED, int kGeneralSplit>
-__global__ void band_mac_general_kernel(const BandItem* __restrict__ items, const NorthRec* __restrict__ north,
+__global__ void __launch_bounds__(kBandThreads * kGeneralPack) band_mac_general_kernel(const BandItem* __restrict__ items, int nitems, const NorthRec* __restrict__ north,
                                         const PairRec* __restrict__ pairs, const T* __restrict__ W,
                                         const RingRec* __restrict__ rings, int R, const cx<T>* __restrict__ specIn,
                                         cx<T>* __restrict__ specOut, int64_t spec_stride, int variant_a)
 {
-    const BandItem it = items[blockIdx.x];
+    // blockDim.y items per block (whole warps each: the shuffles stay inside an item): few large blocks keep this
+    // latency-bound kernel on few SMs instead of a small block on every SM
+    const int item = (int)blockIdx.x * (int)blockDim.y + (int)threadIdx.y;
+    if (item >= nitems) return;
+    const BandItem it = items[item];
     const int i = it.ring, iS = R - 1 - i;
     const RingRec ri = rings[i];
     const int slice = (int)threadIdx.x % kGeneralSplit;
@@ -93,6 +99,9 @@ __global__ void band_mac_general_kernel(const BandItem* __restrict__ items, cons
     const int mp = live ? mp_raw : 0;                           // idle threads follow along (the shuffles need whole warps)
     const cx<T>* __restrict__ in = specIn + (int64_t)blockIdx.y * spec_stride;
     cx<T> accN = mk<T>(0, 0), accS = mk<T>(0, 0);
+    int memo_M[2] = {-1, -1}, memo_par[2] = {-1, -1};
+    cx<T> memo_rot[2], memo_seed[2];
+    memo_rot[0] = memo_rot[1] = memo_seed[0] = memo_seed[1] = mk<T>(0, 0);
     const NorthRec nr = north[i];
     // the records of the next pair travel while this one is worked on (pair record -> ring records -> coefficients is a
     // chain of dependent loads; the kernel is latency-bound)
@@ -110,16 +119,31 @@ __global__ void band_mac_general_kernel(const BandItem* __restrict__ items, cons
         const cx<T>* __restrict__ bS = in + rjS.spec_off;
         const T* __restrict__ w = W + pr.woff;
         const int M = pr.M, Mh = M >> 1;
+#pragma unroll
         for (int fam = 0; fam < 2; ++fam) {
             int wi = fam;
             for (int m = fam ? Ni - mp : mp; m <= Mh; m += Ni, ++wi) {
                 // G_ij[m] = sum_t w[t] cos(m (2t + par) pi / M)
-                const cx<T> rot = cispi_ratio<T>((uint32_t)((2u * (uint32_t)m) % (2u * (uint32_t)M)), (uint32_t)M);
+                // the step exp(2 pi i m / M) and the first seed exp(i pi m par / M) depend on (m, M, par) only and the pairs of a
+                // ring share one or two grids M: kept from the previous pair when they repeat (first term of each family)
+                const bool first = wi == fam;
+                cx<T> rot;
+                if (first && memo_M[fam] == M) rot = memo_rot[fam];
+                else {
+                    rot = cispi_ratio<T>((uint32_t)((2u * (uint32_t)m) % (2u * (uint32_t)M)), (uint32_t)M);
+                    if (first) { memo_M[fam] = M; memo_rot[fam] = rot; memo_par[fam] = -1; }
+                }
                 T G = 0;
                 for (int t0 = 0; t0 < pr.cnt; t0 += RESEED) {
                     // m <= M/2 < 2^15 and 2 t0 + par < 2 M <= 2^17: the product fits 32 bits
-                    const uint32_t q = ((uint32_t)m * (uint32_t)(2 * t0 + pr.par)) % (2u * (uint32_t)M);
-                    cx<T> c = cispi_ratio<T>((uint32_t)q, (uint32_t)M);
+                    cx<T> c;
+                    if (t0 == 0 && pr.par == 0) c = mk<T>((T)1, (T)0);
+                    else if (t0 == 0 && first && memo_par[fam] == 1) c = memo_seed[fam];
+                    else {
+                        const uint32_t q = ((uint32_t)m * (uint32_t)(2 * t0 + pr.par)) % (2u * (uint32_t)M);
+                        c = cispi_ratio<T>((uint32_t)q, (uint32_t)M);
+                        if (t0 == 0 && first) { memo_par[fam] = 1; memo_seed[fam] = c; }
+                    }
                     const int t1 = min(pr.cnt, t0 + RESEED);
                     for (int t = t0; t < t1; ++t) {
                         G += w[t] * c.x;
@@ -161,7 +185,6 @@ namespace arkcos {
 // One thread per folded output mode m'.  For each unfolded mode m that folds onto m' the thread builds the cosines
 // cos(m u pi / M) of the row-sample positions ONCE in registers (rotation, re-seeded every 8 steps from an exact
 // sincospi) and reuses them for all input rings of the band; the rows and the per-pair records sit in shared memory.
-constexpr int kBandThreads = 128;
 constexpr int kMaxPairs = 64;
 constexpr int kBandClasses = 6;   // 0: general kernel; 1..4: band_mac_uniform_kernel<12,odd>, <12>, <20>, <32,odd>; 5: band_mac_capchunk_kernel (cap rings in the single-period regime)
 

@@ -882,25 +882,27 @@ template <class T> int enqueue_convolve(const arkcos_plan* pl, const void* d_in,
     // the band kernels of the different ring classes write disjoint rings: fork them onto the plan's side streams
     // (timing mode 2: one after the other on the caller's stream with an event between them)
     const bool serial = pl->timing == 2;
-    // The big launches (tensor-core / run kernels) go first: each of their blocks takes a whole SM, and a small latency-bound
-    // kernel that got there before them would hold every SM for its whole duration; issued behind them the small ones run in
-    // the gaps of the big launches' last waves.
+    // The small latency-bound kernels (general, pole, uniform classes: 25-45 us each whatever the device gives them) are issued
+    // first, the big launches (tensor-core / run kernels, a whole SM per block) behind them: the big blocks take the SMs the
+    // small kernels leave free and the others as they drain.  (Issued last, the small kernels only start in the big launches'
+    // last wave and the stage ends 15 us later; measured both ways, profiles/r2_final.md.)
     cudaStream_t s0 = serial ? st : pl->side[1], sp = serial ? st : pl->side[5];
     if (!serial) {
         cudaEventRecord(pl->ev_fork, st);
         for (int k = 0; k < 6; ++k) cudaStreamWaitEvent(pl->side[k], pl->ev_fork, 0);
-        launch_uniform(pl, nmaps, st, false, 1);
     }
     if (serial) cudaEventRecord(pl->ev_band[0], st);
     if (pl->nitems[0] > 0) {
-        const dim3 gg((unsigned)pl->nitems[0], (unsigned)nmaps);
+        // the four-threads-per-mode form is latency-bound: six items per block (fewer, larger blocks)
+        const int pk = pl->general_split == 4 ? kGeneralPack : 1;
+        const dim3 gg((unsigned)((pl->nitems[0] + pk - 1) / pk), (unsigned)nmaps), bb((unsigned)kBandThreads, (unsigned)pk);
         if (pl->general_split == 4)
-            band_mac_general_kernel<T, 16, 4><<<gg, kBandThreads, 0, s0>>>(
-                pl->d_items[0], pl->d_north, pl->d_pairs, (const T*)pl->d_W, pl->d_rings, g.R, (const cx<T>*)pl->spec_in(),
+            band_mac_general_kernel<T, 16, 4><<<gg, bb, 0, s0>>>(
+                pl->d_items[0], pl->nitems[0], pl->d_north, pl->d_pairs, (const T*)pl->d_W, pl->d_rings, g.R, (const cx<T>*)pl->spec_in(),
                 (cx<T>*)pl->d_specOut, g.spec_total, pl->opt.variant == 1 ? 1 : 0);
         else
-            band_mac_general_kernel<T, 16, 1><<<gg, kBandThreads, 0, s0>>>(
-                pl->d_items[0], pl->d_north, pl->d_pairs, (const T*)pl->d_W, pl->d_rings, g.R, (const cx<T>*)pl->spec_in(),
+            band_mac_general_kernel<T, 16, 1><<<gg, bb, 0, s0>>>(
+                pl->d_items[0], pl->nitems[0], pl->d_north, pl->d_pairs, (const T*)pl->d_W, pl->d_rings, g.R, (const cx<T>*)pl->spec_in(),
                 (cx<T>*)pl->d_specOut, g.spec_total, pl->opt.variant == 1 ? 1 : 0);
     }
     if (serial) cudaEventRecord(pl->ev_band[1], st);
@@ -920,6 +922,7 @@ template <class T> int enqueue_convolve(const arkcos_plan* pl, const void* d_in,
     }
     if (serial) cudaEventRecord(pl->ev_band[2], st);
     launch_uniform(pl, nmaps, st, serial, serial ? 3 : 2);
+    if (!serial) launch_uniform(pl, nmaps, st, false, 1);
     if (!serial)
         for (int k = 0; k < 6; ++k) {
             cudaEventRecord(pl->ev_join[k], pl->side[k]);
