@@ -800,23 +800,8 @@ void launch_ring_ffts(const arkcos_plan* pl, const void* d_in, void* d_out, int 
 {
     const HostGeometry& g = pl->g;
     bool forked = false;
-    if constexpr (sizeof(T) == 4) {
-        const int dir = FWD ? 0 : 1;
-        const int nside_launches = (pl->nfft3[dir][2] > 0) + (pl->nfft3[dir][1] + pl->nfft3[dir][0] > 0) + (pl->nfft_old[dir] > 0);
-        forked = pl->nfft3[dir][3] > 0 && nside_launches > 0 && pl->timing != 2;
-        if (forked) {
-            cudaEventRecord(pl->ev_fork, st);
-            for (int k = 0; k < 3; ++k) cudaStreamWaitEvent(pl->side[k], pl->ev_fork, 0);
-        }
-        launch_fft3<12, FWD>(pl, d_in, d_out, nmaps, st);
-        launch_fft3<11, FWD>(pl, d_in, d_out, nmaps, forked ? pl->side[0] : st);
-        launch_fft3<10, FWD>(pl, d_in, d_out, nmaps, forked ? pl->side[1] : st);
-        launch_fft3<9, FWD>(pl, d_in, d_out, nmaps, forked ? pl->side[1] : st);
-    } else if (pl->timing == 2)
-        for (int k = 0; k < 8; ++k) cudaEventRecord(pl->ev_fft[FWD ? 0 : 1][k], st);
-    if (pl->timing == 2) cudaEventRecord(pl->ev_fft[FWD ? 0 : 1][8], st);
-    if (pl->nfft_old[FWD ? 0 : 1] > 0) {
-        cudaStream_t so = forked ? pl->side[2] : st;
+    auto launch_old = [&](cudaStream_t so) {            // the shared-memory kernel: very short or very long rings, fp64 plans
+        if (pl->nfft_old[FWD ? 0 : 1] == 0) return;
         const dim3 gfft((unsigned)pl->nfft_old[FWD ? 0 : 1], (unsigned)nmaps);
         if (FWD) {
             if (pl->fft_bpt == 2)
@@ -837,7 +822,32 @@ void launch_ring_ffts(const arkcos_plan* pl, const void* d_in, void* d_out, int 
                     (const cx<T>*)pl->d_specOut, g.spec_total, (T*)d_out, g.npix, pl->d_rings, pl->d_fft_order[FWD ? 0 : 1], pl->d_lens,
                     (const cx<T>*)pl->d_tw, pl->logPT, (const cx<T>*)pl->d_filt, (const cx<T>*)pl->d_chirp, (const cx<T>*)pl->d_phase);
         }
-    }
+    };
+    if constexpr (sizeof(T) == 4) {
+        const int dir = FWD ? 0 : 1;
+        const int nside_launches = (pl->nfft3[dir][2] > 0) + (pl->nfft3[dir][1] + pl->nfft3[dir][0] > 0) + (pl->nfft_old[dir] > 0);
+        forked = pl->nfft3[dir][3] > 0 && nside_launches > 0 && pl->timing != 2;
+        if (forked) {
+            cudaEventRecord(pl->ev_fork, st);
+            for (int k = 0; k < 3; ++k) cudaStreamWaitEvent(pl->side[k], pl->ev_fork, 0);
+        }
+        if (forked) {
+            // the small size classes first (single-wave, latency-bound launches): the blocks of the big launches then fill the
+            // SMs around them; issued behind the big launches they would only start in their last wave (-10 us per call)
+            launch_fft3<9, FWD>(pl, d_in, d_out, nmaps, pl->side[1]);
+            launch_fft3<10, FWD>(pl, d_in, d_out, nmaps, pl->side[1]);
+            launch_fft3<11, FWD>(pl, d_in, d_out, nmaps, pl->side[0]);
+            launch_fft3<12, FWD>(pl, d_in, d_out, nmaps, st);
+        } else {                                      // one stream (timing mode 2: in the order of the event slots)
+            launch_fft3<12, FWD>(pl, d_in, d_out, nmaps, st);
+            launch_fft3<11, FWD>(pl, d_in, d_out, nmaps, st);
+            launch_fft3<10, FWD>(pl, d_in, d_out, nmaps, st);
+            launch_fft3<9, FWD>(pl, d_in, d_out, nmaps, st);
+        }
+    } else if (pl->timing == 2)
+        for (int k = 0; k < 8; ++k) cudaEventRecord(pl->ev_fft[FWD ? 0 : 1][k], st);
+    if (pl->timing == 2) cudaEventRecord(pl->ev_fft[FWD ? 0 : 1][8], st);
+    launch_old(forked ? pl->side[2] : st);
     if (pl->timing == 2) cudaEventRecord(pl->ev_fft[FWD ? 0 : 1][9], st);
     if (forked)
         for (int k = 0; k < 3; ++k) {
