@@ -256,6 +256,34 @@ def test_exact_caps_hard_edged_kernels(dtype, nmaps):
         assert frms(plain, ref1) > 1e-5            # without the option the caps carry the scheme's artifact level
 
 
+@pytest.mark.parametrize("dtype,nmaps", [(arkcos.F64, 3), (arkcos.F32, 5), (arkcos.F32, 2)])
+def test_exact_caps_wide_kernel_long_windows(dtype, nmaps):
+    """exact_caps with a kernel 100 pixels wide (Eq. 6): the input windows of a thread block are longer than the
+    direct-space kernel stages in shared memory (its global-memory path), a ring has more ring pairs than one staging pass of
+    the pair constants holds, whole-ring windows of up to 400 pixels next to the poles (the rotation along the ring runs
+    that long), and the two-map form.  Sampled rings against the brute-force sum."""
+    nside = 256
+    geom = geometry.healpix_ring(nside)
+    tmax = 0.32
+    tab = inputs.gaussian_table(0.25, tmax)
+    x = inputs.white_noise_maps(geom.npix, 7, nmaps)
+    if dtype == arkcos.F64:
+        x = x.astype(np.float64)
+    out, plan = gpu_convolve(("healpix", nside), tab, tmax, x, dtype, exact_caps=1)
+    assert np.isfinite(out).all()
+    R = geom.nrings
+    rings = np.array([0, 1, 5, 50, 99, 120, 200, 255, 256, 300, R - 1 - 301, R - 1 - 120, R - 1 - 50, R - 1])
+    ref1 = direct.direct_sum(geom, tab, tmax, x.astype(np.float64), out_rings=rings)
+    got = take_rings(geom, out, rings)
+    if dtype == arkcos.F64:
+        assert maxrel(got, ref1) <= 1e-12
+    else:
+        # 2e4 input pixels per output pixel summed in fp32: the bound of north_star for HEALPix, not the 1e-6 of compact kernels
+        err = frms(got, ref1)
+        print(f"\nwide kernel, fp32, {nmaps} maps: fractional RMS vs brute force = {err:.2e}")
+        assert err <= 1e-5
+
+
 # ------------------------------------------------------------------ config 3: HEALPix nside 512 --------------------
 
 def test_cfg3_fp32_sampled_rings():
