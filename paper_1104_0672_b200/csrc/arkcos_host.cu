@@ -683,6 +683,36 @@ void launch_uniform(const arkcos_plan* pl, int nmaps, cudaStream_t st, bool seri
 {
     // every small class on a stream of its own: they are latency-bound, tiny grids
     cudaStream_t s1 = serial ? st : pl->side[2], s2 = serial ? st : pl->side[3], s3 = serial ? st : pl->side[4], sc = serial ? st : pl->side[0];
+    auto launch_cap = [&](auto multi_tag, int first, int count, cudaStream_t sc) {
+        constexpr bool MULTI = decltype(multi_tag)::value;
+        if (count <= 0) return;
+        const unsigned n = (unsigned)count;
+        const CapChunkItem* items = pl->d_cap_chunk_items + first;
+        if (pl->d_G && nmaps >= 4)
+            band_mac_capchunk_cached_kernel<4, 4, MULTI, 1><<<dim3(n, (unsigned)((nmaps + 3) / 4)), 256, 0, sc>>>(
+                items, pl->d_cap_chunks, pl->d_north, pl->d_pairs, pl->d_goff, pl->d_G, pl->d_rings, pl->g.R,
+                (const cx<float>*)pl->spec_in(), (cx<float>*)pl->d_specOut, pl->g.spec_total, nmaps);
+        else if (pl->d_G && nmaps > 1)
+            band_mac_capchunk_cached_kernel<4, 2, MULTI, 2><<<dim3(n, (unsigned)((nmaps + 1) / 2)), kBandThreads, 0, sc>>>(
+                items, pl->d_cap_chunks, pl->d_north, pl->d_pairs, pl->d_goff, pl->d_G, pl->d_rings, pl->g.R,
+                (const cx<float>*)pl->spec_in(), (cx<float>*)pl->d_specOut, pl->g.spec_total, nmaps);
+        else if (pl->d_G)
+            band_mac_capchunk_cached_kernel<4, 1, MULTI, 2><<<dim3(n, 1), kBandThreads, 0, sc>>>(
+                items, pl->d_cap_chunks, pl->d_north, pl->d_pairs, pl->d_goff, pl->d_G, pl->d_rings, pl->g.R,
+                (const cx<float>*)pl->spec_in(), (cx<float>*)pl->d_specOut, pl->g.spec_total, nmaps);
+        else if (pl->use_tc) {
+            if (pl->ntc_items[MULTI ? 2 : 1] > 0)
+                tc_launch(pl->tc_cfg, MULTI ? 3 : 2, (unsigned)pl->ntc_items[MULTI ? 2 : 1], (unsigned)nmaps, sc, pl->d_tc_items[MULTI ? 2 : 1],
+                          pl->d_tc_chunks, pl->d_tc_tiles, pl->d_tc_cols, pl->d_tc_rings, (const float*)pl->d_W, pl->g.R,
+                          (const cx<float>*)pl->spec_in(), (cx<float>*)pl->d_specOut, pl->g.spec_total);
+        } else
+            band_mac_capchunk_kernel<4, 20, MULTI><<<dim3(n, (unsigned)nmaps), kBandThreads, 0, sc>>>(
+                items, pl->d_cap_chunks, pl->d_north, pl->d_pairs, (const float*)pl->d_W, pl->d_rings, pl->g.R,
+                (const cx<float>*)pl->spec_in(), (cx<float>*)pl->d_specOut, pl->g.spec_total);
+    };
+    // the runs whose grids span several periods are few blocks (fewer than SMs): on a stream of their own and ahead of the
+    // launches that fill the device; behind the single-period runs on one stream they ran alone on a quarter of the SMs
+    if (!serial && (which & 1) && pl->ncapitems > 0) launch_cap(std::true_type{}, pl->ncapsingle, pl->ncapitems - pl->ncapsingle, pl->side[6]);
     if (!(which & 1)) {
     } else if (pl->neqchunks > 0 && pl->d_G) {
         const unsigned gx = (unsigned)((pl->eq_mh + 255) / 256);
@@ -727,36 +757,11 @@ void launch_uniform(const arkcos_plan* pl, int nmaps, cudaStream_t st, bool seri
             (const cx<float>*)pl->spec_in(), (cx<float>*)pl->d_specOut, pl->g.spec_total);
     if (serial) cudaEventRecord(pl->ev_band[7], st);
     if (pl->ncapitems > 0 && (which & 1)) {
-        auto launch_cap = [&](auto multi_tag, int first, int count) {
-            constexpr bool MULTI = decltype(multi_tag)::value;
-            if (count <= 0) return;
-            const unsigned n = (unsigned)count;
-            const CapChunkItem* items = pl->d_cap_chunk_items + first;
-            if (pl->d_G && nmaps >= 4)
-                band_mac_capchunk_cached_kernel<4, 4, MULTI, 1><<<dim3(n, (unsigned)((nmaps + 3) / 4)), 256, 0, sc>>>(
-                    items, pl->d_cap_chunks, pl->d_north, pl->d_pairs, pl->d_goff, pl->d_G, pl->d_rings, pl->g.R,
-                    (const cx<float>*)pl->spec_in(), (cx<float>*)pl->d_specOut, pl->g.spec_total, nmaps);
-            else if (pl->d_G && nmaps > 1)
-                band_mac_capchunk_cached_kernel<4, 2, MULTI, 2><<<dim3(n, (unsigned)((nmaps + 1) / 2)), kBandThreads, 0, sc>>>(
-                    items, pl->d_cap_chunks, pl->d_north, pl->d_pairs, pl->d_goff, pl->d_G, pl->d_rings, pl->g.R,
-                    (const cx<float>*)pl->spec_in(), (cx<float>*)pl->d_specOut, pl->g.spec_total, nmaps);
-            else if (pl->d_G)
-                band_mac_capchunk_cached_kernel<4, 1, MULTI, 2><<<dim3(n, 1), kBandThreads, 0, sc>>>(
-                    items, pl->d_cap_chunks, pl->d_north, pl->d_pairs, pl->d_goff, pl->d_G, pl->d_rings, pl->g.R,
-                    (const cx<float>*)pl->spec_in(), (cx<float>*)pl->d_specOut, pl->g.spec_total, nmaps);
-            else if (pl->use_tc) {
-                if (pl->ntc_items[MULTI ? 2 : 1] > 0)
-                    tc_launch(pl->tc_cfg, MULTI ? 3 : 2, (unsigned)pl->ntc_items[MULTI ? 2 : 1], (unsigned)nmaps, sc, pl->d_tc_items[MULTI ? 2 : 1],
-                              pl->d_tc_chunks, pl->d_tc_tiles, pl->d_tc_cols, pl->d_tc_rings, (const float*)pl->d_W, pl->g.R,
-                              (const cx<float>*)pl->spec_in(), (cx<float>*)pl->d_specOut, pl->g.spec_total);
-            } else
-                band_mac_capchunk_kernel<4, 20, MULTI><<<dim3(n, (unsigned)nmaps), kBandThreads, 0, sc>>>(
-                    items, pl->d_cap_chunks, pl->d_north, pl->d_pairs, (const float*)pl->d_W, pl->d_rings, pl->g.R,
-                    (const cx<float>*)pl->spec_in(), (cx<float>*)pl->d_specOut, pl->g.spec_total);
-        };
-        launch_cap(std::false_type{}, 0, pl->ncapsingle);
-        if (serial) cudaEventRecord(pl->ev_band[8], st);
-        launch_cap(std::true_type{}, pl->ncapsingle, pl->ncapitems - pl->ncapsingle);
+        launch_cap(std::false_type{}, 0, pl->ncapsingle, sc);
+        if (serial) {
+            cudaEventRecord(pl->ev_band[8], st);
+            launch_cap(std::true_type{}, pl->ncapsingle, pl->ncapitems - pl->ncapsingle, sc);
+        }
     } else if (serial) cudaEventRecord(pl->ev_band[8], st);
     if (serial) cudaEventRecord(pl->ev_band[9], st);
 }
@@ -899,7 +904,7 @@ template <class T> int enqueue_convolve(const arkcos_plan* pl, const void* d_in,
     cudaStream_t s0 = serial ? st : pl->side[1], sp = serial ? st : pl->side[5];
     if (!serial) {
         cudaEventRecord(pl->ev_fork, st);
-        for (int k = 0; k < 6; ++k) cudaStreamWaitEvent(pl->side[k], pl->ev_fork, 0);
+        for (int k = 0; k < 7; ++k) cudaStreamWaitEvent(pl->side[k], pl->ev_fork, 0);
     }
     if (serial) cudaEventRecord(pl->ev_band[0], st);
     if (pl->nitems[0] > 0) {
@@ -934,7 +939,7 @@ template <class T> int enqueue_convolve(const arkcos_plan* pl, const void* d_in,
     launch_uniform(pl, nmaps, st, serial, serial ? 3 : 2);
     if (!serial) launch_uniform(pl, nmaps, st, false, 1);
     if (!serial)
-        for (int k = 0; k < 6; ++k) {
+        for (int k = 0; k < 7; ++k) {
             cudaEventRecord(pl->ev_join[k], pl->side[k]);
             cudaStreamWaitEvent(st, pl->ev_join[k], 0);
         }

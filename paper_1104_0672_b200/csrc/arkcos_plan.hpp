@@ -126,8 +126,8 @@ struct arkcos_plan {
     mutable cudaEvent_t ev_band[10] = {};
     mutable cudaEvent_t ev_fft[2][10] = {};      // timing mode 2: before each ring-FFT launch of a direction and after the last
     // fork/join of the band kernels of the different ring classes
-    // side streams 0-2: ring-FFT size classes and the big band launches; 0-5: the band kernels of the ring classes
-    cudaStream_t side[6] = {}, side_rows = nullptr;
-    cudaEvent_t ev_fork = nullptr, ev_join[6] = {};
+    // side streams 0-2: ring-FFT size classes and the big band launches; 0-6: the band kernels of the ring classes
+    cudaStream_t side[7] = {}, side_rows = nullptr;
+    cudaEvent_t ev_fork = nullptr, ev_join[7] = {};
     cudaEvent_t ev_rows_fork = nullptr, ev_rows_done = nullptr;   // kernel-row generator beside the forward FFTs
 };
