@@ -90,7 +90,7 @@ typedef struct {
  *  no_tensor_cores   0: float plans run the kernel-row phi-transform of the class-E and cap-ring runs as
  *                       3xTF32 tcgen05 matrix products (FP32-level accuracy); 1: every band kernel
  *                       uses FP32 FMAs only (the round-1 kernels; also what small grids and cached-spectra plans use).
- *  no_cuda_graph     0: arkcos_convolve captures the launches of a call (about 30 kernels on the caller's stream and six plan-owned
+ *  no_cuda_graph     0: arkcos_convolve captures the launches of a call (about 30 kernels on the caller's stream and seven plan-owned
  *                       streams, with their event dependencies) into a CUDA graph the first time it sees a combination of
  *                       (d_in, d_out, nmaps, stream) and replays that graph afterwards (the four most recent combinations are
  *                       kept); not on the NULL / legacy default stream, not while the stream is being captured by the caller
