@@ -43,7 +43,21 @@ int fft3_setup()
     if ((e = set_smem<9>()) != cudaSuccess) return (int)e;
     if ((e = set_smem<10>()) != cudaSuccess) return (int)e;
     if ((e = set_smem<11>()) != cudaSuccess) return (int)e;
-    return (int)set_smem<12>();
+    if ((e = set_smem<12>()) != cudaSuccess) return (int)e;
+    const int full = (int)Fft3<12>::smem_bytes;
+    if ((e = cudaFuncSetAttribute(ring_fft3_direct2_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, full)) != cudaSuccess) return (int)e;
+    return (int)cudaFuncSetAttribute(ring_fft3_direct2_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, full);
+}
+
+void fft3_launch_direct2(bool fwd, const FftJob* jobs, unsigned njobs, unsigned nmaps, cudaStream_t st, const Fft3Args& a)
+{
+    const dim3 grid(njobs, nmaps);
+    if (fwd)
+        ring_fft3_direct2_kernel<true><<<grid, Fft3<12>::T, Fft3<12>::smem_bytes, st>>>(
+            a.in, a.outmap, a.npix, a.spec, a.spec_stride, jobs, a.tw, a.logPT, a.tw16, a.tw3, a.phase);
+    else
+        ring_fft3_direct2_kernel<false><<<grid, Fft3<12>::T, Fft3<12>::smem_bytes, st>>>(
+            a.in, a.outmap, a.npix, a.spec, a.spec_stride, jobs, a.tw, a.logPT, a.tw16, a.tw3, a.phase);
 }
 
 #define ARKCOS_FFT3_DISPATCH(fn, ...)                                       \

@@ -346,3 +346,79 @@ ring_fft3_direct1_kernel(const float* __restrict__ in, float* __restrict__ outma
 }
 
 }  // namespace arkcos
+
+namespace arkcos {
+
+// Power-of-two rings of twice the largest transform size (L = 2 Q = 8192 complex points: the belt of HEALPix nside 4096, ECP
+// rings of 16384 pixels; PAPER.md:231 names nside 4096 as the next size).  One ring per block as TWO size-Q transforms side by
+// side - the even and the odd samples of the packed ring (decimation in time) - and one radix-2 step in registers,
+//     Z[k] = E[k] + w^k O[k],   Z[k + Q] = E[k] - w^k O[k],   w = exp(-2 pi i / 2Q),
+// with the split / packing of the real ring as in the other kernels.  grid = (jobs, nmaps), block = Q/16 threads, job.r0 only.
+template <bool FWD>
+__global__ void __launch_bounds__(Fft3<12>::T, Fft3<12>::MINB)
+ring_fft3_direct2_kernel(const float* __restrict__ in, float* __restrict__ outmap, int64_t npix,
+                         cx<float>* __restrict__ spec, int64_t spec_stride, const FftJob* __restrict__ jobs,
+                         const cx<float>* __restrict__ tw, int logPT, const cx<float>* __restrict__ tw16,
+                         const cx<float>* __restrict__ tw3, const cx<float>* __restrict__ phase)
+{
+    using F = Fft3<12>;
+    constexpr int T = F::T, Q = F::Q, L = 2 * Q;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cx<float>* s = reinterpret_cast<cx<float>*>(smem_raw);
+    const int t = (int)threadIdx.x;
+    const FftJob& job = jobs[blockIdx.x];
+    const RingRec rr = job.r0;
+    const cx<float>* __restrict__ ph = phase + job.f.ph_off;                   // exp(-i pi k / N), k = 0 .. L
+    cx<float>* __restrict__ sp = spec + (int64_t)blockIdx.y * spec_stride + rr.spec_off;
+    const int shW = logPT - 13;                                                // w^k = tw[k << shW]
+    cx<float> u[2][16];
+    if (FWD) {
+        const cx<float>* __restrict__ x0 = reinterpret_cast<const cx<float>*>(in + (int64_t)blockIdx.y * npix + rr.pix_off);
+#pragma unroll
+        for (int r = 0; r < 16; ++r) {
+            const int m = t + T * r;
+            u[0][r] = x0[2 * m];
+            u[1][r] = x0[2 * m + 1];
+        }
+        fft3<12, 2>(u, s, tw, logPT, tw16, tw3);
+#pragma unroll
+        for (int q = 0; q < 16; ++q) {
+            const cx<float> wo = cmul(tw[(t + T * q) << shW], u[1][q]);
+            u[1][q] = u[0][q] - wo;                                            // Z[k + Q]
+            u[0][q] = u[0][q] + wo;                                            // Z[k]
+        }
+        __syncthreads();
+#pragma unroll
+        for (int q = 0; q < 16; ++q) {
+            s[phys(t + T * q)] = u[0][q];
+            s[phys(t + T * q + Q)] = u[1][q];
+        }
+        __syncthreads();
+#pragma unroll
+        for (int q = 0; q < 16; ++q) {
+            const int k = t + T * q;
+            sp[k] = split_fwd(u[0][q], cconj(s[phys(k == 0 ? 0 : L - k)]), ph[k], rr.shifted);
+            sp[k + Q] = split_fwd(u[1][q], cconj(s[phys(Q - k)]), ph[k + Q], rr.shifted);
+        }
+        if (t == 0) sp[L] = split_fwd(u[0][0], cconj(u[0][0]), ph[L], rr.shifted);
+    } else {
+#pragma unroll
+        for (int r = 0; r < 16; ++r) {
+            const int k0 = 2 * (t + T * r), k1 = k0 + 1;
+            const cx<float> h0 = cconj(ph[k0]), h1 = cconj(ph[k1]);            // exp(+i pi k / N); exp(i pi (L-k)/N) = i conj(h)
+            u[0][r] = pack_inv(sp[k0], sp[L - k0], h0, mk<float>(h0.y, h0.x), rr.shifted);
+            u[1][r] = pack_inv(sp[k1], sp[L - k1], h1, mk<float>(h1.y, h1.x), rr.shifted);
+        }
+        fft3<12, 2>(u, s, tw, logPT, tw16, tw3);
+        cx<float>* __restrict__ o0 = reinterpret_cast<cx<float>*>(outmap + (int64_t)blockIdx.y * npix + rr.pix_off);
+#pragma unroll
+        for (int q = 0; q < 16; ++q) {
+            const int k = t + T * q;
+            const cx<float> wo = cmul(tw[k << shW], u[1][q]);
+            o0[k] = cconj(u[0][q] + wo);
+            o0[k + Q] = cconj(u[0][q] - wo);
+        }
+    }
+}
+
+}  // namespace arkcos

@@ -330,7 +330,8 @@ def test_cfg4_full_size_sampled_rings():
 
 
 def test_nside4096_maximum_size_sampled_rings():
-    """The largest HEALPix grid an fp32 plan accepts (ring length 16384: the shared-memory FFT path for the belt)."""
+    """The largest HEALPix grid an fp32 plan accepts (ring length 16384: the belt as two size-4096 transforms per ring, the cap
+    rings longer than 8192 pixels through the shared-memory FFT path)."""
     nside = 4096
     geom = geometry.healpix_ring(nside)
     fwhm, tmax = 2.5 * ARCMIN, 7.5 * ARCMIN
@@ -341,6 +342,21 @@ def test_nside4096_maximum_size_sampled_rings():
     rings = np.array([0, 3, 700, 2047, 2048, 3000, nside - 1, nside, nside + 5, 2 * nside - 1, 3 * nside + 2, geom.nrings - 1])
     ref = direct.direct_sum(geom, tab, tmax, x.astype(np.float64), out_rings=rings)
     assert frms(take_rings(geom, out, rings), ref) <= 1e-5
+
+
+def test_ecp_rings_of_16384_pixels():
+    """ECP rings of 16384 pixels (8192 complex points: two register-resident size-4096 transforms and a radix-2 step per ring,
+    PAPER.md:125 / 142 for the ring transforms): every pair is exact on ECP, so the fp32 bound of 1e-6 applies."""
+    pix = ("ecp", 24, 16384)
+    geom = geom_of(pix)
+    tmax = 0.15                         # neighbouring rings are 0.13 apart: bands of three rings, rows of up to 800 samples
+    tab = inputs.gaussian_table(0.1, tmax)
+    x = inputs.white_noise_maps(geom.npix, 8, 2)
+    out, plan = gpu_convolve(pix, tab, tmax, x)
+    assert np.isfinite(out).all()
+    rings = np.array([0, 1, 7, 11, 12, 16, 23])
+    ref = direct.direct_sum(geom, tab, tmax, x.astype(np.float64), out_rings=rings)
+    assert frms(take_rings(geom, out, rings), ref) <= 1e-6
 
 
 # ------------------------------------------------------------------ API behaviour -----------------------------------
