@@ -46,7 +46,20 @@ int fft3_setup()
     if ((e = set_smem<12>()) != cudaSuccess) return (int)e;
     const int full = (int)Fft3<12>::smem_bytes;
     if ((e = cudaFuncSetAttribute(ring_fft3_direct2_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, full)) != cudaSuccess) return (int)e;
-    return (int)cudaFuncSetAttribute(ring_fft3_direct2_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, full);
+    if ((e = cudaFuncSetAttribute(ring_fft3_direct2_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, full)) != cudaSuccess) return (int)e;
+    if ((e = cudaFuncSetAttribute(ring_fft3_bluestein2_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, full)) != cudaSuccess) return (int)e;
+    return (int)cudaFuncSetAttribute(ring_fft3_bluestein2_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, full);
+}
+
+void fft3_launch_bluestein2(bool fwd, const FftJob* jobs, unsigned njobs, unsigned nmaps, cudaStream_t st, const Fft3Args& a)
+{
+    const dim3 grid(njobs, nmaps);
+    if (fwd)
+        ring_fft3_bluestein2_kernel<true><<<grid, Fft3<12>::T, Fft3<12>::smem_bytes, st>>>(
+            a.in, a.outmap, a.npix, a.spec, a.spec_stride, jobs, a.tw, a.logPT, a.tw16, a.tw3, a.filt, a.chirp, a.phase);
+    else
+        ring_fft3_bluestein2_kernel<false><<<grid, Fft3<12>::T, Fft3<12>::smem_bytes, st>>>(
+            a.in, a.outmap, a.npix, a.spec, a.spec_stride, jobs, a.tw, a.logPT, a.tw16, a.tw3, a.filt, a.chirp, a.phase);
 }
 
 void fft3_launch_direct2(bool fwd, const FftJob* jobs, unsigned njobs, unsigned nmaps, cudaStream_t st, const Fft3Args& a)

@@ -422,3 +422,169 @@ ring_fft3_direct2_kernel(const float* __restrict__ in, float* __restrict__ outma
 }
 
 }  // namespace arkcos
+
+namespace arkcos {
+
+// Size-8192 transforms of one sequence held as u[0][.] / u[1][.] by 256 threads, built from two size-4096 transforms side by
+// side.  Two layouts: "blocked" u[0][q] = x[k], u[1][q] = x[k + Q], k = t + T q, and "interleaved" u[0][r] = x[2m],
+// u[1][r] = x[2m + 1], m = t + T r.  Decimation in time takes interleaved input to blocked output, decimation in frequency
+// blocked input to interleaved output, so a transform pair (forward, pointwise product, forward again) needs no reordering.
+// Entry: earlier readers of s have passed a barrier.  w = exp(-2 pi i / 8192) = tw[1 << shW].
+__device__ __forceinline__ void fft8192_dit(cx<float> (&u)[2][16], cx<float>* __restrict__ s, const cx<float>* __restrict__ tw,
+                                            int logPT, const cx<float>* __restrict__ tw16, const cx<float>* __restrict__ tw3)
+{
+    constexpr int T = Fft3<12>::T;
+    const int t = (int)threadIdx.x, shW = logPT - 13;
+    fft3<12, 2>(u, s, tw, logPT, tw16, tw3);
+#pragma unroll
+    for (int q = 0; q < 16; ++q) {
+        const cx<float> wo = cmul(tw[(t + T * q) << shW], u[1][q]);
+        u[1][q] = u[0][q] - wo;
+        u[0][q] = u[0][q] + wo;
+    }
+}
+__device__ __forceinline__ void fft8192_dif(cx<float> (&u)[2][16], cx<float>* __restrict__ s, const cx<float>* __restrict__ tw,
+                                            int logPT, const cx<float>* __restrict__ tw16, const cx<float>* __restrict__ tw3)
+{
+    constexpr int T = Fft3<12>::T;
+    const int t = (int)threadIdx.x, shW = logPT - 13;
+#pragma unroll
+    for (int q = 0; q < 16; ++q) {
+        const cx<float> a = u[0][q], b = u[1][q];
+        u[0][q] = a + b;
+        u[1][q] = cmul(a - b, tw[(t + T * q) << shW]);
+    }
+    fft3<12, 2>(u, s, tw, logPT, tw16, tw3);
+}
+
+// One half (even bins: half = 0, odd bins: half = 1) of the Bluestein convolution of length P = 16384 for a ring of
+// 4096 < L <= 8192 complex points: on entry u = the chirped input (interleaved layout, zero beyond L; for half 1 already
+// multiplied by w_P^n); on exit u = conj(E[n]) or conj(O[n]) (interleaved layout), cf. bluestein_core.
+__device__ __forceinline__ void bluestein16k_half(cx<float> (&u)[2][16], cx<float>* __restrict__ s, int half, const cx<float>* __restrict__ fl,
+                                                  const cx<float>* __restrict__ tw, int logPT, const cx<float>* __restrict__ tw16,
+                                                  const cx<float>* __restrict__ tw3)
+{
+    constexpr int T = Fft3<12>::T, Q = Fft3<12>::Q;
+    const int t = (int)threadIdx.x;
+    fft8192_dit(u, s, tw, logPT, tw16, tw3);
+#pragma unroll
+    for (int q = 0; q < 16; ++q) {
+        const int k = t + T * q;                                               // filter table: F[2k], F[2k + 1] side by side
+        u[0][q] = cconj(cmul(u[0][q], fl[2 * k + half]));
+        u[1][q] = cconj(cmul(u[1][q], fl[2 * (k + Q) + half]));
+    }
+    __syncthreads();
+    fft8192_dif(u, s, tw, logPT, tw16, tw3);
+}
+
+// Steps 1 + 2 / 6 + 7 for Bluestein rings of 4096 < L <= 8192 complex points (the long cap rings of HEALPix nside 4096): the two
+// halves of the convolution one after the other, the first one parked in the ring's own output row meanwhile (spectrum row of
+// L + 1 coefficients / map ring of L pixel pairs; every thread reads back what it wrote).  grid = (jobs, nmaps), 256 threads.
+template <bool FWD>
+__global__ void __launch_bounds__(Fft3<12>::T, Fft3<12>::MINB)
+ring_fft3_bluestein2_kernel(const float* __restrict__ in, float* __restrict__ outmap, int64_t npix,
+                            cx<float>* __restrict__ spec, int64_t spec_stride, const FftJob* __restrict__ jobs,
+                            const cx<float>* __restrict__ tw, int logPT, const cx<float>* __restrict__ tw16,
+                            const cx<float>* __restrict__ tw3, const cx<float>* __restrict__ filt,
+                            const cx<float>* __restrict__ chirp, const cx<float>* __restrict__ phase)
+{
+    using F = Fft3<12>;
+    constexpr int T = F::T;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cx<float>* s = reinterpret_cast<cx<float>*>(smem_raw);
+    const int t = (int)threadIdx.x;
+    const FftJob& job = jobs[blockIdx.x];
+    const RingRec r0 = job.r0;
+    const FftLen f = job.f;
+    const int L = f.L;
+    const int shP = logPT - 14;                                                // w_P^n = tw[n << shP], P = 16384
+    const cx<float>* __restrict__ ph = phase + f.ph_off;
+    const cx<float>* __restrict__ cw = chirp + f.chirp_off;
+    const cx<float>* __restrict__ fl = filt + f.filt_off;
+    cx<float>* __restrict__ sp = spec + (int64_t)blockIdx.y * spec_stride + r0.spec_off;
+    cx<float> u[2][16];
+    if (FWD) {
+        const cx<float>* __restrict__ x0 = reinterpret_cast<const cx<float>*>(in + (int64_t)blockIdx.y * npix + r0.pix_off);
+        cx<float>* park = sp;                                                  // conj(E[n]), n < L
+#pragma unroll 1
+        for (int half = 0; half < 2; ++half) {
+#pragma unroll
+            for (int r = 0; r < 16; ++r) {
+#pragma unroll
+                for (int b = 0; b < 2; ++b) {
+                    const int n = 2 * (t + T * r) + b;
+                    cx<float> a = n < L ? cmul(x0[n], cw[n]) : mk<float>(0.f, 0.f);
+                    if (half == 1 && n < L) a = cmul(a, tw[n << shP]);
+                    u[b][r] = a;
+                }
+            }
+            if (half == 1) __syncthreads();
+            bluestein16k_half(u, s, half, fl, tw, logPT, tw16, tw3);
+            if (half == 0) {
+#pragma unroll
+                for (int r = 0; r < 16; ++r)
+#pragma unroll
+                    for (int b = 0; b < 2; ++b) {
+                        const int n = 2 * (t + T * r) + b;
+                        if (n < L) park[n] = u[b][r];
+                    }
+            }
+        }
+        __syncthreads();
+        // conj(y) = conj(E) + w_P^n conj(O);  Z[n] = chirp[n] y[n]
+#pragma unroll
+        for (int r = 0; r < 16; ++r)
+#pragma unroll
+            for (int b = 0; b < 2; ++b) {
+                const int n = 2 * (t + T * r) + b;
+                if (n < L) {
+                    const cx<float> cy = park[n] + cmul(u[b][r], tw[n << shP]);
+                    s[phys(n)] = cmul(cw[n], cconj(cy));
+                }
+            }
+        __syncthreads();
+        for (int k = t; k < L; k += T)
+            sp[k] = split_fwd(s[phys(k)], cconj(s[phys(k == 0 ? 0 : L - k)]), ph[k], r0.shifted);
+        if (t == 0) sp[L] = split_fwd(s[phys(0)], cconj(s[phys(0)]), ph[L], r0.shifted);
+    } else {
+        cx<float>* __restrict__ o0 = reinterpret_cast<cx<float>*>(outmap + (int64_t)blockIdx.y * npix + r0.pix_off);
+#pragma unroll 1
+        for (int half = 0; half < 2; ++half) {
+#pragma unroll
+            for (int r = 0; r < 16; ++r) {
+#pragma unroll
+                for (int b = 0; b < 2; ++b) {
+                    const int k = 2 * (t + T * r) + b;
+                    cx<float> v = mk<float>(0.f, 0.f);
+                    if (k < L) {
+                        const cx<float> hk = cconj(ph[k]), hl = mk<float>(hk.y, hk.x);     // exp(i pi (L-k)/N) = i conj(exp(i pi k/N))
+                        v = cmul(pack_inv(sp[k], sp[L - k], hk, hl, r0.shifted), cw[k]);
+                        if (half == 1) v = cmul(v, tw[k << shP]);
+                    }
+                    u[b][r] = v;
+                }
+            }
+            if (half == 1) __syncthreads();
+            bluestein16k_half(u, s, half, fl, tw, logPT, tw16, tw3);
+            if (half == 0) {
+#pragma unroll
+                for (int r = 0; r < 16; ++r)
+#pragma unroll
+                    for (int b = 0; b < 2; ++b) {
+                        const int n = 2 * (t + T * r) + b;
+                        if (n < L) o0[n] = u[b][r];                            // parked in the ring's own pixels
+                    }
+            }
+        }
+        // z'[n] = chirp[n] y[n]; out = conj(z') = conj(chirp[n]) conj(y[n])
+#pragma unroll
+        for (int r = 0; r < 16; ++r)
+#pragma unroll
+            for (int b = 0; b < 2; ++b) {
+                const int n = 2 * (t + T * r) + b;
+                if (n < L) o0[n] = cmulc(o0[n] + cmul(u[b][r], tw[n << shP]), cw[n]);
+            }
+    }
+}
+
+}  // namespace arkcos

@@ -31,6 +31,8 @@ int fft3_setup();               // shared-memory limits of all instantiations; r
 void fft3_launch_direct(int logq, bool fwd, const FftJob* jobs, unsigned njobs, unsigned nmaps, cudaStream_t st, const Fft3Args& a);
 // power-of-two rings of 8192 complex points: one ring (job.r0) per block, two size-4096 transforms and a radix-2 step
 void fft3_launch_direct2(bool fwd, const FftJob* jobs, unsigned njobs, unsigned nmaps, cudaStream_t st, const Fft3Args& a);
+// Bluestein rings of 4096 < L <= 8192 complex points: one ring (job.r0) per block, eight size-4096 transforms
+void fft3_launch_bluestein2(bool fwd, const FftJob* jobs, unsigned njobs, unsigned nmaps, cudaStream_t st, const Fft3Args& a);
 // Bluestein rings: one ring per block; sm_count sizes the look-ahead of the L2 prefetch
 void fft3_launch_bluestein(int logq, bool fwd, const FftJob* jobs, unsigned njobs, unsigned nmaps, cudaStream_t st, const Fft3Args& a,
                            int sm_count);

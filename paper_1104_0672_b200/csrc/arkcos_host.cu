@@ -185,6 +185,7 @@ struct HostTables {
     std::vector<int> fft_order[2];       // rings of the shared-memory FFT kernels, sorted by decreasing transform size
     std::vector<FftJob> fft3_jobs[2][4]; // jobs of the register-resident FFT kernels, Q = 512 << k
     std::vector<FftJob> fft3_d2[2];      // power-of-two rings of 8192 complex points (ring_fft3_direct2_kernel), one ring per job
+    std::vector<FftJob> fft3_b2[2];      // Bluestein rings of 4096 < L <= 8192 complex points (ring_fft3_bluestein2_kernel), mirror rings adjacent
     int64_t filt_total = 0, chirp_total = 0, ph_total = 0, nsamples = 0;
     int logPT = 1;
 };
@@ -280,6 +281,20 @@ void build_fft_lens(const HostGeometry& g, HostTables& t, Stats& st, bool use_ff
             j.f = f;
             t.fft3_d2[d].push_back(j);
         }
+        for (int i = g.R / 2; i >= 0; --i) {                 // Bluestein rings with a convolution of 16384 points, longest first
+            const int twin[2] = {i, g.R - 1 - i};
+            for (int h = 0; h < 2; ++h) {
+                const int r = twin[h];
+                const FftLen& f = t.lens[t.rings[r].len_id];
+                if (taken[r] || !use_fft3 || f.pow2 || f.logP != 14) continue;
+                taken[r] = 1;
+                if (!need[d][r]) continue;
+                FftJob j{};
+                j.r0 = t.rings[r];
+                j.f = f;
+                t.fft3_b2[d].push_back(j);
+            }
+        }
         for (int i = 0; i < g.R; ++i)
             if (!taken[i] && need[d][i]) t.fft_order[d].push_back(i);
         std::stable_sort(t.fft_order[d].begin(), t.fft_order[d].end(), [&](int a, int b) {
@@ -297,6 +312,7 @@ void build_fft_lens(const HostGeometry& g, HostTables& t, Stats& st, bool use_ff
         }
     for (int i : t.fft_order[0]) st.fft_pixels[8] += g.n[i];
     for (const FftJob& j : t.fft3_d2[0]) st.fft_pixels[8] += j.r0.n;      // launched beside the shared-memory kernel
+    for (const FftJob& j : t.fft3_b2[0]) st.fft_pixels[8] += j.r0.n;
 }
 
 // Ring-pair table for the northern output rings (the southern ones reuse the rows of their mirror images).
@@ -588,6 +604,8 @@ template <class T> int setup_fft3(arkcos_plan* pl, const HostTables& t)
     for (int d = 0; d < 2; ++d) {
         pl->nfft3_d2[d] = (int)t.fft3_d2[d].size();
         if (int rc = upload(&pl->d_fft3_d2[d], t.fft3_d2[d], &pl->stats.workspace_bytes)) return rc;
+        pl->nfft3_b2[d] = (int)t.fft3_b2[d].size();
+        if (int rc = upload(&pl->d_fft3_b2[d], t.fft3_b2[d], &pl->stats.workspace_bytes)) return rc;
     }
     std::vector<cx<float>> tw16(256);
     for (int k = 0; k < 16; ++k)
@@ -823,7 +841,7 @@ void launch_ring_ffts(const arkcos_plan* pl, const void* d_in, void* d_out, int 
     bool forked = false;
     auto launch_old = [&](cudaStream_t so) {            // the shared-memory kernel: very short or very long rings, fp64 plans
         if constexpr (sizeof(T) == 4) {
-            if (pl->nfft3_d2[FWD ? 0 : 1] > 0) {            // 8192-point power-of-two rings: two size-4096 transforms per block
+            if (pl->nfft3_d2[FWD ? 0 : 1] + pl->nfft3_b2[FWD ? 0 : 1] > 0) {   // rings of 8194 .. 16384 pixels on size-4096 transforms
                 Fft3Args a{};
                 a.in = (const float*)d_in;
                 a.outmap = (float*)d_out;
@@ -835,7 +853,12 @@ void launch_ring_ffts(const arkcos_plan* pl, const void* d_in, void* d_out, int 
                 a.tw3 = (const cx<float>*)pl->d_tw3 + pl->tw3_off[3];
                 a.phase = (const cx<float>*)pl->d_phase;
                 a.logPT = pl->logPT;
-                fft3_launch_direct2(FWD, pl->d_fft3_d2[FWD ? 0 : 1], (unsigned)pl->nfft3_d2[FWD ? 0 : 1], (unsigned)nmaps, so, a);
+                a.filt = (const cx<float>*)pl->d_filt;
+                a.chirp = (const cx<float>*)pl->d_chirp;
+                if (pl->nfft3_b2[FWD ? 0 : 1] > 0)
+                    fft3_launch_bluestein2(FWD, pl->d_fft3_b2[FWD ? 0 : 1], (unsigned)pl->nfft3_b2[FWD ? 0 : 1], (unsigned)nmaps, so, a);
+                if (pl->nfft3_d2[FWD ? 0 : 1] > 0)
+                    fft3_launch_direct2(FWD, pl->d_fft3_d2[FWD ? 0 : 1], (unsigned)pl->nfft3_d2[FWD ? 0 : 1], (unsigned)nmaps, so, a);
             }
         }
         if (pl->nfft_old[FWD ? 0 : 1] == 0) return;
@@ -862,7 +885,7 @@ void launch_ring_ffts(const arkcos_plan* pl, const void* d_in, void* d_out, int 
     };
     if constexpr (sizeof(T) == 4) {
         const int dir = FWD ? 0 : 1;
-        const int nside_launches = (pl->nfft3[dir][2] > 0) + (pl->nfft3[dir][1] + pl->nfft3[dir][0] > 0) + (pl->nfft_old[dir] + pl->nfft3_d2[dir] > 0);
+        const int nside_launches = (pl->nfft3[dir][2] > 0) + (pl->nfft3[dir][1] + pl->nfft3[dir][0] > 0) + (pl->nfft_old[dir] + pl->nfft3_d2[dir] + pl->nfft3_b2[dir] > 0);
         forked = pl->nfft3[dir][3] > 0 && nside_launches > 0 && pl->timing != 2;
         if (forked) {
             cudaEventRecord(pl->ev_fork, st);
@@ -1456,7 +1479,7 @@ int arkcos_plan_destroy(arkcos_plan* pl)
     void* ptrs[] = {pl->d_rings, pl->d_lens, pl->d_pairs, pl->d_north, pl->d_items[0], pl->d_items[1], pl->d_items[2], pl->d_items[3],
                     pl->d_items[4], pl->d_items[5], pl->d_eqchunks, pl->d_pole, pl->d_chirp, pl->d_phase, pl->d_fft_order[0], pl->d_fft_order[1], pl->d_table, pl->d_table2, pl->d_tw, pl->d_filt,
                     pl->d_W, pl->d_specIn, pl->d_specOut, pl->d_stage_in, pl->d_stage_out,
-                    pl->d_cap_chunks, pl->d_cap_chunk_items, pl->d_tc_chunks, pl->d_tc_tiles, pl->d_tc_cols, pl->d_tc_rings, pl->d_tc_items[0], pl->d_tc_items[1], pl->d_tc_items[2], pl->d_goff, pl->d_G, pl->d_pole_scratch, pl->d_nyq, pl->d_direct_items, pl->d_tw3, pl->d_tw16, pl->d_fft3_d2[0], pl->d_fft3_d2[1], pl->d_fft3_jobs[0][0], pl->d_fft3_jobs[0][1], pl->d_fft3_jobs[0][2], pl->d_fft3_jobs[0][3],
+                    pl->d_cap_chunks, pl->d_cap_chunk_items, pl->d_tc_chunks, pl->d_tc_tiles, pl->d_tc_cols, pl->d_tc_rings, pl->d_tc_items[0], pl->d_tc_items[1], pl->d_tc_items[2], pl->d_goff, pl->d_G, pl->d_pole_scratch, pl->d_nyq, pl->d_direct_items, pl->d_tw3, pl->d_tw16, pl->d_fft3_d2[0], pl->d_fft3_d2[1], pl->d_fft3_b2[0], pl->d_fft3_b2[1], pl->d_fft3_jobs[0][0], pl->d_fft3_jobs[0][1], pl->d_fft3_jobs[0][2], pl->d_fft3_jobs[0][3],
                     pl->d_fft3_jobs[1][0], pl->d_fft3_jobs[1][1], pl->d_fft3_jobs[1][2], pl->d_fft3_jobs[1][3]};
     for (void* p : ptrs) if (p) cudaFree(p);
     for (auto& e : pl->ev) if (e) cudaEventDestroy(e);
@@ -1599,7 +1622,7 @@ int arkcos_plan_launches_per_convolve(const arkcos_plan* pl)
     if (!pl) return -1;
     int n = (pl->opt.cache_kernel_rows || pl->npairs == 0) ? 0 : 1;
     for (int d = 0; d < 2; ++d) {
-        n += (pl->nfft_old[d] > 0 ? 1 : 0) + (pl->nfft3_d2[d] > 0 ? 1 : 0);
+        n += (pl->nfft_old[d] > 0 ? 1 : 0) + (pl->nfft3_d2[d] > 0 ? 1 : 0) + (pl->nfft3_b2[d] > 0 ? 1 : 0);
         for (int c = 0; c < 4; ++c) n += (pl->nfft3_bluestein[d][c] > 0 ? 1 : 0) + (pl->nfft3[d][c] > pl->nfft3_bluestein[d][c] ? 1 : 0);
     }
     n += (pl->nitems[0] > 0) + (pl->pole_warp_per_mode ? 2 : 1) * (pl->npole > 0) + (pl->neqchunks > 0);

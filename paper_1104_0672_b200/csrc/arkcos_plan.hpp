@@ -99,6 +99,8 @@ struct arkcos_plan {
     int nfft3[2][4] = {};
     arkcos::FftJob* d_fft3_d2[2] = {};   // power-of-two rings of 8192 complex points (ring_fft3_direct2_kernel)
     int nfft3_d2[2] = {};
+    arkcos::FftJob* d_fft3_b2[2] = {};   // Bluestein rings of 4096 < L <= 8192 complex points (ring_fft3_bluestein2_kernel)
+    int nfft3_b2[2] = {};
     int nfft3_bluestein[2][4] = {};   // the first jobs of each list are the Bluestein rings, the rest pairs of power-of-two rings
     void* d_tw3 = nullptr;       // cx<float>: pass-3 twiddles of the four transform sizes, see arkcos_fft3.cuh
     int tw3_off[4] = {0, 0, 0, 0};

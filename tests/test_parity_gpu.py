@@ -330,8 +330,9 @@ def test_cfg4_full_size_sampled_rings():
 
 
 def test_nside4096_maximum_size_sampled_rings():
-    """The largest HEALPix grid an fp32 plan accepts (ring length 16384: the belt as two size-4096 transforms per ring, the cap
-    rings longer than 8192 pixels through the shared-memory FFT path)."""
+    """The largest HEALPix grid an fp32 plan accepts: the belt rings of 16384 pixels as two size-4096 transforms
+    per ring, the cap rings of 8196 .. 16380 pixels by a Bluestein convolution of 16384 points built from the same transforms
+    (rings 2048, 2049, 3000, 4094 and a mirror ring), the shorter ones as at the smaller sizes."""
     nside = 4096
     geom = geometry.healpix_ring(nside)
     fwhm, tmax = 2.5 * ARCMIN, 7.5 * ARCMIN
@@ -339,7 +340,8 @@ def test_nside4096_maximum_size_sampled_rings():
     x = inputs.white_noise(geom.npix, 6)
     out, _ = gpu_convolve(("healpix", nside), tab, tmax, x)
     assert np.isfinite(out).all()
-    rings = np.array([0, 3, 700, 2047, 2048, 3000, nside - 1, nside, nside + 5, 2 * nside - 1, 3 * nside + 2, geom.nrings - 1])
+    rings = np.array([0, 3, 700, 2047, 2048, 2049, 3000, nside - 2, nside - 1, nside, nside + 5, 2 * nside - 1, 3 * nside + 2,
+                      geom.nrings - 1 - 3000, geom.nrings - 1])
     ref = direct.direct_sum(geom, tab, tmax, x.astype(np.float64), out_rings=rings)
     assert frms(take_rings(geom, out, rings), ref) <= 1e-5
 
