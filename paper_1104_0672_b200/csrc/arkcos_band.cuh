@@ -29,35 +29,34 @@ struct NorthRec { int pair_lo, pair_hi; };     // pairs of northern output ring 
 struct BandItem { int ring, m0; };             // one block of the band kernel: output ring, first folded mode
 
 // Step 3: evaluate the tabulated profile on the half-row of every ring pair.  The distance is
-// computed in double precision for both dtypes.  One block per pair.
-template <class T> __global__ void __launch_bounds__(128) kernel_rows_kernel(const PairRec* __restrict__ pairs, int npairs,
-                                                      const double* __restrict__ table, int ntab, double theta_max,
-                                                      T* __restrict__ W)
+// computed in double precision for both dtypes.  One thread per stored sample (rows are zero-padded to
+// multiples of four samples: wpair[g / 4] is the ring pair of the four samples from g on).
+template <class T> __global__ void __launch_bounds__(128) kernel_rows_kernel(const PairRec* __restrict__ pairs, const int* __restrict__ wpair,
+                                                      int64_t nsamples, const double* __restrict__ table, int ntab,
+                                                      double theta_max, T* __restrict__ W)
 {
-    const int p = (int)blockIdx.x * 4 + ((int)threadIdx.x >> 5);     // one warp per ring pair, four pairs per block
-    if (p >= npairs) return;
-    const PairRec pr = pairs[p];
+    const int64_t g = (int64_t)blockIdx.x * 128 + (int64_t)threadIdx.x;
+    if (g >= nsamples) return;
+    const PairRec pr = pairs[wpair[g >> 2]];
+    const int t = (int)(g - pr.woff);
+    if (t >= pr.cnt) { W[g] = (T)0; return; }
     const double inv2M = 1.0 / (2.0 * (double)pr.M);
     const double tscale = (double)(ntab - 1) / theta_max;
-    const int cnt4 = (pr.cnt + 3) & ~3;
-    for (int t = threadIdx.x & 31; t < cnt4; t += 32) {
-        if (t >= pr.cnt) { W[pr.woff + t] = (T)0; continue; }
-        const int u = 2 * t + pr.par;
-        const double sh = sinpi((double)u * inv2M);                    // sin(psi/2), psi = u pi / M
-        const double x = pr.A + pr.B * sh * sh;
-        const double gamma = gamma_of_chord2(x);
-        double val = 0.0;
-        if (gamma < theta_max) {
-            const double uu = gamma * tscale;
-            int tt = (int)floor(uu);
-            tt = max(0, min(tt, ntab - 2));
-            const double f = uu - (double)tt;
-            const double k0 = table[tt], k1 = table[tt + 1];
-            const double mult = (u == 0 || u == pr.M) ? 1.0 : 2.0;
-            val = (k0 + f * (k1 - k0)) * pr.scale * mult;
-        }
-        W[pr.woff + t] = (T)val;
+    const int u = 2 * t + pr.par;
+    const double sh = sinpi((double)u * inv2M);                        // sin(psi/2), psi = u pi / M
+    const double x = pr.A + pr.B * sh * sh;
+    const double gamma = gamma_of_chord2(x);
+    double val = 0.0;
+    if (gamma < theta_max) {
+        const double uu = gamma * tscale;
+        int tt = (int)floor(uu);
+        tt = max(0, min(tt, ntab - 2));
+        const double f = uu - (double)tt;
+        const double k0 = table[tt], k1 = table[tt + 1];
+        const double mult = (u == 0 || u == pr.M) ? 1.0 : 2.0;
+        val = (k0 + f * (k1 - k0)) * pr.scale * mult;
     }
+    W[g] = (T)val;
 }
 
 // Bp_j extended to any mode m >= 0 from the stored half spectrum b[0 .. N/2] (periodic extension).

@@ -697,9 +697,9 @@ namespace {
 
 template <class T> int enqueue_rows(const arkcos_plan* pl, cudaStream_t st)
 {
-    if (pl->npairs > 0)
-        kernel_rows_kernel<T><<<(pl->npairs + 3) / 4, 128, 0, st>>>(pl->d_pairs, pl->npairs, pl->d_table, pl->ntab, pl->theta_max,
-                                                         (T*)pl->d_W);
+    if (pl->npairs > 0 && pl->nsamples > 0)
+        kernel_rows_kernel<T><<<(unsigned)((pl->nsamples + 127) / 128), 128, 0, st>>>(pl->d_pairs, pl->d_wpair, pl->nsamples, pl->d_table, pl->ntab,
+                                                                                      pl->theta_max, (T*)pl->d_W);
     return 0;
 }
 
@@ -1155,6 +1155,13 @@ static int plan_create_impl(arkcos_plan** out, const arkcos_pixelization* pix, c
     if (int rc = upload(&pl->d_rings, t.rings, wsb)) return rc;
     if (int rc = upload(&pl->d_lens, t.lens, wsb)) return rc;
     if (int rc = upload(&pl->d_pairs, t.pairs, wsb)) return rc;
+    {
+        // ring pair of every group of four stored row samples (kernel_rows_kernel: one thread per sample)
+        std::vector<int> wpair((size_t)(t.nsamples / 4), 0);
+        for (size_t p = 0; p < t.pairs.size(); ++p)
+            for (int64_t q = t.pairs[p].woff / 4, e = q + (t.pairs[p].cnt + 3) / 4; q < e; ++q) wpair[(size_t)q] = (int)p;
+        if (int rc = upload(&pl->d_wpair, wpair, wsb)) return rc;
+    }
     if (int rc = upload(&pl->d_north, t.north, wsb)) return rc;
     for (int c = 0; c < kBandClasses; ++c)
         if (int rc = upload(&pl->d_items[c], t.items[c], wsb)) return rc;
@@ -1479,7 +1486,7 @@ int arkcos_plan_destroy(arkcos_plan* pl)
     void* ptrs[] = {pl->d_rings, pl->d_lens, pl->d_pairs, pl->d_north, pl->d_items[0], pl->d_items[1], pl->d_items[2], pl->d_items[3],
                     pl->d_items[4], pl->d_items[5], pl->d_eqchunks, pl->d_pole, pl->d_chirp, pl->d_phase, pl->d_fft_order[0], pl->d_fft_order[1], pl->d_table, pl->d_table2, pl->d_tw, pl->d_filt,
                     pl->d_W, pl->d_specIn, pl->d_specOut, pl->d_stage_in, pl->d_stage_out,
-                    pl->d_cap_chunks, pl->d_cap_chunk_items, pl->d_tc_chunks, pl->d_tc_tiles, pl->d_tc_cols, pl->d_tc_rings, pl->d_tc_items[0], pl->d_tc_items[1], pl->d_tc_items[2], pl->d_goff, pl->d_G, pl->d_pole_scratch, pl->d_nyq, pl->d_direct_items, pl->d_tw3, pl->d_tw16, pl->d_fft3_d2[0], pl->d_fft3_d2[1], pl->d_fft3_b2[0], pl->d_fft3_b2[1], pl->d_fft3_jobs[0][0], pl->d_fft3_jobs[0][1], pl->d_fft3_jobs[0][2], pl->d_fft3_jobs[0][3],
+                    pl->d_cap_chunks, pl->d_cap_chunk_items, pl->d_tc_chunks, pl->d_tc_tiles, pl->d_tc_cols, pl->d_tc_rings, pl->d_tc_items[0], pl->d_tc_items[1], pl->d_tc_items[2], pl->d_goff, pl->d_G, pl->d_pole_scratch, pl->d_nyq, pl->d_direct_items, pl->d_tw3, pl->d_tw16, pl->d_fft3_d2[0], pl->d_fft3_d2[1], pl->d_fft3_b2[0], pl->d_fft3_b2[1], pl->d_wpair, pl->d_fft3_jobs[0][0], pl->d_fft3_jobs[0][1], pl->d_fft3_jobs[0][2], pl->d_fft3_jobs[0][3],
                     pl->d_fft3_jobs[1][0], pl->d_fft3_jobs[1][1], pl->d_fft3_jobs[1][2], pl->d_fft3_jobs[1][3]};
     for (void* p : ptrs) if (p) cudaFree(p);
     for (auto& e : pl->ev) if (e) cudaEventDestroy(e);

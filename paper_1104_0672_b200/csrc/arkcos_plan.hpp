@@ -86,6 +86,7 @@ struct arkcos_plan {
     bool pole_warp_per_mode = false;
     arkcos::BandItem* d_items[arkcos::kBandClasses] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
     double* d_table = nullptr;
+    int* d_wpair = nullptr;       // ring pair of every group of four stored kernel-row samples
     double* d_table2 = nullptr;   // exact_caps: (K[t], K[t+1] - K[t]) pairs
     void* d_tw = nullptr;        // cx<T>[PT/2]
     void* d_filt = nullptr;      // cx<T>[...] Bluestein filter spectra
