@@ -256,6 +256,24 @@ def test_exact_caps_hard_edged_kernels(dtype, nmaps):
         assert frms(plain, ref1) > 1e-5            # without the option the caps carry the scheme's artifact level
 
 
+@pytest.mark.parametrize("nside", [1, 2, 4, 8])
+def test_exact_caps_tiny_grids_and_map_counts(nside):
+    """exact_caps on the smallest grids (rings of 4 .. 32 pixels: quadrants of one pixel, whole-ring windows, most threads of
+    a block idle) and with 1, 5, 17 maps (one, eight and a partial chunk of maps per thread; 3 fp64 maps) against the
+    brute-force sum (Eq. 6)."""
+    geom = geometry.healpix_ring(nside)
+    pixsz = np.sqrt(4 * np.pi / geom.npix)
+    for tmax in (1.5 * pixsz, min(4.0 * pixsz, 3.0)):
+        tab = inputs.gaussian_table(tmax / 2, tmax)
+        for dtype, nmaps in ((arkcos.F32, 1), (arkcos.F32, 5), (arkcos.F64, 3), (arkcos.F32, 17)):
+            x = inputs.white_noise_maps(geom.npix, 3, nmaps)
+            if dtype == arkcos.F64:
+                x = x.astype(np.float64)
+            out, _ = gpu_convolve(("healpix", nside), tab, tmax, x, dtype, exact_caps=1)
+            ref = direct.direct_sum(geom, tab, tmax, x.astype(np.float64))
+            assert maxrel(out, ref) <= (1e-12 if dtype == arkcos.F64 else 2e-6)
+
+
 @pytest.mark.parametrize("dtype,nmaps", [(arkcos.F64, 3), (arkcos.F32, 5), (arkcos.F32, 2)])
 def test_exact_caps_wide_kernel_long_windows(dtype, nmaps):
     """exact_caps with a kernel 100 pixels wide (Eq. 6): the input windows of a thread block are longer than the
