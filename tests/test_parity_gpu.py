@@ -355,7 +355,7 @@ def test_nside4096_maximum_size_sampled_rings():
     geom = geometry.healpix_ring(nside)
     fwhm, tmax = 2.5 * ARCMIN, 7.5 * ARCMIN
     tab = inputs.gaussian_table(fwhm, tmax)
-    x = inputs.white_noise(geom.npix, 6)
+    x = inputs.white_noise_maps(geom.npix, 6, 2)
     out, _ = gpu_convolve(("healpix", nside), tab, tmax, x)
     assert np.isfinite(out).all()
     rings = np.array([0, 3, 700, 2047, 2048, 2049, 3000, nside - 2, nside - 1, nside, nside + 5, 2 * nside - 1, 3 * nside + 2,
