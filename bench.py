@@ -421,6 +421,18 @@ def run_ours(args):
             blk[kspec["kernel"]] = row
         extra["cfg5"] = blk
         del x5, o5
+        torch.cuda.empty_cache()
+        # nside 4096 (the paper's next size; not a BASELINE.json config): rings of up to 16384 pixels
+        ns = 4096
+        np4 = 12 * ns * ns
+        fw4, tm4 = 2.5 * inputs.ARCMIN, 7.5 * inputs.ARCMIN
+        x4 = torch.randn(np4, dtype=torch.float32, device="cuda", generator=torch.Generator(device="cuda").manual_seed(4096))
+        o4 = torch.empty_like(x4)
+        p4 = arkcos.Plan(("healpix", ns), inputs.gaussian_table(fw4, tm4), tm4, dtype)
+        ms4 = timed(p4, 1, x4, o4, 10)
+        extra["nside4096"] = {"workload": "HEALPix nside=4096 (201 Mpix), Gaussian FWHM 2.5' cut at 7.5', 1 map",
+                              "ms_per_map": ms4, "gpix_per_s": np4 / (ms4 * 1e-3) / 1e9}
+        del p4, x4, o4
 
     cpu = time_oracle(c, tab, x, args.oracle_rings)
     cpu_val = cpu["pixels"] * cpu["maps"] / cpu["seconds"] / 1e6
